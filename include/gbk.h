@@ -1,0 +1,174 @@
+/*
+ * gbk.h -- C ABI of libgbk: batched residual / chi^2 evaluation of GBKFIT-style
+ * kinematic models of disc galaxies on NVIDIA B200 (sm_100a).
+ *
+ * The operation is the paper's "intensity cube modelling strategy"
+ * (Bekiaris et al., arXiv:1510.01815; citations are /root/reference/PAPER.md
+ * lines): one fitting iteration = evaluate the model cube (PAPER.md:63,
+ * 197-210), convolve it with the PSF and LSF,
+ * down-sample, extract velocity and dispersion maps as the
+ * first and second moments, and form the error-weighted
+ * residual and chi^2 against the observed maps (eq. 11).
+ * Every optimiser of the paper (LM, nested sampling, nested grids;
+ * PAPER.md:265-289) calls that iteration thousands of times; here it is
+ * batched: K parameter rows per call.
+ *
+ * Plain C, no torch types.  Every pointer says whether it is HOST or DEVICE
+ * memory.  No function throws or aborts; all return GBK_OK or an error code
+ * and leave a message for gbk_last_error().  There is NO CPU fallback: without
+ * a CUDA device every compute call returns GBK_ERR_CUDA.
+ *
+ * Model row (GBK_P = 10 floats):
+ *   [0] x_o, [1] y_o    kinematic centre, data pixels (pixel j is centred on j)
+ *   [2] PA   degrees    position angle (eq. 1-2)
+ *   [3] i    degrees    inclination (eq. 3)
+ *   [4] V_sys km/s      systemic velocity (eq. 8)
+ *   [5] V_t  km/s, [6] r_t px   rotation curve (eq. 6; or ramp)
+ *   [7] sigma_0 km/s    intrinsic dispersion
+ *   [8] r_0 px, [9] I_0 exponential disc (eq. 5)
+ *
+ * Out-of-domain rows are not errors: a row with a non-finite parameter,
+ * sigma_0 <= 0, r_0 <= 0, r_t <= 0, I_0 <= 0 or |cos i| < 1e-6, or with an
+ * unmasked spaxel that is model-dark (m0 < 1e-30 * I_0) or has non-finite
+ * moments, gets chi2 = +INF (an optimiser rejects it).
+ */
+#ifndef GBK_H_
+#define GBK_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GBK_P 10
+
+enum { GBK_OK = 0, GBK_ERR_ARG = 1, GBK_ERR_ALLOC = 2, GBK_ERR_CUDA = 3, GBK_ERR_UNSUPPORTED = 4 };
+enum { GBK_RC_ARCTAN = 0, GBK_RC_RAMP = 1 };     /* eq. 6; V_t*min(r/r_t,1) */
+enum { GBK_PSF_GAUSSIAN = 0, GBK_PSF_IMAGE = 1 }; /* eq. 9; image */
+
+typedef struct gbk_problem gbk_problem; /* opaque; owns device copies of the observation */
+
+/*
+ * Problem descriptor: the observation a batch of rows is compared with
+ * (velocity and dispersion maps with optional error and mask maps,
+ * PAPER.md:185; PSF and LSF; grid and up-sampling factor,
+ * PAPER.md:201; rotation-curve choice).
+ * All pointers are HOST memory, read during gbk_create_problem only; the caller
+ * may free them afterwards.  Maps are [n_gal][ny][nx], x fastest.
+ */
+typedef struct {
+  int32_t nx, ny, nv;   /* spaxels and velocity channels of the observation               */
+  int32_t u;            /* spatial up-sampling factor >= 1; the model is evaluated on a     */
+                        /* (u*nx) x (u*ny) fine grid and block-averaged */
+  float v_center, dv;   /* km/s; channel k has velocity v_center + (k-(nv-1)/2)*dv          */
+  int32_t rc_model;     /* GBK_RC_*                                                        */
+  int32_t n_gal;        /* data sets held by this problem (>= 1)                           */
+  const float *vobs;    /* observed velocity map, km/s (required)                          */
+  const float *verr;    /* its 1-sigma error map, > 0 where unmasked (required)            */
+  const float *sobs;    /* observed dispersion map; NULL with serr NULL drops the second   */
+  const float *serr;    /* term of eq. 11.  W of eq. 11 is pre-folded by    */
+                        /* the caller as serr / sqrt(W)                     */
+  const uint8_t *mask;  /* 0 = masked spaxel; NULL = all valid              */
+  int32_t psf_kind;     /* GBK_PSF_*                                                       */
+  const float *psf_fwhm;  /* GAUSSIAN: FWHM in DATA pixels, [n_gal] if psf_per_gal else [1]; */
+                          /* taps exp(-j^2/2s^2), s = u*FWHM/(2 sqrt(2 ln 2)) fine pixels,   */
+                          /* j in [-R,R], R = ceil(4 s), normalised to sum 1; FWHM <= 0 is   */
+                          /* the delta PSF                                                  */
+  const float *psf_image; /* IMAGE: [n_gal or 1][psf_n][psf_n] sampled on the FINE grid,     */
+  int32_t psf_n;          /* psf_n odd; normalised to sum 1 at create; applied as a true     */
+                          /* convolution (kernel flipped)                                   */
+  int32_t psf_per_gal;  /* 0: one PSF shared by all data sets                              */
+  float lsf_sigma;      /* km/s; Gaussian LSF, taps R = ceil(4*sigma/dv) channels,           */
+                        /* normalised; <= 0 is the delta LSF                               */
+  int32_t tile_w, tile_h; /* spatial tile of one thread block in SPAXELS; 0 = automatic     */
+  int32_t device;       /* CUDA device ordinal; < 0 = the current device                   */
+} gbk_problem_desc;
+
+/* What gbk_create_problem decided (for tests, benchmarks and op counting). */
+typedef struct {
+  int32_t nx, ny, nv, u, n_gal;
+  int32_t r_v;            /* LSF tap radius, channels                                      */
+  int32_t r_p_max;        /* largest PSF tap radius over the data sets, fine pixels        */
+  int32_t tile_w, tile_h; /* tile in spaxels                                               */
+  int32_t tiles_x, tiles_y;
+  int32_t block_threads;  /* threads per block of the fused kernel                        */
+  int32_t smem_bytes;     /* dynamic shared memory per block                              */
+  int32_t blocks_per_sm;  /* occupancy of the fused kernel as reported by the runtime      */
+  int32_t sm_count;
+  int64_t ext_voxels_per_eval; /* sum over tiles of (tw+2R)(th+2R)(nv+2R_v), R = r_p_max   */
+} gbk_problem_info;
+
+/*
+ * Validates the descriptor, copies the observation to the device, builds tap
+ * and channel tables, picks the tiling.  *out receives the handle.
+ * Errors: GBK_ERR_ARG (NULL/shape/non-finite unmasked data/even psf_n/non-
+ * positive error at an unmasked spaxel), GBK_ERR_UNSUPPORTED (tile does not
+ * fit in shared memory, PSF radius beyond the supported maximum),
+ * GBK_ERR_ALLOC, GBK_ERR_CUDA.
+ */
+int gbk_create_problem(const gbk_problem_desc *desc, gbk_problem **out);
+
+int gbk_get_info(const gbk_problem *p, gbk_problem_info *info);
+
+/*
+ * The hot path (PAPER.md:63-66 steps 1-3 for K rows), fused: the model cube is
+ * never written to memory.  Asynchronous on `cuda_stream`; never synchronises
+ * or allocates except to grow the cross-tile scratch when K grows (first call
+ * with a larger K).
+ *   params     DEVICE [K][GBK_P] float32, row-major
+ *   gal_index  DEVICE [K] int32 in [0, n_gal), or NULL (all rows use data set 0)
+ *   chi2       DEVICE [K] float32, required (eq. 11)
+ *   m0,m1,m2   DEVICE [K][ny][nx] float32 each, any may be NULL: flux (sum over
+ *              channels), velocity (first moment) and dispersion (sqrt of the
+ *              second central moment) maps of the model
+ *   resid      DEVICE [K][2][ny][nx] float32 or NULL: (model-obs)/err for the
+ *              velocity and dispersion maps, 0 where masked
+ *   cuda_stream  a cudaStream_t (NULL = the legacy default stream)
+ * The caller owns all buffers.
+ */
+int gbk_eval_batch(gbk_problem *p, const float *params, const int32_t *gal_index, int64_t K,
+                   float *chi2, float *m0, float *m1, float *m2, float *resid,
+                   void *cuda_stream);
+
+/*
+ * Comparison path, same contract: one kernel per step of the paper's pipeline
+ * (PAPER.md:197-251), with the FP32 model cube written to device memory
+ * between steps (the paper's own structure minus the FFT).  Processes the rows
+ * in chunks that fit its scratch buffer.
+ */
+int gbk_eval_batch_unfused(gbk_problem *p, const float *params, const int32_t *gal_index,
+                           int64_t K, float *chi2, float *m0, float *m1, float *m2, float *resid,
+                           void *cuda_stream);
+
+/*
+ * End-to-end entry with HOST buffers: copies params (and gal_index) to the
+ * device, runs gbk_eval_batch, copies chi2 back and waits for `cuda_stream`.
+ * params/gal_index/chi2 are HOST pointers (pinned memory makes the copies
+ * asynchronous and faster; pageable memory also works).
+ */
+int gbk_eval_batch_host(gbk_problem *p, const float *params, const int32_t *gal_index, int64_t K,
+                        float *chi2, void *cuda_stream);
+
+/* Frees device memory.  NULL is a no-op. */
+int gbk_destroy(gbk_problem *p);
+
+/* Thread-local message of the last failing call on this thread ("" if none). */
+const char *gbk_last_error(void);
+
+/*
+ * Pipe-throughput probes used for the roofline denominators (DESIGN.md
+ * "Roofline"): a register-only loop of independent MUFU.EX2 (which = 0) or
+ * FFMA (which = 1) instructions on every SM.  Launches one kernel on
+ * `cuda_stream` executing `iters` x 16 instructions per thread in
+ * `blocks` x `threads`; `sink` is a DEVICE float buffer of at least one element
+ * (written only to keep the loop alive).  *ops_per_launch receives the number
+ * of lane-level operations the launch executes.
+ */
+int gbk_probe_pipe(int which, int64_t iters, int blocks, int threads, float *sink,
+                   double *ops_per_launch, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GBK_H_ */

@@ -1,0 +1,381 @@
+// Host side of libgbk: descriptor validation, table building, tiling, the C ABI of include/gbk.h.
+// No CPU fallback: every compute call ends in a kernel launch or an error code.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "gbk_internal.h"
+
+using namespace gbk;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define GBK_CUDA(expr)                                                                  \
+  do {                                                                                  \
+    cudaError_t e_ = (expr);                                                            \
+    if (e_ != cudaSuccess)                                                              \
+      return fail(e_ == cudaErrorMemoryAllocation ? GBK_ERR_ALLOC : GBK_ERR_CUDA,       \
+                  "%s: %s", #expr, cudaGetErrorString(e_));                             \
+  } while (0)
+
+int round_up4(int v) { return (v + 3) & ~3; }
+
+// Gaussian taps exp(-j^2 / 2 sigma^2), j in [-R, R], R = ceil(4 sigma), normalised to sum 1
+// (eq. 9 of the paper sampled on the grid).  sigma <= 0: delta.
+std::vector<double> gaussian_taps(double sigma) {
+  if (!(sigma > 0.0)) return {1.0};
+  const int R = (int)ceil(4.0 * sigma);
+  std::vector<double> t(2 * R + 1);
+  double sum = 0.0;
+  for (int j = -R; j <= R; ++j) sum += (t[j + R] = exp(-0.5 * (double)j * j / (sigma * sigma)));
+  for (double& v : t) v /= sum;
+  return t;
+}
+
+}  // namespace
+
+struct gbk_problem {
+  gbk_problem_desc d{};       // scalars only are meaningful after create
+  DevProblem dp{};
+  FusedLaunch fl{};
+  int device = 0;
+  int sm_count = 0, blocks_per_sm = 0;
+  long long ext_voxels = 0;
+  // device allocations owned by the problem
+  float4* chan_tab = nullptr;
+  float* psf_taps = nullptr;
+  int* psf_r = nullptr;
+  float4* obs = nullptr;
+  float* partial = nullptr;
+  long long partial_cap = 0;    // rows
+  // staging for gbk_eval_batch_host
+  float* st_params = nullptr;
+  int32_t* st_gal = nullptr;
+  float* st_chi2 = nullptr;
+  long long st_cap = 0;
+  // scratch of the unfused path
+  float* uf_scratch = nullptr;
+  size_t uf_bytes = 0;
+};
+
+extern "C" const char* gbk_last_error(void) { return g_err; }
+
+extern "C" int gbk_destroy(gbk_problem* p) {
+  if (!p) return GBK_OK;
+  cudaFree(p->chan_tab);
+  cudaFree(p->psf_taps);
+  cudaFree(p->psf_r);
+  cudaFree(p->obs);
+  cudaFree(p->partial);
+  cudaFree(p->st_params);
+  cudaFree(p->st_gal);
+  cudaFree(p->st_chi2);
+  cudaFree(p->uf_scratch);
+  delete p;
+  return GBK_OK;
+}
+
+extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) {
+  g_err[0] = 0;
+  if (!d || !out) return fail(GBK_ERR_ARG, "null descriptor or output pointer");
+  *out = nullptr;
+  if (d->nx < 1 || d->ny < 1 || d->nv < 1 || d->u < 1 || d->n_gal < 1)
+    return fail(GBK_ERR_ARG, "nx, ny, nv, u and n_gal must be >= 1");
+  if ((long long)d->nx * d->u > 16384 || (long long)d->ny * d->u > 16384 || d->nv > 16384)
+    return fail(GBK_ERR_ARG, "grid too large");
+  if (!(d->dv > 0.f) || !isfinite(d->dv) || !isfinite(d->v_center))
+    return fail(GBK_ERR_ARG, "dv must be > 0 and finite, v_center finite");
+  if (d->rc_model != GBK_RC_ARCTAN && d->rc_model != GBK_RC_RAMP)
+    return fail(GBK_ERR_ARG, "unknown rc_model %d", d->rc_model);
+  if (!d->vobs || !d->verr) return fail(GBK_ERR_ARG, "vobs and verr are required");
+  if ((d->sobs == nullptr) != (d->serr == nullptr))
+    return fail(GBK_ERR_ARG, "sobs and serr must both be given or both be NULL");
+  if (d->psf_kind != GBK_PSF_GAUSSIAN && d->psf_kind != GBK_PSF_IMAGE)
+    return fail(GBK_ERR_ARG, "unknown psf_kind %d", d->psf_kind);
+  if (!isfinite(d->lsf_sigma)) return fail(GBK_ERR_ARG, "lsf_sigma must be finite");
+
+  const int n_psf = d->psf_per_gal ? d->n_gal : 1;
+  const size_t npix = (size_t)d->nx * d->ny;
+
+  // ---- LSF taps and the LSF-folded channel weights (a4) ---------------------------------
+  const std::vector<double> lsf = gaussian_taps(d->lsf_sigma > 0.f ? (double)d->lsf_sigma / d->dv : 0.0);
+  const int r_v = (int)(lsf.size() / 2);
+  if (r_v > kMaxLsfR) return fail(GBK_ERR_UNSUPPORTED, "LSF radius %d > %d channels", r_v, kMaxLsfR);
+  const int nvx = d->nv + 2 * r_v;
+  // w_q[c] = sum over in-band channels k of L[k - ch] * v'_k^q, ch = c - r_v,
+  // v'_k = (k - (nv-1)/2) dv  (velocities relative to v_center).
+  std::vector<float4> chan(nvx);
+  for (int c = 0; c < nvx; ++c) {
+    const int ch = c - r_v;
+    double w[3] = {0, 0, 0};
+    for (int k = std::max(0, ch - r_v); k <= std::min(d->nv - 1, ch + r_v); ++k) {
+      const double L = lsf[(k - ch) + r_v];
+      const double v = ((double)k - 0.5 * (d->nv - 1)) * (double)d->dv;
+      w[0] += L;
+      w[1] += L * v;
+      w[2] += L * v * v;
+    }
+    chan[c] = make_float4((float)c, (float)w[0], (float)w[1], (float)w[2]);
+  }
+
+  // ---- PSF sets ------------------------------------------------------------------------
+  std::vector<int> psf_r(n_psf);
+  std::vector<float> psf_taps;
+  int psf_stride = 0, r_p_max = 0;
+  if (d->psf_kind == GBK_PSF_GAUSSIAN) {
+    if (!d->psf_fwhm) return fail(GBK_ERR_ARG, "psf_fwhm is required for a Gaussian PSF");
+    std::vector<std::vector<double>> sets(n_psf);
+    for (int g = 0; g < n_psf; ++g) {
+      const double fwhm = d->psf_fwhm[g];
+      if (!isfinite(fwhm)) return fail(GBK_ERR_ARG, "psf_fwhm[%d] is not finite", g);
+      const double sigma_f = (double)d->u * fwhm / (2.0 * sqrt(2.0 * log(2.0)));
+      sets[g] = gaussian_taps(sigma_f);
+      psf_r[g] = (int)(sets[g].size() / 2);
+      r_p_max = std::max(r_p_max, psf_r[g]);
+    }
+    if (r_p_max > kMaxSepR)
+      return fail(GBK_ERR_UNSUPPORTED, "Gaussian PSF radius %d fine pixels > %d", r_p_max, kMaxSepR);
+    psf_stride = 2 * r_p_max + 1;
+    psf_taps.assign((size_t)n_psf * psf_stride, 0.f);
+    for (int g = 0; g < n_psf; ++g)
+      for (size_t j = 0; j < sets[g].size(); ++j) psf_taps[(size_t)g * psf_stride + j] = (float)sets[g][j];
+  } else {
+    if (!d->psf_image) return fail(GBK_ERR_ARG, "psf_image is required for an image PSF");
+    if (d->psf_n < 1 || (d->psf_n & 1) == 0) return fail(GBK_ERR_ARG, "psf_n must be odd and >= 1");
+    if (d->psf_n > kMaxPsfN) return fail(GBK_ERR_UNSUPPORTED, "psf_n %d > %d", d->psf_n, kMaxPsfN);
+    const int n = d->psf_n;
+    psf_stride = n * n;
+    r_p_max = n / 2;
+    psf_taps.resize((size_t)n_psf * psf_stride);
+    for (int g = 0; g < n_psf; ++g) {
+      const float* img = d->psf_image + (size_t)g * psf_stride;
+      double sum = 0.0;
+      for (int i = 0; i < psf_stride; ++i) {
+        if (!isfinite(img[i])) return fail(GBK_ERR_ARG, "psf_image has a non-finite value");
+        sum += img[i];
+      }
+      if (!(sum > 0.0)) return fail(GBK_ERR_ARG, "psf_image must have a positive sum");
+      // stored flipped: the kernel correlates, which is then the true convolution
+      for (int y = 0; y < n; ++y)
+        for (int x = 0; x < n; ++x)
+          psf_taps[(size_t)g * psf_stride + y * n + x] = (float)(img[(n - 1 - y) * n + (n - 1 - x)] / sum);
+      psf_r[g] = n / 2;
+    }
+  }
+
+  // ---- packed observation: {vobs - v_center, 1/E_v (0 = masked), sobs, 1/E_s} ------------
+  std::vector<float4> obs((size_t)d->n_gal * npix);
+  for (size_t i = 0; i < obs.size(); ++i) {
+    const bool unmasked = !d->mask || d->mask[i] != 0;
+    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (unmasked) {
+      const float v = d->vobs[i], ev = d->verr[i];
+      if (!isfinite(v) || !isfinite(ev) || !(ev > 0.f))
+        return fail(GBK_ERR_ARG, "unmasked spaxel %zu: vobs/verr must be finite and verr > 0", i);
+      o.x = (float)((double)v - (double)d->v_center);
+      o.y = (float)(1.0 / (double)ev);
+      if (d->sobs) {
+        const float s = d->sobs[i], es = d->serr[i];
+        if (!isfinite(s) || !isfinite(es) || !(es > 0.f))
+          return fail(GBK_ERR_ARG, "unmasked spaxel %zu: sobs/serr must be finite and serr > 0", i);
+        o.z = s;
+        o.w = (float)(1.0 / (double)es);
+      }
+      if (!(o.y > 0.f)) return fail(GBK_ERR_ARG, "unmasked spaxel %zu: verr too large", i);
+    }
+    obs[i] = o;
+  }
+
+  // ---- device and tiling ---------------------------------------------------------------
+  int dev = d->device;
+  if (dev < 0) GBK_CUDA(cudaGetDevice(&dev));
+  GBK_CUDA(cudaSetDevice(dev));
+  cudaDeviceProp prop;
+  GBK_CUDA(cudaGetDeviceProperties(&prop, dev));
+  const size_t smem_cap = prop.sharedMemPerBlockOptin;
+
+  gbk_problem* p = new (std::nothrow) gbk_problem;
+  if (!p) return fail(GBK_ERR_ALLOC, "out of host memory");
+  p->d = *d;
+  p->device = dev;
+  p->sm_count = prop.multiProcessorCount;
+  DevProblem& dp = p->dp;
+  dp.nx = d->nx, dp.ny = d->ny, dp.nv = d->nv, dp.u = d->u, dp.n_gal = d->n_gal;
+  dp.fw = d->u * d->nx, dp.fh = d->u * d->ny;
+  dp.r_v = r_v, dp.nvx = nvx;
+  dp.rc_model = d->rc_model, dp.psf_kind = d->psf_kind;
+  dp.has_disp = d->sobs ? 1 : 0, dp.psf_per_gal = d->psf_per_gal ? 1 : 0;
+  dp.r_p_max = r_p_max, dp.psf_stride = psf_stride;
+  dp.dv = d->dv, dp.v_center = d->v_center;
+  dp.vrel_first = (float)((-(double)r_v - 0.5 * (d->nv - 1)) * (double)d->dv);
+  dp.inv_u = 1.0f / (float)d->u, dp.inv_u2 = 1.0f / ((float)d->u * (float)d->u);
+
+  auto set_tile = [&](int tws, int ths) {   // in spaxels
+    dp.tile_w = tws * d->u, dp.tile_h = ths * d->u;
+    dp.tiles_x = (d->nx + tws - 1) / tws, dp.tiles_y = (d->ny + ths - 1) / ths;
+    dp.ntiles = dp.tiles_x * dp.tiles_y;
+    dp.ews = round_up4(dp.tile_w) + 4 * ((2 * r_p_max + 4 + 3) / 4) - 4;
+    dp.ehs = dp.tile_h + 2 * r_p_max;
+    return fused_smem_bytes(dp);
+  };
+  int tws = d->tile_w > 0 ? std::min(d->tile_w, d->nx) : d->nx;
+  int ths = d->tile_h > 0 ? std::min(d->tile_h, d->ny) : d->ny;
+  size_t smem = set_tile(tws, ths);
+  if (d->tile_w <= 0 || d->tile_h <= 0) {
+    // automatic: halve the longer side until two blocks fit on an SM (or at least one does)
+    const size_t want = (smem_cap - 2048) / 2;
+    while (smem > want && (tws > 8 || ths > 8)) {
+      if (d->tile_w <= 0 && (tws >= ths || d->tile_h > 0) && tws > 8) tws = (tws + 1) / 2;
+      else if (d->tile_h <= 0 && ths > 8) ths = (ths + 1) / 2;
+      else break;
+      smem = set_tile(tws, ths);
+    }
+  }
+  if (smem > smem_cap) {
+    delete p;
+    return fail(GBK_ERR_UNSUPPORTED, "tile %dx%d spaxels needs %zu B of shared memory (max %zu)", tws,
+                ths, smem, smem_cap);
+  }
+  // launch shape: P pixels per thread in the voxel loop, threads per block
+  const int n_ext = (dp.tile_w + 2 * r_p_max) * (dp.tile_h + 2 * r_p_max);
+  p->fl.smem_bytes = (int)smem;
+  p->fl.pixels_per_thread = 4;
+  p->fl.threads = std::min(384, std::max(64, ((n_ext + 3) / 4 + 31) / 32 * 32));
+  long long ext = 0;
+  for (int ty = 0; ty < dp.tiles_y; ++ty)
+    for (int tx = 0; tx < dp.tiles_x; ++tx) {
+      const int tw = std::min(dp.tile_w, dp.fw - tx * dp.tile_w), th = std::min(dp.tile_h, dp.fh - ty * dp.tile_h);
+      ext += (long long)(tw + 2 * r_p_max) * (th + 2 * r_p_max) * nvx;
+    }
+  p->ext_voxels = ext;
+
+  auto bail = [&](int code) {
+    gbk_destroy(p);
+    return code;
+  };
+#define GBK_CUDA_P(expr)                                                                       \
+  do {                                                                                         \
+    cudaError_t e_ = (expr);                                                                   \
+    if (e_ != cudaSuccess)                                                                     \
+      return bail(fail(e_ == cudaErrorMemoryAllocation ? GBK_ERR_ALLOC : GBK_ERR_CUDA, "%s: %s", \
+                       #expr, cudaGetErrorString(e_)));                                        \
+  } while (0)
+  GBK_CUDA_P(cudaMalloc(&p->chan_tab, sizeof(float4) * nvx));
+  GBK_CUDA_P(cudaMalloc(&p->psf_taps, sizeof(float) * psf_taps.size()));
+  GBK_CUDA_P(cudaMalloc(&p->psf_r, sizeof(int) * n_psf));
+  GBK_CUDA_P(cudaMalloc(&p->obs, sizeof(float4) * obs.size()));
+  GBK_CUDA_P(cudaMemcpy(p->chan_tab, chan.data(), sizeof(float4) * nvx, cudaMemcpyHostToDevice));
+  GBK_CUDA_P(cudaMemcpy(p->psf_taps, psf_taps.data(), sizeof(float) * psf_taps.size(), cudaMemcpyHostToDevice));
+  GBK_CUDA_P(cudaMemcpy(p->psf_r, psf_r.data(), sizeof(int) * n_psf, cudaMemcpyHostToDevice));
+  GBK_CUDA_P(cudaMemcpy(p->obs, obs.data(), sizeof(float4) * obs.size(), cudaMemcpyHostToDevice));
+  dp.chan_tab = p->chan_tab, dp.psf_taps = p->psf_taps, dp.psf_r = p->psf_r, dp.obs = p->obs;
+  GBK_CUDA_P(fused_prepare(p->fl));
+  GBK_CUDA_P(fused_occupancy(p->fl, &p->blocks_per_sm));
+#undef GBK_CUDA_P
+  // host pointers of the descriptor are not kept
+  p->d.vobs = p->d.verr = p->d.sobs = p->d.serr = nullptr;
+  p->d.mask = nullptr;
+  p->d.psf_fwhm = p->d.psf_image = nullptr;
+  *out = p;
+  return GBK_OK;
+}
+
+extern "C" int gbk_get_info(const gbk_problem* p, gbk_problem_info* info) {
+  if (!p || !info) return fail(GBK_ERR_ARG, "null argument");
+  const DevProblem& dp = p->dp;
+  info->nx = dp.nx, info->ny = dp.ny, info->nv = dp.nv, info->u = dp.u, info->n_gal = dp.n_gal;
+  info->r_v = dp.r_v, info->r_p_max = dp.r_p_max;
+  info->tile_w = dp.tile_w / dp.u, info->tile_h = dp.tile_h / dp.u;
+  info->tiles_x = dp.tiles_x, info->tiles_y = dp.tiles_y;
+  info->block_threads = p->fl.threads, info->smem_bytes = p->fl.smem_bytes;
+  info->blocks_per_sm = p->blocks_per_sm, info->sm_count = p->sm_count;
+  info->ext_voxels_per_eval = p->ext_voxels;
+  return GBK_OK;
+}
+
+static int check_eval_args(gbk_problem* p, const float* params, int64_t K, float* chi2) {
+  if (!p) return fail(GBK_ERR_ARG, "null problem");
+  if (K < 0) return fail(GBK_ERR_ARG, "K must be >= 0");
+  if (K > 0 && (!params || !chi2)) return fail(GBK_ERR_ARG, "params and chi2 are required");
+  if (K * (int64_t)p->dp.ntiles > 0x7fffffffLL) return fail(GBK_ERR_ARG, "K * tiles exceeds the grid limit");
+  return GBK_OK;
+}
+
+extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
+                              float* chi2, float* m0, float* m1, float* m2, float* resid,
+                              void* cuda_stream) {
+  g_err[0] = 0;
+  if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  if (K == 0) return GBK_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  GBK_CUDA(cudaSetDevice(p->device));
+  if (p->dp.ntiles > 1 && K > p->partial_cap) {
+    if (p->partial) GBK_CUDA(cudaFree(p->partial));   // synchronises; only when K grows
+    p->partial = nullptr, p->partial_cap = 0;
+    GBK_CUDA(cudaMalloc(&p->partial, sizeof(float) * (size_t)K * p->dp.ntiles));
+    p->partial_cap = K;
+  }
+  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, p->partial};
+  GBK_CUDA(launch_fused(p->dp, a, p->fl, st));
+  return GBK_OK;
+}
+
+extern "C" int gbk_eval_batch_host(gbk_problem* p, const float* params, const int32_t* gal_index,
+                                   int64_t K, float* chi2, void* cuda_stream) {
+  g_err[0] = 0;
+  if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  if (K == 0) return GBK_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  GBK_CUDA(cudaSetDevice(p->device));
+  if (K > p->st_cap) {
+    cudaFree(p->st_params), cudaFree(p->st_gal), cudaFree(p->st_chi2);
+    p->st_params = nullptr, p->st_gal = nullptr, p->st_chi2 = nullptr, p->st_cap = 0;
+    GBK_CUDA(cudaMalloc(&p->st_params, sizeof(float) * GBK_P * (size_t)K));
+    GBK_CUDA(cudaMalloc(&p->st_gal, sizeof(int32_t) * (size_t)K));
+    GBK_CUDA(cudaMalloc(&p->st_chi2, sizeof(float) * (size_t)K));
+    p->st_cap = K;
+  }
+  GBK_CUDA(cudaMemcpyAsync(p->st_params, params, sizeof(float) * GBK_P * (size_t)K, cudaMemcpyHostToDevice, st));
+  if (gal_index)
+    GBK_CUDA(cudaMemcpyAsync(p->st_gal, gal_index, sizeof(int32_t) * (size_t)K, cudaMemcpyHostToDevice, st));
+  if (int rc = gbk_eval_batch(p, p->st_params, gal_index ? p->st_gal : nullptr, K, p->st_chi2, nullptr,
+                              nullptr, nullptr, nullptr, cuda_stream))
+    return rc;
+  GBK_CUDA(cudaMemcpyAsync(chi2, p->st_chi2, sizeof(float) * (size_t)K, cudaMemcpyDeviceToHost, st));
+  GBK_CUDA(cudaStreamSynchronize(st));
+  return GBK_OK;
+}
+
+extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const int32_t* gal_index,
+                                      int64_t K, float* chi2, float* m0, float* m1, float* m2,
+                                      float* resid, void* cuda_stream) {
+  (void)gal_index, (void)m0, (void)m1, (void)m2, (void)resid, (void)cuda_stream;
+  g_err[0] = 0;
+  if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  return fail(GBK_ERR_UNSUPPORTED, "unfused comparison path not built yet");
+}
+
+extern "C" int gbk_probe_pipe(int which, int64_t iters, int blocks, int threads, float* sink,
+                              double* ops_per_launch, void* cuda_stream) {
+  g_err[0] = 0;
+  if ((which != 0 && which != 1) || iters < 1 || blocks < 1 || threads < 32 || threads > 1024 || !sink)
+    return fail(GBK_ERR_ARG, "bad probe arguments");
+  if (ops_per_launch) *ops_per_launch = 16.0 * (double)iters * (double)blocks * (double)threads;
+  GBK_CUDA(launch_probe(which, iters, blocks, threads, sink, (cudaStream_t)cuda_stream));
+  return GBK_OK;
+}

@@ -1,0 +1,79 @@
+// Internal declarations shared by the translation units of libgbk (CUDA side only; the CPU
+// oracle under oracle/ shares nothing with this tree).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gbk.h"
+
+namespace gbk {
+
+constexpr int kMaxSepR = 16;    // largest separable (Gaussian) PSF tap radius, fine pixels
+constexpr int kMaxPsfN = 33;    // largest PSF image side
+constexpr int kMaxLsfR = 64;    // largest LSF tap radius, channels
+constexpr int kVBlock = 8;      // output rows per thread in the vertical pass
+
+// Everything the kernels need to know about a problem; passed by value (__grid_constant__).
+struct DevProblem {
+  int nx, ny, nv, u;        // spaxels, channels, up-sampling
+  int n_gal;
+  int fw, fh;               // fine grid = u*nx, u*ny
+  int r_v, nvx;             // LSF radius, nv + 2 r_v extended channels
+  int rc_model, psf_kind, has_disp, psf_per_gal;
+  int tile_w, tile_h;       // tile, fine pixels (multiples of u)
+  int tiles_x, tiles_y, ntiles;
+  int r_p_max;              // largest PSF radius
+  int ews, ehs;             // shared-memory row stride (floats) and rows of one moment map
+  int psf_stride;           // floats per PSF set in psf_taps
+  float dv, v_center;
+  float vrel_first;         // velocity of extended channel 0 relative to v_center
+  float inv_u, inv_u2;
+  const float4* chan_tab;   // [nvx] {channel index as float, w0, w1, w2}: LSF-folded moment weights
+  const float* psf_taps;    // [n_psf][psf_stride]: Gaussian 1-D taps, or flipped PSF image
+  const int* psf_r;         // [n_psf] tap radius of each PSF set
+  const float4* obs;        // [n_gal][ny][nx] {vobs - v_center, 1/E_v (0 = masked), sobs, 1/E_s}
+};
+
+struct EvalArgs {
+  const float* params;      // [K][GBK_P]
+  const int32_t* gal_index; // [K] or null
+  long long K;
+  float* chi2;              // [K]
+  float *m0, *m1, *m2;      // [K][ny][nx] or null
+  float* resid;             // [K][2][ny][nx] or null
+  float* partial;           // [K][ntiles] cross-tile scratch (ntiles > 1)
+};
+
+// Per-row constants (a1 of SURVEY.md section 8(a)), computed once per block.
+struct RowConst {
+  float xo, yo, sp, cp, inv_ci;
+  float vrot_scale;   // arctan: (2/pi) V_t sin i;  ramp: V_t sin i
+  float inv_rt;
+  float nl2e_inv_r0;  // -log2(e)/r0
+  float vsys_rel;     // V_sys - v_center
+  float s;            // 1/(sigma0 sqrt(2 ln 2)):  exp(-dv^2/(2 sigma0^2)) = 2^-(s dv)^2
+  float step;         // s * dv
+  float d_first;      // s * vrel_first
+  float amp;          // I0 * dv / (sigma0 sqrt(2 pi) u^2): scales the S0 block sum to m0
+  float dark_s0;      // S0 block sums below this are model-dark (m0 < 1e-30 I0)
+  int valid;
+  int r_p;            // PSF radius of this row's data set
+  int psf_set, gal;
+};
+
+struct FusedLaunch {
+  int threads;
+  int smem_bytes;
+  int pixels_per_thread;  // P of the voxel loop
+};
+
+cudaError_t launch_fused(const DevProblem& dp, const EvalArgs& a, const FusedLaunch& fl,
+                         cudaStream_t st);
+cudaError_t fused_occupancy(const FusedLaunch& fl, int* blocks_per_sm);
+cudaError_t fused_prepare(const FusedLaunch& fl);  // opt in to large dynamic shared memory
+size_t fused_smem_bytes(const DevProblem& dp);
+
+cudaError_t launch_probe(int which, long long iters, int blocks, int threads, float* sink,
+                         cudaStream_t st);
+
+}  // namespace gbk

@@ -1,0 +1,329 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: m0 1e-4 relative, m1/m2 0.05 km/s absolute,
+chi^2 1e-4 relative (see parity_util.compare).  All tests here need a GPU.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1510_01815_b200 import workloads as wl
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu tests need a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gbk():
+    from paper_1510_01815_b200 import gbk as g
+    g.lib()
+    return g
+
+
+def _gpu_eval(torch, gbk, desc, rows, gal_index=None, want_maps=True, want_resid=False,
+              unfused=False):
+    with gbk.Problem(**desc) as prob:
+        p = torch.from_numpy(np.ascontiguousarray(rows, dtype=np.float32)).cuda()
+        gi = None if gal_index is None else torch.from_numpy(
+            np.ascontiguousarray(gal_index, dtype=np.int32)).cuda()
+        out = prob.eval(p, gi, want_maps=want_maps, want_resid=want_resid, unfused=unfused)
+        torch.cuda.synchronize()
+        res = {k: v.cpu().numpy() for k, v in out.items()}
+        res["info"] = prob.info
+    return res
+
+
+def _rows_near(w, true_row, rng, n):
+    """n trial rows scattered around the true row (10 % of the box width), plus the true row."""
+    b = wl.box(w)
+    width = b[:, 1] - b[:, 0]
+    rows = np.repeat(np.asarray(true_row, dtype=np.float64).reshape(1, -1), n, axis=0)
+    rows[1:] += 0.1 * width * rng.uniform(-1, 1, (n - 1, wl.P))
+    rows[:, wl.IX_INC] = np.clip(rows[:, wl.IX_INC], 5.0, 85.0)
+    rows[:, wl.IX_RT] = np.clip(rows[:, wl.IX_RT], 0.5, None)
+    return rows.astype(np.float32)
+
+
+# ------------------------------------------------------------------------- config 1 ----
+
+@pytest.mark.parametrize("tile", [(0, 0), (16, 16), (12, 10), (8, 32)])
+def test_cfg1_maps_and_chi2(oracle, torch_cuda, gbk, tile):
+    w = wl.config(1)
+    rng = wl.rng_for(1)
+    true = wl.cfg1_true_row(rng)
+    g, obs = pu.single_galaxy_case(oracle, w, true[0], rng)
+    rows = np.concatenate([wl.cfg1_trial_row(), true, _rows_near(w, true[0], rng, 6)])
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True, want_resid=True)
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1]), rows,
+                    want_resid=True)
+    worst = pu.compare(ref, got, rows, want_maps=True, label=f"cfg1 tile={tile}")
+    m = obs.mask[0] != 0
+    dres = np.abs(got["resid"] - ref["resid"])[:, :, m]
+    assert dres.max() <= pu.TOL_M12_ABS / 5.0 + 1e-6          # residual = map difference / 5 km/s
+    assert np.all(got["resid"][:, :, ~m] == 0)
+    if tile != (0, 0):
+        assert got["info"].tiles_x * got["info"].tiles_y > 1
+    print("cfg1", tile, worst)
+
+
+# ------------------------------------------------- config 2 (u = 2), reduced and sampled ----
+
+def test_cfg2_reduced_supersampled(oracle, torch_cuda, gbk):
+    w = wl.config(2).scaled(nx=22, ny=18, nv=48)
+    rng = wl.rng_for(2)
+    true = wl.draw_rows(w, rng, 1)[0]
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = wl.lm_rows(w, true)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    for tile in [(0, 0), (8, 6)]:
+        got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1]), rows)
+        print("cfg2-reduced", tile, pu.compare(ref, got, rows, True, f"cfg2r tile={tile}"))
+
+
+def test_cfg2_full_size_sampled_rows(oracle, torch_cuda, gbk):
+    w = wl.config(2)
+    rng = wl.rng_for(2, 1)
+    true = wl.draw_rows(w, rng, 1)[0]
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = wl.lm_rows(w, true)                       # K = 8, the launch shape of the LM driver
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows)
+    pick = [0, 3, 7]
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0],
+                           rows[pick], want_maps=True)
+    sub = {k: v[pick] for k, v in got.items() if k != "info"}
+    print("cfg2-full", pu.compare(ref, sub, rows[pick], True, "cfg2 full"))
+
+
+# ----------------------------------------------------- config 3: the headline launch ----
+
+def test_cfg3_full_launch_sampled_rows(oracle, torch_cuda, gbk):
+    w = wl.config(3)
+    rng = wl.rng_for(3)
+    true = wl.draw_rows(w, rng, 1)[0]
+    true[[wl.IX_XO, wl.IX_YO, wl.IX_VSYS]] = (31.7, 32.4, 0.0)
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = wl.nested_grid_rows(w, true, level=0)      # K = 4096, chi^2 only (bench configuration)
+    assert rows.shape == (4096, wl.P)
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows, want_maps=False)
+    pick = rng.choice(4096, size=48, replace=False)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0],
+                           rows[pick])
+    sub = {"chi2": got["chi2"][pick]}
+    print("cfg3", pu.compare(ref, sub, rows[pick], False, "cfg3"))
+    # the grid minimum found on the GPU is the oracle's minimum among the sampled rows
+    assert pick[np.argmin(ref["chi2"])] == pick[np.argmin(sub["chi2"])]
+    # maps for a few rows as well
+    got_m = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows[pick[:6]])
+    ref_m = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0],
+                             rows[pick[:6]], want_maps=True)
+    print("cfg3 maps", pu.compare(ref_m, got_m, rows[pick[:6]], True, "cfg3 maps"))
+
+
+# ------------------------------------------------------- config 4: image PSF, ramp ----
+
+def test_cfg4_reduced_moffat_ramp(oracle, torch_cuda, gbk):
+    w = wl.config(4).scaled(nx=44, ny=36)
+    rng = wl.rng_for(4)
+    true = wl.draw_rows(w, rng, 1)[0]
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    assert 0.25 < 1.0 - obs.mask.mean() < 0.35        # ~30 % masked
+    rows = np.concatenate([true[None], wl.draw_rows(w, rng, 11)])
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    for tile in [(0, 0), (16, 12)]:
+        got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1]), rows)
+        print("cfg4-reduced", tile, pu.compare(ref, got, rows, True, f"cfg4r tile={tile}"))
+
+
+def test_cfg4_full_size_sampled_rows(oracle, torch_cuda, gbk):
+    w = wl.config(4)
+    rng = wl.rng_for(4, 1)
+    true = wl.draw_rows(w, rng, 1)[0]
+    true[wl.IX_R0] = 30.0
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = wl.draw_rows(w, rng, w.K)
+    rows[0] = true
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows, want_maps=True)
+    pick = [0, 17, 101]
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0],
+                           rows[pick], want_maps=True)
+    sub = {k: v[pick] for k, v in got.items() if k != "info"}
+    print("cfg4-full", pu.compare(ref, sub, rows[pick], True, "cfg4 full"))
+
+
+# ------------------------------------------------ config 5: mixed-galaxy batches ----
+
+def test_cfg5_mixed_galaxies(oracle, torch_cuda, gbk):
+    n_gal = 6
+    w = wl.config(5).scaled(n_gal=n_gal)
+    rng = wl.rng_for(5)
+    fwhms = wl.galaxy_fwhms(w, rng)
+    trues = wl.draw_rows(w, rng, n_gal)
+    grids, clean = [], []
+    for gi in range(n_gal):
+        g = pu.oracle_grid(oracle, w, fwhms[gi])
+        grids.append(g)
+        clean.append(oracle.model_maps(g, trues[gi].astype(np.float64)))
+    m0, m1, m2 = (np.stack([c[i] for c in clean]) for i in range(3))
+    obs = wl.observe(w, m0, m1, m2, rng)
+    rows, gal = [], []
+    for gi in range(n_gal):                          # LM-shaped slots: base + 7 forward differences
+        rows.append(wl.lm_rows(w, trues[gi]))
+        gal += [gi] * 8
+    rows = np.concatenate(rows)
+    gal = np.asarray(gal, dtype=np.int32)
+    perm = rng.permutation(len(gal))                  # mixed order
+    rows, gal = rows[perm], gal[perm]
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs, fwhms=fwhms), rows, gal_index=gal)
+    assert got["info"].r_p_max == max(int(math.ceil(4 * oracle.fwhm_to_sigma(pu.f32(f)))) for f in fwhms)
+    for gi in range(n_gal):
+        sel = np.nonzero(gal == gi)[0]
+        ref = oracle.eval_rows(grids[gi], obs.vobs[gi], obs.verr[gi], obs.sobs[gi], obs.serr[gi],
+                               obs.mask[gi], rows[sel], want_maps=True)
+        sub = {k: v[sel] for k, v in got.items() if k != "info"}
+        print("cfg5 gal", gi, float(fwhms[gi]), pu.compare(ref, sub, rows[sel], True, f"cfg5 gal {gi}"))
+
+
+# ------------------------------------------------------------------- edge cases ----
+
+def _tiny_case(oracle, **kw):
+    w = wl.config(1).scaled(**{**dict(nx=14, ny=11, nv=40), **kw})
+    rng = np.random.default_rng(11)
+    true = np.array([6.2, 5.1, 140.0, 50.0, 8.0, 180.0, 2.0, 40.0, 3.0, 1.5], dtype=np.float32)
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    return w, g, obs, true, rng
+
+
+def test_out_of_domain_rows_and_empty_batch(oracle, torch_cuda, gbk):
+    w, g, obs, true, rng = _tiny_case(oracle)
+    rows = np.repeat(true[None], 8, axis=0)
+    rows[1, wl.IX_SIG] = 0.0
+    rows[2, wl.IX_R0] = -1.0
+    rows[3, wl.IX_RT] = 0.0
+    rows[4, wl.IX_INC] = 90.0
+    rows[5, wl.IX_VT] = np.nan
+    rows[6, wl.IX_I0] = 0.0
+    rows[7, wl.IX_XO] = np.inf
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    for tile in [(0, 0), (5, 4)]:
+        got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1]), rows,
+                        want_resid=True)
+        assert np.isfinite(got["chi2"][0]) and np.all(np.isposinf(got["chi2"][1:]))
+        assert np.all(np.isposinf(ref["chi2"][1:]))
+        assert np.isnan(got["m1"][1:]).all() and np.isnan(got["resid"][1:]).all()
+        pu.compare(ref, got, rows, True, "domain")
+    # K = 0 is a no-op
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        p = torch_cuda.empty((0, 10), dtype=torch_cuda.float32, device="cuda")
+        assert prob.eval(p)["chi2"].numel() == 0
+    # a gal_index outside [0, n_gal) makes the row +INF instead of reading out of bounds
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows[:2],
+                    gal_index=np.array([0, 3], dtype=np.int32), want_maps=False)
+    assert np.isfinite(got["chi2"][0]) and np.isposinf(got["chi2"][1])
+
+
+def test_model_dark_unmasked_spaxel_gives_inf(oracle, torch_cuda, gbk):
+    w, g, obs, true, rng = _tiny_case(oracle)
+    rows = np.repeat(true[None], 2, axis=0)
+    rows[1, wl.IX_R0] = 0.02         # exp(-r/r0) falls below 1e-30 inside the field
+    obs.mask[:] = 1                   # nothing masked: dark spaxels count
+    obs.verr[:] = 5.0
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows)
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows, want_maps=False)
+    assert np.isposinf(ref["chi2"][1]) and np.isposinf(got["chi2"][1])
+    assert np.isfinite(got["chi2"][0])
+
+
+def test_masks_and_missing_dispersion_term(oracle, torch_cuda, gbk):
+    w, g, obs, true, rng = _tiny_case(oracle)
+    rows = _rows_near(w, true, rng, 4)
+    # all masked: chi^2 = 0
+    all_masked = wl.Observed(obs.vobs, obs.verr, obs.sobs, obs.serr, np.zeros_like(obs.mask))
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, all_masked), rows, want_maps=False)
+    assert np.all(got["chi2"] == 0.0)
+    # no dispersion map: second term of eq. 11 dropped
+    d = pu.gbk_desc(w, obs)
+    d["sobs"] = d["serr"] = None
+    got = _gpu_eval(torch_cuda, gbk, d, rows, want_maps=False)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], None, None, obs.mask[0], rows)
+    pu.compare(ref, got, rows, False, "no dispersion")
+    # mask = None: every spaxel counts
+    d = pu.gbk_desc(w, obs)
+    d["mask"] = None
+    full = wl.Observed(obs.vobs, obs.verr, obs.sobs, obs.serr, np.ones_like(obs.mask))
+    got = _gpu_eval(torch_cuda, gbk, d, rows, want_maps=False)
+    ref = oracle.eval_rows(g, full.vobs[0], full.verr[0], full.sobs[0], full.serr[0], None, rows)
+    pu.compare(ref, got, rows, False, "no mask")
+
+
+@pytest.mark.parametrize("kw", [dict(psf_fwhm=0.0, lsf_sigma=0.0), dict(psf_fwhm=0.7),
+                                dict(u=3, psf_fwhm=1.2), dict(u=4, nx=6, ny=5, psf_fwhm=1.6),
+                                dict(v_center=1500.0), dict(rc_model=wl.RC_RAMP),
+                                dict(psf_fwhm=6.7, nx=9, ny=7)])
+def test_variants(oracle, torch_cuda, gbk, kw):
+    w, g, obs, true, rng = _tiny_case(oracle, **kw)
+    if "v_center" in kw:
+        true = true.copy()
+        true[wl.IX_VSYS] += kw["v_center"]
+        g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = _rows_near(w, true, rng, 5)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows)
+    print("variant", kw, pu.compare(ref, got, rows, True, f"variant {kw}"))
+
+
+def test_bitwise_reproducible_and_host_entry(oracle, torch_cuda, gbk):
+    torch = torch_cuda
+    w, g, obs, true, rng = _tiny_case(oracle)
+    rows = _rows_near(w, true, rng, 64)
+    with gbk.Problem(**pu.gbk_desc(w, obs, tile_w=5, tile_h=4)) as prob:
+        p = torch.from_numpy(rows).cuda()
+        a = prob.eval(p)["chi2"].cpu().numpy()
+        b = prob.eval(p)["chi2"].cpu().numpy()
+        assert np.array_equal(a, b)                      # fixed-order reductions, no float atomics
+        host_params = torch.from_numpy(rows).pin_memory()
+        host_chi2 = torch.empty(64, dtype=torch.float32).pin_memory()
+        gbk.gbk_eval_batch_host(prob.handle, host_params, None, 64, host_chi2,
+                                torch.cuda.current_stream().cuda_stream)
+        assert np.array_equal(host_chi2.numpy(), a)
+        pageable = np.empty(64, dtype=np.float32)
+        gbk.gbk_eval_batch_host(prob.handle, rows, None, 64, pageable)
+        assert np.array_equal(pageable, a)
+
+
+def test_create_rejects_bad_descriptors(oracle, torch_cuda, gbk):
+    w, g, obs, true, rng = _tiny_case(oracle)
+    d = pu.gbk_desc(w, obs)
+    bad = dict(d)
+    bad["dv"] = 0.0
+    with pytest.raises(gbk.GbkError) as e:
+        gbk.Problem(**bad)
+    assert e.value.code == gbk.GBK_ERR_ARG
+    bad = dict(d)
+    v = obs.vobs.copy()
+    v[0][obs.mask[0] != 0] = np.nan
+    bad["vobs"] = v
+    with pytest.raises(gbk.GbkError):
+        gbk.Problem(**bad)
+    bad = dict(d)
+    bad["psf_kind"], bad["psf_image"] = gbk.GBK_PSF_IMAGE, np.ones((4, 4), dtype=np.float32)
+    with pytest.raises(gbk.GbkError):
+        gbk.Problem(**bad)
+    bad = dict(d)
+    bad["psf_fwhm"] = np.array([40.0], dtype=np.float32)          # radius beyond the supported maximum
+    with pytest.raises(gbk.GbkError) as e:
+        gbk.Problem(**bad)
+    assert e.value.code == gbk.GBK_ERR_UNSUPPORTED
