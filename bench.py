@@ -1,0 +1,390 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of libgbk on B200 (contract: see the task prompt / DESIGN.md
+"Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+
+One "step" = one pass of the whole hot path over one batch:
+`gbk_eval_batch` on K_rows parameter rows of BASELINE.json config 3 (64x64 spaxels x 64 channels,
+K_rows = 4096 = one nested-grid level, chi^2 only), the configuration BASELINE.json's metric is
+quoted on.  Prints ONE JSON line on rank 0.
+
+  value      model evaluations / s, inputs resident in HBM, CUDA events around each launch on the
+             launching stream, L2 flushed between timed launches, max over ranks
+  e2e        the same through gbk_eval_batch_host: HOST (pinned) params in, HOST chi^2 out, copies
+             inside the timed region (wall clock around a blocking call)
+  roofline   the fused kernel against the SM arithmetic pipe that bounds it (MUFU, "alu")
+  cpu_baseline   the CPU oracle (oracle/, untouched) on a bounded sample of the same rows
+
+The oracle is executed only by the cpu_baseline leg and by --impl reference.  Nothing here reads
+/root/reference.  All inputs are seeded and synthetic (paper_1510_01815_b200/workloads.py).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1510_01815_b200 import workloads as wl  # noqa: E402
+
+METRIC = "model evals/sec (cube+PSF+moments+\u03c7\u00b2) at 64\u00d764\u00d764, K=4096; % FP32/SFU peak"
+UNIT = "evals/s"
+SM_COUNT_B200 = 148
+MUFU_LANES_PER_SM_CLK = 16      # 4 SMSPs x 4 MUFU lanes
+FP32_LANES_PER_SM_CLK = 128
+
+
+# ------------------------------------------------------------------------------ inputs ----
+
+def true_row_for(cfg: int, w: wl.Workload, rng) -> np.ndarray:
+    true = wl.draw_rows(w, rng, 1)[0]
+    if cfg == 3:   # centre and V_sys fixed at truth; DESIGN.md "Input recipe"
+        true[[wl.IX_XO, wl.IX_YO, wl.IX_VSYS]] = (31.7, 32.4, 0.0)
+    return true
+
+
+def batch_rows(cfg: int, w: wl.Workload, true: np.ndarray, rng, n_batches: int) -> list:
+    """The parameter batches the timed steps cycle through (float32 [K, P] each)."""
+    if cfg == 3:   # the four nested-grid levels, each 8^4 nodes, re-centred on the truth
+        centre = true[[wl.IX_PA, wl.IX_INC, wl.IX_VT, wl.IX_RT]].astype(np.float64)
+        return [wl.nested_grid_rows(w, true, level=l, centre=None if l == 0 else centre)
+                for l in range(min(4, max(1, n_batches)))]
+    return [wl.draw_rows(w, rng, w.K) for _ in range(min(4, max(1, n_batches)))]
+
+
+def desc_for(w: wl.Workload, obs: wl.Observed) -> dict:
+    d = dict(nx=w.nx, ny=w.ny, nv=w.nv, u=w.u, v_center=w.v_center, dv=w.dv, rc_model=w.rc_model,
+             n_gal=1, vobs=obs.vobs, verr=obs.verr, sobs=obs.sobs, serr=obs.serr, mask=obs.mask,
+             psf_kind=w.psf_kind, lsf_sigma=w.lsf_sigma)
+    if w.psf_kind == wl.PSF_GAUSSIAN:
+        d["psf_fwhm"] = np.asarray([w.psf_fwhm], dtype=np.float32)
+    else:
+        d["psf_image"] = wl.moffat_image(w.psf_fwhm, w.moffat_beta, w.psf_n)
+    return d
+
+
+def observation_from_gpu(gbk, torch, w: wl.Workload, true: np.ndarray, rng) -> wl.Observed:
+    """Clean maps of the true row from the CUDA path itself (the GPU leg never calls the oracle),
+    then seeded noise / errors / mask."""
+    blank = wl.Observed(*(np.zeros((1, w.ny, w.nx), np.float32) for _ in range(2)),
+                        *(np.zeros((1, w.ny, w.nx), np.float32) for _ in range(2)),
+                        np.zeros((1, w.ny, w.nx), np.uint8))
+    blank.verr[:] = 1.0
+    blank.serr[:] = 1.0
+    with gbk.Problem(**desc_for(w, blank)) as prob:
+        out = prob.eval(torch.from_numpy(true[None].copy()).cuda(), want_maps=True)
+        torch.cuda.synchronize()
+        m0, m1, m2 = (out[k].cpu().numpy().astype(np.float64) for k in ("m0", "m1", "m2"))
+    return wl.observe(w, m0, m1, m2, rng)
+
+
+# ------------------------------------------------------------------------------ clocks ----
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (profiling recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        rows = [l for (t, l) in self.lines if t0 <= t <= t1 + 0.11] or [l for (_, l) in self.lines]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in rows:
+            f = [x.strip() for x in l.split(",")]
+            try:
+                sm.append(float(f[0])), mx.append(float(f[1])), pw.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------- the CPU oracle legs ----
+
+def oracle_grid(oracle, w: wl.Workload):
+    """Oracle Grid of workload w (its own tap builders; nothing shared with the CUDA path)."""
+    f32 = lambda x: float(np.float32(x))
+    if w.psf_kind == wl.PSF_GAUSSIAN:
+        psf = oracle.psf_gaussian_image(f32(w.psf_fwhm), w.u)
+    else:
+        img = wl.moffat_image(w.psf_fwhm, w.moffat_beta, w.psf_n).astype(np.float64)
+        psf = img / img.sum()
+    lsf = oracle.gaussian_taps(f32(w.lsf_sigma) / f32(w.dv) if w.lsf_sigma > 0 else 0.0)
+    return oracle.Grid(nx=w.nx, ny=w.ny, nv=w.nv, u=w.u, v_center=f32(w.v_center), dv=f32(w.dv),
+                       rc_model=w.rc_model, psf=psf, lsf=lsf)
+
+
+def host_cores() -> int:
+    return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
+def oracle_case(cfg: int):
+    """Workload, oracle grid, observation (clean maps from the ORACLE here) and batches."""
+    from oracle import gbk_oracle as oracle
+    w = wl.config(cfg)
+    rng = wl.rng_for(cfg, 100)
+    true = true_row_for(cfg, w, rng)
+    g = oracle_grid(oracle, w)
+    m0, m1, m2 = oracle.model_maps(g, true.astype(np.float64))
+    obs = wl.observe(w, m0[None], m1[None], m2[None], rng)
+    return oracle, w, g, obs, batch_rows(cfg, w, true, rng, 4)
+
+
+def time_oracle(cfg: int, rows_per_step: int, steps: int, warmup: int, threads: int) -> dict:
+    """The oracle as it stands on `threads` host threads: `steps` timed calls of `rows_per_step`
+    rows each (the first rows of the batches the GPU leg cycles through)."""
+    oracle, w, g, obs, batches = oracle_case(cfg)
+    o = obs
+    call = lambda rows: oracle.eval_rows(g, o.vobs[0], o.verr[0], o.sobs[0], o.serr[0], o.mask[0],
+                                         rows, nthreads=threads)
+    for i in range(warmup):
+        call(batches[i % len(batches)][:max(1, min(rows_per_step, threads))])
+    t0 = time.perf_counter()
+    for i in range(steps):
+        call(batches[i % len(batches)][:rows_per_step])
+    dt = time.perf_counter() - t0
+    return {"value": rows_per_step * steps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "seconds": dt,
+            "sample": f"first {rows_per_step} rows of each of {steps} config-{cfg} batches "
+                      f"(K={w.K} per batch on the GPU), double precision, OpenMP over rows"}
+
+
+def run_reference(args, ranks) -> None:
+    """--impl reference: the oracle is this tier's reference arm.  Rank 0 only."""
+    if not ranks.is_main:
+        return
+    cores = host_cores()
+    rows_per_step = args.ref_rows or max(cores, 4 * cores)
+    r = time_oracle(args.config, rows_per_step, args.steps, min(args.warmup, 1), cores)
+    w = wl.config(args.config)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * r["seconds"] / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {args.config}: {w.nx}x{w.ny} spaxels x {w.nv} channels, "
+                               f"u={w.u}; each step = {rows_per_step} rows sampled from a K={w.K} batch",
+                   "rows_per_step": rows_per_step},
+        "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------- the GPU leg ----
+
+def measure_pipe_peaks(gbk, torch, sm_count: int) -> dict:
+    """Register-only MUFU.EX2 and FFMA loops on every SM (gbk_probe_pipe): the measured
+    denominators quoted beside the derived ones."""
+    sink = torch.zeros(4, dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    out = {}
+    for which, name, iters in ((0, "mufu", 4096), (1, "ffma", 32768)):
+        best = 0.0
+        for rep in range(4):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ops = gbk.gbk_probe_pipe(which, iters, sm_count * 8, 256, sink, st)
+            e1.record()
+            e1.synchronize()
+            if rep:
+                best = max(best, ops / (e0.elapsed_time(e1) * 1e-3))
+        out[name + "_gops_measured"] = best / 1e9
+    return out
+
+
+def run_ours(args, ranks) -> None:
+    import torch
+    from paper_1510_01815_b200 import dist, gbk
+    gbk.lib()                                   # raises if libgbk.so is missing: no fallback
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(ranks.local_rank)
+    cfg = args.config
+    w = wl.config(cfg)
+    rng = wl.rng_for(cfg, 100 + ranks.rank)     # every rank its own galaxy: weak scaling
+    true = true_row_for(cfg, w, rng)
+    obs = observation_from_gpu(gbk, torch, w, true, rng)
+    batches = batch_rows(cfg, w, true, rng, 4)
+    K = batches[0].shape[0]
+    prob = gbk.Problem(**desc_for(w, obs))
+    info = prob.info
+    dev_batches = [torch.from_numpy(b).cuda() for b in batches]
+    chi2 = torch.empty(K, dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB of L2
+    stream = torch.cuda.current_stream()
+    st = stream.cuda_stream
+    launches_per_step = 1 if info.tiles_x * info.tiles_y == 1 else 2
+
+    def step(i):
+        gbk.gbk_eval_batch(prob.handle, dev_batches[i % len(dev_batches)], None, K, chi2, stream=st)
+
+    sampler = ClockSampler(ranks.local_rank)
+    sampler.start()
+    t_warm = time.perf_counter()
+    for i in range(max(args.warmup, 3)):
+        flush.zero_()
+        step(i)
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: CUDA events on the launching stream, L2 flushed between ----
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    dist.barrier(ranks)
+    torch.cuda.synchronize()
+    for i in range(args.steps):
+        flush.zero_()
+        ev[i][0].record(stream)
+        step(i)
+        ev[i][1].record(stream)
+    torch.cuda.synchronize()
+    dist.barrier(ranks)
+    t_end = time.perf_counter()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    sec_rank = sum(ms) * 1e-3
+    checksum = float(chi2[torch.isfinite(chi2)].sum().item())
+    value, sec_max = dist.aggregate_throughput(ranks, K * args.steps, sec_rank)
+
+    # ---- end to end through the host entry: pinned host params in, host chi^2 out ----------
+    host_batches = [torch.from_numpy(b).pin_memory() for b in batches]
+    host_chi2 = torch.empty(K, dtype=torch.float32).pin_memory()
+    for i in range(3):
+        gbk.gbk_eval_batch_host(prob.handle, host_batches[i % len(host_batches)], None, K, host_chi2, st)
+    dist.barrier(ranks)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        gbk.gbk_eval_batch_host(prob.handle, host_batches[i % len(host_batches)], None, K, host_chi2, st)
+    torch.cuda.synchronize()
+    e2e_rank = time.perf_counter() - t0
+    t_end = time.perf_counter()
+    e2e_value, _ = dist.aggregate_throughput(ranks, K * args.steps, e2e_rank)
+    clocks = sampler.stop(t_warm, t_end)
+    same = bool(np.array_equal(host_chi2.numpy(),
+                               _chi2_of(gbk, prob, dev_batches[(args.steps - 1) % len(dev_batches)], K, torch)))
+
+    # ---- roofline of the dominant kernel (the fused kernel: the only one at one tile) ------
+    nvx = info.nv + 2 * info.r_v
+    ext_samples = info.ext_voxels_per_eval // nvx
+    mufu_per_eval = info.ext_voxels_per_eval + 3 * ext_samples
+    fp32_per_eval = 5 * info.ext_voxels_per_eval + 45 * ext_samples \
+        + 3 * 2 * (2 * info.r_p_max + 1) * (info.u * info.nx) * (info.u * info.ny) + 12 * info.nx * info.ny
+    sm_max = (clocks.get("sm_max_mhz") or 1965.0)
+    peak_mufu = info.sm_count * MUFU_LANES_PER_SM_CLK * sm_max * 1e6 / 1e9           # Gop/s
+    achieved = mufu_per_eval * K * args.steps / sec_rank / 1e9
+    roofline = {"bound": "alu", "pipe": "MUFU (ex2/rsqrt), 16 lanes/clk/SM", "achieved": achieved,
+                "peak": peak_mufu, "unit": "Gop/s", "frac": achieved / peak_mufu, "traffic": None,
+                "peak_how": f"derived: {info.sm_count} SMs x 16 MUFU lanes x {sm_max:.0f} MHz (max SM clock)",
+                "ops_per_eval": int(mufu_per_eval), "fp32_instr_per_eval": int(fp32_per_eval),
+                "kernel_ms_avg": statistics.mean(ms), "kernel_ms_min": min(ms)}
+    if ranks.is_main:
+        pk = measure_pipe_peaks(gbk, torch, info.sm_count)
+        roofline.update(pk)
+        roofline["frac_of_measured"] = achieved / pk["mufu_gops_measured"]
+        if clocks.get("sm_mhz"):
+            roofline["frac_at_sampled_clock"] = achieved / (peak_mufu * clocks["sm_mhz"] / sm_max)
+
+    cpu = None
+    if ranks.is_main and ranks.world == 1 and not args.no_cpu_baseline:
+        cores = host_cores()
+        cpu = time_oracle(cfg, args.cpu_rows or 32 * cores, 1, 1, cores)
+        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    if ranks.is_main:
+        core_vox = w.nx * w.ny * w.nv * w.u * w.u
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ranks.world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * sec_max / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": f"config {cfg}: {w.nx}x{w.ny} spaxels x {w.nv} channels, u={w.u}, "
+                                   f"K={K} rows per launch (nested-grid levels 0-3 cycled), chi2 only",
+                       "rows_per_launch": K, "l2": "flushed between timed launches (256 MiB memset)",
+                       "tile": [info.tile_w, info.tile_h], "block_threads": info.block_threads,
+                       "smem_bytes": info.smem_bytes, "blocks_per_sm": info.blocks_per_sm,
+                       "ext_voxels_per_eval": int(info.ext_voxels_per_eval),
+                       "parallelism": f"rows sharded, {ranks.world} rank(s), no collective"},
+            "voxels_per_s": value * core_vox, "ext_voxels_per_s": value * info.ext_voxels_per_eval,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": K * wl.P * 4,
+                    "d2h_bytes_per_step": K * 4, "matches_device_path": same},
+            "gpu_launches": launches_per_step * args.steps,
+            "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "checksum": checksum,
+        }
+        print(json.dumps(line), flush=True)
+    prob.close()
+
+
+def _chi2_of(gbk, prob, params, K, torch):
+    out = torch.empty(K, dtype=torch.float32, device="cuda")
+    gbk.gbk_eval_batch(prob.handle, params, None, K, out, stream=torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number (metric: 3)")
+    ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the cpu_baseline sample")
+    ap.add_argument("--ref-rows", type=int, default=0, help="rows per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_1510_01815_b200 import dist
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        if rank == 0:
+            run_reference(args, dist.Ranks())
+        return
+    ranks = dist.init_from_env("nccl")
+    try:
+        run_ours(args, ranks)
+    finally:
+        dist.finalize(ranks)
+
+
+if __name__ == "__main__":
+    main()

@@ -230,7 +230,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     dp.tiles_x = (d->nx + tws - 1) / tws, dp.tiles_y = (d->ny + ths - 1) / ths;
     dp.ntiles = dp.tiles_x * dp.tiles_y;
     dp.ews = round_up4(dp.tile_w) + 4 * ((2 * r_p_max + 4 + 3) / 4) - 4;
-    dp.ehs = dp.tile_h + 2 * r_p_max;
+    dp.ehs = (dp.tile_h + kVBlock - 1) / kVBlock * kVBlock + 2 * r_p_max;  // the vertical pass reads whole blocks
     return fused_smem_bytes(dp);
   };
   int tws = d->tile_w > 0 ? std::min(d->tile_w, d->nx) : d->nx;

@@ -20,6 +20,12 @@
 // (LSF taps L and band edges folded in exactly; built in gbk_api.cu).  Only three 2-D maps per
 // tile are convolved.  m1 = S1/S0, m2 = sqrt(S2/S0 - m1^2).  Velocities are measured from
 // v_center so the FP32 cancellation in m2 stays ~1e-4 km/s.
+//
+// Instruction economy: the kernel is bound by the MUFU pipe (one ex2 per
+// extended voxel, 16 lanes/clk/SM) only if everything else fits in the issue slots left over, so
+// all FP32 arithmetic is written for Blackwell's packed FFMA2/FMUL2 (two FP32 lanes per issued
+// instruction): pixels are processed in horizontally adjacent pairs in the voxel loop, and the
+// separable PSF passes update output pairs with tap pairs (t[k], t[k-1]) times a broadcast input.
 #include <math.h>
 
 #include "gbk_internal.h"
@@ -30,7 +36,29 @@ namespace {
 
 constexpr int kMaxThreads = 384;
 constexpr int kMinBlocks = 2;
+constexpr int kPairs = 2;        // pixel pairs per lane in the voxel loop (4 pixels per thread)
 
+typedef unsigned long long u64;  // two packed floats {lo, hi}
+
+__device__ __forceinline__ u64 pk(float lo, float hi) {
+  u64 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ u64 pk1(float v) { return pk(v, v); }
+__device__ __forceinline__ void upk(u64 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
+  u64 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
+  u64 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -41,7 +69,15 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __host__ __device__ __forceinline__ int round_up4(int v) { return (v + 3) & ~3; }
+
+__device__ __forceinline__ float f_inf() { return __int_as_float(0x7f800000); }
+__device__ __forceinline__ float f_nan() { return __int_as_float(0x7fc00000); }
 
 struct Smem {
   float* maps;      // 3 x ehs x ews
@@ -83,18 +119,22 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->psf_set = dp.psf_per_gal ? gal : 0;
   rc->r_p = dp.psf_r[rc->psf_set];
   rc->valid = (ok && gal_ok) ? 1 : 0;
+  const float inv_ci = 1.0f / ci;
+  const float s = 1.0f / (sigma0 * 1.1774100225154747f);  // sqrt(2 ln 2): 2^-(s dv)^2 = exp(-dv^2/2sigma0^2)
+  const float vrot_scale = (dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134f : 1.0f) * v[5] * si;
   rc->xo = v[0];
   rc->yo = v[1];
   rc->sp = sp;
   rc->cp = cp;
-  rc->inv_ci = 1.0f / ci;
-  rc->vrot_scale = (dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134f : 1.0f) * v[5] * si;
+  rc->nsp = -sp;
+  rc->ncp_ci = -cp * inv_ci;
+  rc->nsp_ci = -sp * inv_ci;
   rc->inv_rt = 1.0f / rt;
+  rc->rt = rt;
   rc->nl2e_inv_r0 = -1.4426950408889634f / r0;
-  rc->vsys_rel = v[4] - dp.v_center;
-  rc->s = 1.0f / (sigma0 * 1.1774100225154747f);  // sqrt(2 ln 2)
-  rc->step = rc->s * dp.dv;
-  rc->d_first = rc->s * dp.vrel_first;
+  rc->step = s * dp.dv;
+  rc->k1 = -s * vrot_scale;                                  // d0 = k1 * f(r) * cos(theta) + k0
+  rc->k0 = s * dp.vrel_first - s * (v[4] - dp.v_center);
   const float line_amp = dp.dv / (sigma0 * 2.5066282746310002f) * dp.inv_u2;  // sqrt(2 pi)
   rc->amp = i0 * line_amp;
   rc->dark_s0 = 1e-30f / line_amp;
@@ -102,53 +142,63 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
 
 // ---------------------------------------------------------------------------- a7, a8, a9 ----
 // One spaxel: moments from the block sums, residuals, chi^2 contribution, optional outputs.
+// The packed observation has 1/E = 0 where masked and {0, 0} for a missing dispersion map, so
+// neither needs a branch.  OUT = false is the chi^2-only instantiation (no output predicates).
+template <bool OUT>
 __device__ __forceinline__ float spaxel_finish(const DevProblem& dp, const EvalArgs& a,
-                                               const RowConst& rc, long long k, int X, int Y,
-                                               float S0, float S1, float S2) {
-  const int npix = dp.nx * dp.ny;
-  const int pix = Y * dp.nx + X;
-  const float4 ob = __ldg(&dp.obs[(size_t)rc.gal * npix + pix]);
-  const float inv = 1.0f / S0;
+                                               const RowConst& rc, long long k, int pix,
+                                               const float4 ob, float S0, float S1, float S2) {
+  const float inv = rcp_approx(S0);
   float m1r = S1 * inv;
   const float var = fmaf(-m1r, m1r, S2 * inv);
-  float m2 = sqrtf(fmaxf(var, 0.0f));
-  if (var != var) m2 = var;                       // fmaxf drops NaN
+  float m2 = var > 1e-30f ? var * rsqrt_approx(var) : 0.0f;   // sqrt(max(var, 0)); no denormal * inf
+  if (var != var) m2 = var;                                     // keep a NaN visible
   const bool dark = !(S0 >= rc.dark_s0);
-  if (dark) m1r = m2 = __int_as_float(0x7fc00000);
-  const bool bad = dark || !isfinite(m1r) || !isfinite(m2);
   const bool unmasked = ob.y > 0.0f;
-  float t = 0.0f, s = 0.0f, contrib = 0.0f;
-  if (unmasked) {
-    if (bad) {
-      t = s = __int_as_float(0x7fc00000);
-      contrib = __int_as_float(0x7f800000);
-    } else {
-      t = (m1r - ob.x) * ob.y;
-      s = dp.has_disp ? (m2 - ob.z) * ob.w : 0.0f;
-      contrib = fmaf(t, t, s * s);
+  float t = (m1r - ob.x) * ob.y;
+  float s = (m2 - ob.z) * ob.w;
+  float contrib = fmaf(t, t, s * s);
+  const bool bad = dark || !(contrib < f_inf());                // NaN or Inf moments
+  contrib = unmasked ? (bad ? f_inf() : contrib) : 0.0f;
+  if (OUT) {
+    if (dark) m1r = m2 = f_nan();
+    if (!unmasked) t = s = 0.0f;
+    else if (bad) t = s = f_nan();
+    const size_t npix = (size_t)dp.nx * dp.ny;
+    const size_t o = (size_t)k * npix + pix;
+    if (a.m0) a.m0[o] = rc.amp * S0;
+    if (a.m1) a.m1[o] = m1r + dp.v_center;
+    if (a.m2) a.m2[o] = m2;
+    if (a.resid) {
+      a.resid[2 * (size_t)k * npix + pix] = t;
+      a.resid[(2 * (size_t)k + 1) * npix + pix] = s;
     }
-  }
-  const size_t o = (size_t)k * npix + pix;
-  if (a.m0) a.m0[o] = rc.amp * S0;
-  if (a.m1) a.m1[o] = m1r + dp.v_center;
-  if (a.m2) a.m2[o] = m2;
-  if (a.resid) {
-    a.resid[2 * (size_t)k * npix + pix] = t;
-    a.resid[(2 * (size_t)k + 1) * npix + pix] = s;
   }
   return contrib;
 }
 
+__device__ __forceinline__ float4 load_obs(const DevProblem& dp, const RowConst& rc, int pix) {
+  return __ldg(&dp.obs[(size_t)rc.gal * ((size_t)dp.nx * dp.ny) + pix]);
+}
+
 // ---------------------------------------------------------------------------------- a5 ------
-// Horizontal pass of the separable PSF, in place: a row is owned by one group of lanes, which
-// loads everything it needs before it stores (true convolution: out[x] = sum_k T[k] in[x+2R-k]).
+// Separable Gaussian PSF.  Taps are symmetric, so out[x] = sum_{j=0..2R} t[j] in[x + j].
+// An output PAIR (out[x], out[x+1]) receives from input in[x + i], i = 0..2R+1, the tap pair
+// tp[i] = (t[i], t[i-1]) (t[-1] = t[2R+1] = 0): one FFMA2 with a broadcast input per pair and
+// input, i.e. (R + 1) instructions per output instead of (2R + 1).
+template <int R>
+__device__ __forceinline__ void load_tap_pairs(const float* taps, u64 (&tp)[2 * R + 2]) {
+#pragma unroll
+  for (int i = 0; i < 2 * R + 2; ++i)
+    tp[i] = pk(i <= 2 * R ? taps[i] : 0.0f, i >= 1 ? taps[i - 1] : 0.0f);
+}
+
+// Horizontal pass, in place: a row is owned by one group of lanes of one warp, which loads
+// everything it needs before it stores.  A lane produces 4 consecutive outputs.
 template <int R>
 __device__ __forceinline__ void hpass(float* maps, int map_stride, int ews, int EH, int tw,
-                                      const float* taps, int tid, int nthreads) {
-  constexpr int NT = 2 * R + 1, NV4 = (4 + 2 * R + 3) / 4;
-  float t[R + 1];   // Gaussian taps are symmetric: tap(k) = t[|k - R|]
-#pragma unroll
-  for (int j = 0; j <= R; ++j) t[j] = taps[R + j];
+                                      const u64 (&tp)[2 * R + 2], int tid, int nthreads) {
+  constexpr int NV4 = (4 + 2 * R + 3) / 4;
   const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
   const int nx4 = (tw + 3) >> 2;
   int lpr_log = 0;
@@ -159,8 +209,8 @@ __device__ __forceinline__ void hpass(float* maps, int map_stride, int ews, int 
   const int nchunks = (nx4 + lpr - 1) >> lpr_log;
   const int npass = (EH + rpp - 1) / rpp;
   for (int job = warp; job < 3 * npass; job += nwarps) {
-    const int q = job / npass, pass = job - q * npass;
-    const int row = pass * rpp + rsub;
+    const int q = job >= 2 * npass ? 2 : (job >= npass ? 1 : 0);
+    const int row = (job - q * npass) * rpp + rsub;
     float* rowp = maps + q * map_stride + row * ews;
     for (int chunk = 0; chunk < nchunks; ++chunk) {
       const int x0 = ((chunk << lpr_log) + l) << 2;
@@ -175,58 +225,70 @@ __device__ __forceinline__ void hpass(float* maps, int map_stride, int ews, int 
       }
       __syncwarp();
       if (active) {
-        float o[4] = {0.f, 0.f, 0.f, 0.f};
+        u64 o0 = pk(0.f, 0.f), o1 = o0;
 #pragma unroll
-        for (int kk = 0; kk < NT; ++kk)
-#pragma unroll
-          for (int i = 0; i < 4; ++i) o[i] = fmaf(t[kk < R ? R - kk : kk - R], v[i + 2 * R - kk], o[i]);
-        *reinterpret_cast<float4*>(rowp + x0) = make_float4(o[0], o[1], o[2], o[3]);
+        for (int i = 0; i < 2 * R + 2; ++i) {
+          o0 = fma2(pk1(v[i]), tp[i], o0);
+          o1 = fma2(pk1(v[i + 2]), tp[i], o1);
+        }
+        float4 f;
+        upk(o0, f.x, f.y);
+        upk(o1, f.z, f.w);
+        *reinterpret_cast<float4*>(rowp + x0) = f;
       }
       __syncwarp();
     }
   }
 }
 
+// Vertical pass of kVBlock output rows of one column of one map into registers.
+template <int R>
+__device__ __forceinline__ void vcolumn(const float* col, int ews, const u64 (&tp)[2 * R + 2],
+                                        float (&res)[kVBlock]) {
+  constexpr int BY = kVBlock;
+  u64 acc[BY / 2];
+#pragma unroll
+  for (int m = 0; m < BY / 2; ++m) acc[m] = pk(0.f, 0.f);
+#pragma unroll
+  for (int i = 0; i < BY + 2 * R; ++i) {
+    const u64 v = pk1(col[i * ews]);
+#pragma unroll
+    for (int m = 0; m < BY / 2; ++m) {
+      const int ti = i - 2 * m;
+      if (ti >= 0 && ti < 2 * R + 2) acc[m] = fma2(v, tp[ti], acc[m]);
+    }
+  }
+#pragma unroll
+  for (int m = 0; m < BY / 2; ++m) upk(acc[m], res[2 * m], res[2 * m + 1]);
+}
+
 // Vertical pass fused with moments and chi^2 (u == 1): a thread owns kVBlock consecutive rows of
 // one column; lanes run along x, so shared-memory reads are conflict-free and global accesses
-// coalesced.
-template <int R>
+// coalesced.  Rows past the tile are read from the (allocated, possibly uninitialised) padding of
+// the plane and only feed outputs that are discarded.
+template <int R, bool OUT>
 __device__ __forceinline__ float vpass_moments(const DevProblem& dp, const EvalArgs& a,
                                                const RowConst& rc, long long k, const float* maps,
-                                               int map_stride, int ews, int EH, int tw, int th,
-                                               int tx0, int ty0, const float* taps, int tid,
+                                               int map_stride, int ews, int tw, int th, int tx0,
+                                               int ty0, const u64 (&tp)[2 * R + 2], int tid,
                                                int nthreads) {
-  constexpr int NT = 2 * R + 1, BY = kVBlock;
-  float t[R + 1];
-#pragma unroll
-  for (int j = 0; j <= R; ++j) t[j] = taps[R + j];
+  constexpr int BY = kVBlock;
   const int nyb = (th + BY - 1) / BY;
+  const unsigned magic = 0xFFFFFFFFu / (unsigned)tw + 1u;
   float chi = 0.0f;
   for (int item = tid; item < tw * nyb; item += nthreads) {
-    const int yb = item / tw, x = item - yb * tw, y0 = yb * BY;
+    const int yb = (int)__umulhi((unsigned)item, magic), x = item - yb * tw, y0 = yb * BY;
     float res[3][BY];
 #pragma unroll
-    for (int q = 0; q < 3; ++q) {
-      const float* col = maps + q * map_stride + y0 * ews + x;
-      float acc[BY];
-#pragma unroll
-      for (int o = 0; o < BY; ++o) acc[o] = 0.0f;
-#pragma unroll
-      for (int i = 0; i < BY + 2 * R; ++i) {
-        const float v = (y0 + i < EH) ? col[i * ews] : 0.0f;
-#pragma unroll
-        for (int o = 0; o < BY; ++o) {
-          const int kk = 2 * R - (i - o);
-          if (kk >= 0 && kk < NT) acc[o] = fmaf(t[kk < R ? R - kk : kk - R], v, acc[o]);
-        }
-      }
-#pragma unroll
-      for (int o = 0; o < BY; ++o) res[q][o] = acc[o];
-    }
+    for (int q = 0; q < 3; ++q) vcolumn<R>(maps + q * map_stride + y0 * ews + x, ews, tp, res[q]);
+    const int pix0 = (ty0 + y0) * dp.nx + tx0 + x;
 #pragma unroll
     for (int o = 0; o < BY; ++o)
-      if (y0 + o < th)
-        chi += spaxel_finish(dp, a, rc, k, tx0 + x, ty0 + y0 + o, res[0][o], res[1][o], res[2][o]);
+      if (y0 + o < th) {
+        const int pix = pix0 + o * dp.nx;
+        chi += spaxel_finish<OUT>(dp, a, rc, k, pix, load_obs(dp, rc, pix), res[0][o], res[1][o],
+                                  res[2][o]);
+      }
   }
   return chi;
 }
@@ -234,36 +296,24 @@ __device__ __forceinline__ float vpass_moments(const DevProblem& dp, const EvalA
 // Vertical pass in place (u > 1): a thread owns one column of one map and walks it top to bottom
 // in chunks, so the rows it overwrites are never read again.
 template <int R>
-__device__ __forceinline__ void vpass_inplace(float* maps, int map_stride, int ews, int EH, int tw,
-                                              int th, const float* taps, int tid, int nthreads) {
-  constexpr int NT = 2 * R + 1, BY = kVBlock;
-  float t[R + 1];
-#pragma unroll
-  for (int j = 0; j <= R; ++j) t[j] = taps[R + j];
+__device__ __forceinline__ void vpass_inplace(float* maps, int map_stride, int ews, int tw, int th,
+                                              const u64 (&tp)[2 * R + 2], int tid, int nthreads) {
+  constexpr int BY = kVBlock;
   for (int item = tid; item < 3 * tw; item += nthreads) {
-    const int q = item / tw, x = item - q * tw;
+    const int q = item >= 2 * tw ? 2 : (item >= tw ? 1 : 0), x = item - q * tw;
     float* col = maps + q * map_stride + x;
     for (int y0 = 0; y0 < th; y0 += BY) {
-      float acc[BY];
-#pragma unroll
-      for (int o = 0; o < BY; ++o) acc[o] = 0.0f;
-#pragma unroll
-      for (int i = 0; i < BY + 2 * R; ++i) {
-        const float v = (y0 + i < EH) ? col[(y0 + i) * ews] : 0.0f;
-#pragma unroll
-        for (int o = 0; o < BY; ++o) {
-          const int kk = 2 * R - (i - o);
-          if (kk >= 0 && kk < NT) acc[o] = fmaf(t[kk < R ? R - kk : kk - R], v, acc[o]);
-        }
-      }
+      float res[BY];
+      vcolumn<R>(col + y0 * ews, ews, tp, res);
 #pragma unroll
       for (int o = 0; o < BY; ++o)
-        if (y0 + o < th) col[(y0 + o) * ews] = acc[o];
+        if (y0 + o < th) col[(y0 + o) * ews] = res[o];
     }
   }
 }
 
 // a6 + a7/a8 for u > 1 after both in-place passes: block sums over u x u fine pixels.
+template <bool OUT>
 __device__ __forceinline__ float moments_blocks(const DevProblem& dp, const EvalArgs& a,
                                                 const RowConst& rc, long long k, const float* maps,
                                                 int map_stride, int ews, int tw, int th, int tx0,
@@ -272,25 +322,30 @@ __device__ __forceinline__ float moments_blocks(const DevProblem& dp, const Eval
   float chi = 0.0f;
   for (int item = tid; item < sw * sh; item += nthreads) {
     const int Y = item / sw, X = item - Y * sw;
+    const int pix = (ty0 / u + Y) * dp.nx + tx0 / u + X;
+    const float4 ob = load_obs(dp, rc, pix);
     float s[3] = {0.f, 0.f, 0.f};
     for (int q = 0; q < 3; ++q)
       for (int dy = 0; dy < u; ++dy)
         for (int dx = 0; dx < u; ++dx) s[q] += maps[q * map_stride + (Y * u + dy) * ews + X * u + dx];
-    chi += spaxel_finish(dp, a, rc, k, tx0 / u + X, ty0 / u + Y, s[0], s[1], s[2]);
+    chi += spaxel_finish<OUT>(dp, a, rc, k, pix, ob, s[0], s[1], s[2]);
   }
   return chi;
 }
 
 // General 2-D PSF image (any u): direct sum per spaxel from shared memory.  The image is stored
 // flipped at create, so this correlation is the true convolution.
+template <bool OUT>
 __device__ __noinline__ float conv2d_moments(const DevProblem& dp, const EvalArgs& a,
-                                                const RowConst& rc, long long k, const float* maps,
-                                                int map_stride, int ews, int tw, int th, int tx0,
-                                                int ty0, const float* taps, int tid, int nthreads) {
+                                             const RowConst& rc, long long k, const float* maps,
+                                             int map_stride, int ews, int tw, int th, int tx0,
+                                             int ty0, const float* taps, int tid, int nthreads) {
   const int u = dp.u, sw = tw / u, sh = th / u, n = 2 * rc.r_p + 1;
   float chi = 0.0f;
   for (int item = tid; item < sw * sh; item += nthreads) {
     const int Y = item / sw, X = item - Y * sw;
+    const int pix = (ty0 / u + Y) * dp.nx + tx0 / u + X;
+    const float4 ob = load_obs(dp, rc, pix);
     float s0 = 0.f, s1 = 0.f, s2 = 0.f;
     for (int dy = 0; dy < u; ++dy)
       for (int dx = 0; dx < u; ++dx) {
@@ -304,28 +359,142 @@ __device__ __noinline__ float conv2d_moments(const DevProblem& dp, const EvalArg
             s2 = fmaf(w, pp[2 * map_stride], s2);
           }
       }
-    chi += spaxel_finish(dp, a, rc, k, tx0 / u + X, ty0 / u + Y, s0, s1, s2);
+    chi += spaxel_finish<OUT>(dp, a, rc, k, pix, ob, s0, s1, s2);
   }
   return chi;
 }
 
-template <int R>
+template <int R, bool OUT>
 __device__ __noinline__ float separable_phase(const DevProblem& dp, const EvalArgs& a,
-                                                 const RowConst& rc, long long k, float* maps,
-                                                 int map_stride, int EH, int tw, int th, int tx0,
-                                                 int ty0, const float* taps, int tid, int nthreads) {
-  hpass<R>(maps, map_stride, dp.ews, EH, tw, taps, tid, nthreads);
+                                              const RowConst& rc, long long k, float* maps,
+                                              int map_stride, int EH, int tw, int th, int tx0,
+                                              int ty0, const float* taps, int tid, int nthreads) {
+  u64 tp[2 * R + 2];
+  load_tap_pairs<R>(taps, tp);
+  hpass<R>(maps, map_stride, dp.ews, EH, tw, tp, tid, nthreads);
   __syncthreads();
   if (dp.u == 1)
-    return vpass_moments<R>(dp, a, rc, k, maps, map_stride, dp.ews, EH, tw, th, tx0, ty0, taps, tid,
-                            nthreads);
-  vpass_inplace<R>(maps, map_stride, dp.ews, EH, tw, th, taps, tid, nthreads);
+    return vpass_moments<R, OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0, tp, tid,
+                                 nthreads);
+  vpass_inplace<R>(maps, map_stride, dp.ews, tw, th, tp, tid, nthreads);
   __syncthreads();
-  return moments_blocks(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0, tid, nthreads);
+  return moments_blocks<OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0, tid, nthreads);
+}
+
+// ------------------------------------------------------------------------ a2, a3, a4 --------
+// atan(z) for z in [0, 1] as z * P(z^2) (8 terms, max error 1.4e-7 rad evaluated in FP32;
+// DESIGN.md "Precision"), packed for a pixel pair.
+__device__ __forceinline__ u64 atan01_2(u64 z) {
+  const u64 t = mul2(z, z);
+  u64 p = pk1(-0.00405439967289567f);
+  p = fma2(p, t, pk1(0.02186231128871441f));
+  p = fma2(p, t, pk1(-0.05591132491827011f));
+  p = fma2(p, t, pk1(0.09642117470502853f));
+  p = fma2(p, t, pk1(-0.13908594846725464f));
+  p = fma2(p, t, pk1(0.1994655877351761f));
+  p = fma2(p, t, pk1(-0.33329859375953674f));
+  p = fma2(p, t, pk1(0.9999993443489075f));
+  return mul2(p, z);
+}
+
+// Geometry of one horizontally adjacent pixel pair (dx = x - x_o of both, dy = y - y_o shared):
+// returns the line-centre offsets d0 (in units of 1/s, from extended channel 0) and writes the
+// brightness I/I0 of both.
+__device__ __forceinline__ u64 pair_geometry(const DevProblem& dp, const RowConst& rc, u64 dx,
+                                             float dy, u64& brightness) {
+  const u64 xe = fma2(pk1(rc.nsp), dx, pk1(dy * rc.cp));            // eq. 1
+  const u64 yd = fma2(pk1(rc.ncp_ci), dx, pk1(dy * rc.nsp_ci));     // eq. 2 / cos i
+  const u64 r2 = fma2(xe, xe, mul2(yd, yd));                         // eq. 3
+  float r2a, r2b;
+  upk(r2, r2a, r2b);
+  // r < 1e-15 px is r = 0: cos(theta) := 0 and V_rot(0) = 0 (A8)
+  const u64 rs = pk(r2a > 1e-30f ? rsqrt_approx(r2a) : 0.0f, r2b > 1e-30f ? rsqrt_approx(r2b) : 0.0f);
+  const u64 r = mul2(r2, rs);
+  const u64 cos_t = mul2(xe, rs);                                    // eq. 4
+  float ea, eb;
+  upk(mul2(r, pk1(rc.nl2e_inv_r0)), ea, eb);
+  brightness = pk(ex2_approx(ea), ex2_approx(eb));                   // eq. 5 / I0
+  const u64 q = mul2(r, pk1(rc.inv_rt));
+  u64 f;
+  if (dp.rc_model == GBK_RC_ARCTAN) {                                // eq. 6 without (2/pi) V_t
+    float qa, qb, ia, ib;
+    upk(q, qa, qb);
+    upk(mul2(rs, pk1(rc.rt)), ia, ib);                               // 1/q = r_t / r
+    const bool biga = qa > 1.0f, bigb = qb > 1.0f;
+    const u64 at = atan01_2(pk(biga ? ia : qa, bigb ? ib : qb));
+    // atan(q) = pi/2 - atan(1/q) for q > 1
+    f = fma2(at, pk(biga ? -1.0f : 1.0f, bigb ? -1.0f : 1.0f),
+             pk(biga ? 1.5707963267948966f : 0.0f, bigb ? 1.5707963267948966f : 0.0f));
+  } else {                                                           // ramp: min(r/r_t, 1)
+    float qa, qb;
+    upk(q, qa, qb);
+    f = pk(fminf(qa, 1.0f), fminf(qb, 1.0f));
+  }
+  return fma2(mul2(f, pk1(rc.k1)), cos_t, pk1(rc.k0));               // eq. 8 -> line centre
+}
+
+// The voxel loop: a warp takes items of 32 lanes x kPairs pixel pairs, evaluates the Gaussian line
+// of each pixel at every extended channel and accumulates the three LSF-folded weighted sums.
+__device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst& rc, const Smem& sm,
+                                            int tx0, int ty0, int EW, int EH, int R, int tid,
+                                            int nthreads) {
+  const int ppr = (EW + 1) >> 1;                  // pixel pairs per extended row
+  const int npairs = ppr * EH;
+  const unsigned magic = 0xFFFFFFFFu / (unsigned)ppr + 1u;   // exact quotient for these sizes
+  const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+  constexpr int kPerItem = 32 * kPairs;
+  const int nitems = (npairs + kPerItem - 1) / kPerItem;
+  const int map_stride = dp.ehs * dp.ews;
+  const float inv_u = dp.inv_u;
+  const int nvx = dp.nvx;
+  const u64 st2 = pk1(rc.step);
+  for (int item = warp; item < nitems; item += nwarps) {
+    u64 d0[kPairs], In[kPairs];
+    int sidx[kPairs];
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) {
+      const int pi = item * kPerItem + j * 32 + lane;
+      const int pic = min(pi, npairs - 1);
+      const int ey = (int)__umulhi((unsigned)pic, magic), ex = (pic - ey * ppr) << 1;
+      sidx[j] = pi < npairs ? ey * dp.ews + ex : -1;
+      const float gx = (float)(tx0 + ex - R), gy = (float)(ty0 + ey - R);
+      const float xa = (gx + 0.5f) * inv_u - 0.5f, xb = (gx + 1.5f) * inv_u - 0.5f;
+      const float y = (gy + 0.5f) * inv_u - 0.5f;
+      d0[j] = pair_geometry(dp, rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo, In[j]);
+    }
+    u64 s0[kPairs], s1[kPairs], s2[kPairs];
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) s0[j] = s1[j] = s2[j] = pk(0.f, 0.f);
+#pragma unroll 4
+    for (int c = 0; c < nvx; ++c) {
+      const float4 w = sm.chan[c];
+#pragma unroll
+      for (int j = 0; j < kPairs; ++j) {
+        const u64 d = fma2(pk1(w.x), st2, d0[j]);
+        float ea, eb;
+        upk(mul2(d, d), ea, eb);
+        const u64 g = pk(ex2_approx(-ea), ex2_approx(-eb));          // Gaussian line
+        s0[j] = fma2(pk1(w.y), g, s0[j]);
+        s1[j] = fma2(pk1(w.z), g, s1[j]);
+        s2[j] = fma2(pk1(w.w), g, s2[j]);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j)
+      if (sidx[j] >= 0) {
+        float2 v;
+        upk(mul2(s0[j], In[j]), v.x, v.y);
+        *reinterpret_cast<float2*>(sm.maps + sidx[j]) = v;
+        upk(mul2(s1[j], In[j]), v.x, v.y);
+        *reinterpret_cast<float2*>(sm.maps + map_stride + sidx[j]) = v;
+        upk(mul2(s2[j], In[j]), v.x, v.y);
+        *reinterpret_cast<float2*>(sm.maps + 2 * map_stride + sidx[j]) = v;
+      }
+  }
 }
 
 // ------------------------------------------------------------------------------ the kernel ---
-template <int P>
+template <bool OUT>
 __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     fused_kernel(const __grid_constant__ DevProblem dp, const __grid_constant__ EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -349,89 +518,32 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   float chi = 0.0f;
   if (!rc.valid) {
     // out-of-domain row: chi^2 = +INF, NaN maps and residuals for this tile's spaxels
-    const int u = dp.u, sw = tw / u, sh = th / u, npix = dp.nx * dp.ny;
-    const float qnan = __int_as_float(0x7fc00000);
-    for (int item = tid; item < sw * sh; item += nthreads) {
-      const int Y = item / sw, X = item - Y * sw;
-      const size_t pix = (size_t)(ty0 / u + Y) * dp.nx + tx0 / u + X;
-      if (a.m0) a.m0[k * npix + pix] = qnan;
-      if (a.m1) a.m1[k * npix + pix] = qnan;
-      if (a.m2) a.m2[k * npix + pix] = qnan;
-      if (a.resid) a.resid[2 * k * npix + pix] = a.resid[(2 * k + 1) * npix + pix] = qnan;
+    if (OUT) {
+      const int u = dp.u, sw = tw / u, sh = th / u, npix = dp.nx * dp.ny;
+      for (int item = tid; item < sw * sh; item += nthreads) {
+        const int Y = item / sw, X = item - Y * sw;
+        const size_t pix = (size_t)(ty0 / u + Y) * dp.nx + tx0 / u + X;
+        if (a.m0) a.m0[k * npix + pix] = f_nan();
+        if (a.m1) a.m1[k * npix + pix] = f_nan();
+        if (a.m2) a.m2[k * npix + pix] = f_nan();
+        if (a.resid) a.resid[2 * k * npix + pix] = a.resid[(2 * k + 1) * npix + pix] = f_nan();
+      }
     }
-    chi = __int_as_float(0x7f800000);
+    chi = f_inf();
   } else {
-    // ------------------------------------------------------------------ a2, a3, a4 -------
     const int R = rc.r_p;
-    const int EW = tw + 2 * R, EH = th + 2 * R, n_ext = EW * EH;
-    const float step = rc.step, inv_u = dp.inv_u;
-    const int nvx = dp.nvx;
-    for (int base = 0; base < n_ext; base += nthreads * P) {
-      float d0[P], In[P];
-      int sidx[P];
-#pragma unroll
-      for (int p = 0; p < P; ++p) {
-        const int idx = base + p * nthreads + tid;
-        const int idc = min(idx, n_ext - 1);
-        const int ey = idc / EW, ex = idc - ey * EW;
-        sidx[p] = idx < n_ext ? ey * dp.ews + ex : -1;
-        const float x = ((float)(tx0 + ex - R) + 0.5f) * inv_u - 0.5f;
-        const float y = ((float)(ty0 + ey - R) + 0.5f) * inv_u - 0.5f;
-        const float dx = x - rc.xo, dy = y - rc.yo;
-        const float xe = fmaf(dy, rc.cp, -dx * rc.sp);            // eq. 1
-        const float ye = -fmaf(dx, rc.cp, dy * rc.sp);            // eq. 2
-        const float yd = ye * rc.inv_ci;
-        const float r2 = fmaf(xe, xe, yd * yd);                   // eq. 3
-        const float rs = r2 > 0.0f ? rsqrt_approx(r2) : 0.0f;
-        const float r = r2 * rs;
-        const float cos_t = xe * rs;                              // eq. 4 (0 at r = 0)
-        In[p] = ex2_approx(r * rc.nl2e_inv_r0);                   // eq. 5 / I0
-        const float q = r * rc.inv_rt;
-        const float vrot = rc.vrot_scale * (dp.rc_model == GBK_RC_ARCTAN ? atanf(q) : fminf(q, 1.0f));
-        const float vlos_rel = fmaf(vrot, cos_t, rc.vsys_rel);    // eq. 8 (minus v_center)
-        d0[p] = fmaf(-rc.s, vlos_rel, rc.d_first);
-      }
-      float s0[P], s1[P], s2[P];
-#pragma unroll
-      for (int p = 0; p < P; ++p) s0[p] = s1[p] = s2[p] = 0.0f;
-#pragma unroll 4
-      for (int c = 0; c < nvx; ++c) {
-        const float4 w = sm.chan[c];
-#pragma unroll
-        for (int p = 0; p < P; ++p) {
-          const float d = fmaf(w.x, step, d0[p]);
-          const float g = ex2_approx(-d * d);                     // Gaussian line
-          s0[p] = fmaf(w.y, g, s0[p]);
-          s1[p] = fmaf(w.z, g, s1[p]);
-          s2[p] = fmaf(w.w, g, s2[p]);
-        }
-      }
-#pragma unroll
-      for (int p = 0; p < P; ++p)
-        if (sidx[p] >= 0) {
-          sm.maps[sidx[p]] = s0[p] * In[p];
-          sm.maps[map_stride + sidx[p]] = s1[p] * In[p];
-          sm.maps[2 * map_stride + sidx[p]] = s2[p] * In[p];
-        }
-    }
-    // zero the pad columns the vectorised horizontal pass may read
-    const int padw = dp.ews - EW;
-    for (int i = tid; i < 3 * EH * padw; i += nthreads) {
-      const int q = i / (EH * padw), rem = i - q * (EH * padw);
-      const int row = rem / padw, col = EW + rem - row * padw;
-      sm.maps[q * map_stride + row * dp.ews + col] = 0.0f;
-    }
+    const int EW = tw + 2 * R, EH = th + 2 * R;
+    voxel_phase(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads);
     __syncthreads();
-
     // ------------------------------------------------------------------ a5 .. a9 ---------
     if (dp.psf_kind == GBK_PSF_IMAGE) {
-      chi = conv2d_moments(dp, a, rc, k, sm.maps, map_stride, dp.ews, tw, th, tx0, ty0, sm.taps, tid,
-                           nthreads);
+      chi = conv2d_moments<OUT>(dp, a, rc, k, sm.maps, map_stride, dp.ews, tw, th, tx0, ty0, sm.taps,
+                                tid, nthreads);
     } else {
-#define GBK_SEP_CASE(RR)                                                                        \
-  case RR:                                                                                      \
-    chi = separable_phase<RR>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0, sm.taps, \
-                              tid, nthreads);                                                   \
+#define GBK_SEP_CASE(RR)                                                                          \
+  case RR:                                                                                        \
+    chi = separable_phase<RR, OUT>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0,       \
+                                   sm.taps, tid, nthreads);                                       \
     break;
       switch (R) {
         GBK_SEP_CASE(0) GBK_SEP_CASE(1) GBK_SEP_CASE(2) GBK_SEP_CASE(3) GBK_SEP_CASE(4)
@@ -447,13 +559,12 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   // ------------------------------------------------ block reduction, fixed order ----------
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) chi += __shfl_down_sync(0xffffffffu, chi, off);
-  __syncthreads();  // all reads of the maps are done; red[] does not alias them, but keep order
   if ((tid & 31) == 0) sm.red[tid >> 5] = chi;
   __syncthreads();
   if (tid == 0) {
     float tot = 0.0f;
     for (int w = 0; w < (nthreads >> 5); ++w) tot += sm.red[w];
-    if (!(tot < __int_as_float(0x7f800000))) tot = __int_as_float(0x7f800000);
+    if (!(tot < f_inf())) tot = f_inf();
     if (dp.ntiles == 1)
       a.chi2[k] = tot;
     else
@@ -471,26 +582,6 @@ __global__ void finish_kernel(const float* __restrict__ partial, int ntiles, lon
   chi2[k] = tot;
 }
 
-template <int P>
-cudaError_t launch_p(const DevProblem& dp, const EvalArgs& a, const FusedLaunch& fl,
-                     cudaStream_t st) {
-  const long long nblocks = a.K * dp.ntiles;
-  fused_kernel<P><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
-  return cudaGetLastError();
-}
-
-template <int P>
-cudaError_t prepare_p(const FusedLaunch& fl) {
-  return cudaFuncSetAttribute(fused_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              fl.smem_bytes);
-}
-
-template <int P>
-cudaError_t occupancy_p(const FusedLaunch& fl, int* n) {
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(n, fused_kernel<P>, fl.threads,
-                                                       fl.smem_bytes);
-}
-
 }  // namespace
 
 size_t fused_smem_bytes(const DevProblem& dp) {
@@ -499,16 +590,26 @@ size_t fused_smem_bytes(const DevProblem& dp) {
 }
 
 cudaError_t fused_prepare(const FusedLaunch& fl) {
-  return prepare_p<4>(fl);
+  cudaError_t e = cudaFuncSetAttribute(fused_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       fl.smem_bytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(fused_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              fl.smem_bytes);
 }
 
 cudaError_t fused_occupancy(const FusedLaunch& fl, int* n) {
-  return occupancy_p<4>(fl, n);
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(n, fused_kernel<false>, fl.threads,
+                                                       fl.smem_bytes);
 }
 
 cudaError_t launch_fused(const DevProblem& dp, const EvalArgs& a, const FusedLaunch& fl,
                          cudaStream_t st) {
-  cudaError_t e = launch_p<4>(dp, a, fl, st);
+  const long long nblocks = a.K * dp.ntiles;
+  if (a.m0 || a.m1 || a.m2 || a.resid)
+    fused_kernel<true><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
+  else
+    fused_kernel<false><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
+  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (dp.ntiles > 1) {
     const int th = 128;

@@ -46,14 +46,16 @@ struct EvalArgs {
 
 // Per-row constants (a1 of SURVEY.md section 8(a)), computed once per block.
 struct RowConst {
-  float xo, yo, sp, cp, inv_ci;
-  float vrot_scale;   // arctan: (2/pi) V_t sin i;  ramp: V_t sin i
-  float inv_rt;
+  float xo, yo, sp, cp;
+  float nsp;          // -sin(PA):            x_e = nsp * dx + cp * dy             (eq. 1)
+  float ncp_ci;       // -cos(PA) / cos(i):   y_e / cos i = ncp_ci * dx + nsp_ci * dy   (eq. 2-3)
+  float nsp_ci;       // -sin(PA) / cos(i)
+  float inv_rt, rt;
   float nl2e_inv_r0;  // -log2(e)/r0
-  float vsys_rel;     // V_sys - v_center
-  float s;            // 1/(sigma0 sqrt(2 ln 2)):  exp(-dv^2/(2 sigma0^2)) = 2^-(s dv)^2
-  float step;         // s * dv
-  float d_first;      // s * vrel_first
+  float step;         // s * dv with s = 1/(sigma0 sqrt(2 ln 2)): exp(-dv^2/(2 sigma0^2)) = 2^-(s dv)^2
+  float k1;           // -s * V_t sin i (* 2/pi for the arctan curve)
+  float k0;           // s * (velocity of extended channel 0 - V_sys): the line-centre offset of a
+                      // sample from extended channel 0 is  d0 = k1 * f(r/r_t) * cos(theta) + k0
   float amp;          // I0 * dv / (sigma0 sqrt(2 pi) u^2): scales the S0 block sum to m0
   float dark_s0;      // S0 block sums below this are model-dark (m0 < 1e-30 I0)
   int valid;
