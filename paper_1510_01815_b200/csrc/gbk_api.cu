@@ -70,7 +70,8 @@ struct gbk_problem {
   long long st_cap = 0;
   // scratch of the unfused path
   float* uf_scratch = nullptr;
-  size_t uf_bytes = 0;
+  long long uf_rows = 0;        // rows the scratch holds
+  float* lsf_taps = nullptr;    // [2 r_v + 1], unfused path only
 };
 
 extern "C" const char* gbk_last_error(void) { return g_err; }
@@ -86,6 +87,7 @@ extern "C" int gbk_destroy(gbk_problem* p) {
   cudaFree(p->st_gal);
   cudaFree(p->st_chi2);
   cudaFree(p->uf_scratch);
+  cudaFree(p->lsf_taps);
   delete p;
   return GBK_OK;
 }
@@ -279,6 +281,11 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   GBK_CUDA_P(cudaMalloc(&p->psf_taps, sizeof(float) * psf_taps.size()));
   GBK_CUDA_P(cudaMalloc(&p->psf_r, sizeof(int) * n_psf));
   GBK_CUDA_P(cudaMalloc(&p->obs, sizeof(float4) * obs.size()));
+  {
+    std::vector<float> lsf_f(lsf.begin(), lsf.end());
+    GBK_CUDA_P(cudaMalloc(&p->lsf_taps, sizeof(float) * lsf_f.size()));
+    GBK_CUDA_P(cudaMemcpy(p->lsf_taps, lsf_f.data(), sizeof(float) * lsf_f.size(), cudaMemcpyHostToDevice));
+  }
   GBK_CUDA_P(cudaMemcpy(p->chan_tab, chan.data(), sizeof(float4) * nvx, cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->psf_taps, psf_taps.data(), sizeof(float) * psf_taps.size(), cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->psf_r, psf_r.data(), sizeof(int) * n_psf, cudaMemcpyHostToDevice));
@@ -364,10 +371,24 @@ extern "C" int gbk_eval_batch_host(gbk_problem* p, const float* params, const in
 extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const int32_t* gal_index,
                                       int64_t K, float* chi2, float* m0, float* m1, float* m2,
                                       float* resid, void* cuda_stream) {
-  (void)gal_index, (void)m0, (void)m1, (void)m2, (void)resid, (void)cuda_stream;
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
-  return fail(GBK_ERR_UNSUPPORTED, "unfused comparison path not built yet");
+  if (K == 0) return GBK_OK;
+  GBK_CUDA(cudaSetDevice(p->device));
+  // scratch: two cubes + one contribution map per row, for a chunk of rows (<= 2 GiB, grown lazily)
+  const size_t per_row = unfused_bytes_per_row(p->dp);
+  const long long cap_rows = std::max<long long>(1, (long long)((size_t(2) << 30) / per_row));
+  const long long want = std::min<long long>(K, cap_rows);
+  if (want > p->uf_rows) {
+    if (p->uf_scratch) GBK_CUDA(cudaFree(p->uf_scratch));
+    p->uf_scratch = nullptr, p->uf_rows = 0;
+    GBK_CUDA(cudaMalloc(&p->uf_scratch, per_row * (size_t)want));
+    p->uf_rows = want;
+  }
+  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, nullptr};
+  GBK_CUDA(launch_unfused(p->dp, a, p->lsf_taps, p->uf_scratch, p->uf_rows, p->sm_count,
+                          (cudaStream_t)cuda_stream));
+  return GBK_OK;
 }
 
 extern "C" int gbk_probe_pipe(int which, int64_t iters, int blocks, int threads, float* sink,

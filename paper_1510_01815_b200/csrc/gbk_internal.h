@@ -75,6 +75,12 @@ cudaError_t fused_occupancy(const FusedLaunch& fl, int* blocks_per_sm);
 cudaError_t fused_prepare(const FusedLaunch& fl);  // opt in to large dynamic shared memory
 size_t fused_smem_bytes(const DevProblem& dp);
 
+// unfused comparison path (gbk_unfused.cu)
+size_t unfused_bytes_per_row(const DevProblem& dp);
+double unfused_algorithmic_bytes_per_row(const DevProblem& dp);
+cudaError_t launch_unfused(const DevProblem& dp, const EvalArgs& a, const float* lsf_taps, float* scratch,
+                           long long chunk_rows, int sm_count, cudaStream_t st);
+
 cudaError_t launch_probe(int which, long long iters, int blocks, int threads, float* sink,
                          cudaStream_t st);
 
