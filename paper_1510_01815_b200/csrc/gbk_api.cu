@@ -121,7 +121,9 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   const int nvx = d->nv + 2 * r_v;
   // w_q[c] = sum over in-band channels k of L[k - ch] * v'_k^q, ch = c - r_v,
   // v'_k = (k - (nv-1)/2) dv  (velocities relative to v_center).
-  std::vector<float4> chan(nvx);
+  const int nvx_pad = (nvx + kChanBlock - 1) / kChanBlock * kChanBlock;
+  std::vector<float4> chan(nvx_pad);
+  for (int c = nvx; c < nvx_pad; ++c) chan[c] = make_float4((float)c, 0.f, 0.f, 0.f);  // weightless padding
   for (int c = 0; c < nvx; ++c) {
     const int ch = c - r_v;
     double w[3] = {0, 0, 0};
@@ -219,7 +221,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   DevProblem& dp = p->dp;
   dp.nx = d->nx, dp.ny = d->ny, dp.nv = d->nv, dp.u = d->u, dp.n_gal = d->n_gal;
   dp.fw = d->u * d->nx, dp.fh = d->u * d->ny;
-  dp.r_v = r_v, dp.nvx = nvx;
+  dp.r_v = r_v, dp.nvx = nvx, dp.nvx_pad = nvx_pad;
   dp.rc_model = d->rc_model, dp.psf_kind = d->psf_kind;
   dp.has_disp = d->sobs ? 1 : 0, dp.psf_per_gal = d->psf_per_gal ? 1 : 0;
   dp.r_p_max = r_p_max, dp.psf_stride = psf_stride;
@@ -257,7 +259,9 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   const int n_ext = (dp.tile_w + 2 * r_p_max) * (dp.tile_h + 2 * r_p_max);
   p->fl.smem_bytes = (int)smem;
   p->fl.pixels_per_thread = 4;
-  p->fl.threads = std::min(384, std::max(64, ((n_ext + 3) / 4 + 31) / 32 * 32));
+  // 256 threads: three blocks of a whole-field config-3 tile are resident per SM (70.7 KB and
+  // <= 85 registers x 256 threads each), so their phases overlap (measured best of 128..384)
+  p->fl.threads = std::min(256, std::max(64, ((n_ext + 3) / 4 + 31) / 32 * 32));
   long long ext = 0;
   for (int ty = 0; ty < dp.tiles_y; ++ty)
     for (int tx = 0; tx < dp.tiles_x; ++tx) {
@@ -277,7 +281,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
       return bail(fail(e_ == cudaErrorMemoryAllocation ? GBK_ERR_ALLOC : GBK_ERR_CUDA, "%s: %s", \
                        #expr, cudaGetErrorString(e_)));                                        \
   } while (0)
-  GBK_CUDA_P(cudaMalloc(&p->chan_tab, sizeof(float4) * nvx));
+  GBK_CUDA_P(cudaMalloc(&p->chan_tab, sizeof(float4) * nvx_pad));
   GBK_CUDA_P(cudaMalloc(&p->psf_taps, sizeof(float) * psf_taps.size()));
   GBK_CUDA_P(cudaMalloc(&p->psf_r, sizeof(int) * n_psf));
   GBK_CUDA_P(cudaMalloc(&p->obs, sizeof(float4) * obs.size()));
@@ -286,7 +290,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     GBK_CUDA_P(cudaMalloc(&p->lsf_taps, sizeof(float) * lsf_f.size()));
     GBK_CUDA_P(cudaMemcpy(p->lsf_taps, lsf_f.data(), sizeof(float) * lsf_f.size(), cudaMemcpyHostToDevice));
   }
-  GBK_CUDA_P(cudaMemcpy(p->chan_tab, chan.data(), sizeof(float4) * nvx, cudaMemcpyHostToDevice));
+  GBK_CUDA_P(cudaMemcpy(p->chan_tab, chan.data(), sizeof(float4) * nvx_pad, cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->psf_taps, psf_taps.data(), sizeof(float) * psf_taps.size(), cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->psf_r, psf_r.data(), sizeof(int) * n_psf, cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->obs, obs.data(), sizeof(float4) * obs.size(), cudaMemcpyHostToDevice));

@@ -12,6 +12,8 @@ constexpr int kMaxSepR = 16;    // largest separable (Gaussian) PSF tap radius, 
 constexpr int kMaxPsfN = 33;    // largest PSF image side
 constexpr int kMaxLsfR = 64;    // largest LSF tap radius, channels
 constexpr int kVBlock = 8;      // output rows per thread in the vertical pass
+constexpr int kChanBlock = 8;   // channels between two restarts of the line recurrence (gbk_fused.cu)
+constexpr float kRecMaxStep = 0.8f;  // the recurrence is used for step <= this (sigma0/dv >= 1.06)
 
 // Everything the kernels need to know about a problem; passed by value (__grid_constant__).
 struct DevProblem {
@@ -19,6 +21,7 @@ struct DevProblem {
   int n_gal;
   int fw, fh;               // fine grid = u*nx, u*ny
   int r_v, nvx;             // LSF radius, nv + 2 r_v extended channels
+  int nvx_pad;              // nvx rounded up to kChanBlock; the padding channels have zero weights
   int rc_model, psf_kind, has_disp, psf_per_gal;
   int tile_w, tile_h;       // tile, fine pixels (multiples of u)
   int tiles_x, tiles_y, ntiles;
@@ -53,6 +56,10 @@ struct RowConst {
   float inv_rt, rt;
   float nl2e_inv_r0;  // -log2(e)/r0
   float step;         // s * dv with s = 1/(sigma0 sqrt(2 ln 2)): exp(-dv^2/(2 sigma0^2)) = 2^-(s dv)^2
+  float q;            // 2^(-2 step^2): ratio of consecutive line ratios (recurrence of the voxel loop)
+  float m2step;       // -2 step
+  float mstep2;       // -step^2
+  int use_rec;        // step <= kRecMaxStep: the multiplicative recurrence is safe
   float k1;           // -s * V_t sin i (* 2/pi for the arctan curve)
   float k0;           // s * (velocity of extended channel 0 - V_sys): the line-centre offset of a
                       // sample from extended channel 0 is  d0 = k1 * f(r/r_t) * cos(theta) + k0
