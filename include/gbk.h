@@ -97,6 +97,7 @@ typedef struct {
   int32_t blocks_per_sm;  /* occupancy of the fused kernel as reported by the runtime      */
   int32_t sm_count;
   int64_t ext_voxels_per_eval; /* sum over tiles of (tw+2R)(th+2R)(nv+2R_v), R = r_p_max   */
+  int32_t device;         /* CUDA device ordinal the problem lives on                      */
 } gbk_problem_info;
 
 /*
@@ -167,6 +168,68 @@ const char *gbk_last_error(void);
  */
 int gbk_probe_pipe(int which, int64_t iters, int blocks, int threads, float *sink,
                    double *ops_per_launch, void *cuda_stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Host drivers: the paper's three optimisers re-stated as callers of the
+ * batched hot path.  Each builds batches of rows, calls gbk_eval_batch on `cuda_stream`, reduces
+ * on the device what can be reduced there (argmin, J^T J) and reads back a few numbers per
+ * iteration.  All array arguments are HOST memory.  They block until the fit is done.
+ * MPFIT and MultiNest themselves are third-party codes and are not reproduced; these are plain
+ * re-statements of the published algorithms.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct {
+  int64_t evals;       /* rows evaluated                                                      */
+  int32_t launches;    /* gbk_eval_batch calls                                                */
+  int32_t iterations;  /* NG: levels; LM: largest iteration count over the fits; NS: batches  */
+  int32_t converged;   /* fits that met their stopping rule                                   */
+  float ms_total;      /* wall clock of the call, ms                                          */
+} gbk_fit_stats;
+
+/*
+ * Nested grids (refinement rule: DESIGN.md reading A19).  `n_axes` parameters
+ * (indices axis_param[a] into the row, box [axis_lo[a], axis_hi[a]]) are gridded with `nodes`
+ * nodes each, the other parameters stay at base_row.  Level l has spacing h = (hi-lo)/(nodes 2^l)
+ * and nodes c + (j - (nodes-1)/2) h; c = box centre at level 0, then the best node of the level
+ * before.  An axis on PA (index 2) whose box spans >= 360 degrees wraps; any other axis is shifted
+ * to stay inside its box.  Ties in chi^2 take the lowest flat index (axis 0 slowest).
+ * nodes^n_axes <= 2^24.  best_row [GBK_P] and best_chi2 [1] receive the final level's best node.
+ */
+int gbk_fit_ng(gbk_problem *p, const float *base_row, int32_t gal, int32_t n_axes,
+               const int32_t *axis_param, const float *axis_lo, const float *axis_hi, int32_t nodes,
+               int32_t levels, float *best_row, float *best_chi2, gbk_fit_stats *stats,
+               void *cuda_stream);
+
+/*
+ * Levenberg-Marquardt for n_fits independent fits at once (config 5: one fit
+ * per galaxy; config 2: n_fits = 1).  Per iteration ONE batch of n_active*(n_free+1) rows (base +
+ * forward differences of rel_step x box width, backward at the upper bound) with weighted
+ * residuals, J^T J and J^T r reduced on the device, the damped normal equations
+ * solved on the host, and ONE batch of n_active*4 trial rows (four damping factors) for chi^2.
+ * Parameters are clipped to [lo, hi].  A fit stops when the relative chi^2 decrease of an accepted
+ * step is < ftol, when no damping factor up to 1e10 lowers chi^2, or after max_iter iterations.
+ *   start_rows [n_fits][GBK_P], gal [n_fits] or NULL (all 0), free_param/lo/hi [n_free]
+ *   fit_rows [n_fits][GBK_P], fit_chi2 [n_fits], fit_iters [n_fits] or NULL
+ * A fit whose start row has chi^2 = +INF is returned unchanged with chi^2 = +INF.
+ */
+int gbk_fit_lm(gbk_problem *p, int32_t n_fits, const float *start_rows, const int32_t *gal,
+               int32_t n_free, const int32_t *free_param, const float *lo, const float *hi,
+               float rel_step, int32_t max_iter, float ftol, float *fit_rows, float *fit_chi2,
+               int32_t *fit_iters, gbk_fit_stats *stats, void *cuda_stream);
+
+/*
+ * Nested sampling with ln L = -chi^2/2 (A20) and a uniform prior on
+ * the box: n_live live points; every batch draws `batch` candidates uniformly from the bounding
+ * box of the live points enlarged by `enlarge` (>= 0, fraction of its width; clipped to the prior
+ * box) and evaluates them in one launch; each candidate that beats the current worst live point
+ * replaces it (prior volume X_i = exp(-i/n_live), evidence by the trapezoid-free simple rule).
+ * Stops when L_max X_i < tol x Z or after max_batches.  Outputs: the best row, its chi^2, the
+ * posterior-mean row and ln Z.  `seed` seeds the driver's own generator (xoshiro256**).
+ */
+int gbk_fit_ns(gbk_problem *p, const float *base_row, int32_t gal, int32_t n_free,
+               const int32_t *free_param, const float *lo, const float *hi, int32_t n_live,
+               int32_t batch, int32_t max_batches, float enlarge, float tol, uint64_t seed,
+               float *best_row, float *best_chi2, float *mean_row, double *log_evidence,
+               gbk_fit_stats *stats, void *cuda_stream);
 
 #ifdef __cplusplus
 }

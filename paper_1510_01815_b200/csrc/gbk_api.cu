@@ -14,9 +14,10 @@
 using namespace gbk;
 
 namespace {
-
 thread_local char g_err[512] = "";
+}
 
+namespace gbk {
 int fail(int code, const char* fmt, ...) {
   va_list ap;
   va_start(ap, fmt);
@@ -24,6 +25,10 @@ int fail(int code, const char* fmt, ...) {
   va_end(ap);
   return code;
 }
+void clear_error() { g_err[0] = 0; }
+}  // namespace gbk
+
+namespace {
 
 #define GBK_CUDA(expr)                                                                  \
   do {                                                                                  \
@@ -316,6 +321,7 @@ extern "C" int gbk_get_info(const gbk_problem* p, gbk_problem_info* info) {
   info->block_threads = p->fl.threads, info->smem_bytes = p->fl.smem_bytes;
   info->blocks_per_sm = p->blocks_per_sm, info->sm_count = p->sm_count;
   info->ext_voxels_per_eval = p->ext_voxels;
+  info->device = p->device;
   return GBK_OK;
 }
 

@@ -1,0 +1,615 @@
+// Host drivers of libgbk: nested grids, Levenberg-Marquardt and nested sampling
+// written as callers of the batched hot path.  They use only the public calls of include/gbk.h
+// (gbk_get_info, gbk_eval_batch) plus three small device reductions of their own (row building,
+// argmin, J^T J), so an optimiser iteration moves a few hundred bytes across PCIe instead of the
+// residual maps the paper copies back every iteration.
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#include <algorithm>
+#include <chrono>
+#include <vector>
+
+#include "gbk_internal.h"
+
+using namespace gbk;
+
+namespace {
+
+#define DRV_CUDA(expr)                                                                      \
+  do {                                                                                      \
+    cudaError_t e_ = (expr);                                                                \
+    if (e_ != cudaSuccess)                                                                  \
+      return fail(e_ == cudaErrorMemoryAllocation ? GBK_ERR_ALLOC : GBK_ERR_CUDA, "%s: %s", \
+                  #expr, cudaGetErrorString(e_));                                           \
+  } while (0)
+#define DRV_TRY(expr)            \
+  do {                           \
+    if (int rc_ = (expr)) return rc_; \
+  } while (0)
+
+// Device / pinned-host buffer pair that frees itself (the drivers allocate per call, off the hot path).
+template <typename T>
+struct Buf {
+  T* d = nullptr;
+  T* h = nullptr;
+  size_t n = 0;
+  ~Buf() {
+    cudaFree(d);
+    cudaFreeHost(h);
+  }
+  cudaError_t alloc(size_t count, bool host = true, bool dev = true) {
+    n = count;
+    cudaError_t e = cudaSuccess;
+    if (dev) e = cudaMalloc(&d, sizeof(T) * std::max<size_t>(count, 1));
+    if (e == cudaSuccess && host) e = cudaMallocHost(&h, sizeof(T) * std::max<size_t>(count, 1));
+    return e;
+  }
+  cudaError_t to_device(size_t count, cudaStream_t st) {
+    return cudaMemcpyAsync(d, h, sizeof(T) * count, cudaMemcpyHostToDevice, st);
+  }
+  cudaError_t to_host(size_t count, cudaStream_t st) {
+    return cudaMemcpyAsync(h, d, sizeof(T) * count, cudaMemcpyDeviceToHost, st);
+  }
+};
+
+struct Clock {
+  std::chrono::steady_clock::time_point t0 = std::chrono::steady_clock::now();
+  float ms() const {
+    return std::chrono::duration<float, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  }
+};
+
+bool finite_row(const float* r) {
+  for (int j = 0; j < GBK_P; ++j)
+    if (!isfinite(r[j])) return false;
+  return true;
+}
+
+int check_box(int n, const int32_t* idx, const float* lo, const float* hi) {
+  if (n < 1 || n > GBK_P || !idx || !lo || !hi) return fail(GBK_ERR_ARG, "bad parameter box");
+  for (int a = 0; a < n; ++a) {
+    if (idx[a] < 0 || idx[a] >= GBK_P) return fail(GBK_ERR_ARG, "parameter index %d out of range", idx[a]);
+    if (!isfinite(lo[a]) || !isfinite(hi[a]) || !(hi[a] > lo[a]))
+      return fail(GBK_ERR_ARG, "box of parameter %d is empty or not finite", idx[a]);
+    for (int b = 0; b < a; ++b)
+      if (idx[b] == idx[a]) return fail(GBK_ERR_ARG, "parameter %d listed twice", idx[a]);
+  }
+  return GBK_OK;
+}
+
+// ------------------------------------------------------------------------- nested grids ----
+constexpr int kNgMaxAxes = 6, kNgMaxNodes = 32;
+
+struct NgAxes {
+  int n_axes, nodes;
+  int param[kNgMaxAxes];
+  float value[kNgMaxAxes][kNgMaxNodes];
+  float base[GBK_P];
+};
+
+// Row r of the level: flat index with axis 0 slowest.
+__global__ void ng_rows_kernel(const __grid_constant__ NgAxes ax, int n_rows, float* __restrict__ rows) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n_rows) return;
+  float row[GBK_P];
+#pragma unroll
+  for (int j = 0; j < GBK_P; ++j) row[j] = ax.base[j];
+  int rem = r;
+  for (int a = ax.n_axes - 1; a >= 0; --a) {
+    const int j = rem % ax.nodes;
+    rem /= ax.nodes;
+    row[ax.param[a]] = ax.value[a][j];
+  }
+#pragma unroll
+  for (int j = 0; j < GBK_P; ++j) rows[(size_t)r * GBK_P + j] = row[j];
+}
+
+// Smallest chi^2 and its lowest index (NaN never wins; +INF only if everything is +INF).
+__global__ void argmin_kernel(const float* __restrict__ chi2, int n, int* __restrict__ out_idx,
+                              float* __restrict__ out_val) {
+  __shared__ float sv[1024];
+  __shared__ int si[1024];
+  float best = __int_as_float(0x7f800000);
+  int bi = 0x7fffffff;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    const float v = chi2[i];
+    if (v < best || (v == best && i < bi)) best = v, bi = i;
+  }
+  sv[threadIdx.x] = best, si[threadIdx.x] = bi;
+  __syncthreads();
+  for (int s = blockDim.x >> 1; s > 0; s >>= 1) {
+    if (threadIdx.x < s) {
+      const float v = sv[threadIdx.x + s];
+      const int i = si[threadIdx.x + s];
+      if (v < sv[threadIdx.x] || (v == sv[threadIdx.x] && i < si[threadIdx.x]))
+        sv[threadIdx.x] = v, si[threadIdx.x] = i;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out_idx[0] = si[0] == 0x7fffffff ? 0 : si[0], out_val[0] = sv[0];
+}
+
+}  // namespace
+
+extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, int32_t n_axes,
+                          const int32_t* axis_param, const float* axis_lo, const float* axis_hi,
+                          int32_t nodes, int32_t levels, float* best_row, float* best_chi2,
+                          gbk_fit_stats* stats, void* cuda_stream) {
+  clear_error();
+  Clock clock;
+  gbk_problem_info info;
+  DRV_TRY(gbk_get_info(p, &info));
+  if (!base_row || !best_row || !best_chi2) return fail(GBK_ERR_ARG, "null argument");
+  if (n_axes > kNgMaxAxes || nodes < 2 || nodes > kNgMaxNodes || levels < 1 || levels > 30)
+    return fail(GBK_ERR_ARG, "need n_axes <= %d, 2 <= nodes <= %d, 1 <= levels <= 30", kNgMaxAxes, kNgMaxNodes);
+  DRV_TRY(check_box(n_axes, axis_param, axis_lo, axis_hi));
+  if (gal < 0 || gal >= info.n_gal) return fail(GBK_ERR_ARG, "gal out of range");
+  double n_rows_d = 1.0;
+  for (int a = 0; a < n_axes; ++a) n_rows_d *= nodes;
+  if (n_rows_d > (double)(1 << 24)) return fail(GBK_ERR_ARG, "nodes^n_axes exceeds 2^24 rows");
+  const int n_rows = (int)n_rows_d;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DRV_CUDA(cudaSetDevice(info.device));
+
+  Buf<float> rows, chi2, best_v;
+  Buf<int> best_i, gal_idx;
+  DRV_CUDA(rows.alloc((size_t)n_rows * GBK_P, false));
+  DRV_CUDA(chi2.alloc(n_rows, false));
+  DRV_CUDA(best_v.alloc(1));
+  DRV_CUDA(best_i.alloc(1));
+  if (gal != 0) {
+    DRV_CUDA(gal_idx.alloc(n_rows));
+    std::fill(gal_idx.h, gal_idx.h + n_rows, gal);
+    DRV_CUDA(gal_idx.to_device(n_rows, st));
+  }
+
+  NgAxes ax;
+  memset(&ax, 0, sizeof(ax));
+  ax.n_axes = n_axes, ax.nodes = nodes;
+  memcpy(ax.base, base_row, sizeof(float) * GBK_P);
+  double centre[kNgMaxAxes];
+  for (int a = 0; a < n_axes; ++a) {
+    ax.param[a] = axis_param[a];
+    centre[a] = 0.5 * ((double)axis_lo[a] + (double)axis_hi[a]);
+  }
+  gbk_fit_stats fs{};
+  for (int level = 0; level < levels; ++level) {
+    for (int a = 0; a < n_axes; ++a) {
+      const double lo = axis_lo[a], hi = axis_hi[a];
+      const double h = (hi - lo) / ((double)nodes * (double)(1u << level));
+      const bool wraps = axis_param[a] == 2 && hi - lo >= 360.0;
+      double first = centre[a] - 0.5 * (nodes - 1) * h;
+      if (!wraps) {   // shift the whole axis back inside the box
+        const double last = first + (nodes - 1) * h;
+        first += std::max(0.0, lo - first) - std::max(0.0, last - hi);
+      }
+      for (int j = 0; j < nodes; ++j) {
+        double v = first + j * h;
+        if (wraps) v = lo + fmod(fmod(v - lo, 360.0) + 360.0, 360.0);
+        ax.value[a][j] = (float)v;
+      }
+    }
+    ng_rows_kernel<<<(n_rows + 255) / 256, 256, 0, st>>>(ax, n_rows, rows.d);
+    DRV_CUDA(cudaGetLastError());
+    DRV_TRY(gbk_eval_batch(p, rows.d, gal != 0 ? gal_idx.d : nullptr, n_rows, chi2.d, nullptr, nullptr,
+                           nullptr, nullptr, cuda_stream));
+    argmin_kernel<<<1, 1024, 0, st>>>(chi2.d, n_rows, best_i.d, best_v.d);
+    DRV_CUDA(cudaGetLastError());
+    DRV_CUDA(best_i.to_host(1, st));
+    DRV_CUDA(best_v.to_host(1, st));
+    DRV_CUDA(cudaStreamSynchronize(st));
+    int rem = best_i.h[0];
+    for (int a = n_axes - 1; a >= 0; --a) {
+      centre[a] = ax.value[a][rem % nodes];
+      rem /= nodes;
+    }
+    fs.evals += n_rows, fs.launches += 1, fs.iterations += 1;
+  }
+  memcpy(best_row, base_row, sizeof(float) * GBK_P);
+  for (int a = 0; a < n_axes; ++a) best_row[axis_param[a]] = (float)centre[a];
+  *best_chi2 = best_v.h[0];
+  fs.converged = isfinite(best_v.h[0]) ? 1 : 0;
+  fs.ms_total = clock.ms();
+  if (stats) *stats = fs;
+  return GBK_OK;
+}
+
+// ------------------------------------------------------------------ Levenberg-Marquardt ----
+namespace {
+
+// One block per (term, fit).  Terms: n(n+1)/2 entries of J^T J (upper triangle, row-major),
+// n entries of J^T r, and r.r; J_a = (r_a - r_0) / h_a from the forward-difference rows.
+// resid: [n_fits][n+1][M]; h: [n_fits][n]; out: [n_fits][n_terms] (double).
+__global__ void lm_normal_kernel(const float* __restrict__ resid, const float* __restrict__ h, int n,
+                                 int M, double* __restrict__ out) {
+  const int n_tri = n * (n + 1) / 2, n_terms = n_tri + n + 1;
+  const int term = blockIdx.x, fit = blockIdx.y;
+  int a = -1, b = -1;   // a = b = -1: r.r;  b = -1: (J^T r)_a
+  if (term < n_tri) {
+    int t = term;
+    a = 0;
+    while (t >= n - a) t -= n - a, ++a;
+    b = a + t;
+  } else if (term < n_tri + n) {
+    a = term - n_tri;
+  }
+  const float* r0 = resid + (size_t)fit * (n + 1) * M;
+  const float* ra = a >= 0 ? r0 + (size_t)(a + 1) * M : r0;
+  const float* rb = b >= 0 ? r0 + (size_t)(b + 1) * M : r0;
+  double acc = 0.0;
+  for (int i = threadIdx.x; i < M; i += blockDim.x) {
+    const double z = r0[i];
+    const double x = a >= 0 ? (double)ra[i] - z : z;
+    const double y = b >= 0 ? (double)rb[i] - z : z;
+    acc += x * y;
+  }
+  __shared__ double red[256];
+  red[threadIdx.x] = acc;
+  __syncthreads();
+  for (int s = blockDim.x >> 1; s > 0; s >>= 1) {
+    if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    double v = red[0];
+    if (a >= 0) v /= (double)h[(size_t)fit * n + a];
+    if (b >= 0) v /= (double)h[(size_t)fit * n + b];
+    out[(size_t)fit * n_terms + term] = v;
+  }
+}
+
+// Solves (A + lambda diag(A)) x = -g by Cholesky (A symmetric, upper triangle packed row-major).
+bool solve_damped(int n, const double* tri, const double* g, double lambda, double* x) {
+  double L[GBK_P][GBK_P];
+  int t = 0;
+  for (int a = 0; a < n; ++a)
+    for (int b = a; b < n; ++b, ++t) L[a][b] = L[b][a] = tri[t];
+  for (int a = 0; a < n; ++a) {
+    if (!(L[a][a] > 0.0) || !isfinite(L[a][a])) return false;
+    L[a][a] *= 1.0 + lambda;
+  }
+  for (int j = 0; j < n; ++j) {
+    double d = L[j][j];
+    for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
+    if (!(d > 0.0) || !isfinite(d)) return false;
+    L[j][j] = sqrt(d);
+    for (int i = j + 1; i < n; ++i) {
+      double s = L[i][j];
+      for (int k = 0; k < j; ++k) s -= L[i][k] * L[j][k];
+      L[i][j] = s / L[j][j];
+    }
+  }
+  double y[GBK_P];
+  for (int i = 0; i < n; ++i) {
+    double s = -g[i];
+    for (int k = 0; k < i; ++k) s -= L[i][k] * y[k];
+    y[i] = s / L[i][i];
+  }
+  for (int i = n - 1; i >= 0; --i) {
+    double s = y[i];
+    for (int k = i + 1; k < n; ++k) s -= L[k][i] * x[k];
+    x[i] = s / L[i][i];
+    if (!isfinite(x[i])) return false;
+  }
+  return true;
+}
+
+constexpr int kLmTrials = 4;
+const double kLmFactor[kLmTrials] = {0.1, 1.0, 10.0, 100.0};
+
+struct LmFit {
+  float row[GBK_P];
+  double chi2 = INFINITY, lambda = 1e-3;
+  int iters = 0, gal = 0;
+  bool active = true, converged = false;
+};
+
+}  // namespace
+
+extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_rows, const int32_t* gal,
+                          int32_t n_free, const int32_t* free_param, const float* lo, const float* hi,
+                          float rel_step, int32_t max_iter, float ftol, float* fit_rows,
+                          float* fit_chi2, int32_t* fit_iters, gbk_fit_stats* stats,
+                          void* cuda_stream) {
+  clear_error();
+  Clock clock;
+  gbk_problem_info info;
+  DRV_TRY(gbk_get_info(p, &info));
+  if (n_fits < 0 || (n_fits > 0 && (!start_rows || !fit_rows || !fit_chi2)))
+    return fail(GBK_ERR_ARG, "null argument");
+  if (!(rel_step > 0.f) || !isfinite(rel_step) || max_iter < 0 || !(ftol >= 0.f))
+    return fail(GBK_ERR_ARG, "need rel_step > 0, max_iter >= 0, ftol >= 0");
+  DRV_TRY(check_box(n_free, free_param, lo, hi));
+  for (int f = 0; f < n_fits; ++f)
+    if (gal && (gal[f] < 0 || gal[f] >= info.n_gal)) return fail(GBK_ERR_ARG, "gal[%d] out of range", f);
+  gbk_fit_stats fs{};
+  if (n_fits == 0) {
+    if (stats) *stats = fs;
+    return GBK_OK;
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DRV_CUDA(cudaSetDevice(info.device));
+  const int n = n_free, M = 2 * info.nx * info.ny;
+  const int n_tri = n * (n + 1) / 2, n_terms = n_tri + n + 1;
+  // fits per chunk: the residual buffer of a chunk stays below 1 GiB
+  const size_t resid_per_fit = sizeof(float) * (size_t)(n + 1) * M;
+  const int chunk = (int)std::max<size_t>(1, std::min<size_t>(n_fits, (size_t(1) << 30) / resid_per_fit));
+  const int rows_per_fit = std::max(n + 1, kLmTrials);
+  Buf<float> rows, chi2, resid, hstep;
+  Buf<int> gidx;
+  Buf<double> normal;
+  DRV_CUDA(rows.alloc((size_t)chunk * rows_per_fit * GBK_P));
+  DRV_CUDA(chi2.alloc((size_t)chunk * rows_per_fit));
+  DRV_CUDA(gidx.alloc((size_t)chunk * rows_per_fit));
+  DRV_CUDA(resid.alloc((size_t)chunk * (n + 1) * M, false));
+  DRV_CUDA(hstep.alloc((size_t)chunk * n));
+  DRV_CUDA(normal.alloc((size_t)chunk * n_terms));
+
+  std::vector<LmFit> fits(n_fits);
+  for (int f = 0; f < n_fits; ++f) {
+    memcpy(fits[f].row, start_rows + (size_t)f * GBK_P, sizeof(float) * GBK_P);
+    fits[f].gal = gal ? gal[f] : 0;
+    for (int a = 0; a < n; ++a)   // start inside the box
+      fits[f].row[free_param[a]] = std::min(hi[a], std::max(lo[a], fits[f].row[free_param[a]]));
+    if (!finite_row(fits[f].row)) fits[f].active = false;
+  }
+
+  for (int c0 = 0; c0 < n_fits; c0 += chunk) {
+    const int c1 = std::min(n_fits, c0 + chunk);
+    for (int iter = 0;; ++iter) {
+      std::vector<int> act;
+      for (int f = c0; f < c1; ++f)
+        if (fits[f].active) act.push_back(f);
+      if (act.empty()) break;
+      const int na = (int)act.size();
+      // ---- Jacobian batch: base + n one-sided differences per active fit ----
+      for (int i = 0; i < na; ++i) {
+        const LmFit& ft = fits[act[i]];
+        for (int r = 0; r <= n; ++r) {
+          float* row = rows.h + ((size_t)i * (n + 1) + r) * GBK_P;
+          memcpy(row, ft.row, sizeof(float) * GBK_P);
+          gidx.h[(size_t)i * (n + 1) + r] = ft.gal;
+          if (r > 0) {
+            const int a = r - 1, j = free_param[a];
+            float h = rel_step * (hi[a] - lo[a]);
+            if (row[j] + h > hi[a]) h = -h;
+            const float moved = row[j] + h;
+            hstep.h[(size_t)i * n + a] = moved - row[j];   // the step actually taken in FP32
+            row[j] = moved;
+          }
+        }
+      }
+      const int kj = na * (n + 1);
+      DRV_CUDA(rows.to_device((size_t)kj * GBK_P, st));
+      DRV_CUDA(gidx.to_device(kj, st));
+      DRV_CUDA(hstep.to_device((size_t)na * n, st));
+      DRV_TRY(gbk_eval_batch(p, rows.d, gidx.d, kj, chi2.d, nullptr, nullptr, nullptr, resid.d, cuda_stream));
+      lm_normal_kernel<<<dim3(n_terms, na), 256, 0, st>>>(resid.d, hstep.d, n, M, normal.d);
+      DRV_CUDA(cudaGetLastError());
+      DRV_CUDA(normal.to_host((size_t)na * n_terms, st));
+      DRV_CUDA(chi2.to_host(kj, st));
+      DRV_CUDA(cudaStreamSynchronize(st));
+      fs.evals += kj, fs.launches += 1;
+      // ---- trial rows: four damping factors per fit ----
+      std::vector<int> live;   // indices into act with a usable base row
+      for (int i = 0; i < na; ++i) {
+        LmFit& ft = fits[act[i]];
+        ft.chi2 = chi2.h[(size_t)i * (n + 1)];
+        if (!isfinite(ft.chi2) || iter >= max_iter) {
+          ft.active = false;
+          continue;
+        }
+        live.push_back(i);
+      }
+      const int nl = (int)live.size();
+      if (nl == 0) continue;
+      for (int q = 0; q < nl; ++q) {
+        const int i = live[q];
+        const LmFit& ft = fits[act[i]];
+        const double* nm = normal.h + (size_t)i * n_terms;
+        for (int t = 0; t < kLmTrials; ++t) {
+          float* row = rows.h + ((size_t)q * kLmTrials + t) * GBK_P;
+          memcpy(row, ft.row, sizeof(float) * GBK_P);
+          gidx.h[(size_t)q * kLmTrials + t] = ft.gal;
+          double dx[GBK_P];
+          if (solve_damped(n, nm, nm + n_tri, ft.lambda * kLmFactor[t], dx))
+            for (int a = 0; a < n; ++a) {
+              const int j = free_param[a];
+              row[j] = (float)std::min<double>(hi[a], std::max<double>(lo[a], (double)row[j] + dx[a]));
+            }
+        }
+      }
+      const int kt = nl * kLmTrials;
+      DRV_CUDA(rows.to_device((size_t)kt * GBK_P, st));
+      DRV_CUDA(gidx.to_device(kt, st));
+      DRV_TRY(gbk_eval_batch(p, rows.d, gidx.d, kt, chi2.d, nullptr, nullptr, nullptr, nullptr, cuda_stream));
+      DRV_CUDA(chi2.to_host(kt, st));
+      DRV_CUDA(cudaStreamSynchronize(st));
+      fs.evals += kt, fs.launches += 1;
+      for (int q = 0; q < nl; ++q) {
+        LmFit& ft = fits[act[live[q]]];
+        int best = -1;
+        double best_chi = ft.chi2;
+        for (int t = 0; t < kLmTrials; ++t) {
+          const double c = chi2.h[(size_t)q * kLmTrials + t];
+          if (c < best_chi) best_chi = c, best = t;
+        }
+        ft.iters += 1;
+        if (best >= 0) {
+          const double rel = (ft.chi2 - best_chi) / ft.chi2;
+          memcpy(ft.row, rows.h + ((size_t)q * kLmTrials + best) * GBK_P, sizeof(float) * GBK_P);
+          ft.lambda = std::max(1e-9, ft.lambda * kLmFactor[best] * 0.3);
+          ft.chi2 = best_chi;
+          if (rel < (double)ftol) ft.active = false, ft.converged = true;
+        } else {
+          ft.lambda *= 1e4;
+          if (ft.lambda > 1e10) ft.active = false, ft.converged = true;   // no downhill step left
+        }
+      }
+    }
+  }
+  for (int f = 0; f < n_fits; ++f) {
+    memcpy(fit_rows + (size_t)f * GBK_P, fits[f].row, sizeof(float) * GBK_P);
+    fit_chi2[f] = (float)fits[f].chi2;
+    if (fit_iters) fit_iters[f] = fits[f].iters;
+    fs.iterations = std::max(fs.iterations, fits[f].iters);
+    fs.converged += fits[f].converged ? 1 : 0;
+  }
+  fs.ms_total = clock.ms();
+  if (stats) *stats = fs;
+  return GBK_OK;
+}
+
+// --------------------------------------------------------------------- nested sampling ----
+namespace {
+
+struct Xoshiro {   // xoshiro256** seeded by splitmix64 (public-domain algorithm, re-stated)
+  uint64_t s[4];
+  explicit Xoshiro(uint64_t seed) {
+    for (int i = 0; i < 4; ++i) {
+      seed += 0x9E3779B97F4A7C15ull;
+      uint64_t z = seed;
+      z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+      z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+      s[i] = z ^ (z >> 31);
+    }
+  }
+  static uint64_t rotl(uint64_t x, int k) { return (x << k) | (x >> (64 - k)); }
+  uint64_t next() {
+    const uint64_t r = rotl(s[1] * 5, 7) * 9, t = s[1] << 17;
+    s[2] ^= s[0], s[3] ^= s[1], s[1] ^= s[2], s[0] ^= s[3], s[2] ^= t, s[3] = rotl(s[3], 45);
+    return r;
+  }
+  double uniform() { return (double)(next() >> 11) * (1.0 / 9007199254740992.0); }
+};
+
+double log_add(double a, double b) {
+  if (a == -INFINITY) return b;
+  if (b == -INFINITY) return a;
+  const double m = std::max(a, b);
+  return m + log(exp(a - m) + exp(b - m));
+}
+
+}  // namespace
+
+extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, int32_t n_free,
+                          const int32_t* free_param, const float* lo, const float* hi, int32_t n_live,
+                          int32_t batch, int32_t max_batches, float enlarge, float tol, uint64_t seed,
+                          float* best_row, float* best_chi2, float* mean_row, double* log_evidence,
+                          gbk_fit_stats* stats, void* cuda_stream) {
+  clear_error();
+  Clock clock;
+  gbk_problem_info info;
+  DRV_TRY(gbk_get_info(p, &info));
+  if (!base_row || !best_row || !best_chi2) return fail(GBK_ERR_ARG, "null argument");
+  if (n_live < 2 || batch < 1 || max_batches < 0 || !(enlarge >= 0.f) || !(tol > 0.f))
+    return fail(GBK_ERR_ARG, "need n_live >= 2, batch >= 1, max_batches >= 0, enlarge >= 0, tol > 0");
+  DRV_TRY(check_box(n_free, free_param, lo, hi));
+  if (gal < 0 || gal >= info.n_gal) return fail(GBK_ERR_ARG, "gal out of range");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DRV_CUDA(cudaSetDevice(info.device));
+  const int n = n_free, cap = std::max(n_live, batch);
+  Buf<float> rows, chi2;
+  Buf<int> gidx;
+  DRV_CUDA(rows.alloc((size_t)cap * GBK_P));
+  DRV_CUDA(chi2.alloc(cap));
+  DRV_CUDA(gidx.alloc(cap));
+  std::fill(gidx.h, gidx.h + cap, gal);
+  DRV_CUDA(gidx.to_device(cap, st));
+  Xoshiro rng(seed);
+  gbk_fit_stats fs{};
+
+  auto evaluate = [&](int k) -> int {   // rows.h[0..k) -> chi2.h[0..k)
+    DRV_CUDA(rows.to_device((size_t)k * GBK_P, st));
+    DRV_TRY(gbk_eval_batch(p, rows.d, gidx.d, k, chi2.d, nullptr, nullptr, nullptr, nullptr, cuda_stream));
+    DRV_CUDA(chi2.to_host(k, st));
+    DRV_CUDA(cudaStreamSynchronize(st));
+    fs.evals += k, fs.launches += 1;
+    return GBK_OK;
+  };
+  auto draw = [&](float* row, const double* blo, const double* bhi) {
+    memcpy(row, base_row, sizeof(float) * GBK_P);
+    for (int a = 0; a < n; ++a) row[free_param[a]] = (float)(blo[a] + (bhi[a] - blo[a]) * rng.uniform());
+  };
+
+  // live points from the whole prior box
+  std::vector<double> plo(lo, lo + n), phi(hi, hi + n);
+  std::vector<float> live((size_t)n_live * GBK_P);
+  std::vector<double> live_lnl(n_live);
+  for (int i = 0; i < n_live; ++i) draw(rows.h + (size_t)i * GBK_P, plo.data(), phi.data());
+  DRV_TRY(evaluate(n_live));
+  memcpy(live.data(), rows.h, sizeof(float) * live.size());
+  for (int i = 0; i < n_live; ++i) live_lnl[i] = isfinite(chi2.h[i]) ? -0.5 * (double)chi2.h[i] : -INFINITY;
+
+  // dead points: ln L, ln w and the free parameters, for the evidence and the posterior mean
+  std::vector<double> dead_lnl, dead_lnw, dead_x;
+  double lnz = -INFINITY;
+  long long n_dead = 0;
+  bool done = false;
+  std::vector<double> blo(n), bhi(n);
+  for (int b = 0; b < max_batches && !done; ++b) {
+    // sampling box: bounding box of the live points, enlarged, clipped to the prior
+    double ln_shrink = 0.0;   // ln(volume of the sampling box / prior volume): bookkeeping only
+    for (int a = 0; a < n; ++a) {
+      double mn = INFINITY, mx = -INFINITY;
+      for (int i = 0; i < n_live; ++i) {
+        const double v = live[(size_t)i * GBK_P + free_param[a]];
+        mn = std::min(mn, v), mx = std::max(mx, v);
+      }
+      const double pad = 0.5 * enlarge * (mx - mn) + 1e-6 * (phi[a] - plo[a]);
+      blo[a] = std::max(plo[a], mn - pad), bhi[a] = std::min(phi[a], mx + pad);
+      ln_shrink += log((bhi[a] - blo[a]) / (phi[a] - plo[a]));
+    }
+    (void)ln_shrink;
+    for (int i = 0; i < batch; ++i) draw(rows.h + (size_t)i * GBK_P, blo.data(), bhi.data());
+    DRV_TRY(evaluate(batch));
+    fs.iterations += 1;
+    for (int i = 0; i < batch && !done; ++i) {
+      const double lnl = isfinite(chi2.h[i]) ? -0.5 * (double)chi2.h[i] : -INFINITY;
+      int worst = 0;
+      for (int j = 1; j < n_live; ++j)
+        if (live_lnl[j] < live_lnl[worst]) worst = j;
+      if (!(lnl > live_lnl[worst])) continue;   // rejected: outside the current iso-likelihood contour
+      // the worst live point dies: X_i = exp(-i / n_live), w_i = X_{i-1} - X_i
+      const double x_prev = -(double)n_dead / n_live, x_now = -(double)(n_dead + 1) / n_live;
+      const double lnw = x_prev + log1p(-exp(x_now - x_prev));
+      dead_lnl.push_back(live_lnl[worst]), dead_lnw.push_back(lnw);
+      for (int a = 0; a < n; ++a) dead_x.push_back(live[(size_t)worst * GBK_P + free_param[a]]);
+      lnz = log_add(lnz, live_lnl[worst] + lnw);
+      ++n_dead;
+      memcpy(&live[(size_t)worst * GBK_P], rows.h + (size_t)i * GBK_P, sizeof(float) * GBK_P);
+      live_lnl[worst] = lnl;
+      const double lmax = *std::max_element(live_lnl.begin(), live_lnl.end());
+      if (lmax + x_now < lnz + log((double)tol)) done = true;   // what is left cannot change Z by > tol
+    }
+  }
+  // the live points share the remaining volume X = exp(-n_dead / n_live)
+  const double ln_rest = -(double)n_dead / n_live - log((double)n_live);
+  for (int i = 0; i < n_live; ++i) {
+    dead_lnl.push_back(live_lnl[i]), dead_lnw.push_back(ln_rest);
+    for (int a = 0; a < n; ++a) dead_x.push_back(live[(size_t)i * GBK_P + free_param[a]]);
+    lnz = log_add(lnz, live_lnl[i] + ln_rest);
+  }
+  int best = 0;
+  for (int j = 1; j < n_live; ++j)
+    if (live_lnl[j] > live_lnl[best]) best = j;
+  memcpy(best_row, &live[(size_t)best * GBK_P], sizeof(float) * GBK_P);
+  *best_chi2 = live_lnl[best] == -INFINITY ? INFINITY : (float)(-2.0 * live_lnl[best]);
+  if (mean_row) {
+    memcpy(mean_row, base_row, sizeof(float) * GBK_P);
+    std::vector<double> acc(n, 0.0);
+    for (size_t i = 0; i < dead_lnl.size(); ++i) {
+      const double w = exp(dead_lnl[i] + dead_lnw[i] - lnz);
+      if (w > 0.0)
+        for (int a = 0; a < n; ++a) acc[a] += w * dead_x[i * n + a];
+    }
+    for (int a = 0; a < n; ++a) mean_row[free_param[a]] = (float)acc[a];
+  }
+  if (log_evidence) *log_evidence = lnz;
+  fs.converged = done ? 1 : 0;
+  fs.ms_total = clock.ms();
+  if (stats) *stats = fs;
+  return GBK_OK;
+}

@@ -88,6 +88,10 @@ double unfused_algorithmic_bytes_per_row(const DevProblem& dp);
 cudaError_t launch_unfused(const DevProblem& dp, const EvalArgs& a, const float* lsf_taps, float* scratch,
                            long long chunk_rows, int sm_count, cudaStream_t st);
 
+// error reporting shared by the translation units (message read by gbk_last_error)
+int fail(int code, const char* fmt, ...);
+void clear_error();
+
 cudaError_t launch_probe(int which, long long iters, int blocks, int threads, float* sink,
                          cudaStream_t st);
 

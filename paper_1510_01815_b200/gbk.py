@@ -56,6 +56,14 @@ class gbk_problem_info(C.Structure):
         ("tiles_y", C.c_int32), ("block_threads", C.c_int32), ("smem_bytes", C.c_int32),
         ("blocks_per_sm", C.c_int32), ("sm_count", C.c_int32),
         ("ext_voxels_per_eval", C.c_int64),
+        ("device", C.c_int32),
+    ]
+
+
+class gbk_fit_stats(C.Structure):
+    _fields_ = [
+        ("evals", C.c_int64), ("launches", C.c_int32), ("iterations", C.c_int32),
+        ("converged", C.c_int32), ("ms_total", C.c_float),
     ]
 
 
@@ -89,6 +97,17 @@ def lib():
         L.gbk_probe_pipe.argtypes = [C.c_int, C.c_int64, C.c_int, C.c_int, vp,
                                      C.POINTER(C.c_double), vp]
         L.gbk_probe_pipe.restype = C.c_int
+        sp = C.POINTER(gbk_fit_stats)
+        L.gbk_fit_ng.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, C.c_int32, vp,
+                                 vp, sp, vp]
+        L.gbk_fit_ng.restype = C.c_int
+        L.gbk_fit_lm.argtypes = [vp, C.c_int32, vp, vp, C.c_int32, vp, vp, vp, C.c_float, C.c_int32,
+                                 C.c_float, vp, vp, vp, sp, vp]
+        L.gbk_fit_lm.restype = C.c_int
+        L.gbk_fit_ns.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, C.c_int32,
+                                 C.c_int32, C.c_float, C.c_float, C.c_uint64, vp, vp, vp,
+                                 C.POINTER(C.c_double), sp, vp]
+        L.gbk_fit_ns.restype = C.c_int
         _lib = L
     return _lib
 
@@ -189,6 +208,69 @@ def gbk_probe_pipe(which: int, iters: int, blocks: int, threads: int, sink, stre
     _check(lib().gbk_probe_pipe(which, iters, blocks, threads, _ptr(sink), C.byref(ops),
                                 stream or None))
     return ops.value
+
+
+def _stats_dict(st: gbk_fit_stats) -> dict:
+    return {k: getattr(st, k) for k, _ in gbk_fit_stats._fields_}
+
+
+def _box(params, lo, hi):
+    idx = np.ascontiguousarray(params, dtype=np.int32)
+    lo = np.ascontiguousarray(lo, dtype=np.float32)
+    hi = np.ascontiguousarray(hi, dtype=np.float32)
+    if not (idx.size == lo.size == hi.size):
+        raise ValueError("params, lo and hi must have the same length")
+    return idx, lo, hi
+
+
+def gbk_fit_ng(handle, base_row, gal, axis_param, axis_lo, axis_hi, nodes, levels, stream=0):
+    """Nested grids (host arrays in, host results out) -> (best_row [P], best_chi2, stats)."""
+    base = _host_f32(base_row, (GBK_P,))
+    idx, lo, hi = _box(axis_param, axis_lo, axis_hi)
+    best = np.empty(GBK_P, np.float32)
+    chi = np.empty(1, np.float32)
+    st = gbk_fit_stats()
+    _check(lib().gbk_fit_ng(handle, _ptr(base), int(gal), idx.size, _ptr(idx), _ptr(lo), _ptr(hi),
+                            int(nodes), int(levels), _ptr(best), _ptr(chi), C.byref(st),
+                            stream or None))
+    return best, float(chi[0]), _stats_dict(st)
+
+
+def gbk_fit_lm(handle, start_rows, gal, free_param, lo, hi, rel_step=1e-3, max_iter=50, ftol=1e-6,
+               stream=0):
+    """Levenberg-Marquardt for n_fits rows at once -> (fit_rows [n, P], chi2 [n], iters [n], stats)."""
+    start = np.ascontiguousarray(start_rows, dtype=np.float32).reshape(-1, GBK_P)
+    n = start.shape[0]
+    g = None if gal is None else np.ascontiguousarray(gal, dtype=np.int32)
+    if g is not None and g.size != n:
+        raise ValueError("gal must have one entry per fit")
+    idx, lo, hi = _box(free_param, lo, hi)
+    rows = np.empty((n, GBK_P), np.float32)
+    chi = np.empty(n, np.float32)
+    iters = np.empty(n, np.int32)
+    st = gbk_fit_stats()
+    _check(lib().gbk_fit_lm(handle, n, _ptr(start), _ptr(g), idx.size, _ptr(idx), _ptr(lo), _ptr(hi),
+                            float(rel_step), int(max_iter), float(ftol), _ptr(rows), _ptr(chi),
+                            _ptr(iters), C.byref(st), stream or None))
+    return rows, chi, iters, _stats_dict(st)
+
+
+def gbk_fit_ns(handle, base_row, gal, free_param, lo, hi, n_live=256, batch=256, max_batches=200,
+               enlarge=0.2, tol=0.01, seed=1, stream=0):
+    """Nested sampling -> dict(best_row, best_chi2, mean_row, log_evidence, stats)."""
+    base = _host_f32(base_row, (GBK_P,))
+    idx, lo, hi = _box(free_param, lo, hi)
+    best = np.empty(GBK_P, np.float32)
+    mean = np.empty(GBK_P, np.float32)
+    chi = np.empty(1, np.float32)
+    lnz = C.c_double()
+    st = gbk_fit_stats()
+    _check(lib().gbk_fit_ns(handle, _ptr(base), int(gal), idx.size, _ptr(idx), _ptr(lo), _ptr(hi),
+                            int(n_live), int(batch), int(max_batches), float(enlarge), float(tol),
+                            int(seed), _ptr(best), _ptr(chi), _ptr(mean), C.byref(lnz), C.byref(st),
+                            stream or None))
+    return dict(best_row=best, best_chi2=float(chi[0]), mean_row=mean, log_evidence=lnz.value,
+                stats=_stats_dict(st))
 
 
 # ------------------------------------------------------------------------ convenience ----

@@ -59,7 +59,7 @@ def test_library_exports_every_declared_symbol(libgbk):
 
 
 def test_binding_struct_layout_follows_the_header(libgbk):
-    for cname in ("gbk_problem_desc", "gbk_problem_info"):
+    for cname in ("gbk_problem_desc", "gbk_problem_info", "gbk_fit_stats"):
         want = _struct_fields(cname)
         got = [f[0] for f in getattr(libgbk, cname)._fields_]
         assert got == want, (cname, got, want)

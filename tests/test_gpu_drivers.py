@@ -1,0 +1,183 @@
+"""The host drivers (gbk_fit_ng / gbk_fit_lm / gbk_fit_ns) on the GPU.
+
+Several optimiser paths are correct, so what is compared is what is unique: the nested-grid path
+is deterministic given the chi^2 values and must equal a replica of rule A19 driven by the same
+chi^2 (gbk_eval_batch, itself parity-checked against the oracle elsewhere); LM and NS must recover
+the parameters of noise-free synthetic data within the thresholds the paper uses for its own mock
+data (Table 3: 1 px, 1 degree, 5 km/s).
+"""
+import numpy as np
+import pytest
+
+from paper_1510_01815_b200 import workloads as wl
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+FREE7 = [wl.IX_XO, wl.IX_YO, wl.IX_PA, wl.IX_INC, wl.IX_VSYS, wl.IX_VT, wl.IX_RT]
+FREE4 = [wl.IX_PA, wl.IX_INC, wl.IX_VT, wl.IX_RT]
+TABLE3 = {wl.IX_XO: 1.0, wl.IX_YO: 1.0, wl.IX_PA: 1.0, wl.IX_INC: 1.0, wl.IX_VSYS: 5.0, wl.IX_VT: 5.0,
+          wl.IX_RT: 1.0}
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu tests need a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gbk():
+    from paper_1510_01815_b200 import gbk as g
+    g.lib()
+    return g
+
+
+def _case(oracle, cfg, true, **scale):
+    w = wl.config(cfg).scaled(noise=0.0, **scale)
+    rng = wl.rng_for(cfg, 7)
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    return w, obs
+
+
+def _true_row(w):
+    t = np.array([0.5 * w.nx + 0.4, 0.5 * w.ny - 0.3, 123.0, 52.0, 8.0, 180.0, 3.5, w.sigma0,
+                  w.r0_lo, 1.0], dtype=np.float32)
+    return t
+
+
+def _pa_diff(a, b):
+    return abs((a - b + 180.0) % 360.0 - 180.0)
+
+
+def test_nested_grids_follow_rule_a19_and_find_the_truth(oracle, torch_cuda, gbk):
+    torch = torch_cuda
+    w0 = wl.config(3).scaled(nx=32, ny=32, nv=48)
+    true = _true_row(w0)
+    w, obs = _case(oracle, 3, true, nx=32, ny=32, nv=48)
+    b = wl.box(w)
+    nodes, levels = 6, 4
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        best, chi, st = gbk.gbk_fit_ng(prob.handle, true, 0, FREE4, b[FREE4, 0], b[FREE4, 1], nodes,
+                                       levels)
+        # replica of A19 in numpy, driven by the same chi^2
+        centre = None
+        for level in range(levels):
+            rows = wl.nested_grid_rows(w, true, level=level, centre=centre, nodes=nodes)
+            out = prob.eval(torch.from_numpy(rows).cuda())
+            k = int(torch.argmin(out["chi2"]).item())
+            centre = rows[k, FREE4].astype(np.float64)
+            chi_rep = float(out["chi2"][k].item())
+    assert st["launches"] == levels and st["evals"] == levels * nodes ** 4 and st["iterations"] == levels
+    np.testing.assert_allclose(best[FREE4], centre, rtol=0, atol=1e-3)
+    assert chi == pytest.approx(chi_rep, rel=1e-6)
+    # the last level's spacing bounds the distance to the truth (noise-free data)
+    h = (b[FREE4, 1] - b[FREE4, 0]) / (nodes * 2 ** (levels - 1))
+    assert _pa_diff(best[wl.IX_PA], true[wl.IX_PA]) <= 1.5 * h[0]
+    for a, j in enumerate(FREE4[1:], start=1):
+        assert abs(best[j] - true[j]) <= 1.5 * h[a], (j, best[j], true[j])
+    assert np.array_equal(np.delete(best, FREE4), np.delete(true, FREE4))
+
+
+def test_levenberg_marquardt_recovers_noise_free_parameters(oracle, torch_cuda, gbk):
+    w0 = wl.config(1)
+    true = _true_row(w0)
+    w, obs = _case(oracle, 1, true)
+    b = wl.box(w)
+    b[wl.IX_PA] = (true[wl.IX_PA] - 90.0, true[wl.IX_PA] + 90.0)    # PA does not wrap in LM
+    rng = wl.rng_for(1, 11)
+    starts = np.repeat(true[None], 4, axis=0).astype(np.float64)
+    width = b[FREE7, 1] - b[FREE7, 0]
+    starts[:, FREE7] += 0.1 * width * rng.uniform(-1, 1, (4, 7))
+    starts[3, wl.IX_INC] = 90.0       # cos i = 0: out of domain, chi^2 = +INF at the start
+    lo, hi = b[FREE7, 0].copy(), b[FREE7, 1].copy()
+    hi[FREE7.index(wl.IX_INC)] = 90.0
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        rows, chi, iters, st = gbk.gbk_fit_lm(prob.handle, starts, None, FREE7, lo, hi,
+                                              rel_step=1e-3, max_iter=50, ftol=1e-6)
+    assert np.isinf(chi[3]) and iters[3] == 0
+    np.testing.assert_array_equal(rows[3], starts[3].astype(np.float32))
+    for f in range(3):
+        assert np.isfinite(chi[f]) and chi[f] < 1.0, (f, chi[f])     # noise-free: chi^2 -> 0
+        for j in FREE7:
+            d = _pa_diff(rows[f, j], true[j]) if j == wl.IX_PA else abs(rows[f, j] - true[j])
+            assert d <= TABLE3[j], (f, j, rows[f, j], true[j])
+        assert 1 <= iters[f] <= 50
+    assert st["converged"] >= 3 and st["launches"] >= 2 and st["evals"] > 0
+
+
+def test_levenberg_marquardt_mixed_galaxies(oracle, torch_cuda, gbk):
+    """Config-5 style: several galaxies, each its own data set and PSF, fitted in one call."""
+    w = wl.config(5).scaled(nx=24, ny=24, nv=64, n_gal=3)
+    rng = wl.rng_for(5, 3)
+    fw = np.array([1.6, 2.4, 3.3], np.float32)
+    trues, maps = [], []
+    for g in range(3):
+        t = _true_row(w)
+        t[[wl.IX_PA, wl.IX_INC, wl.IX_VT]] += (40.0 * g, 6.0 * g, -30.0 * g)
+        t[wl.IX_R0] = 5.0 + g
+        trues.append(t)
+        grid = pu.oracle_grid(oracle, w, fwhm=float(fw[g]))
+        maps.append(oracle.model_maps(grid, t.astype(np.float64)))
+    m0, m1, m2 = (np.stack([m[i] for m in maps]) for i in range(3))
+    obs = wl.observe(w, m0, m1, m2, rng)
+    trues = np.stack(trues)
+    b = wl.box(w)
+    starts = trues.astype(np.float64)
+    starts[:, FREE7] += 0.05 * (b[FREE7, 1] - b[FREE7, 0]) * rng.uniform(-1, 1, (3, 7))
+    lo, hi = b[FREE7, 0].copy(), b[FREE7, 1].copy()
+    lo[2], hi[2] = -360.0, 720.0
+    with gbk.Problem(**pu.gbk_desc(w, obs, fwhms=fw)) as prob:
+        rows, chi, iters, st = gbk.gbk_fit_lm(prob.handle, starts, np.arange(3), FREE7, lo, hi)
+        gi = torch_cuda.arange(3, dtype=torch_cuda.int32, device="cuda")
+        chi_true = prob.eval(torch_cuda.from_numpy(trues).cuda(), gi)["chi2"].cpu().numpy()
+        chi_fit = prob.eval(torch_cuda.from_numpy(rows).cuda(), gi)["chi2"].cpu().numpy()
+    # config 5 draws noise N(0, E) with per-spaxel errors: the fit must do at least as well as the
+    # truth on the noisy data, report the chi^2 of the row it returns, and stay near the truth
+    np.testing.assert_allclose(chi, chi_fit, rtol=1e-6)
+    for f in range(3):
+        assert chi[f] <= chi_true[f] * (1.0 + 1e-4), (f, chi[f], chi_true[f])
+        for j in FREE7:
+            d = _pa_diff(rows[f, j], trues[f, j]) if j == wl.IX_PA else abs(rows[f, j] - trues[f, j])
+            assert d <= 3.0 * TABLE3[j], (f, j, rows[f, j], trues[f, j])
+
+
+def test_nested_sampling_finds_the_mode(oracle, torch_cuda, gbk):
+    w0 = wl.config(1)
+    true = _true_row(w0)
+    w, obs = _case(oracle, 1, true)
+    b = wl.box(w)
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        r = gbk.gbk_fit_ns(prob.handle, true, 0, FREE4, b[FREE4, 0], b[FREE4, 1], n_live=200,
+                           batch=1024, max_batches=150, enlarge=0.3, tol=0.01, seed=20151001)
+        r2 = gbk.gbk_fit_ns(prob.handle, true, 0, FREE4, b[FREE4, 0], b[FREE4, 1], n_live=200,
+                            batch=1024, max_batches=150, enlarge=0.3, tol=0.01, seed=20151001)
+    assert np.isfinite(r["log_evidence"]) and np.isfinite(r["best_chi2"])
+    assert r["stats"]["evals"] >= 200 and r["stats"]["launches"] == r["stats"]["iterations"] + 1
+    for row in (r["best_row"], r["mean_row"]):
+        assert _pa_diff(row[wl.IX_PA], true[wl.IX_PA]) <= 2.0
+        assert abs(row[wl.IX_INC] - true[wl.IX_INC]) <= 2.0
+        assert abs(row[wl.IX_VT] - true[wl.IX_VT]) <= 10.0
+        assert abs(row[wl.IX_RT] - true[wl.IX_RT]) <= 1.0
+    # same seed, same path (the kernels are bit-reproducible)
+    assert r2["log_evidence"] == r["log_evidence"] and np.array_equal(r2["best_row"], r["best_row"])
+
+
+def test_driver_argument_errors(oracle, torch_cuda, gbk):
+    w0 = wl.config(1)
+    true = _true_row(w0)
+    w, obs = _case(oracle, 1, true)
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        for call in (
+            lambda: gbk.gbk_fit_ng(prob.handle, true, 0, [2, 2], [0, 0], [1, 1], 4, 2),       # twice
+            lambda: gbk.gbk_fit_ng(prob.handle, true, 0, [2], [1.0], [1.0], 4, 2),            # empty box
+            lambda: gbk.gbk_fit_ng(prob.handle, true, 5, [2], [0.0], [1.0], 4, 2),            # gal
+            lambda: gbk.gbk_fit_lm(prob.handle, true[None], None, [11], [0.0], [1.0]),        # index
+            lambda: gbk.gbk_fit_ns(prob.handle, true, 0, [2], [0.0], [1.0], n_live=1),
+        ):
+            with pytest.raises(gbk.GbkError) as ei:
+                call()
+            assert ei.value.code == gbk.GBK_ERR_ARG
