@@ -340,6 +340,7 @@ def run_ours(args, ranks) -> None:
         cpu = time_oracle(cfg, args.cpu_rows or 32 * cores, 1, 1, cores)
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
 
+    fits = time_fits(gbk, torch, prob, w, true) if (ranks.is_main and cfg == 3 and not args.no_fits) else None
     if ranks.is_main:
         core_vox = w.nx * w.ny * w.nv * w.u * w.u
         line = {
@@ -359,9 +360,43 @@ def run_ours(args, ranks) -> None:
                     "d2h_bytes_per_step": K * 4, "matches_device_path": same},
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "checksum": checksum,
+            "fits": fits,
         }
         print(json.dumps(line), flush=True)
     prob.close()
+
+
+def time_fits(gbk, torch, prob3, w3, true3) -> dict:
+    """Wall time to a converged fit through the host drivers (outside the timed region; rank 0):
+    nested grids on the config-3 problem (4 levels x 8^4 rows) and LM on a config-2
+    problem (64x64x128, u=2, 7 free parameters, K=8 per iteration)."""
+    out = {}
+    b = wl.box(w3)
+    free4 = [wl.IX_PA, wl.IX_INC, wl.IX_VT, wl.IX_RT]
+    gbk.gbk_fit_ng(prob3.handle, true3, 0, free4, b[free4, 0], b[free4, 1], 8, 4)      # warm-up
+    best, chi, st = gbk.gbk_fit_ng(prob3.handle, true3, 0, free4, b[free4, 0], b[free4, 1], 8, 4)
+    out["ng_cfg3"] = {"ms": st["ms_total"], "evals": st["evals"], "levels": st["iterations"],
+                      "chi2": chi, "abs_err": [float(abs(best[j] - true3[j])) for j in free4]}
+    w2 = wl.config(2)
+    rng = wl.rng_for(2, 200)
+    true2 = wl.draw_rows(w2, rng, 1)[0]
+    obs2 = observation_from_gpu(gbk, torch, w2, true2, rng)
+    b2 = wl.box(w2)
+    free7 = [wl.IX_XO, wl.IX_YO, wl.IX_PA, wl.IX_INC, wl.IX_VSYS, wl.IX_VT, wl.IX_RT]
+    lo, hi = b2[free7, 0].copy(), b2[free7, 1].copy()
+    lo[2], hi[2] = -360.0, 720.0                      # PA is periodic: no wall for LM
+    start = true2.astype(np.float64)
+    start[free7] += 0.1 * (b2[free7, 1] - b2[free7, 0]) * rng.uniform(-1, 1, 7)
+    start[wl.IX_INC] = np.clip(start[wl.IX_INC], 20.0, 80.0)
+    start[wl.IX_RT] = np.clip(start[wl.IX_RT], 1.0, 8.0)
+    with gbk.Problem(**desc_for(w2, obs2)) as prob2:
+        gbk.gbk_fit_lm(prob2.handle, start, None, free7, lo, hi, max_iter=2)             # warm-up
+        rows, chi2, iters, st = gbk.gbk_fit_lm(prob2.handle, start, None, free7, lo, hi,
+                                               rel_step=1e-3, max_iter=50, ftol=1e-6)
+    out["lm_cfg2"] = {"ms": st["ms_total"], "evals": st["evals"], "iterations": int(iters[0]),
+                      "converged": st["converged"], "chi2": float(chi2[0]),
+                      "abs_err": [float(abs(rows[0, j] - true2[j])) for j in free7]}
+    return out
 
 
 def _chi2_of(gbk, prob, params, K, torch):
@@ -381,6 +416,7 @@ def main() -> None:
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the cpu_baseline sample")
     ap.add_argument("--ref-rows", type=int, default=0, help="rows per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fits", action="store_true", help="skip the wall-time-to-fit legs")
     args = ap.parse_args()
     from paper_1510_01815_b200 import dist
     if args.impl == "reference":
