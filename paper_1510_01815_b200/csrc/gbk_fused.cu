@@ -36,6 +36,7 @@ namespace {
 
 constexpr int kMaxThreads = 256;
 constexpr int kMinBlocks = 3;
+constexpr int kVBlockX = 4;      // output rows per thread in the x-packed vertical pass (divides kVBlock)
 constexpr int kPairs = 2;        // pixel pairs per lane in the voxel loop (4 pixels per thread)
 
 typedef unsigned long long u64;  // two packed floats {lo, hi}
@@ -316,6 +317,121 @@ __device__ __forceinline__ void vpass_inplace(float* maps, int map_stride, int e
   }
 }
 
+// ---- x-packed passes (the fast path) -----------------------------------------------------
+// Both passes keep two horizontally adjacent pixels in one 64-bit register pair and multiply by a
+// broadcast tap pair (t, t), so every FFMA2 does two useful FMAs and no instruction is spent on
+// building broadcast inputs.  Symmetric taps: only R + 1 tap pairs live in registers.
+template <int R>
+__device__ __forceinline__ void load_tap_bcast(const float* taps, u64 (&tb)[R + 1]) {
+#pragma unroll
+  for (int i = 0; i <= R; ++i) tb[i] = pk1(taps[i]);
+}
+template <int R>
+__device__ __forceinline__ u64 tap_sym(const u64 (&tb)[R + 1], int j) {   // j in [0, 2R]
+  return tb[j <= R ? j : 2 * R - j];
+}
+
+// Horizontal pass, in place.  A row of one map is owned by a group of lanes of one warp (each lane
+// 4 consecutive outputs), which loads everything it needs before it stores.
+template <int R>
+__device__ __forceinline__ void hpass_x(float* maps, int map_stride, int ews, int EH, int tw,
+                                        const u64 (&tb)[R + 1], int tid, int nthreads) {
+  constexpr int NV4 = (4 + 2 * R + 3) / 4;
+  const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+  const int nx4 = (tw + 3) >> 2;
+  int lpr_log = 0;
+  while ((1 << lpr_log) < nx4 && lpr_log < 5) ++lpr_log;
+  const int lpr = 1 << lpr_log;                 // lanes per row
+  const int rpp = 32 >> lpr_log;                // rows per pass
+  const int l = lane & (lpr - 1), rsub = lane >> lpr_log;
+  const int nchunks = (nx4 + lpr - 1) >> lpr_log;
+  const int npass = (EH + rpp - 1) / rpp;
+  for (int job = warp; job < npass; job += nwarps) {
+    const int row = job * rpp + rsub;
+    for (int chunk = 0; chunk < nchunks; ++chunk) {
+      const int x0 = ((chunk << lpr_log) + l) << 2;
+      const bool active = row < EH && x0 < tw;
+      float* rowp = maps + row * ews + x0;
+      float4 res[3];
+      if (active) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+          float v[NV4 * 4];
+#pragma unroll
+          for (int i = 0; i < NV4; ++i) {
+            const float4 f = *reinterpret_cast<const float4*>(rowp + q * map_stride + 4 * i);
+            v[4 * i] = f.x, v[4 * i + 1] = f.y, v[4 * i + 2] = f.z, v[4 * i + 3] = f.w;
+          }
+          u64 o0 = pk(0.f, 0.f), o1 = o0;
+#pragma unroll
+          for (int j = 0; j <= 2 * R; ++j) {
+            o0 = fma2(tap_sym<R>(tb, j), pk(v[j], v[j + 1]), o0);
+            o1 = fma2(tap_sym<R>(tb, j), pk(v[j + 2], v[j + 3]), o1);
+          }
+          upk(o0, res[q].x, res[q].y);
+          upk(o1, res[q].z, res[q].w);
+        }
+      }
+      __syncwarp();
+      if (active) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) *reinterpret_cast<float4*>(rowp + q * map_stride) = res[q];
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// Vertical pass fused with moments and chi^2 (u == 1): a thread owns BY consecutive rows of a
+// column PAIR; lanes run along x, so the 8-byte shared-memory reads are conflict-free and the
+// global accesses coalesced.  Rows past the tile are read from the (allocated, possibly
+// uninitialised) padding of the plane and only feed outputs that are discarded; likewise the
+// second column of the last pair when the tile width is odd.
+template <int R, int BY, bool OUT>
+__device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const EvalArgs& a,
+                                                 const RowConst& rc, long long k, const float* maps,
+                                                 int map_stride, int ews, int tw, int th, int tx0,
+                                                 int ty0, const u64 (&tb)[R + 1], int tid,
+                                                 int nthreads) {
+  const int nxp = (tw + 1) >> 1, nyb = (th + BY - 1) / BY;
+  const unsigned magic = 0xFFFFFFFFu / (unsigned)nxp + 1u;
+  float chi = 0.0f;
+  for (int item = tid; item < nxp * nyb; item += nthreads) {
+    const int yb = (int)__umulhi((unsigned)item, magic), x = (item - yb * nxp) << 1, y0 = yb * BY;
+    u64 res[3][BY];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const float* col = maps + q * map_stride + y0 * ews + x;
+#pragma unroll
+      for (int m = 0; m < BY; ++m) res[q][m] = pk(0.f, 0.f);
+#pragma unroll
+      for (int i = 0; i < BY + 2 * R; ++i) {
+        const u64 v = *reinterpret_cast<const u64*>(col + i * ews);
+#pragma unroll
+        for (int m = 0; m < BY; ++m) {
+          const int ti = i - m;
+          if (ti >= 0 && ti <= 2 * R) res[q][m] = fma2(tap_sym<R>(tb, ti), v, res[q][m]);
+        }
+      }
+    }
+    const int pix0 = (ty0 + y0) * dp.nx + tx0 + x;
+    const bool second = x + 1 < tw;
+#pragma unroll
+    for (int m = 0; m < BY; ++m)
+      if (y0 + m < th) {
+        const int pix = pix0 + m * dp.nx;
+        float s0a, s0b, s1a, s1b, s2a, s2b;
+        upk(res[0][m], s0a, s0b);
+        upk(res[1][m], s1a, s1b);
+        upk(res[2][m], s2a, s2b);
+        chi += spaxel_finish<OUT>(dp, a, rc, k, pix, load_obs(dp, rc, pix), s0a, s1a, s2a);
+        if (second)
+          chi += spaxel_finish<OUT>(dp, a, rc, k, pix + 1, load_obs(dp, rc, pix + 1), s0b, s1b, s2b);
+      }
+  }
+  return chi;
+}
+
 // a6 + a7/a8 for u > 1 after both in-place passes: block sums over u x u fine pixels.
 template <bool OUT>
 __device__ __forceinline__ float moments_blocks(const DevProblem& dp, const EvalArgs& a,
@@ -373,13 +489,18 @@ __device__ __noinline__ float separable_phase(const DevProblem& dp, const EvalAr
                                               const RowConst& rc, long long k, float* maps,
                                               int map_stride, int EH, int tw, int th, int tx0,
                                               int ty0, const float* taps, int tid, int nthreads) {
+  if (dp.u == 1) {
+    u64 tb[R + 1];
+    load_tap_bcast<R>(taps, tb);
+    hpass_x<R>(maps, map_stride, dp.ews, EH, tw, tb, tid, nthreads);
+    __syncthreads();
+    return vpass_x_moments<R, kVBlockX, OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0,
+                                             tb, tid, nthreads);
+  }
   u64 tp[2 * R + 2];
   load_tap_pairs<R>(taps, tp);
   hpass<R>(maps, map_stride, dp.ews, EH, tw, tp, tid, nthreads);
   __syncthreads();
-  if (dp.u == 1)
-    return vpass_moments<R, OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0, tp, tid,
-                                 nthreads);
   vpass_inplace<R>(maps, map_stride, dp.ews, tw, th, tp, tid, nthreads);
   __syncthreads();
   return moments_blocks<OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0, tid, nthreads);
