@@ -70,6 +70,11 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ float sqrt_approx(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ float rcp_approx(float x) {
   float y;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -153,17 +158,18 @@ template <bool OUT>
 __device__ __forceinline__ float spaxel_finish(const DevProblem& dp, const EvalArgs& a,
                                                const RowConst& rc, long long k, int pix,
                                                const float4 ob, float S0, float S1, float S2) {
-  const float inv = rcp_approx(S0);
+  // A model-dark spaxel (S0 below the threshold, or not a number) poisons the moments with NaN,
+  // so the one test "contrib < inf" below catches dark, NaN and overflowing spaxels alike.
+  const bool dark = !(S0 >= rc.dark_s0);
+  const float inv = dark ? f_nan() : rcp_approx(S0);
   float m1r = S1 * inv;
   const float var = fmaf(-m1r, m1r, S2 * inv);
-  float m2 = var > 1e-30f ? var * rsqrt_approx(var) : 0.0f;   // sqrt(max(var, 0)); no denormal * inf
-  if (var != var) m2 = var;                                     // keep a NaN visible
-  const bool dark = !(S0 >= rc.dark_s0);
+  float m2 = sqrt_approx(fmaxf(var, 0.0f));                     // fmaxf drops a NaN var: m1r carries it
   const bool unmasked = ob.y > 0.0f;
   float t = (m1r - ob.x) * ob.y;
   float s = (m2 - ob.z) * ob.w;
   float contrib = fmaf(t, t, s * s);
-  const bool bad = dark || !(contrib < f_inf());                // NaN or Inf moments
+  const bool bad = !(contrib < f_inf());                        // NaN or Inf moments
   contrib = unmasked ? (bad ? f_inf() : contrib) : 0.0f;
   if (OUT) {
     if (dark) m1r = m2 = f_nan();
@@ -265,37 +271,6 @@ __device__ __forceinline__ void vcolumn(const float* col, int ews, const u64 (&t
   }
 #pragma unroll
   for (int m = 0; m < BY / 2; ++m) upk(acc[m], res[2 * m], res[2 * m + 1]);
-}
-
-// Vertical pass fused with moments and chi^2 (u == 1): a thread owns kVBlock consecutive rows of
-// one column; lanes run along x, so shared-memory reads are conflict-free and global accesses
-// coalesced.  Rows past the tile are read from the (allocated, possibly uninitialised) padding of
-// the plane and only feed outputs that are discarded.
-template <int R, bool OUT>
-__device__ __forceinline__ float vpass_moments(const DevProblem& dp, const EvalArgs& a,
-                                               const RowConst& rc, long long k, const float* maps,
-                                               int map_stride, int ews, int tw, int th, int tx0,
-                                               int ty0, const u64 (&tp)[2 * R + 2], int tid,
-                                               int nthreads) {
-  constexpr int BY = kVBlock;
-  const int nyb = (th + BY - 1) / BY;
-  const unsigned magic = 0xFFFFFFFFu / (unsigned)tw + 1u;
-  float chi = 0.0f;
-  for (int item = tid; item < tw * nyb; item += nthreads) {
-    const int yb = (int)__umulhi((unsigned)item, magic), x = item - yb * tw, y0 = yb * BY;
-    float res[3][BY];
-#pragma unroll
-    for (int q = 0; q < 3; ++q) vcolumn<R>(maps + q * map_stride + y0 * ews + x, ews, tp, res[q]);
-    const int pix0 = (ty0 + y0) * dp.nx + tx0 + x;
-#pragma unroll
-    for (int o = 0; o < BY; ++o)
-      if (y0 + o < th) {
-        const int pix = pix0 + o * dp.nx;
-        chi += spaxel_finish<OUT>(dp, a, rc, k, pix, load_obs(dp, rc, pix), res[0][o], res[1][o],
-                                  res[2][o]);
-      }
-  }
-  return chi;
 }
 
 // Vertical pass in place (u > 1): a thread owns one column of one map and walks it top to bottom
@@ -406,7 +381,8 @@ __device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const Eva
       for (int m = 0; m < BY; ++m) res[q][m] = pk(0.f, 0.f);
 #pragma unroll
       for (int i = 0; i < BY + 2 * R; ++i) {
-        const u64 v = *reinterpret_cast<const u64*>(col + i * ews);
+        const u64 v = *reinterpret_cast<const u64*>(col);
+        col += ews;
 #pragma unroll
         for (int m = 0; m < BY; ++m) {
           const int ti = i - m;
