@@ -308,8 +308,10 @@ def run_ours(args, ranks) -> None:
     nvx = info.nv + 2 * info.r_v
     ext_samples = info.ext_voxels_per_eval // nvx
     mufu_per_eval = info.ext_voxels_per_eval + 3 * ext_samples
+    taps = 2 * info.r_p_max + 1
+    psf_fma = (taps * taps if w.psf_kind == wl.PSF_IMAGE else 2 * taps)       # per map and fine pixel
     fp32_per_eval = 5 * info.ext_voxels_per_eval + 45 * ext_samples \
-        + 3 * 2 * (2 * info.r_p_max + 1) * (info.u * info.nx) * (info.u * info.ny) + 12 * info.nx * info.ny
+        + 3 * psf_fma * (info.u * info.nx) * (info.u * info.ny) + 12 * info.nx * info.ny
     sm_max = (clocks.get("sm_max_mhz") or 1965.0)
     # The voxel loop evaluates the Gaussian line by its multiplicative recurrence along v (two FP32
     # multiplies per voxel, one MUFU.EX2 pair per kChanBlock channels), so the binding pipe is the
@@ -323,7 +325,7 @@ def run_ours(args, ranks) -> None:
                 "traffic": None,
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
                 "ops_per_eval": int(fp32_per_eval),
-                "ops_how": "algorithmic FP32 lane-ops: 5/ext voxel + 45/ext sample + 3 maps x 2 passes x taps/fine pixel + 12/spaxel",
+                "ops_how": "algorithmic FP32 lane-ops: 5/ext voxel + 45/ext sample + 3 maps x (2 x taps separable | taps^2 image)/fine pixel + 12/spaxel",
                 "mufu_ops_per_eval_direct": int(mufu_per_eval),
                 "mufu_frac_if_direct": mufu_per_eval * K * args.steps / sec_rank / 1e9 / peak_mufu,
                 "kernel_ms_avg": statistics.mean(ms), "kernel_ms_min": min(ms)}

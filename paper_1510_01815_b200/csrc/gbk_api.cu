@@ -240,6 +240,16 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     dp.ntiles = dp.tiles_x * dp.tiles_y;
     dp.ews = round_up4(dp.tile_w) + 4 * ((2 * r_p_max + 4 + 3) / 4) - 4;
     dp.ehs = (dp.tile_h + kVBlock - 1) / kVBlock * kVBlock + 2 * r_p_max;  // the vertical pass reads whole blocks
+    dp.img_fast = d->psf_kind == GBK_PSF_IMAGE && d->psf_n <= kMaxFastPsfN ? 1 : 0;
+    dp.spare_plane = 0;
+    if (dp.img_fast) {
+      // the 2-D pass reads 8-pixel chunks plus the kernel width as float4s, with lanes along y:
+      // a row stride = 4 (mod 8) floats keeps those 16-byte reads free of bank conflicts
+      const int nxc = (dp.tile_w + 7) / 8, nv4 = (8 + 2 * r_p_max + 3) / 4;
+      dp.ews = std::max(dp.ews, 8 * nxc - 8 + 4 * nv4);
+      while (dp.ews % 8 != 4) ++dp.ews;
+      dp.spare_plane = dp.tile_h * dp.ews;
+    }
     return fused_smem_bytes(dp);
   };
   int tws = d->tile_w > 0 ? std::min(d->tile_w, d->nx) : d->nx;

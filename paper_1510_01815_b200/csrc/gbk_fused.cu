@@ -85,8 +85,14 @@ __host__ __device__ __forceinline__ int round_up4(int v) { return (v + 3) & ~3; 
 __device__ __forceinline__ float f_inf() { return __int_as_float(0x7f800000); }
 __device__ __forceinline__ float f_nan() { return __int_as_float(0x7fc00000); }
 
+// floats of the PSF tap area: image taps of the register-tiled pass are stored as (w, w) pairs
+__host__ __device__ __forceinline__ int taps_floats(const DevProblem& dp) {
+  return round_up4(dp.psf_stride) * (dp.img_fast ? 2 : 1);
+}
+
 struct Smem {
   float* maps;      // 3 x ehs x ews
+  float* spare;     // tile_h x ews (register-tiled image-PSF pass only)
   float4* chan;     // nvx
   float* taps;      // round_up4(psf_stride)
   RowConst* rc;
@@ -96,9 +102,10 @@ struct Smem {
 __device__ __forceinline__ Smem carve(const DevProblem& dp, unsigned char* raw) {
   Smem s;
   s.maps = reinterpret_cast<float*>(raw);
-  s.chan = reinterpret_cast<float4*>(s.maps + 3 * dp.ehs * dp.ews);
+  s.spare = s.maps + 3 * dp.ehs * dp.ews;
+  s.chan = reinterpret_cast<float4*>(s.spare + dp.spare_plane);
   s.taps = reinterpret_cast<float*>(s.chan + dp.nvx_pad);
-  s.rc = reinterpret_cast<RowConst*>(s.taps + round_up4(dp.psf_stride));
+  s.rc = reinterpret_cast<RowConst*>(s.taps + taps_floats(dp));
   s.red = reinterpret_cast<float*>(s.rc + 1);
   return s;
 }
@@ -411,9 +418,10 @@ __device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const Eva
 // a6 + a7/a8 for u > 1 after both in-place passes: block sums over u x u fine pixels.
 template <bool OUT>
 __device__ __forceinline__ float moments_blocks(const DevProblem& dp, const EvalArgs& a,
-                                                const RowConst& rc, long long k, const float* maps,
-                                                int map_stride, int ews, int tw, int th, int tx0,
-                                                int ty0, int tid, int nthreads) {
+                                                const RowConst& rc, long long k, const float* p0,
+                                                const float* p1, const float* p2, int ews, int tw,
+                                                int th, int tx0, int ty0, int tid, int nthreads) {
+  const float* const plane[3] = {p0, p1, p2};
   const int u = dp.u, sw = tw / u, sh = th / u;
   float chi = 0.0f;
   for (int item = tid; item < sw * sh; item += nthreads) {
@@ -423,7 +431,7 @@ __device__ __forceinline__ float moments_blocks(const DevProblem& dp, const Eval
     float s[3] = {0.f, 0.f, 0.f};
     for (int q = 0; q < 3; ++q)
       for (int dy = 0; dy < u; ++dy)
-        for (int dx = 0; dx < u; ++dx) s[q] += maps[q * map_stride + (Y * u + dy) * ews + X * u + dx];
+        for (int dx = 0; dx < u; ++dx) s[q] += plane[q][(Y * u + dy) * ews + X * u + dx];
     chi += spaxel_finish<OUT>(dp, a, rc, k, pix, ob, s[0], s[1], s[2]);
   }
   return chi;
@@ -460,6 +468,81 @@ __device__ __noinline__ float conv2d_moments(const DevProblem& dp, const EvalArg
   return chi;
 }
 
+// Register-tiled general 2-D PSF (image side N <= kMaxFastPsfN): out[y][x] = sum_ky sum_kx
+// W[ky][kx] in[y + ky][x + kx] with W the flipped image (true convolution).  A thread produces an
+// 8-pixel chunk of two rows (y and y + th/2): per kernel row it holds the N taps as (w, w) pairs
+// (one 8-byte broadcast read each) and applies them to the two input rows (float4 reads; lanes run
+// along y and the row stride is 4 mod 8 floats, so they are conflict-free), i.e. 8 N FFMA2 for
+// N + 2 NV4 shared-memory reads.  `out` is a different plane than `in`.
+template <int N>
+__device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ews, int tw, int th,
+                                             const u64* w64, int tid, int nthreads) {
+  constexpr int NV4 = (8 + N - 1 + 3) / 4;
+  const int nxc = (tw + 7) >> 3, half = (th + 1) >> 1;
+  const unsigned magic = 0xFFFFFFFFu / (unsigned)half + 1u;
+  for (int item = tid; item < nxc * half; item += nthreads) {
+    const int xc = (int)__umulhi((unsigned)item, magic), l = item - xc * half;
+    const bool two = l + half < th;
+    const int yy[2] = {l, two ? l + half : l};
+    u64 acc[2][4];
+#pragma unroll
+    for (int m = 0; m < 2; ++m)
+#pragma unroll
+      for (int p = 0; p < 4; ++p) acc[m][p] = pk(0.f, 0.f);
+#pragma unroll 1
+    for (int ky = 0; ky < N; ++ky) {
+      u64 w[N];
+#pragma unroll
+      for (int kx = 0; kx < N; ++kx) w[kx] = w64[ky * N + kx];
+#pragma unroll
+      for (int m = 0; m < 2; ++m) {
+        const float* rowp = in + (yy[m] + ky) * ews + (xc << 3);
+        float v[NV4 * 4];
+#pragma unroll
+        for (int i = 0; i < NV4; ++i) {
+          const float4 f = *reinterpret_cast<const float4*>(rowp + 4 * i);
+          v[4 * i] = f.x, v[4 * i + 1] = f.y, v[4 * i + 2] = f.z, v[4 * i + 3] = f.w;
+        }
+#pragma unroll
+        for (int kx = 0; kx < N; ++kx)
+#pragma unroll
+          for (int p = 0; p < 4; ++p)
+            acc[m][p] = fma2(w[kx], pk(v[kx + 2 * p], v[kx + 2 * p + 1]), acc[m][p]);
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < 2; ++m)
+      if (m == 0 || two) {
+        float4 f0, f1;
+        upk(acc[m][0], f0.x, f0.y);
+        upk(acc[m][1], f0.z, f0.w);
+        upk(acc[m][2], f1.x, f1.y);
+        upk(acc[m][3], f1.z, f1.w);
+        float* o = out + yy[m] * ews + (xc << 3);
+        *reinterpret_cast<float4*>(o) = f0;
+        *reinterpret_cast<float4*>(o + 4) = f1;
+      }
+  }
+}
+
+// a5..a9 for an image PSF on the fast path: the three maps are convolved plane by plane, each into
+// a plane that is free by then (S0 -> spare, S1 -> plane 0, S2 -> plane 1), then block sums.
+template <int N, bool OUT>
+__device__ __noinline__ float image_phase(const DevProblem& dp, const EvalArgs& a, const RowConst& rc,
+                                          long long k, float* maps, float* spare, int map_stride, int tw,
+                                          int th, int tx0, int ty0, const float* taps, int tid,
+                                          int nthreads) {
+  const u64* w64 = reinterpret_cast<const u64*>(taps);
+  conv2d_plane<N>(maps, spare, dp.ews, tw, th, w64, tid, nthreads);
+  __syncthreads();
+  conv2d_plane<N>(maps + map_stride, maps, dp.ews, tw, th, w64, tid, nthreads);
+  __syncthreads();
+  conv2d_plane<N>(maps + 2 * map_stride, maps + map_stride, dp.ews, tw, th, w64, tid, nthreads);
+  __syncthreads();
+  return moments_blocks<OUT>(dp, a, rc, k, spare, maps, maps + map_stride, dp.ews, tw, th, tx0, ty0, tid,
+                             nthreads);
+}
+
 template <int R, bool OUT>
 __device__ __noinline__ float separable_phase(const DevProblem& dp, const EvalArgs& a,
                                               const RowConst& rc, long long k, float* maps,
@@ -479,7 +562,8 @@ __device__ __noinline__ float separable_phase(const DevProblem& dp, const EvalAr
   __syncthreads();
   vpass_inplace<R>(maps, map_stride, dp.ews, tw, th, tp, tid, nthreads);
   __syncthreads();
-  return moments_blocks<OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0, tid, nthreads);
+  return moments_blocks<OUT>(dp, a, rc, k, maps, maps + map_stride, maps + 2 * map_stride, dp.ews, tw, th,
+                             tx0, ty0, tid, nthreads);
 }
 
 // ------------------------------------------------------------------------ a2, a3, a4 --------
@@ -650,8 +734,13 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   for (int c = tid; c < dp.nvx_pad; c += nthreads) sm.chan[c] = dp.chan_tab[c];
   __syncthreads();
   const RowConst rc = *sm.rc;   // by value: registers, no aliasing with the map stores
-  for (int j = tid; j < dp.psf_stride; j += nthreads)
-    sm.taps[j] = dp.psf_taps[(size_t)rc.psf_set * dp.psf_stride + j];
+  for (int j = tid; j < dp.psf_stride; j += nthreads) {
+    const float t = dp.psf_taps[(size_t)rc.psf_set * dp.psf_stride + j];
+    if (dp.img_fast)
+      reinterpret_cast<u64*>(sm.taps)[j] = pk1(t);
+    else
+      sm.taps[j] = t;
+  }
 
   float chi = 0.0f;
   if (!rc.valid) {
@@ -674,7 +763,19 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     voxel_phase(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads);
     __syncthreads();
     // ------------------------------------------------------------------ a5 .. a9 ---------
-    if (dp.psf_kind == GBK_PSF_IMAGE) {
+    if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {
+#define GBK_IMG_CASE(NN)                                                                          \
+  case NN:                                                                                        \
+    chi = image_phase<NN, OUT>(dp, a, rc, k, sm.maps, sm.spare, map_stride, tw, th, tx0, ty0,     \
+                               sm.taps, tid, nthreads);                                           \
+    break;
+      switch (2 * R + 1) {
+        GBK_IMG_CASE(1) GBK_IMG_CASE(3) GBK_IMG_CASE(5) GBK_IMG_CASE(7) GBK_IMG_CASE(9)
+        GBK_IMG_CASE(11) GBK_IMG_CASE(13) GBK_IMG_CASE(15)
+        default: break;
+      }
+#undef GBK_IMG_CASE
+    } else if (dp.psf_kind == GBK_PSF_IMAGE) {
       chi = conv2d_moments<OUT>(dp, a, rc, k, sm.maps, map_stride, dp.ews, tw, th, tx0, ty0, sm.taps,
                                 tid, nthreads);
     } else {
@@ -723,8 +824,8 @@ __global__ void finish_kernel(const float* __restrict__ partial, int ntiles, lon
 }  // namespace
 
 size_t fused_smem_bytes(const DevProblem& dp) {
-  return sizeof(float) * 3 * (size_t)dp.ehs * dp.ews + sizeof(float4) * dp.nvx_pad +
-         sizeof(float) * round_up4(dp.psf_stride) + sizeof(RowConst) + sizeof(float) * 32;
+  return sizeof(float) * (3 * (size_t)dp.ehs * dp.ews + dp.spare_plane) + sizeof(float4) * dp.nvx_pad +
+         sizeof(float) * taps_floats(dp) + sizeof(RowConst) + sizeof(float) * 32;
 }
 
 cudaError_t fused_prepare(const FusedLaunch& fl) {

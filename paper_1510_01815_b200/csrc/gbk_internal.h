@@ -10,6 +10,7 @@ namespace gbk {
 
 constexpr int kMaxSepR = 16;    // largest separable (Gaussian) PSF tap radius, fine pixels
 constexpr int kMaxPsfN = 33;    // largest PSF image side
+constexpr int kMaxFastPsfN = 15; // largest PSF image side of the register-tiled 2-D pass
 constexpr int kMaxLsfR = 64;    // largest LSF tap radius, channels
 constexpr int kVBlock = 8;      // output rows per thread in the vertical pass
 constexpr int kChanBlock = 8;   // channels between two restarts of the line recurrence (gbk_fused.cu)
@@ -28,6 +29,8 @@ struct DevProblem {
   int r_p_max;              // largest PSF radius
   int ews, ehs;             // shared-memory row stride (floats) and rows of one moment map
   int psf_stride;           // floats per PSF set in psf_taps
+  int img_fast;             // image PSF small enough for the register-tiled 2-D pass (gbk_fused.cu)
+  int spare_plane;          // floats of the extra output plane of that pass (0 if unused)
   float dv, v_center;
   float vrel_first;         // velocity of extended channel 0 relative to v_center
   float inv_u, inv_u2;
