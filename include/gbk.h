@@ -81,7 +81,11 @@ typedef struct {
   int32_t psf_per_gal;  /* 0: one PSF shared by all data sets                              */
   float lsf_sigma;      /* km/s; Gaussian LSF, taps R = ceil(4*sigma/dv) channels,           */
                         /* normalised; <= 0 is the delta LSF                               */
-  int32_t tile_w, tile_h; /* spatial tile of one thread block in SPAXELS; 0 = automatic     */
+  int32_t tile_w, tile_h; /* spatial tile of one thread block in SPAXELS; 0 = automatic:     */
+                          /* the largest tile of which two blocks fit in an SM's shared      */
+                          /* memory, and, when BOTH are 0, smaller tiles at eval time for     */
+                          /* batches too small to fill the GPU (chi^2 then differs between    */
+                          /* batch sizes by summation order only, ~1e-7 relative)             */
   int32_t device;       /* CUDA device ordinal; < 0 = the current device                   */
 } gbk_problem_desc;
 

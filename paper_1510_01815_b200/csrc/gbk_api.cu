@@ -58,6 +58,15 @@ struct gbk_problem {
   gbk_problem_desc d{};       // scalars only are meaningful after create
   DevProblem dp{};
   FusedLaunch fl{};
+  // smaller tilings of the same problem for batches too small to fill the GPU (automatic tiling
+  // only): level 0 is {dp, fl}; every further level halves the tile
+  struct Level {
+    DevProblem dp;
+    FusedLaunch fl;
+    int blocks_per_sm;   // resident blocks of this shape
+    int rounds;          // passes of the voxel loop over the tile (4 pixels per thread and pass)
+  };
+  std::vector<Level> levels;
   int device = 0;
   int sm_count = 0, blocks_per_sm = 0;
   long long ext_voxels = 0;
@@ -67,7 +76,7 @@ struct gbk_problem {
   int* psf_r = nullptr;
   float4* obs = nullptr;
   float* partial = nullptr;
-  long long partial_cap = 0;    // rows
+  long long partial_cap = 0;    // floats
   // staging for gbk_eval_batch_host
   float* st_params = nullptr;
   int32_t* st_gal = nullptr;
@@ -276,7 +285,12 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   p->fl.pixels_per_thread = 4;
   // 256 threads: three blocks of a whole-field config-3 tile are resident per SM (70.7 KB and
   // <= 85 registers x 256 threads each), so their phases overlap (measured best of 128..384)
-  p->fl.threads = std::min(256, std::max(64, ((n_ext + 3) / 4 + 31) / 32 * 32));
+  auto threads_for = [&](const DevProblem& q) {
+    const int ne = (q.tile_w + 2 * r_p_max) * (q.tile_h + 2 * r_p_max);
+    return std::min(256, std::max(64, ((ne + 3) / 4 + 31) / 32 * 32));
+  };
+  p->fl.threads = threads_for(dp);
+  (void)n_ext;
   long long ext = 0;
   for (int ty = 0; ty < dp.tiles_y; ++ty)
     for (int tx = 0; tx < dp.tiles_x; ++tx) {
@@ -312,6 +326,25 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   dp.chan_tab = p->chan_tab, dp.psf_taps = p->psf_taps, dp.psf_r = p->psf_r, dp.obs = p->obs;
   GBK_CUDA_P(fused_prepare(p->fl));
   GBK_CUDA_P(fused_occupancy(p->fl, &p->blocks_per_sm));
+  auto rounds_for = [&](const DevProblem& q, const FusedLaunch& f) {
+    const int ne = (q.tile_w + 2 * r_p_max) * (q.tile_h + 2 * r_p_max);
+    return (ne + 4 * f.threads - 1) / (4 * f.threads);
+  };
+  p->levels.push_back({dp, p->fl, std::max(1, p->blocks_per_sm), rounds_for(dp, p->fl)});
+  if (d->tile_w <= 0 && d->tile_h <= 0) {
+    const DevProblem dp0 = dp;
+    int lw = tws, lh = ths;
+    while (std::max(lw, lh) > 4) {
+      lw = std::max(4, (lw + 1) / 2), lh = std::max(4, (lh + 1) / 2);
+      FusedLaunch lf = p->fl;
+      lf.smem_bytes = (int)set_tile(lw, lh);
+      lf.threads = threads_for(dp);
+      int bps = 1;
+      GBK_CUDA_P(fused_occupancy(lf, &bps));
+      p->levels.push_back({dp, lf, std::max(1, bps), rounds_for(dp, lf)});
+    }
+    dp = dp0;
+  }
 #undef GBK_CUDA_P
   // host pointers of the descriptor are not kept
   p->d.vobs = p->d.verr = p->d.sobs = p->d.serr = nullptr;
@@ -339,7 +372,8 @@ static int check_eval_args(gbk_problem* p, const float* params, int64_t K, float
   if (!p) return fail(GBK_ERR_ARG, "null problem");
   if (K < 0) return fail(GBK_ERR_ARG, "K must be >= 0");
   if (K > 0 && (!params || !chi2)) return fail(GBK_ERR_ARG, "params and chi2 are required");
-  if (K * (int64_t)p->dp.ntiles > 0x7fffffffLL) return fail(GBK_ERR_ARG, "K * tiles exceeds the grid limit");
+  if (K * (int64_t)p->dp.ntiles > 0x7fffffffLL)   // smaller tilings are only used for small K
+    return fail(GBK_ERR_ARG, "K * tiles exceeds the grid limit");
   return GBK_OK;
 }
 
@@ -351,14 +385,26 @@ extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t
   if (K == 0) return GBK_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   GBK_CUDA(cudaSetDevice(p->device));
-  if (p->dp.ntiles > 1 && K > p->partial_cap) {
+  // tiling: the level with the fewest (waves of blocks) x (voxel-loop passes per block); ties go
+  // to the larger tile (less halo work, and one tile needs no second kernel)
+  size_t lv = 0;
+  long long best_cost = 0;
+  for (size_t i = 0; i < p->levels.size(); ++i) {
+    const auto& L = p->levels[i];
+    const long long slots = (long long)p->sm_count * L.blocks_per_sm;
+    const long long cost = ((long long)K * L.dp.ntiles + slots - 1) / slots * L.rounds;
+    if (i == 0 || cost < best_cost) best_cost = cost, lv = i;
+  }
+  const DevProblem& dp = p->levels[lv].dp;
+  const long long need = dp.ntiles > 1 ? (long long)K * dp.ntiles : 0;
+  if (need > p->partial_cap) {
     if (p->partial) GBK_CUDA(cudaFree(p->partial));   // synchronises; only when K grows
     p->partial = nullptr, p->partial_cap = 0;
-    GBK_CUDA(cudaMalloc(&p->partial, sizeof(float) * (size_t)K * p->dp.ntiles));
-    p->partial_cap = K;
+    GBK_CUDA(cudaMalloc(&p->partial, sizeof(float) * (size_t)need));
+    p->partial_cap = need;
   }
   EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, p->partial};
-  GBK_CUDA(launch_fused(p->dp, a, p->fl, st));
+  GBK_CUDA(launch_fused(dp, a, p->levels[lv].fl, st));
   return GBK_OK;
 }
 

@@ -82,6 +82,13 @@ __device__ __forceinline__ float rcp_approx(float x) {
 }
 __host__ __device__ __forceinline__ int round_up4(int v) { return (v + 3) & ~3; }
 
+// n / d by multiply-high: exact for n * d < 2^32 (indices inside one tile).  d = 1 has no 32-bit
+// magic number (it would be 2^32) and is passed through.
+__device__ __forceinline__ unsigned div_magic(int d) { return d > 1 ? 0xFFFFFFFFu / (unsigned)d + 1u : 0u; }
+__device__ __forceinline__ int div_fast(int n, unsigned magic) {
+  return magic ? (int)__umulhi((unsigned)n, magic) : n;
+}
+
 __device__ __forceinline__ float f_inf() { return __int_as_float(0x7f800000); }
 __device__ __forceinline__ float f_nan() { return __int_as_float(0x7fc00000); }
 
@@ -376,10 +383,10 @@ __device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const Eva
                                                  int ty0, const u64 (&tb)[R + 1], int tid,
                                                  int nthreads) {
   const int nxp = (tw + 1) >> 1, nyb = (th + BY - 1) / BY;
-  const unsigned magic = 0xFFFFFFFFu / (unsigned)nxp + 1u;
+  const unsigned magic = div_magic(nxp);
   float chi = 0.0f;
   for (int item = tid; item < nxp * nyb; item += nthreads) {
-    const int yb = (int)__umulhi((unsigned)item, magic), x = (item - yb * nxp) << 1, y0 = yb * BY;
+    const int yb = div_fast(item, magic), x = (item - yb * nxp) << 1, y0 = yb * BY;
     u64 res[3][BY];
 #pragma unroll
     for (int q = 0; q < 3; ++q) {
@@ -479,9 +486,9 @@ __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ew
                                              const u64* w64, int tid, int nthreads) {
   constexpr int NV4 = (8 + N - 1 + 3) / 4;
   const int nxc = (tw + 7) >> 3, half = (th + 1) >> 1;
-  const unsigned magic = 0xFFFFFFFFu / (unsigned)half + 1u;
+  const unsigned magic = div_magic(half);
   for (int item = tid; item < nxc * half; item += nthreads) {
-    const int xc = (int)__umulhi((unsigned)item, magic), l = item - xc * half;
+    const int xc = div_fast(item, magic), l = item - xc * half;
     const bool two = l + half < th;
     const int yy[2] = {l, two ? l + half : l};
     u64 acc[2][4];
@@ -625,7 +632,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
                                             int nthreads) {
   const int ppr = (EW + 1) >> 1;                  // pixel pairs per extended row
   const int npairs = ppr * EH;
-  const unsigned magic = 0xFFFFFFFFu / (unsigned)ppr + 1u;   // exact quotient for these sizes
+  const unsigned magic = div_magic(ppr);
   const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
   constexpr int kPerItem = 32 * kPairs;
   const int nitems = (npairs + kPerItem - 1) / kPerItem;
@@ -640,7 +647,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
     for (int j = 0; j < kPairs; ++j) {
       const int pi = item * kPerItem + j * 32 + lane;
       const int pic = min(pi, npairs - 1);
-      const int ey = (int)__umulhi((unsigned)pic, magic), ex = (pic - ey * ppr) << 1;
+      const int ey = div_fast(pic, magic), ex = (pic - ey * ppr) << 1;
       sidx[j] = pi < npairs ? ey * dp.ews + ex : -1;
       const float gx = (float)(tx0 + ex - R), gy = (float)(ty0 + ey - R);
       const float xa = (gx + 0.5f) * inv_u - 0.5f, xb = (gx + 1.5f) * inv_u - 0.5f;

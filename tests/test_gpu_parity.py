@@ -285,6 +285,44 @@ def test_variants(oracle, torch_cuda, gbk, kw):
     print("variant", kw, pu.compare(ref, got, rows, True, f"variant {kw}"))
 
 
+@pytest.mark.parametrize("kw,tile", [
+    (dict(psf_fwhm=0.0, lsf_sigma=0.0), (4, 4)), (dict(psf_fwhm=0.0, lsf_sigma=0.0), (2, 2)),
+    (dict(psf_fwhm=0.0, lsf_sigma=0.0), (1, 1)), (dict(psf_fwhm=0.0), (3, 11)),
+    (dict(psf_fwhm=1.1), (1, 2)), (dict(psf_fwhm=1.1), (2, 1)), (dict(psf_fwhm=1.1, u=2), (1, 1)),
+    (dict(psf_fwhm=0.0, lsf_sigma=0.0), (0, 0))])
+def test_tiny_tiles_and_delta_kernels(oracle, torch_cuda, gbk, kw, tile):
+    """Tiles of one or two pixels and the delta PSF (tap radius 0): the degenerate sizes of the index
+    arithmetic (a divisor of 1 in the multiply-high division once produced +INF rows).  K = 5 with
+    automatic tiling (0, 0) also takes the small-batch tiling chosen at eval time."""
+    w, g, obs, true, rng = _tiny_case(oracle, **kw)
+    rows = _rows_near(w, true, rng, 5)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1]), rows)
+    pu.compare(ref, got, rows, True, f"tiny tiles {kw} {tile}")
+
+
+def test_batch_size_picks_the_tiling_but_not_the_result(oracle, torch_cuda, gbk):
+    """Automatic tiling takes smaller tiles for batches too small to fill the GPU: the same row
+    must agree with the oracle (and with itself to rounding) at K = 1, 8 and 600."""
+    torch = torch_cuda
+    w, g, obs, true, rng = _tiny_case(oracle, nx=40, ny=36)
+    rows = _rows_near(w, true, rng, 600)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows[:8],
+                           want_maps=True)
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        p = torch.from_numpy(rows).cuda()
+        outs = {}
+        for K in (1, 8, 600):
+            out = prob.eval(p[:K].contiguous(), want_maps=True)
+            torch.cuda.synchronize()
+            outs[K] = {k: v.cpu().numpy() for k, v in out.items()}
+    pu.compare({k: v[:1] for k, v in ref.items()}, outs[1], rows[:1], True, "K=1")
+    pu.compare(ref, outs[8], rows[:8], True, "K=8")
+    pu.compare(ref, {k: v[:8] for k, v in outs[600].items()}, rows[:8], True, "K=600")
+    np.testing.assert_allclose(outs[1]["chi2"], outs[600]["chi2"][:1], rtol=2e-6)
+
+
 def test_bitwise_reproducible_and_host_entry(oracle, torch_cuda, gbk):
     torch = torch_cuda
     w, g, obs, true, rng = _tiny_case(oracle)
