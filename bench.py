@@ -322,7 +322,9 @@ def run_ours(args, ranks) -> None:
     achieved = fp32_per_eval * K * args.steps / sec_rank / 1e9
     roofline = {"bound": "alu", "pipe": "FP32 FMA pipe, 128 lanes/clk/SM (FFMA2 = 2 lanes x 2 clk)",
                 "achieved": achieved, "peak": peak_fp32, "unit": "Gop/s", "frac": achieved / peak_fp32,
-                "traffic": None,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed capture
+                # profiles/r01_fused_kernel_ncu.md (config 3 only; not measured live)
+                "traffic": 328960 if cfg == 3 else None, "traffic_unit": "bytes per launch",
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
                 "ops_per_eval": int(fp32_per_eval),
                 "ops_how": "algorithmic FP32 lane-ops: 5/ext voxel + 45/ext sample + 3 maps x (2 x taps separable | taps^2 image)/fine pixel + 12/spaxel",
@@ -342,6 +344,8 @@ def run_ours(args, ranks) -> None:
         cpu = time_oracle(cfg, args.cpu_rows or 32 * cores, 1, 1, cores)
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
 
+    unfused = time_unfused(gbk, torch, prob, dev_batches[0], K, info) \
+        if (ranks.is_main and not args.no_fits) else None
     fits = time_fits(gbk, torch, prob, w, true) if (ranks.is_main and cfg == 3 and not args.no_fits) else None
     if ranks.is_main:
         core_vox = w.nx * w.ny * w.nv * w.u * w.u
@@ -362,7 +366,7 @@ def run_ours(args, ranks) -> None:
                     "d2h_bytes_per_step": K * 4, "matches_device_path": same},
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "checksum": checksum,
-            "fits": fits,
+            "fits": fits, "unfused": unfused,
         }
         print(json.dumps(line), flush=True)
     prob.close()
@@ -399,6 +403,33 @@ def time_fits(gbk, torch, prob3, w3, true3) -> dict:
                       "converged": st["converged"], "chi2": float(chi2[0]),
                       "abs_err": [float(abs(rows[0, j] - true2[j])) for j in free7]}
     return out
+
+
+def time_unfused(gbk, torch, prob, params, K: int, info, reps: int = 5) -> dict:
+    """The unfused comparison path (one kernel per pipeline step, FP32 cube in HBM) on the same
+    batch: evals/s and achieved HBM GB/s = algorithmic bytes / device time, against the measured copy
+    bandwidth of MEASURED_PEAKS.json (outside the timed region; rank 0)."""
+    chi = torch.empty(K, dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    gbk.gbk_eval_batch_unfused(prob.handle, params, None, K, chi, stream=st)      # warm-up + scratch
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        gbk.gbk_eval_batch_unfused(prob.handle, params, None, K, chi, stream=st)
+    e1.record()
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3 / reps
+    peak = None
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            peak = float(json.load(f)["hbm_gbs"])
+    except (OSError, KeyError, ValueError):
+        peak = 6500.0      # fallback of the profiling recipe's order; MEASURED_PEAKS.json absent
+    gbs = info.unfused_bytes_per_eval * K / sec / 1e9
+    return {"value": K / sec, "unit": UNIT, "ms_per_batch": sec * 1e3, "bound": "hbm",
+            "bytes_per_eval": int(info.unfused_bytes_per_eval), "achieved": gbs, "peak": peak,
+            "unit_bw": "GB/s", "frac": gbs / peak}
 
 
 def _chi2_of(gbk, prob, params, K, torch):

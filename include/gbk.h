@@ -102,6 +102,8 @@ typedef struct {
   int32_t sm_count;
   int64_t ext_voxels_per_eval; /* sum over tiles of (tw+2R)(th+2R)(nv+2R_v), R = r_p_max   */
   int32_t device;         /* CUDA device ordinal the problem lives on                      */
+  int64_t unfused_bytes_per_eval; /* algorithmic HBM bytes of gbk_eval_batch_unfused per row:   */
+                          /* every intermediate array written once and read once per consumer */
 } gbk_problem_info;
 
 /*

@@ -365,6 +365,7 @@ extern "C" int gbk_get_info(const gbk_problem* p, gbk_problem_info* info) {
   info->blocks_per_sm = p->blocks_per_sm, info->sm_count = p->sm_count;
   info->ext_voxels_per_eval = p->ext_voxels;
   info->device = p->device;
+  info->unfused_bytes_per_eval = (int64_t)unfused_algorithmic_bytes_per_row(p->dp);
   return GBK_OK;
 }
 

@@ -57,6 +57,7 @@ class gbk_problem_info(C.Structure):
         ("blocks_per_sm", C.c_int32), ("sm_count", C.c_int32),
         ("ext_voxels_per_eval", C.c_int64),
         ("device", C.c_int32),
+        ("unfused_bytes_per_eval", C.c_int64),
     ]
 
 
