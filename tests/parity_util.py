@@ -85,6 +85,8 @@ def compare(oracle_out: dict, gpu_out: dict, rows: np.ndarray, want_maps: bool, 
                 assert np.isnan(g0).all() and np.isnan(g1).all() and np.isnan(g2).all()
                 continue
             bright = o0 > DARK_GUARD * 1e-30 * float(rows[k, wl.IX_I0])
+            if not bright.any():        # the whole map is model-dark (line outside the band)
+                continue
             r0 = np.abs(g0 - o0)[bright] / o0[bright]
             d1 = np.abs(g1 - o1)[bright]
             d2 = np.abs(g2 - o2)[bright]

@@ -323,6 +323,34 @@ def test_batch_size_picks_the_tiling_but_not_the_result(oracle, torch_cuda, gbk)
     np.testing.assert_allclose(outs[1]["chi2"], outs[600]["chi2"][:1], rtol=2e-6)
 
 
+@pytest.mark.parametrize("rc_model", [wl.RC_ARCTAN, wl.RC_RAMP])
+def test_line_width_sweep_covers_recurrence_and_direct_loops(oracle, torch_cuda, gbk, rc_model):
+    """The voxel loop evaluates the line by a multiplicative recurrence when sigma_0/dv >= 1.06 and by
+    one ex2 per voxel below that: one batch mixes both, on either side of the
+    switch, with lines that leave the band (large V_sys offsets), very fast and very slow discs."""
+    w, g, obs, true, rng = _tiny_case(oracle, nx=20, ny=17, nv=56, rc_model=rc_model)
+    dv = w.dv
+    rows = []
+    for ratio in (0.45, 0.8, 1.0, 1.05, 1.0617, 1.07, 1.2, 2.0, 5.0):
+        for dvsys, vt in ((0.0, 180.0), (400.0, 250.0), (-700.0, 60.0), (0.0, 1500.0)):
+            r = true.copy()
+            r[wl.IX_SIG] = ratio * dv
+            r[wl.IX_VSYS] += dvsys
+            r[wl.IX_VT] = vt
+            rows.append(r)
+    r = true.copy()
+    r[wl.IX_VSYS] = 5000.0            # the whole line outside the band: model-dark everywhere
+    rows.append(r)
+    rows = np.stack(rows).astype(np.float32)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    for tile in ((0, 0), (7, 6)):
+        got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1]), rows)
+        worst = pu.compare(ref, got, rows, True, f"line width sweep rc={rc_model} tile={tile}")
+        assert worst["skipped_rows"] <= 4, worst
+    assert np.isinf(ref["chi2"][-1])
+
+
 def test_bitwise_reproducible_and_host_entry(oracle, torch_cuda, gbk):
     torch = torch_cuda
     w, g, obs, true, rng = _tiny_case(oracle)
