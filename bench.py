@@ -248,7 +248,7 @@ def run_ours(args, ranks) -> None:
     obs = observation_from_gpu(gbk, torch, w, true, rng)
     batches = batch_rows(cfg, w, true, rng, 4)
     K = batches[0].shape[0]
-    prob = gbk.Problem(**desc_for(w, obs))
+    prob = gbk.Problem(**desc_for(w, obs), tile_w=args.tile[0], tile_h=args.tile[1])
     info = prob.info
     dev_batches = [torch.from_numpy(b).cuda() for b in batches]
     chi2 = torch.empty(K, dtype=torch.float32, device="cuda")
@@ -497,6 +497,8 @@ def main() -> None:
     ap.add_argument("--ref-rows", type=int, default=0, help="rows per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fits", action="store_true", help="skip the wall-time-to-fit legs")
+    ap.add_argument("--tile", type=int, nargs=2, default=(0, 0), metavar=("W", "H"),
+                    help="spatial tile in spaxels (default 0 0 = the library's automatic tiling)")
     args = ap.parse_args()
     from paper_1510_01815_b200 import dist
     if args.impl == "reference":
