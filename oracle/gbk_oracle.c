@@ -394,6 +394,53 @@ int gbko_eval_rows(const gbko_grid *g, const float *vobs, const float *verr, con
   return fail ? -1 : 0;
 }
 
+/* ---------------------------------------------------- velocity field ---- */
+
+/* Velocity-field modelling strategy (section 2.2.1): eq. 8
+ * evaluated at every spaxel centre (x = column, y = row; reading A1), no cube,
+ * no PSF, no LSF (the paper skips steps 2.2.2-2.2.5), then the
+ * velocity residual and the first term of eq. 11 only
+ * (no dispersion map is modelled).  Only the seven kinematic
+ * parameters p[0..6] are used; a row is out of domain when one of them is not
+ * finite, r_t <= 0 or |cos i| < 1e-6 (chi2 = +INF, NaN maps).
+ * Outputs: chi2[K]; vmap[K][ny][nx] and resid[K][ny][nx] may be NULL.        */
+int gbko_vfield_rows(const gbko_grid *g, const float *vobs, const float *verr, const uint8_t *mask,
+                     const float *params, int64_t K, double *chi2, double *vmap, double *resid,
+                     int nthreads) {
+  const size_t npix = (size_t)g->nx * g->ny;
+#ifdef _OPENMP
+  if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+  (void)nthreads;
+#endif
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t k = 0; k < K; ++k) {
+    double p[GBKO_P];
+    int ok = 1;
+    for (int j = 0; j < GBKO_P; ++j) p[j] = (double)params[k * GBKO_P + j];
+    for (int j = 0; j < 7; ++j)
+      if (!isfinite(p[j])) ok = 0;
+    if (ok && (!(p[6] > 0.0) || fabs(cos(p[3] * GBKO_PI / 180.0)) < 1e-6)) ok = 0;
+    p[7] = 1.0, p[8] = 1.0, p[9] = 1.0;   /* unused by eq. 8; keep the brightness finite */
+    double sum = 0.0;
+    for (size_t q = 0; q < npix; ++q) {
+      const int iy = (int)(q / (size_t)g->nx), ix = (int)(q % (size_t)g->nx);
+      double I, v = NAN;
+      if (ok) gbko_disc_point(p, g->rc_model, (double)ix, (double)iy, &I, &v);
+      const int unmasked = !mask || mask[q] != 0;
+      double t = 0.0;
+      if (unmasked) {
+        t = (v - (double)vobs[q]) / (double)verr[q];
+        if (!isfinite(t)) sum = INFINITY; else if (isfinite(sum)) sum += t * t;
+      }
+      if (vmap) vmap[(size_t)k * npix + q] = v;
+      if (resid) resid[(size_t)k * npix + q] = unmasked ? (ok ? t : NAN) : 0.0;
+    }
+    chi2[k] = ok ? sum : INFINITY;
+  }
+  return 0;
+}
+
 int gbko_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -87,6 +87,8 @@ def lib():
         L.gbko_eval_rows.argtypes = [gp, fp, fp, fp, fp, u8p, fp, C.c_int64, dp, dp, dp, dp, dp,
                                      C.c_int]
         L.gbko_eval_rows.restype = C.c_int
+        L.gbko_vfield_rows.argtypes = [gp, fp, fp, u8p, fp, C.c_int64, dp, dp, dp, C.c_int]
+        L.gbko_vfield_rows.restype = C.c_int
         L.gbko_max_threads.argtypes = []
         L.gbko_max_threads.restype = C.c_int
         _lib = L
@@ -283,6 +285,25 @@ def eval_rows(grid: Grid, vobs, verr, sobs, serr, mask, params, want_maps=False,
                               int(nthreads))
     if rc != 0:
         raise MemoryError("oracle allocation failed")
+    return out
+
+
+def vfield_rows(grid: Grid, vobs, verr, mask, params, want_maps=False, want_resid=False,
+                nthreads: int = 0):
+    """Velocity-field strategy: K rows -> dict(chi2[, vmap][, resid])."""
+    params = np.ascontiguousarray(params, dtype=np.float32).reshape(-1, P)
+    K = params.shape[0]
+    vobs, verr = _c32(vobs), _c32(verr)
+    mask = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    g = grid.c()
+    out = {"chi2": np.empty(K, dtype=np.float64)}
+    if want_maps:
+        out["vmap"] = np.empty((K, grid.ny, grid.nx), dtype=np.float64)
+    if want_resid:
+        out["resid"] = np.empty((K, grid.ny, grid.nx), dtype=np.float64)
+    lib().gbko_vfield_rows(C.byref(g), _fp(vobs), _fp(verr), _u8p(mask), _fp(params), K,
+                           _dp(out["chi2"]), _dp(out.get("vmap")), _dp(out.get("resid")),
+                           int(nthreads))
     return out
 
 

@@ -469,3 +469,67 @@ def test_golden_hand_values_file(oracle):
             assert v == pytest.approx(v_want, abs=1e-7), line
             n += 1
     assert n >= 8
+
+
+# ------------------------------------------------ velocity-field strategy ----
+
+def _vf_grid(oracle, nx, ny, rc=0):
+    return oracle.Grid(nx=nx, ny=ny, nv=8, u=1, v_center=0.0, dv=10.0, rc_model=rc,
+                       psf=np.ones((1, 1)), lsf=np.ones(1))
+
+
+def test_vfield_map_equals_the_golden_hand_values(oracle):
+    """vmap[y][x] of the velocity-field oracle = the hand-derived eq. 8 values of the golden file
+    (spaxel j is centred on coordinate j, reading A1), for every golden point on the pixel grid."""
+    n = 0
+    with open(os.path.join(GOLDEN, "eq_hand_values.txt")) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if not line:
+                continue
+            tok = line.split()
+            rc = {"arctan": 0, "ramp": 1}[tok[0]]
+            p = np.array([float(t) for t in tok[1:11]], dtype=np.float32)
+            x, y, _, v_want = (float(t) for t in tok[11:15])
+            if x < 0 or y < 0 or x != int(x) or y != int(y):
+                continue
+            g = _vf_grid(oracle, 16, 16, rc)
+            z = np.zeros((16, 16), np.float32)
+            out = oracle.vfield_rows(g, z, z + 1, None, p[None], want_maps=True)
+            assert out["vmap"][0, int(y), int(x)] == pytest.approx(v_want, abs=1e-5), line
+            n += 1
+    assert n >= 7
+
+
+def test_vfield_chi2_by_hand_masks_and_domain(oracle):
+    g = _vf_grid(oracle, 2, 2)
+    # face-on disc: v = V_sys = 12 everywhere (eq. 8 with sin i = 0)
+    p = np.array([[0.5, 0.5, 30.0, 0.0, 12.0, 200.0, 3.0, np.nan, np.nan, np.nan]], dtype=np.float32)
+    vobs = np.array([[10.0, 12.0], [15.0, 0.0]], np.float32)
+    verr = np.array([[1.0, 2.0], [3.0, 4.0]], np.float32)
+    out = oracle.vfield_rows(g, vobs, verr, None, p, want_maps=True, want_resid=True)
+    assert np.allclose(out["vmap"][0], 12.0, atol=1e-12)
+    assert out["chi2"][0] == pytest.approx(2.0 ** 2 + 0.0 + 1.0 ** 2 + 3.0 ** 2)      # 4 + 0 + 1 + 9
+    assert np.allclose(out["resid"][0], [[2.0, 0.0], [-1.0, 3.0]])
+    mask = np.array([[1, 1], [1, 0]], np.uint8)
+    out = oracle.vfield_rows(g, vobs, verr, mask, p, want_resid=True)
+    assert out["chi2"][0] == pytest.approx(5.0) and out["resid"][0, 1, 1] == 0.0
+    # sigma_0, r_0, I_0 are not part of eq. 8 (NaN above was harmless); the kinematic ones are
+    for j, bad in ((6, 0.0), (3, 90.0), (5, np.inf), (0, np.nan)):
+        q = p.copy()
+        q[0, j] = bad
+        assert np.isinf(oracle.vfield_rows(g, vobs, verr, None, q)["chi2"][0]), j
+
+
+def test_vfield_is_antisymmetric_about_the_centre_and_equals_delta_kernel_m1(oracle):
+    """v(c + d) + v(c - d) = 2 V_sys (eq. 1, 4, 8), and the velocity field is the m1 map of the cube
+    strategy with delta PSF and LSF (the strategies differ only in steps 2.2.2-2.2.5)."""
+    p = np.array([[7.0, 6.0, 123.0, 50.0, 8.0, 180.0, 2.5, 40.0, 3.0, 1.5]], dtype=np.float32)
+    for rc in (0, 1):
+        g = oracle.Grid(nx=15, ny=13, nv=96, u=1, v_center=0.0, dv=12.0, rc_model=rc,
+                        psf=np.ones((1, 1)), lsf=np.ones(1))
+        z = np.zeros((13, 15), np.float32)
+        v = oracle.vfield_rows(g, z, z + 1, None, p, want_maps=True)["vmap"][0]
+        assert np.allclose(v + v[::-1, ::-1], 16.0, atol=1e-10)
+        m0, m1, m2 = oracle.model_maps(g, p[0].astype(np.float64))
+        assert np.max(np.abs(m1 - v)) < 1e-6
