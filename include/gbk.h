@@ -149,6 +149,21 @@ int gbk_eval_batch_unfused(gbk_problem *p, const float *params, const int32_t *g
                            void *cuda_stream);
 
 /*
+ * The paper's OTHER modelling strategy, velocity-field modelling (section
+ * 2.2.1): eq. 8 evaluated at every spaxel centre of the nx x ny grid -- no cube, no
+ * PSF, no LSF, no up-sampling (the paper skips steps 2.2.2-2.2.5) -- then the
+ * velocity residual and the first term of eq. 11 only.  Uses the
+ * problem's vobs / verr / mask and rc_model; of a row only x_o, y_o, PA, i, V_sys, V_t, r_t are
+ * read (a row is out of domain, chi2 = +INF, when one of those is not finite, r_t <= 0 or
+ * |cos i| < 1e-6).  Asynchronous on `cuda_stream`, no allocation.
+ *   params DEVICE [K][GBK_P]; gal_index DEVICE [K] or NULL; chi2 DEVICE [K], required
+ *   vmap   DEVICE [K][ny][nx] or NULL: the model velocity field
+ *   resid  DEVICE [K][ny][nx] or NULL: (model - vobs) / verr, 0 where masked
+ */
+int gbk_eval_vfield_batch(gbk_problem *p, const float *params, const int32_t *gal_index, int64_t K,
+                          float *chi2, float *vmap, float *resid, void *cuda_stream);
+
+/*
  * End-to-end entry with HOST buffers: copies params (and gal_index) to the
  * device, runs gbk_eval_batch, copies chi2 back and waits for `cuda_stream`.
  * params/gal_index/chi2 are HOST pointers (pinned memory makes the copies

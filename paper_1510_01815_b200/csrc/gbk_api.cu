@@ -409,6 +409,18 @@ extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t
   return GBK_OK;
 }
 
+extern "C" int gbk_eval_vfield_batch(gbk_problem* p, const float* params, const int32_t* gal_index,
+                                     int64_t K, float* chi2, float* vmap, float* resid,
+                                     void* cuda_stream) {
+  g_err[0] = 0;
+  if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  if (K == 0) return GBK_OK;
+  GBK_CUDA(cudaSetDevice(p->device));
+  EvalArgs a{params, gal_index, (long long)K, chi2, nullptr, vmap, nullptr, resid, nullptr};
+  GBK_CUDA(launch_vfield(p->dp, a, (cudaStream_t)cuda_stream));
+  return GBK_OK;
+}
+
 extern "C" int gbk_eval_batch_host(gbk_problem* p, const float* params, const int32_t* gal_index,
                                    int64_t K, float* chi2, void* cuda_stream) {
   g_err[0] = 0;

@@ -89,6 +89,8 @@ def lib():
             f = getattr(L, name)
             f.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp]
             f.restype = C.c_int
+        L.gbk_eval_vfield_batch.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp]
+        L.gbk_eval_vfield_batch.restype = C.c_int
         L.gbk_eval_batch_host.argtypes = [vp, vp, vp, C.c_int64, vp, vp]
         L.gbk_eval_batch_host.restype = C.c_int
         L.gbk_destroy.argtypes = [vp]
@@ -191,6 +193,12 @@ def gbk_eval_batch(handle, params, gal_index, K, chi2, m0=None, m1=None, m2=None
 def gbk_eval_batch_unfused(handle, params, gal_index, K, chi2, m0=None, m1=None, m2=None,
                            resid=None, stream=0):
     gbk_eval_batch(handle, params, gal_index, K, chi2, m0, m1, m2, resid, stream, unfused=True)
+
+
+def gbk_eval_vfield_batch(handle, params, gal_index, K, chi2, vmap=None, resid=None, stream=0):
+    """Velocity-field strategy (device buffers; asynchronous on `stream`)."""
+    _check(lib().gbk_eval_vfield_batch(handle, _ptr(params), _ptr(gal_index), int(K), _ptr(chi2),
+                                       _ptr(vmap), _ptr(resid), stream or None))
 
 
 def gbk_eval_batch_host(handle, params, gal_index, K, chi2, stream=0):
@@ -299,6 +307,24 @@ class Problem:
 
     def __exit__(self, *exc):
         self.close()
+
+    def eval_vfield(self, params, gal_index=None, want_maps=False, want_resid=False, stream=None):
+        """Velocity-field strategy: torch CUDA float32 [K, 10] -> dict(chi2[, vmap][, resid])."""
+        import torch
+        assert params.is_cuda and params.dtype == torch.float32 and params.is_contiguous()
+        K = params.shape[0]
+        i = self.info
+        out = {"chi2": torch.empty(K, dtype=torch.float32, device=params.device)}
+        if want_maps:
+            out["vmap"] = torch.empty((K, i.ny, i.nx), dtype=torch.float32, device=params.device)
+        if want_resid:
+            out["resid"] = torch.empty((K, i.ny, i.nx), dtype=torch.float32, device=params.device)
+        if gal_index is not None:
+            assert gal_index.is_cuda and gal_index.dtype == torch.int32 and gal_index.is_contiguous()
+        st = (stream or torch.cuda.current_stream(params.device)).cuda_stream
+        gbk_eval_vfield_batch(self.handle, params, gal_index, K, out["chi2"], out.get("vmap"),
+                              out.get("resid"), st)
+        return out
 
     def eval(self, params, gal_index=None, want_maps=False, want_resid=False, unfused=False,
              stream=None):
