@@ -195,6 +195,39 @@ def test_cfg5_mixed_galaxies(oracle, torch_cuda, gbk):
         print("cfg5 gal", gi, float(fwhms[gi]), pu.compare(ref, sub, rows[sel], True, f"cfg5 gal {gi}"))
 
 
+def test_cfg5_full_launch_sampled_rows(oracle, torch_cuda, gbk):
+    """Config 5 at the size bench.py's survey leg launches: 1000 data sets with their own PSF, one
+    mixed batch of K = 16384 rows.  The observation is seeded random data (chi^2 parity needs no
+    realistic maps, and clean maps of 1000 galaxies would take the oracle minutes); 24 sampled rows
+    are checked against the oracle with the sampled row's own PSF and data set."""
+    torch = torch_cuda
+    w = wl.config(5)
+    rng = wl.rng_for(5, 9)
+    n = w.n_gal
+    fwhms = wl.galaxy_fwhms(w, rng)
+    shp = (n, w.ny, w.nx)
+    obs = wl.Observed(rng.normal(0.0, 80.0, shp).astype(np.float32),
+                      rng.uniform(3.0, 15.0, shp).astype(np.float32),
+                      rng.uniform(20.0, 80.0, shp).astype(np.float32),
+                      rng.uniform(3.0, 15.0, shp).astype(np.float32),
+                      (rng.random(shp) < 0.8).astype(np.uint8))
+    K = w.K
+    rows = wl.draw_rows(w, rng, K)
+    gal = rng.integers(0, n, K).astype(np.int32)
+    with gbk.Problem(**pu.gbk_desc(w, obs, fwhms=fwhms)) as prob:
+        assert prob.info.n_gal == n
+        out = prob.eval(torch.from_numpy(rows).cuda(), torch.from_numpy(gal).cuda())
+        chi = out["chi2"].cpu().numpy()
+    assert np.isfinite(chi).all()
+    sel = np.concatenate([[0, K - 1], rng.integers(0, K, 22)])
+    for k in sel:
+        gi = int(gal[k])
+        g = pu.oracle_grid(oracle, w, fwhms[gi])
+        ref = oracle.eval_rows(g, obs.vobs[gi], obs.verr[gi], obs.sobs[gi], obs.serr[gi], obs.mask[gi],
+                               rows[k:k + 1])
+        pu.compare(ref, {"chi2": chi[k:k + 1]}, rows[k:k + 1], False, f"cfg5 full row {k} gal {gi}")
+
+
 # ------------------------------------------------------------------- edge cases ----
 
 def _tiny_case(oracle, **kw):
