@@ -11,6 +11,7 @@
 // block sum (bit-reproducible).
 #include <math.h>
 
+#include "gbk_device.cuh"
 #include "gbk_internal.h"
 
 namespace gbk {
@@ -21,33 +22,11 @@ constexpr int kRows = 4;        // parameter rows per block
 constexpr int kThreads = 256;
 
 struct VRow {
-  float xo, yo, cp, nsp, ncp_ci, nsp_ci;   // eq. 1-3 as in RowConst
-  float inv_rt, rt;
-  float k1;                                 // V_t sin i (x 2/pi for the arctan curve)
-  float v0;                                 // V_sys - v_center
+  u64 nsp, ncp_ci, inv_rt, rt, k1, v0;     // packed (c, c): eq. 1-3 constants as in RowConst,
+                                            // k1 = V_t sin i (x 2/pi for the arctan curve), v0 = V_sys - v_center
+  float xo, yo, cp, nsp_ci;
   int valid, gal;
 };
-
-__device__ __forceinline__ float vf_rsqrt(float x) {
-  float y;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-
-// atan(z), z in [0, 1]: z * P(z^2), 8 terms, max error 1.4e-7 rad (the polynomial of the fused
-// kernel, scalar here).
-__device__ __forceinline__ float vf_atan01(float z) {
-  const float t = z * z;
-  float p = -0.00405439967289567f;
-  p = fmaf(p, t, 0.02186231128871441f);
-  p = fmaf(p, t, -0.05591132491827011f);
-  p = fmaf(p, t, 0.09642117470502853f);
-  p = fmaf(p, t, -0.13908594846725464f);
-  p = fmaf(p, t, 0.1994655877351761f);
-  p = fmaf(p, t, -0.33329859375953674f);
-  p = fmaf(p, t, 0.9999993443489075f);
-  return p * z;
-}
 
 __device__ void vf_row(const DevProblem& dp, const EvalArgs& a, long long k, VRow* r) {
   const float* p = a.params + k * GBK_P;
@@ -67,30 +46,39 @@ __device__ void vf_row(const DevProblem& dp, const EvalArgs& a, long long k, VRo
   r->valid = (finite && gal_ok && v[6] > 0.f && !(fabsf(ci) < 1e-6f)) ? 1 : 0;
   const float inv_ci = 1.0f / ci;
   r->xo = v[0], r->yo = v[1];
-  r->cp = cp, r->nsp = -sp, r->ncp_ci = -cp * inv_ci, r->nsp_ci = -sp * inv_ci;
-  r->inv_rt = 1.0f / v[6], r->rt = v[6];
-  r->k1 = (dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134f : 1.0f) * v[5] * si;
-  r->v0 = v[4] - dp.v_center;
+  r->cp = cp, r->nsp_ci = -sp * inv_ci;
+  r->nsp = pk1(-sp), r->ncp_ci = pk1(-cp * inv_ci);
+  r->inv_rt = pk1(1.0f / v[6]), r->rt = pk1(v[6]);
+  r->k1 = pk1((dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134f : 1.0f) * v[5] * si);
+  r->v0 = pk1(v[4] - dp.v_center);
 }
 
-// eq. 1-4, 6 (or the ramp), 8 at the spaxel (x, y): velocity relative to v_center.
-__device__ __forceinline__ float vf_velocity(const DevProblem& dp, const VRow& r, float x, float y) {
-  const float dx = x - r.xo, dy = y - r.yo;
-  const float xe = fmaf(r.nsp, dx, dy * r.cp);              // eq. 1
-  const float yd = fmaf(r.ncp_ci, dx, dy * r.nsp_ci);       // eq. 2 / cos i
-  const float r2 = fmaf(xe, xe, yd * yd);                   // eq. 3
-  const float rs = r2 > 1e-30f ? vf_rsqrt(r2) : 0.0f;       // r = 0: cos(theta) := 0 (A8)
-  const float rad = r2 * rs, cos_t = xe * rs;               // eq. 4
-  const float q = rad * r.inv_rt;
-  float f;
-  if (dp.rc_model == GBK_RC_ARCTAN) {                       // eq. 6 without (2/pi) V_t
-    const bool big = q > 1.0f;
-    const float at = vf_atan01(big ? rs * r.rt : q);
-    f = big ? 1.5707963267948966f - at : at;
+// eq. 1-4, 6 (or the ramp), 8 at the spaxel pair (x, y), (x + 1, y): velocities relative to
+// v_center, in packed FP32.
+__device__ __forceinline__ u64 vf_velocity2(const DevProblem& dp, const VRow& r, u64 dx, float dy) {
+  const u64 xe = fma2(r.nsp, dx, pk1(dy * r.cp));               // eq. 1
+  const u64 yd = fma2(r.ncp_ci, dx, pk1(dy * r.nsp_ci));        // eq. 2 / cos i
+  const u64 r2 = fma2(xe, xe, mul2(yd, yd));                    // eq. 3
+  float r2a, r2b;
+  upk(r2, r2a, r2b);
+  // r = 0: cos(theta) := 0 (A8)
+  const u64 rs = pk(r2a > 1e-30f ? rsqrt_approx(r2a) : 0.0f, r2b > 1e-30f ? rsqrt_approx(r2b) : 0.0f);
+  const u64 rad = mul2(r2, rs), cos_t = mul2(xe, rs);           // eq. 4
+  const u64 q = mul2(rad, r.inv_rt);
+  float qa, qb;
+  upk(q, qa, qb);
+  u64 f;
+  if (dp.rc_model == GBK_RC_ARCTAN) {                           // eq. 6 without (2/pi) V_t
+    float ia, ib;
+    upk(mul2(rs, r.rt), ia, ib);                                // 1/q = r_t / r
+    const bool biga = qa > 1.0f, bigb = qb > 1.0f;
+    const u64 at = atan01_2(pk(biga ? ia : qa, bigb ? ib : qb));
+    f = fma2(at, pk(biga ? -1.0f : 1.0f, bigb ? -1.0f : 1.0f),
+             pk(biga ? 1.5707963267948966f : 0.0f, bigb ? 1.5707963267948966f : 0.0f));
   } else {
-    f = fminf(q, 1.0f);                                     // ramp (A7)
+    f = pk(fminf(qa, 1.0f), fminf(qb, 1.0f));                   // ramp (A7)
   }
-  return fmaf(r.k1 * f, cos_t, r.v0);                       // eq. 8
+  return fma2(mul2(f, r.k1), cos_t, r.v0);                      // eq. 8
 }
 
 template <bool OUT, bool SHARED_OBS>
@@ -108,26 +96,45 @@ __global__ void __launch_bounds__(kThreads) vfield_kernel(const __grid_constant_
   float chi[kRows];
 #pragma unroll
   for (int j = 0; j < kRows; ++j) chi[j] = 0.0f;
-  for (int pix = tid; pix < npix; pix += kThreads) {
-    const int iy = pix / dp.nx, ix = pix - iy * dp.nx;
+  const int ppr = (dp.nx + 1) >> 1;                 // spaxel pairs per map row
+  const unsigned magic = div_magic(ppr);
+  for (int item = tid; item < ppr * dp.ny; item += kThreads) {
+    const int iy = div_fast(item, magic), ix = (item - iy * ppr) << 1;
+    const int pix = iy * dp.nx + ix;
+    const bool second = ix + 1 < dp.nx;
     const float x = (float)ix, y = (float)iy;
-    float4 ob;
-    if (SHARED_OBS) ob = __ldg(&dp.obs[pix]);
+    float4 oa, ob = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (SHARED_OBS) {
+      oa = __ldg(&dp.obs[pix]);
+      if (second) ob = __ldg(&dp.obs[pix + 1]);
+    }
 #pragma unroll
     for (int j = 0; j < kRows; ++j) {
       if (j >= nrows) break;
       const VRow& r = rows[j];
-      if (!SHARED_OBS) ob = __ldg(&dp.obs[(size_t)r.gal * npix + pix]);
-      float v = r.valid ? vf_velocity(dp, r, x, y) : nan;
-      float t = (v - ob.x) * ob.y;
-      const bool unmasked = ob.y > 0.0f;
-      float c = t * t;
-      c = unmasked ? (c < inf ? c : inf) : 0.0f;
-      chi[j] += c;
+      if (!SHARED_OBS) {
+        const float4* o = dp.obs + (size_t)r.gal * npix + pix;
+        oa = __ldg(o);
+        if (second) ob = __ldg(o + 1);
+      }
+      float va, vb;
+      upk(vf_velocity2(dp, r, pk(x - r.xo, x + 1.0f - r.xo), y - r.yo), va, vb);
+      if (!r.valid) va = vb = nan;
+      const float ta = (va - oa.x) * oa.y, tb = (vb - ob.x) * ob.y;
+      float ca = ta * ta, cb = tb * tb;
+      ca = oa.y > 0.0f ? (ca < inf ? ca : inf) : 0.0f;
+      cb = ob.y > 0.0f ? (cb < inf ? cb : inf) : 0.0f;     // ob.y = 0 for the missing second spaxel
+      chi[j] += ca + cb;
       if (OUT) {
         const size_t o = (size_t)(k0 + j) * npix + pix;
-        if (a.m1) a.m1[o] = v + dp.v_center;
-        if (a.resid) a.resid[o] = unmasked ? (c < inf ? t : nan) : 0.0f;
+        if (a.m1) {
+          a.m1[o] = va + dp.v_center;
+          if (second) a.m1[o + 1] = vb + dp.v_center;
+        }
+        if (a.resid) {
+          a.resid[o] = oa.y > 0.0f ? (ca < inf ? ta : nan) : 0.0f;
+          if (second) a.resid[o + 1] = ob.y > 0.0f ? (cb < inf ? tb : nan) : 0.0f;
+        }
       }
     }
   }
