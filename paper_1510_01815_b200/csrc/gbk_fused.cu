@@ -486,7 +486,7 @@ __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ew
 // a5..a9 for an image PSF on the fast path: the three maps are convolved plane by plane, each into
 // a plane that is free by then (S0 -> spare, S1 -> plane 0, S2 -> plane 1), then block sums.
 template <int N, bool OUT>
-__device__ __noinline__ float image_phase(const DevProblem& dp, const EvalArgs& a, const RowConst& rc,
+__device__ __forceinline__ float image_phase(const DevProblem& dp, const EvalArgs& a, const RowConst& rc,
                                           long long k, float* maps, float* spare, int map_stride, int tw,
                                           int th, int tx0, int ty0, const float* taps, int tid,
                                           int nthreads) {
@@ -502,7 +502,7 @@ __device__ __noinline__ float image_phase(const DevProblem& dp, const EvalArgs& 
 }
 
 template <int R, bool OUT>
-__device__ __noinline__ float separable_phase(const DevProblem& dp, const EvalArgs& a,
+__device__ __forceinline__ float separable_phase(const DevProblem& dp, const EvalArgs& a,
                                               const RowConst& rc, long long k, float* maps,
                                               int map_stride, int EH, int tw, int th, int tx0,
                                               int ty0, const float* taps, int tid, int nthreads) {
