@@ -313,8 +313,8 @@ def run_ours(args, ranks) -> None:
     fp32_per_eval = 5 * info.ext_voxels_per_eval + 45 * ext_samples \
         + 3 * psf_fma * (info.u * info.nx) * (info.u * info.ny) + 12 * info.nx * info.ny
     sm_max = (clocks.get("sm_max_mhz") or 1965.0)
-    # The voxel loop evaluates the Gaussian line by its multiplicative recurrence along v (two FP32
-    # multiplies per voxel, one MUFU.EX2 pair per kChanBlock channels), so the binding pipe is the
+    # The voxel loop sums the Gaussian line over blocks of 8 channels as a polynomial in the line
+    # ratio (one MUFU.EX2 pair per pixel and block, no ex2 per voxel), so the binding pipe is the
     # FP32 FMA pipe (quote the fraction against that pipe); the MUFU figures
     # are kept beside it for the direct-evaluation count.
     peak_fp32 = info.sm_count * FP32_LANES_PER_SM_CLK * sm_max * 1e6 / 1e9           # G lane-op/s
@@ -328,6 +328,11 @@ def run_ours(args, ranks) -> None:
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
                 "ops_per_eval": int(fp32_per_eval),
                 "ops_how": "algorithmic FP32 lane-ops: 5/ext voxel + 45/ext sample + 3 maps x (2 x taps separable | taps^2 image)/fine pixel + 12/spaxel",
+                # what the kernel executes: the block polynomial needs 27 FP32 lane-ops per pixel
+                # and 8-channel block (3.4 per voxel) where the algorithmic count above has 5 per voxel
+                "ops_executed_per_eval": int(fp32_per_eval - (5.0 - 27.0 / 8.0) * info.ext_voxels_per_eval),
+                "frac_executed": (fp32_per_eval - (5.0 - 27.0 / 8.0) * info.ext_voxels_per_eval)
+                * K * args.steps / sec_rank / 1e9 / peak_fp32,
                 "mufu_ops_per_eval_direct": int(mufu_per_eval),
                 "mufu_frac_if_direct": mufu_per_eval * K * args.steps / sec_rank / 1e9 / peak_mufu,
                 "kernel_ms_avg": statistics.mean(ms), "kernel_ms_min": min(ms)}

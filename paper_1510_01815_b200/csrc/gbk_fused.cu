@@ -594,11 +594,8 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) s0[j] = s1[j] = s2[j] = pk(0.f, 0.f);
     if (rc.use_rec) {
-      // Line recurrence (exact in exact arithmetic): with d_c = d0 + c step the line is
-      // g_c = 2^-(d_c^2), so g_{c+1} = g_c r_c with r_c = 2^-(2 d_c step + step^2) and
-      // r_{c+1} = r_c q, q = 2^-(2 step^2) a row constant.  Restarted from two ex2 every
-      // kChanBlock channels, so the rounding error of a block stays below ~3e-6 relative
-      // and the MUFU pipe carries 1/4 ex2 per voxel instead of 1.
+      // With d_c = d0 + c step the line is g_c = 2^-(d_c^2), so g_{c+1} = g_c r_c with
+      // r_c = 2^-(2 d_c step + step^2) and r_{c+1} = r_c q, q = 2^-(2 step^2) a row constant.
       // Block polynomial (exact in exact arithmetic): within a block of kChanBlock = 8 channels
       // starting at cb, g_j = g_0 r_0^j q^(j(j-1)/2), so the block's contribution to S_m is
       //   g_0 * sum_j C_m[cb + j] r_0^j,   C_m[c] = w_m[c] q^(j(j-1)/2)  (row table, see prologue):

@@ -13,8 +13,8 @@ constexpr int kMaxPsfN = 33;    // largest PSF image side
 constexpr int kMaxFastPsfN = 15; // largest PSF image side of the register-tiled 2-D pass
 constexpr int kMaxLsfR = 64;    // largest LSF tap radius, channels
 constexpr int kVBlock = 8;      // output rows per thread in the vertical pass
-constexpr int kChanBlock = 8;   // channels between two restarts of the line recurrence (gbk_fused.cu)
-constexpr float kRecMaxStep = 0.8f;  // the recurrence is used for step <= this (sigma0/dv >= 1.06)
+constexpr int kChanBlock = 8;   // channels summed by one block polynomial of the voxel loop (gbk_fused.cu)
+constexpr float kRecMaxStep = 0.8f;  // the block polynomial is used for step <= this (sigma0/dv >= 1.06)
 
 // Everything the kernels need to know about a problem; passed by value (__grid_constant__).
 struct DevProblem {
