@@ -155,8 +155,10 @@ void gbko_disc_point(const double *p, int rc_model, double x, double y, double *
   double vrot;
   if (rc_model == 0)
     vrot = (2.0 / GBKO_PI) * vt * atan(r / rt);         /* eq. 6 */
-  else
+  else if (rc_model == 1)
     vrot = vt * fmin(r / rt, 1.0);                      /* A7 */
+  else                                                  /* eq. 7, velocity-field */
+    vrot = vt * pow(r / rt, p[8]) / (1.0 + pow(r / rt, p[7]));   /* strategy only: a = p[7], g = p[8] */
   *I_out = I;
   *vlos_out = vsys + vrot * si * cos_theta;             /* eq. 8 */
 }
@@ -401,8 +403,9 @@ int gbko_eval_rows(const gbko_grid *g, const float *vobs, const float *verr, con
  * no PSF, no LSF (the paper skips steps 2.2.2-2.2.5), then the
  * velocity residual and the first term of eq. 11 only
  * (no dispersion map is modelled).  Only the seven kinematic
- * parameters p[0..6] are used; a row is out of domain when one of them is not
- * finite, r_t <= 0 or |cos i| < 1e-6 (chi2 = +INF, NaN maps).
+ * parameters p[0..6] are used (plus a = p[7], g = p[8] with the Epinat curve,
+ * rc_model 2, eq. 7); a row is out of domain when one of them is not finite,
+ * r_t <= 0, |cos i| < 1e-6, or a <= 0 or g <= 0 (chi2 = +INF, NaN maps).
  * Outputs: chi2[K]; vmap[K][ny][nx] and resid[K][ny][nx] may be NULL.        */
 int gbko_vfield_rows(const gbko_grid *g, const float *vobs, const float *verr, const uint8_t *mask,
                      const float *params, int64_t K, double *chi2, double *vmap, double *resid,
@@ -421,7 +424,13 @@ int gbko_vfield_rows(const gbko_grid *g, const float *vobs, const float *verr, c
     for (int j = 0; j < 7; ++j)
       if (!isfinite(p[j])) ok = 0;
     if (ok && (!(p[6] > 0.0) || fabs(cos(p[3] * GBKO_PI / 180.0)) < 1e-6)) ok = 0;
-    p[7] = 1.0, p[8] = 1.0, p[9] = 1.0;   /* unused by eq. 8; keep the brightness finite */
+    if (g->rc_model == 2) {               /* Epinat curve: the slopes a = p[7], g = p[8] must be > 0 */
+      if (!isfinite(p[7]) || !isfinite(p[8]) || !(p[7] > 0.0) || !(p[8] > 0.0)) ok = 0;
+      if (!ok) p[7] = 1.0, p[8] = 1.0;
+    } else {
+      p[7] = 1.0, p[8] = 1.0;             /* unused by eq. 8; keep the brightness finite */
+    }
+    p[9] = 1.0;
     double sum = 0.0;
     for (size_t q = 0; q < npix; ++q) {
       const int iy = (int)(q / (size_t)g->nx), ix = (int)(q % (size_t)g->nx);

@@ -461,7 +461,7 @@ def test_golden_hand_values_file(oracle):
             if not line:
                 continue
             tok = line.split()
-            rc = {"arctan": 0, "ramp": 1}[tok[0]]
+            rc = {"arctan": 0, "ramp": 1, "epinat": 2}[tok[0]]
             p = [float(t) for t in tok[1:11]]
             x, y, I_want, v_want = (float(t) for t in tok[11:15])
             I, v = oracle.disc_point(p, rc, x, y)
@@ -488,17 +488,17 @@ def test_vfield_map_equals_the_golden_hand_values(oracle):
             if not line:
                 continue
             tok = line.split()
-            rc = {"arctan": 0, "ramp": 1}[tok[0]]
+            rc = {"arctan": 0, "ramp": 1, "epinat": 2}[tok[0]]
             p = np.array([float(t) for t in tok[1:11]], dtype=np.float32)
             x, y, _, v_want = (float(t) for t in tok[11:15])
             if x < 0 or y < 0 or x != int(x) or y != int(y):
                 continue
-            g = _vf_grid(oracle, 16, 16, rc)
-            z = np.zeros((16, 16), np.float32)
+            g = _vf_grid(oracle, 20, 20, rc)
+            z = np.zeros((20, 20), np.float32)
             out = oracle.vfield_rows(g, z, z + 1, None, p[None], want_maps=True)
             assert out["vmap"][0, int(y), int(x)] == pytest.approx(v_want, abs=1e-5), line
             n += 1
-    assert n >= 7
+    assert n >= 11
 
 
 def test_vfield_chi2_by_hand_masks_and_domain(oracle):
@@ -533,3 +533,23 @@ def test_vfield_is_antisymmetric_about_the_centre_and_equals_delta_kernel_m1(ora
         assert np.allclose(v + v[::-1, ::-1], 16.0, atol=1e-10)
         m0, m1, m2 = oracle.model_maps(g, p[0].astype(np.float64))
         assert np.max(np.abs(m1 - v)) < 1e-6
+
+
+def test_vfield_epinat_plateaus_and_domain(oracle):
+    """Eq. 7: a = g gives a flat plateau V -> V_t, a < g rises, a > g declines
+    (PAPER.md:129); slopes must be > 0."""
+    g = _vf_grid(oracle, 400, 1, rc=2)
+    z = np.zeros((1, 400), np.float32)
+    def curve(a, gg):
+        p = np.array([[0.0, 0.0, 90.0, 90.0 - 1e-3, 0.0, 100.0, 2.0, a, gg, 0.0]], dtype=np.float32)
+        # PA = 90: x_e = -(x - x_o); i ~ 90: sin i = 1 -> v(x) = -V_rot(|x|) on this row
+        return -oracle.vfield_rows(g, z, z + 1, None, p, want_maps=True)["vmap"][0, 0]
+    flat, rising, falling = curve(1.5, 1.5), curve(1.0, 1.5), curve(1.5, 1.0)
+    assert flat[-1] == pytest.approx(100.0, rel=2e-3) and flat[2] == pytest.approx(50.0, rel=1e-9)
+    assert rising[-1] > rising[200] > 100.0 and falling[-1] < falling[200] < falling[4]
+    p = np.array([[0.0, 0.0, 0.0, 30.0, 0.0, 100.0, 2.0, 1.0, 1.0, 0.0]], dtype=np.float32)
+    assert np.isfinite(oracle.vfield_rows(g, z, z + 1, None, p)["chi2"][0])
+    for j, bad in ((7, 0.0), (8, 0.0), (7, -1.0), (8, np.nan)):
+        q = p.copy()
+        q[0, j] = bad
+        assert np.isinf(oracle.vfield_rows(g, z, z + 1, None, q)["chi2"][0]), (j, bad)
