@@ -44,7 +44,12 @@ extern "C" {
 #define GBK_P 10
 
 enum { GBK_OK = 0, GBK_ERR_ARG = 1, GBK_ERR_ALLOC = 2, GBK_ERR_CUDA = 3, GBK_ERR_UNSUPPORTED = 4 };
-enum { GBK_RC_ARCTAN = 0, GBK_RC_RAMP = 1 };     /* eq. 6; V_t*min(r/r_t,1) */
+enum { GBK_RC_ARCTAN = 0, GBK_RC_RAMP = 1, GBK_RC_EPINAT = 2 };
+/* eq. 6; V_t*min(r/r_t,1); eq. 7: V_t q^g/(1+q^a), q = r/r_t.
+ * GBK_RC_EPINAT is the curve the paper pairs with velocity-field modelling and is
+ * available with gbk_eval_vfield_batch only: its slopes travel in the row slots that strategy does
+ * not use, [7] = a > 0 and [8] = g > 0 (the cube strategy would need 12 parameters per row:
+ * gbk_eval_batch and gbk_eval_batch_unfused return GBK_ERR_UNSUPPORTED for it). */
 enum { GBK_PSF_GAUSSIAN = 0, GBK_PSF_IMAGE = 1 }; /* eq. 9; image */
 
 typedef struct gbk_problem gbk_problem; /* opaque; owns device copies of the observation */
@@ -102,6 +107,7 @@ typedef struct {
   int32_t sm_count;
   int64_t ext_voxels_per_eval; /* sum over tiles of (tw+2R)(th+2R)(nv+2R_v), R = r_p_max   */
   int32_t device;         /* CUDA device ordinal the problem lives on                      */
+  int32_t strategy;       /* GBK_STRATEGY_* the host drivers evaluate with (gbk_set_strategy) */
   int64_t unfused_bytes_per_eval; /* algorithmic HBM bytes of gbk_eval_batch_unfused per row:   */
                           /* every intermediate array written once and read once per consumer */
 } gbk_problem_info;
@@ -117,6 +123,15 @@ typedef struct {
 int gbk_create_problem(const gbk_problem_desc *desc, gbk_problem **out);
 
 int gbk_get_info(const gbk_problem *p, gbk_problem_info *info);
+
+/*
+ * Which of the paper's two modelling strategies the host drivers gbk_fit_* evaluate
+ * rows with: the intensity-cube strategy (gbk_eval_batch, the default) or the velocity-field
+ * strategy (gbk_eval_vfield_batch; residual vectors are then ny*nx long instead of 2*ny*nx).
+ * GBK_RC_EPINAT problems start as GBK_STRATEGY_VFIELD.  The eval calls themselves ignore it.
+ */
+enum { GBK_STRATEGY_CUBE = 0, GBK_STRATEGY_VFIELD = 1 };
+int gbk_set_strategy(gbk_problem *p, int32_t strategy);
 
 /*
  * The hot path (PAPER.md:63-66 steps 1-3 for K rows), fused: the model cube is
@@ -154,8 +169,8 @@ int gbk_eval_batch_unfused(gbk_problem *p, const float *params, const int32_t *g
  * PSF, no LSF, no up-sampling (the paper skips steps 2.2.2-2.2.5) -- then the
  * velocity residual and the first term of eq. 11 only.  Uses the
  * problem's vobs / verr / mask and rc_model; of a row only x_o, y_o, PA, i, V_sys, V_t, r_t are
- * read (a row is out of domain, chi2 = +INF, when one of those is not finite, r_t <= 0 or
- * |cos i| < 1e-6).  Asynchronous on `cuda_stream`, no allocation.
+ * read, plus a = row[7], g = row[8] with GBK_RC_EPINAT (a row is out of domain, chi2 = +INF, when
+ * one of those is not finite, r_t <= 0, |cos i| < 1e-6, or a <= 0 or g <= 0).  Asynchronous on `cuda_stream`, no allocation.
  *   params DEVICE [K][GBK_P]; gal_index DEVICE [K] or NULL; chi2 DEVICE [K], required
  *   vmap   DEVICE [K][ny][nx] or NULL: the model velocity field
  *   resid  DEVICE [K][ny][nx] or NULL: (model - vobs) / verr, 0 where masked

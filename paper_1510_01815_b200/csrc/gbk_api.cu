@@ -68,6 +68,7 @@ struct gbk_problem {
   };
   std::vector<Level> levels;
   int device = 0;
+  int strategy = GBK_STRATEGY_CUBE;
   int sm_count = 0, blocks_per_sm = 0;
   long long ext_voxels = 0;
   // device allocations owned by the problem
@@ -116,7 +117,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     return fail(GBK_ERR_ARG, "grid too large");
   if (!(d->dv > 0.f) || !isfinite(d->dv) || !isfinite(d->v_center))
     return fail(GBK_ERR_ARG, "dv must be > 0 and finite, v_center finite");
-  if (d->rc_model != GBK_RC_ARCTAN && d->rc_model != GBK_RC_RAMP)
+  if (d->rc_model != GBK_RC_ARCTAN && d->rc_model != GBK_RC_RAMP && d->rc_model != GBK_RC_EPINAT)
     return fail(GBK_ERR_ARG, "unknown rc_model %d", d->rc_model);
   if (!d->vobs || !d->verr) return fail(GBK_ERR_ARG, "vobs and verr are required");
   if ((d->sobs == nullptr) != (d->serr == nullptr))
@@ -231,6 +232,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   if (!p) return fail(GBK_ERR_ALLOC, "out of host memory");
   p->d = *d;
   p->device = dev;
+  p->strategy = d->rc_model == GBK_RC_EPINAT ? GBK_STRATEGY_VFIELD : GBK_STRATEGY_CUBE;
   p->sm_count = prop.multiProcessorCount;
   DevProblem& dp = p->dp;
   dp.nx = d->nx, dp.ny = d->ny, dp.nv = d->nv, dp.u = d->u, dp.n_gal = d->n_gal;
@@ -365,7 +367,25 @@ extern "C" int gbk_get_info(const gbk_problem* p, gbk_problem_info* info) {
   info->blocks_per_sm = p->blocks_per_sm, info->sm_count = p->sm_count;
   info->ext_voxels_per_eval = p->ext_voxels;
   info->device = p->device;
+  info->strategy = p->strategy;
   info->unfused_bytes_per_eval = (int64_t)unfused_algorithmic_bytes_per_row(p->dp);
+  return GBK_OK;
+}
+
+extern "C" int gbk_set_strategy(gbk_problem* p, int32_t strategy) {
+  g_err[0] = 0;
+  if (!p) return fail(GBK_ERR_ARG, "null problem");
+  if (strategy != GBK_STRATEGY_CUBE && strategy != GBK_STRATEGY_VFIELD)
+    return fail(GBK_ERR_ARG, "unknown strategy %d", strategy);
+  if (strategy == GBK_STRATEGY_CUBE && p->dp.rc_model == GBK_RC_EPINAT)
+    return fail(GBK_ERR_UNSUPPORTED, "the Epinat curve is available with the velocity-field strategy only");
+  p->strategy = strategy;
+  return GBK_OK;
+}
+
+static int check_cube_model(const gbk_problem* p) {
+  if (p && p->dp.rc_model == GBK_RC_EPINAT)
+    return fail(GBK_ERR_UNSUPPORTED, "the Epinat curve is available with gbk_eval_vfield_batch only");
   return GBK_OK;
 }
 
@@ -383,6 +403,7 @@ extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t
                               void* cuda_stream) {
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  if (int rc = check_cube_model(p)) return rc;
   if (K == 0) return GBK_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   GBK_CUDA(cudaSetDevice(p->device));
@@ -452,6 +473,7 @@ extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const
                                       float* resid, void* cuda_stream) {
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  if (int rc = check_cube_model(p)) return rc;
   if (K == 0) return GBK_OK;
   GBK_CUDA(cudaSetDevice(p->device));
   // scratch: two cubes + one contribution map per row, for a chunk of rows (<= 2 GiB, grown lazily)

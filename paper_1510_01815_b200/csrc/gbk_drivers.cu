@@ -61,6 +61,15 @@ struct Clock {
   }
 };
 
+// One batch through the strategy the problem is set to (gbk_set_strategy).  `resid` is
+// [K][2][ny][nx] for the cube strategy and [K][ny][nx] for the velocity-field strategy.
+int eval_rows(gbk_problem* p, const gbk_problem_info& info, const float* rows, const int32_t* gal,
+              int64_t K, float* chi2, float* resid, void* stream) {
+  if (info.strategy == GBK_STRATEGY_VFIELD)
+    return gbk_eval_vfield_batch(p, rows, gal, K, chi2, nullptr, resid, stream);
+  return gbk_eval_batch(p, rows, gal, K, chi2, nullptr, nullptr, nullptr, resid, stream);
+}
+
 bool finite_row(const float* r) {
   for (int j = 0; j < GBK_P; ++j)
     if (!isfinite(r[j])) return false;
@@ -193,8 +202,7 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
     }
     ng_rows_kernel<<<(n_rows + 255) / 256, 256, 0, st>>>(ax, n_rows, rows.d);
     DRV_CUDA(cudaGetLastError());
-    DRV_TRY(gbk_eval_batch(p, rows.d, gal != 0 ? gal_idx.d : nullptr, n_rows, chi2.d, nullptr, nullptr,
-                           nullptr, nullptr, cuda_stream));
+    DRV_TRY(eval_rows(p, info, rows.d, gal != 0 ? gal_idx.d : nullptr, n_rows, chi2.d, nullptr, cuda_stream));
     argmin_kernel<<<1, 1024, 0, st>>>(chi2.d, n_rows, best_i.d, best_v.d);
     DRV_CUDA(cudaGetLastError());
     DRV_CUDA(best_i.to_host(1, st));
@@ -331,7 +339,7 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
   }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DRV_CUDA(cudaSetDevice(info.device));
-  const int n = n_free, M = 2 * info.nx * info.ny;
+  const int n = n_free, M = (info.strategy == GBK_STRATEGY_VFIELD ? 1 : 2) * info.nx * info.ny;
   const int n_tri = n * (n + 1) / 2, n_terms = n_tri + n + 1;
   // fits per chunk: the residual buffer of a chunk stays below 1 GiB
   const size_t resid_per_fit = sizeof(float) * (size_t)(n + 1) * M;
@@ -385,7 +393,7 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
       DRV_CUDA(rows.to_device((size_t)kj * GBK_P, st));
       DRV_CUDA(gidx.to_device(kj, st));
       DRV_CUDA(hstep.to_device((size_t)na * n, st));
-      DRV_TRY(gbk_eval_batch(p, rows.d, gidx.d, kj, chi2.d, nullptr, nullptr, nullptr, resid.d, cuda_stream));
+      DRV_TRY(eval_rows(p, info, rows.d, gidx.d, kj, chi2.d, resid.d, cuda_stream));
       lm_normal_kernel<<<dim3(n_terms, na), 256, 0, st>>>(resid.d, hstep.d, n, M, normal.d);
       DRV_CUDA(cudaGetLastError());
       DRV_CUDA(normal.to_host((size_t)na * n_terms, st));
@@ -424,7 +432,7 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
       const int kt = nl * kLmTrials;
       DRV_CUDA(rows.to_device((size_t)kt * GBK_P, st));
       DRV_CUDA(gidx.to_device(kt, st));
-      DRV_TRY(gbk_eval_batch(p, rows.d, gidx.d, kt, chi2.d, nullptr, nullptr, nullptr, nullptr, cuda_stream));
+      DRV_TRY(eval_rows(p, info, rows.d, gidx.d, kt, chi2.d, nullptr, cuda_stream));
       DRV_CUDA(chi2.to_host(kt, st));
       DRV_CUDA(cudaStreamSynchronize(st));
       fs.evals += kt, fs.launches += 1;
@@ -523,7 +531,7 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
 
   auto evaluate = [&](int k) -> int {   // rows.h[0..k) -> chi2.h[0..k)
     DRV_CUDA(rows.to_device((size_t)k * GBK_P, st));
-    DRV_TRY(gbk_eval_batch(p, rows.d, gidx.d, k, chi2.d, nullptr, nullptr, nullptr, nullptr, cuda_stream));
+    DRV_TRY(eval_rows(p, info, rows.d, gidx.d, k, chi2.d, nullptr, cuda_stream));
     DRV_CUDA(chi2.to_host(k, st));
     DRV_CUDA(cudaStreamSynchronize(st));
     fs.evals += k, fs.launches += 1;

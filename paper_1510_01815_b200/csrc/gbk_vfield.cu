@@ -22,6 +22,7 @@ constexpr int kRows = 4;        // parameter rows per block
 constexpr int kThreads = 256;
 
 struct VRow {
+  u64 ea, eg;                               // Epinat slopes a, g (eq. 7), packed
   u64 nsp, ncp_ci, inv_rt, rt, k1, v0;     // packed (c, c): eq. 1-3 constants as in RowConst,
                                             // k1 = V_t sin i (x 2/pi for the arctan curve), v0 = V_sys - v_center
   float xo, yo, cp, nsp_ci;
@@ -44,6 +45,11 @@ __device__ void vf_row(const DevProblem& dp, const EvalArgs& a, long long k, VRo
   const bool gal_ok = gal >= 0 && gal < dp.n_gal;
   r->gal = gal_ok ? gal : 0;
   r->valid = (finite && gal_ok && v[6] > 0.f && !(fabsf(ci) < 1e-6f)) ? 1 : 0;
+  if (dp.rc_model == GBK_RC_EPINAT) {       // slopes in the row slots eq. 8 does not use
+    const float ea = p[7], eg = p[8];
+    if (!(isfinite(ea) && isfinite(eg) && ea > 0.f && eg > 0.f)) r->valid = 0;
+    r->ea = pk1(ea), r->eg = pk1(eg);
+  }
   const float inv_ci = 1.0f / ci;
   r->xo = v[0], r->yo = v[1];
   r->cp = cp, r->nsp_ci = -sp * inv_ci;
@@ -75,8 +81,15 @@ __device__ __forceinline__ u64 vf_velocity2(const DevProblem& dp, const VRow& r,
     const u64 at = atan01_2(pk(biga ? ia : qa, bigb ? ib : qb));
     f = fma2(at, pk(biga ? -1.0f : 1.0f, bigb ? -1.0f : 1.0f),
              pk(biga ? 1.5707963267948966f : 0.0f, bigb ? 1.5707963267948966f : 0.0f));
-  } else {
+  } else if (dp.rc_model == GBK_RC_RAMP) {
     f = pk(fminf(qa, 1.0f), fminf(qb, 1.0f));                   // ramp (A7)
+  } else {                                                      // eq. 7: q^g / (1 + q^a)
+    const u64 lq = pk(lg2_approx(qa), lg2_approx(qb));          // q = 0: -inf -> q^g = q^a = 0
+    float na, nb, da, db;
+    upk(mul2(lq, r.eg), na, nb);
+    upk(mul2(lq, r.ea), da, db);
+    f = mul2(pk(ex2_approx(na), ex2_approx(nb)),
+             pk(rcp_approx(1.0f + ex2_approx(da)), rcp_approx(1.0f + ex2_approx(db))));
   }
   return fma2(mul2(f, r.k1), cos_t, r.v0);                      // eq. 8
 }

@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libgbk.so")
 
 GBK_P = 10
 GBK_OK, GBK_ERR_ARG, GBK_ERR_ALLOC, GBK_ERR_CUDA, GBK_ERR_UNSUPPORTED = range(5)
-GBK_RC_ARCTAN, GBK_RC_RAMP = 0, 1
+GBK_RC_ARCTAN, GBK_RC_RAMP, GBK_RC_EPINAT = 0, 1, 2
+GBK_STRATEGY_CUBE, GBK_STRATEGY_VFIELD = 0, 1
 GBK_PSF_GAUSSIAN, GBK_PSF_IMAGE = 0, 1
 
 EXPORTS = (
@@ -57,6 +58,7 @@ class gbk_problem_info(C.Structure):
         ("blocks_per_sm", C.c_int32), ("sm_count", C.c_int32),
         ("ext_voxels_per_eval", C.c_int64),
         ("device", C.c_int32),
+        ("strategy", C.c_int32),
         ("unfused_bytes_per_eval", C.c_int64),
     ]
 
@@ -89,6 +91,8 @@ def lib():
             f = getattr(L, name)
             f.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp]
             f.restype = C.c_int
+        L.gbk_set_strategy.argtypes = [vp, C.c_int32]
+        L.gbk_set_strategy.restype = C.c_int
         L.gbk_eval_vfield_batch.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp]
         L.gbk_eval_vfield_batch.restype = C.c_int
         L.gbk_eval_batch_host.argtypes = [vp, vp, vp, C.c_int64, vp, vp]
@@ -193,6 +197,11 @@ def gbk_eval_batch(handle, params, gal_index, K, chi2, m0=None, m1=None, m2=None
 def gbk_eval_batch_unfused(handle, params, gal_index, K, chi2, m0=None, m1=None, m2=None,
                            resid=None, stream=0):
     gbk_eval_batch(handle, params, gal_index, K, chi2, m0, m1, m2, resid, stream, unfused=True)
+
+
+def gbk_set_strategy(handle, strategy: int):
+    """Strategy the host drivers evaluate with (GBK_STRATEGY_CUBE / GBK_STRATEGY_VFIELD)."""
+    _check(lib().gbk_set_strategy(handle, int(strategy)))
 
 
 def gbk_eval_vfield_batch(handle, params, gal_index, K, chi2, vmap=None, resid=None, stream=0):

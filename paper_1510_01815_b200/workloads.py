@@ -23,7 +23,7 @@ import numpy as np
 SEED = 151001815
 P = 10  # xo, yo, pa_deg, inc_deg, vsys, vt, rt, sigma0, r0, i0
 IX_XO, IX_YO, IX_PA, IX_INC, IX_VSYS, IX_VT, IX_RT, IX_SIG, IX_R0, IX_I0 = range(10)
-RC_ARCTAN, RC_RAMP = 0, 1
+RC_ARCTAN, RC_RAMP, RC_EPINAT = 0, 1, 2
 PSF_GAUSSIAN, PSF_IMAGE = 0, 1
 
 
