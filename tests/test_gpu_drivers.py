@@ -227,3 +227,42 @@ def test_nested_grids_with_the_velocity_field_strategy(oracle, torch_cuda, gbk):
         k = int(torch_cuda.argmin(ref).item())
     assert st["evals"] == 3 * 6 ** 4 and np.isfinite(chi)
     assert chi <= float(ref[k].item()) * (1 + 1e-6)       # later levels can only improve on level 0
+
+
+def test_monte_carlo_errors_are_consistent_table5(oracle, torch_cuda, gbk):
+    """Monte-Carlo error estimation as the paper does for DYNAMO (refits of
+    noise-perturbed data) as ONE batched LM call: G galaxies x R noise realisations are R*G data sets
+    of one problem.  The scatter of the refits is the error bar; the standardised residuals of one
+    realisation must then be distributed like Table 5 says (~68 % within 1 sigma,
+    ~95 % within 2 sigma)."""
+    G, R = 20, 48
+    w = wl.config(5).scaled(nx=30, ny=30, nv=64, n_gal=G * R, err_lo=5.0, err_hi=5.0, noise=5.0,
+                            psf_fwhm_hi=0.0, psf_fwhm=2.0)
+    rng = wl.rng_for(5, 77)
+    trues = wl.draw_rows(w, rng, G)
+    trues[:, wl.IX_INC] = rng.uniform(35.0, 70.0, G)      # away from the V_t - i degeneracy's ends
+    trues[:, wl.IX_VT] = rng.uniform(120.0, 300.0, G)
+    g = pu.oracle_grid(oracle, w)
+    clean = [oracle.model_maps(g, t.astype(np.float64)) for t in trues]
+    m0, m1, m2 = (np.repeat(np.stack([c[i] for c in clean]), R, axis=0) for i in range(3))
+    obs = wl.observe(w, m0, m1, m2, rng)                  # independent noise per data set
+    b = wl.box(w)
+    lo, hi = b[FREE7, 0].copy(), b[FREE7, 1].copy()
+    lo[2], hi[2] = -360.0, 720.0
+    lo[3], hi[3] = 5.0, 88.0
+    hi[5] = 600.0
+    starts = np.repeat(trues, R, axis=0).astype(np.float64)
+    starts[:, FREE7] += 0.03 * (b[FREE7, 1] - b[FREE7, 0]) * rng.uniform(-1, 1, (G * R, 7))
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        rows, chi, iters, st = gbk.gbk_fit_lm(prob.handle, starts, np.arange(G * R), FREE7, lo, hi,
+                                              max_iter=60, ftol=1e-7)
+    assert st["converged"] >= 0.98 * G * R and np.isfinite(chi).all()
+    fit = rows[:, FREE7].astype(np.float64).reshape(G, R, 7)
+    sigma = fit[:, 1:].std(axis=1, ddof=1)                 # error bars from realisations 1..R-1
+    z = (fit[:, 0] - trues[:, FREE7]) / sigma              # realisation 0 plays "the observation"
+    f1, f2 = float((np.abs(z) < 1).mean()), float((np.abs(z) < 2).mean())
+    print("Table-5 fractions within 1 and 2 sigma:", f1, f2, "median sigma:", np.median(sigma, axis=0))
+    assert 0.52 <= f1 <= 0.84 and f2 >= 0.86, (f1, f2)
+    # the reduced chi^2 of the fits is ~1 (eq. 11 with the right error bars)
+    ndof = 2 * obs.mask.reshape(G * R, -1).sum(axis=1) - 7
+    assert 0.9 < float(np.median(chi / ndof)) < 1.1
