@@ -47,6 +47,18 @@ __device__ URow uf_row(const DevProblem& dp, const float* params, const int32_t*
   return r;
 }
 
+// Which PSF set a row uses (the convolution kernels need nothing else of the row).
+__device__ __forceinline__ URow uf_row_psf(const DevProblem& dp, const int32_t* gal_index, long long k) {
+  URow r;
+  int gal = gal_index ? gal_index[k] : 0;
+  if (gal < 0 || gal >= dp.n_gal) gal = 0;
+  r.gal = gal;
+  r.psf_set = dp.psf_per_gal ? gal : 0;
+  r.r_p = dp.psf_r[r.psf_set];
+  r.valid = 1;
+  return r;
+}
+
 struct UGeom {         // extended grid of the unfused path
   int R, EW, EH, nvx;
   size_t plane, cube;  // EW*EH, plane*nvx
@@ -133,7 +145,7 @@ __global__ void uf_psf1d_kernel(const __grid_constant__ DevProblem dp, const flo
     const int c = (int)(rem / per_chan);
     rem -= c * per_chan;
     const int yy = (int)(rem / W), xx = (int)(rem - (size_t)yy * W);
-    const URow r = uf_row(dp, params, gal_index, k0 + row);
+    const URow r = uf_row_psf(dp, gal_index, k0 + row);
     const float* taps = dp.psf_taps + (size_t)r.psf_set * dp.psf_stride;
     const int ex = xx + g.R, ey = axis == 0 ? yy : yy + g.R;
     const float* src = in + (size_t)row * g.cube + (size_t)c * g.plane + (size_t)ey * g.EW + ex;
@@ -159,7 +171,7 @@ __global__ void uf_psf2d_kernel(const __grid_constant__ DevProblem dp, const flo
     const int c = (int)(rem / per_chan);
     rem -= c * per_chan;
     const int yy = (int)(rem / dp.fw), xx = (int)(rem - (size_t)yy * dp.fw);
-    const URow r = uf_row(dp, params, gal_index, k0 + row);
+    const URow r = uf_row_psf(dp, gal_index, k0 + row);
     const int nn = 2 * r.r_p + 1;
     const float* taps = dp.psf_taps + (size_t)r.psf_set * dp.psf_stride;
     const float* src = in + (size_t)row * g.cube + (size_t)c * g.plane + (size_t)(yy + g.R - r.r_p) * g.EW +
