@@ -426,3 +426,34 @@ def test_create_rejects_bad_descriptors(oracle, torch_cuda, gbk):
     with pytest.raises(gbk.GbkError) as e:
         gbk.Problem(**bad)
     assert e.value.code == gbk.GBK_ERR_UNSUPPORTED
+
+
+def test_eval_batch_in_a_cuda_graph(oracle, torch_cuda, gbk):
+    """gbk_eval_batch is asynchronous on the caller's stream and allocates nothing once its scratch
+    is sized, so it can be captured in a CUDA graph and replayed on new parameters (bench-style
+    inner loops, optimiser iterations)."""
+    torch = torch_cuda
+    w, g, obs, true, rng = _tiny_case(oracle, nx=40, ny=36)
+    rows_a = _rows_near(w, true, rng, 300)
+    rows_b = _rows_near(w, true, rng, 300)
+    with gbk.Problem(**pu.gbk_desc(w, obs, tile_w=16, tile_h=12)) as prob:   # tiled: two kernels
+        params = torch.from_numpy(rows_a).cuda()
+        chi2 = torch.empty(300, dtype=torch.float32, device="cuda")
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            gbk.gbk_eval_batch(prob.handle, params, None, 300, chi2, stream=side.cuda_stream)  # sizes scratch
+        side.synchronize()
+        eager = chi2.cpu().numpy().copy()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            gbk.gbk_eval_batch(prob.handle, params, None, 300, chi2, stream=side.cuda_stream)
+        chi2.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(chi2.cpu().numpy(), eager)
+        params.copy_(torch.from_numpy(rows_b))
+        graph.replay()
+        torch.cuda.synchronize()
+        got_b = chi2.cpu().numpy()
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows_b[:16])
+    pu.compare(ref, {"chi2": got_b[:16]}, rows_b[:16], False, "graph replay")
