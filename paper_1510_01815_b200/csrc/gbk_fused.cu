@@ -379,18 +379,25 @@ __device__ __forceinline__ float moments_blocks(const DevProblem& dp, const Eval
                                                 const RowConst& rc, long long k, const float* p0,
                                                 const float* p1, const float* p2, int ews, int tw,
                                                 int th, int tx0, int ty0, int tid, int nthreads) {
-  const float* const plane[3] = {p0, p1, p2};
   const int u = dp.u, sw = tw / u, sh = th / u;
+  const unsigned magic = div_magic(sw);
   float chi = 0.0f;
   for (int item = tid; item < sw * sh; item += nthreads) {
-    const int Y = item / sw, X = item - Y * sw;
+    const int Y = div_fast(item, magic), X = item - Y * sw;
     const int pix = (ty0 / u + Y) * dp.nx + tx0 / u + X;
     const float4 ob = load_obs(dp, rc, pix);
-    float s[3] = {0.f, 0.f, 0.f};
-    for (int q = 0; q < 3; ++q)
+    float s0 = 0.f, s1 = 0.f, s2 = 0.f;
+    if (u == 1) {                                  // no down-sampling: one value per map
+      const int o = Y * ews + X;
+      s0 = p0[o], s1 = p1[o], s2 = p2[o];
+    } else {
       for (int dy = 0; dy < u; ++dy)
-        for (int dx = 0; dx < u; ++dx) s[q] += plane[q][(Y * u + dy) * ews + X * u + dx];
-    chi += spaxel_finish<OUT>(dp, a, rc, k, pix, ob, s[0], s[1], s[2]);
+        for (int dx = 0; dx < u; ++dx) {
+          const int o = (Y * u + dy) * ews + X * u + dx;
+          s0 += p0[o], s1 += p1[o], s2 += p2[o];
+        }
+    }
+    chi += spaxel_finish<OUT>(dp, a, rc, k, pix, ob, s0, s1, s2);
   }
   return chi;
 }
