@@ -347,7 +347,10 @@ def run_ours(args, ranks) -> None:
     if ranks.is_main and ranks.world == 1 and not args.no_cpu_baseline:
         cores = host_cores()
         cpu = time_oracle(cfg, args.cpu_rows or 32 * cores, 1, 1, cores)
+        one = time_oracle(cfg, 24, 1, 1, 1)          # the paper's single-thread column
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        cpu["value_1_thread"] = one["value"]
+        cpu["sample_1_thread"] = one["sample"]
 
     unfused = time_unfused(gbk, torch, prob, dev_batches[0], K, info) \
         if (ranks.is_main and not args.no_fits) else None
