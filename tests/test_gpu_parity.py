@@ -457,3 +457,53 @@ def test_eval_batch_in_a_cuda_graph(oracle, torch_cuda, gbk):
         got_b = chi2.cpu().numpy()
     ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows_b[:16])
     pu.compare(ref, {"chi2": got_b[:16]}, rows_b[:16], False, "graph replay")
+
+
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("GBK_FUZZ_CASES", "24"))))
+def test_random_shapes_and_kernels(oracle, torch_cuda, gbk, seed):
+    """Seeded random problems: odd grid sizes, any up-sampling, Gaussian or image PSFs of any small
+    size (symmetric or not), delta or wide LSFs, explicit or automatic tiles, both rotation curves,
+    with and without a dispersion map -- chi^2 and maps against the oracle."""
+    rng = np.random.default_rng(1510_01815 + seed)
+    nx, ny = int(rng.integers(3, 34)), int(rng.integers(3, 30))
+    u = int(rng.choice([1, 1, 1, 2, 3]))
+    nv = int(rng.integers(12, 70))
+    dv = float(rng.choice([10.0, 20.0, 30.0]))
+    image = bool(rng.random() < 0.4)
+    kw = dict(nx=nx, ny=ny, nv=nv, u=u, dv=dv, rc_model=int(rng.integers(0, 2)),
+              lsf_sigma=float(rng.choice([0.0, 0.6, 1.0, 2.3])) * dv)
+    if image:
+        n = int(rng.choice([1, 3, 5, 7, 9, 11, 15, 17]))
+        img = rng.random((n, n)).astype(np.float32) + 0.05          # asymmetric: convolution, not correlation
+        w = wl.config(4).scaled(psf_n=n, sigma0=float(rng.uniform(0.5, 3.0)) * dv, r0_lo=4.0, r0_hi=9.0,
+                                mask_rule="m0_rel", **kw)
+        psf = img.astype(np.float64) / img.astype(np.float64).sum()
+    else:
+        fw = float(rng.choice([0.0, 0.8, 1.7, 2.6, 3.9]))
+        if np.ceil(4.0 * u * fw / 2.3548) > 16:          # the library's separable limit: R <= 16 fine pixels
+            fw = 1.7
+        w = wl.config(1).scaled(psf_fwhm=fw, sigma0=float(rng.uniform(0.5, 3.0)) * dv, **kw)
+        psf = oracle.psf_gaussian_image(pu.f32(fw), u)
+    lsf = oracle.gaussian_taps(pu.f32(w.lsf_sigma) / pu.f32(w.dv) if w.lsf_sigma > 0 else 0.0)
+    g = oracle.Grid(nx=nx, ny=ny, nv=nv, u=u, v_center=0.0, dv=pu.f32(dv), rc_model=w.rc_model, psf=psf,
+                    lsf=lsf)
+    true = np.array([0.5 * nx + rng.uniform(-1, 1), 0.5 * ny + rng.uniform(-1, 1), rng.uniform(0, 360),
+                     rng.uniform(20, 75), rng.uniform(-40, 40), rng.uniform(60, 280), rng.uniform(1, 6),
+                     w.sigma0, rng.uniform(3, 8), rng.uniform(0.5, 3)], dtype=np.float32)
+    m0, m1, m2 = oracle.model_maps(g, true.astype(np.float64))
+    obs = wl.observe(w, m0[None], m1[None], m2[None], rng)
+    K = int(rng.choice([1, 3, 17]))
+    rows = _rows_near(w, true, rng, K)
+    rows[:, wl.IX_SIG] = w.sigma0 * rng.uniform(0.7, 1.5, K)
+    no_disp = bool(rng.random() < 0.25)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], None if no_disp else obs.sobs[0],
+                           None if no_disp else obs.serr[0], obs.mask[0], rows, want_maps=True)
+    d = pu.gbk_desc(w, obs)
+    if image:
+        d["psf_image"] = img
+    if no_disp:
+        d["sobs"] = d["serr"] = None
+    if rng.random() < 0.5:
+        d["tile_w"], d["tile_h"] = int(rng.integers(1, nx + 1)), int(rng.integers(1, ny + 1))
+    got = _gpu_eval(torch_cuda, gbk, d, rows)
+    pu.compare(ref, got, rows, True, f"random case {seed}: {kw} image={image} tile={d.get('tile_w')},{d.get('tile_h')}")
