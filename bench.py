@@ -413,6 +413,22 @@ def time_fits(gbk, torch, prob3, w3, true3) -> dict:
                       "converged": st["converged"], "chi2": float(chi2[0]),
                       "abs_err": [float(abs(rows[0, j] - true2[j])) for j in free7]}
     out["lm_cfg5_survey"] = time_survey(gbk, torch)
+    # config 4: nested sampling with K = 256 live points and batches of 256 candidates
+    # (256x256x48, Moffat 15x15 image PSF, ramp curve)
+    w4 = wl.config(4)
+    rng4 = wl.rng_for(4, 400)
+    true4 = wl.draw_rows(w4, rng4, 1)[0]
+    obs4 = observation_from_gpu(gbk, torch, w4, true4, rng4)
+    b4 = wl.box(w4)
+    free5 = [wl.IX_PA, wl.IX_INC, wl.IX_VSYS, wl.IX_VT, wl.IX_RT]
+    with gbk.Problem(**desc_for(w4, obs4)) as prob4:
+        r = gbk.gbk_fit_ns(prob4.handle, true4, 0, free5, b4[free5, 0], b4[free5, 1], n_live=256,
+                           batch=256, max_batches=1000, enlarge=0.2, tol=0.05, seed=4)
+    err = [float(abs(r["best_row"][j] - true4[j])) for j in free5]
+    err[0] = float(abs((err[0] + 180.0) % 360.0 - 180.0))
+    out["ns_cfg4"] = {"ms": r["stats"]["ms_total"], "evals": r["stats"]["evals"],
+                      "batches": r["stats"]["iterations"], "converged": r["stats"]["converged"],
+                      "chi2": r["best_chi2"], "log_evidence": r["log_evidence"], "abs_err": err}
     return out
 
 

@@ -254,10 +254,12 @@ int gbk_fit_lm(gbk_problem *p, int32_t n_fits, const float *start_rows, const in
 
 /*
  * Nested sampling with ln L = -chi^2/2 (A20) and a uniform prior on
- * the box: n_live live points; every batch draws `batch` candidates uniformly from the bounding
- * box of the live points enlarged by `enlarge` (>= 0, fraction of its width; clipped to the prior
- * box) and evaluates them in one launch; each candidate that beats the current worst live point
- * replaces it (prior volume X_i = exp(-i/n_live), evidence by the trapezoid-free simple rule).
+ * the box: n_live live points; every batch draws `batch` candidates uniformly from the ellipsoid of
+ * the live points (their mean and covariance, scaled to hold them all and enlarged by the fraction
+ * `enlarge` >= 0; intersected with their enlarged bounding box and the prior box; the box alone
+ * while the covariance is singular) and evaluates them in one launch; each candidate that beats
+ * the current worst live point replaces it (prior volume X_i = exp(-i/n_live), evidence by the
+ * simple rule Z += L_i (X_{i-1} - X_i)).
  * Stops when L_max X_i < tol x Z or after max_batches.  Outputs: the best row, its chi^2, the
  * posterior-mean row and ln Z.  `seed` seeds the driver's own generator (xoshiro256**).
  */

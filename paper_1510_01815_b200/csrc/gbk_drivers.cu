@@ -558,8 +558,11 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
   bool done = false;
   std::vector<double> blo(n), bhi(n);
   for (int b = 0; b < max_batches && !done; ++b) {
-    // sampling box: bounding box of the live points, enlarged, clipped to the prior
-    double ln_shrink = 0.0;   // ln(volume of the sampling box / prior volume): bookkeeping only
+    // Sampling region: the ellipsoid of the live points (their mean and covariance, scaled to hold
+    // every live point, then enlarged), intersected with the bounding box of the live points
+    // (enlarged likewise) and the prior box -- single-ellipsoid nested sampling (the scheme
+    // MultiNest generalises).  Falls back to the box alone while the covariance
+    // is singular.  Parameters are scaled to the prior box so the covariance is well conditioned.
     for (int a = 0; a < n; ++a) {
       double mn = INFINITY, mx = -INFINITY;
       for (int i = 0; i < n_live; ++i) {
@@ -568,10 +571,85 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
       }
       const double pad = 0.5 * enlarge * (mx - mn) + 1e-6 * (phi[a] - plo[a]);
       blo[a] = std::max(plo[a], mn - pad), bhi[a] = std::min(phi[a], mx + pad);
-      ln_shrink += log((bhi[a] - blo[a]) / (phi[a] - plo[a]));
     }
-    (void)ln_shrink;
-    for (int i = 0; i < batch; ++i) draw(rows.h + (size_t)i * GBK_P, blo.data(), bhi.data());
+    double mu[GBK_P], Lc[GBK_P][GBK_P], scale = 0.0;
+    bool ellipsoid = n_live > 2 * n;
+    if (ellipsoid) {
+      double cov[GBK_P][GBK_P] = {};
+      for (int a = 0; a < n; ++a) {
+        mu[a] = 0.0;
+        for (int i = 0; i < n_live; ++i)
+          mu[a] += (live[(size_t)i * GBK_P + free_param[a]] - plo[a]) / (phi[a] - plo[a]);
+        mu[a] /= n_live;
+      }
+      for (int i = 0; i < n_live; ++i) {
+        double dlt[GBK_P];
+        for (int a = 0; a < n; ++a)
+          dlt[a] = (live[(size_t)i * GBK_P + free_param[a]] - plo[a]) / (phi[a] - plo[a]) - mu[a];
+        for (int a = 0; a < n; ++a)
+          for (int c = 0; c <= a; ++c) cov[a][c] += dlt[a] * dlt[c] / (n_live - 1);
+      }
+      for (int j = 0; j < n && ellipsoid; ++j) {            // Cholesky, lower triangle
+        double d = cov[j][j];
+        for (int q = 0; q < j; ++q) d -= Lc[j][q] * Lc[j][q];
+        if (!(d > 1e-24)) {
+          ellipsoid = false;
+          break;
+        }
+        Lc[j][j] = sqrt(d);
+        for (int i = j + 1; i < n; ++i) {
+          double t = cov[i][j];
+          for (int q = 0; q < j; ++q) t -= Lc[i][q] * Lc[j][q];
+          Lc[i][j] = t / Lc[j][j];
+        }
+      }
+      if (ellipsoid) {                                       // largest Mahalanobis distance of a live point
+        for (int i = 0; i < n_live; ++i) {
+          double y[GBK_P], d2 = 0.0;
+          for (int a = 0; a < n; ++a) {
+            double t = (live[(size_t)i * GBK_P + free_param[a]] - plo[a]) / (phi[a] - plo[a]) - mu[a];
+            for (int q = 0; q < a; ++q) t -= Lc[a][q] * y[q];
+            y[a] = t / Lc[a][a];
+            d2 += y[a] * y[a];
+          }
+          scale = std::max(scale, d2);
+        }
+        scale = sqrt(scale) * (1.0 + enlarge);
+      }
+    }
+    for (int i = 0; i < batch; ++i) {
+      float* row = rows.h + (size_t)i * GBK_P;
+      if (!ellipsoid) {
+        draw(row, blo.data(), bhi.data());
+        continue;
+      }
+      memcpy(row, base_row, sizeof(float) * GBK_P);
+      for (int attempt = 0;; ++attempt) {
+        // uniform in the unit n-ball: Gaussian direction, radius U^(1/n)
+        double z[GBK_P], nrm = 0.0;
+        for (int a = 0; a < n; a += 2) {
+          const double u1 = std::max(rng.uniform(), 1e-300), u2 = rng.uniform();
+          const double rr = sqrt(-2.0 * log(u1));
+          z[a] = rr * cos(6.283185307179586 * u2);
+          if (a + 1 < n) z[a + 1] = rr * sin(6.283185307179586 * u2);
+        }
+        for (int a = 0; a < n; ++a) nrm += z[a] * z[a];
+        const double rad = scale * pow(rng.uniform(), 1.0 / n) / sqrt(nrm);
+        bool inside = true;
+        for (int a = 0; a < n; ++a) {
+          double t = mu[a];
+          for (int q = 0; q <= a; ++q) t += Lc[a][q] * z[q] * rad;
+          const double v = plo[a] + t * (phi[a] - plo[a]);
+          if (!(v >= blo[a] && v <= bhi[a])) inside = false;
+          row[free_param[a]] = (float)v;
+        }
+        if (inside) break;
+        if (attempt >= 1000) {                               // pathological: fall back to the box
+          draw(row, blo.data(), bhi.data());
+          break;
+        }
+      }
+    }
     DRV_TRY(evaluate(batch));
     fs.iterations += 1;
     for (int i = 0; i < batch && !done; ++i) {
