@@ -625,6 +625,13 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
           g[j] = pk(ex2_approx(-ea), ex2_approx(-eb));
           r[j] = pk(ex2_approx(fminf(ra, rcl)), ex2_approx(fminf(rb, rcl)));
         }
+        // A block whose g_0 has flushed to zero for every pixel of the warp contributes exactly
+        // g_0 * P = 0 to all three sums (P is finite by the clamp): skipping it is bit-identical.
+        // That is the part of the band further than ~13 sigma_0 from the line of all 128 pixels.
+        u64 any_g = g[0];
+#pragma unroll
+        for (int j = 1; j < kPairs; ++j) any_g |= g[j];
+        if (!__any_sync(0xffffffffu, any_g != 0ull)) continue;
         const ulonglong2* C = reinterpret_cast<const ulonglong2*>(sm.coef + b * (3 * kChanBlock));
 #pragma unroll
         for (int m = 0; m < 3; ++m) {
