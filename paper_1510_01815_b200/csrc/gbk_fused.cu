@@ -108,6 +108,7 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->mstep2 = -rc->step * rc->step;
   rc->use_rec = rc->step <= kRecMaxStep ? 1 : 0;
   rc->r_clamp = fmaf(13.0f * rc->step, rc->step, fmaf(10.4f, rc->step, 0.5f));
+  rc->inv_bstep = 1.0f / ((float)kChanBlock * rc->step);
   rc->k1 = -s * vrot_scale;                                  // d0 = k1 * f(r) * cos(theta) + k0
   rc->k0 = s * dp.vrel_first - s * (v[4] - dp.v_center);
   const float line_amp = dp.dv / (sigma0 * 2.5066282746310002f) * dp.inv_u2;  // sqrt(2 pi)
@@ -613,7 +614,22 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       const u64 m2s = pk1(rc.m2step), ms2 = pk1(rc.mstep2);
       const float rcl = rc.r_clamp;
       const int nblk = dp.nvx_pad / kChanBlock;
-      for (int b = 0; b < nblk; ++b) {
+      // Blocks that can hold a non-zero g_0 for some pixel of this warp item: |d_0 + 8 b step| < 11.4
+      // (2^-(11.4^2) is far below the flush threshold 2^-126).  A conservative window; the exact
+      // vote below still decides block by block.  NaN offsets give the full range, infinite ones
+      // an empty one (every g is 0 then).
+      float wlo = 3.0e38f, whi = -3.0e38f;
+#pragma unroll
+      for (int j = 0; j < kPairs; ++j) {
+        float da, db;
+        upk(d0[j], da, db);
+        wlo = fminf(wlo, fminf((-11.4f - da) * rc.inv_bstep, (-11.4f - db) * rc.inv_bstep));
+        whi = fmaxf(whi, fmaxf((11.4f - da) * rc.inv_bstep, (11.4f - db) * rc.inv_bstep));
+        if (da != da || db != db) wlo = -3.0e38f, whi = 3.0e38f;
+      }
+      const int b_lo = __reduce_min_sync(0xffffffffu, (int)fminf(fmaxf(floorf(wlo), 0.0f), (float)nblk));
+      const int b_hi = __reduce_max_sync(0xffffffffu, (int)fmaxf(fminf(ceilf(whi), (float)(nblk - 1)), -1.0f));
+      for (int b = b_lo; b <= b_hi; ++b) {
         u64 g[kPairs], r[kPairs];
         const float cf = (float)(b * kChanBlock);
 #pragma unroll
