@@ -337,6 +337,10 @@ def run_ours(args, ranks) -> None:
                 "ops_executed_max_per_eval": int(fp32_per_eval - (5.0 - 27.0 / 8.0) * info.ext_voxels_per_eval),
                 "frac_executed_max": (fp32_per_eval - (5.0 - 27.0 / 8.0) * info.ext_voxels_per_eval)
                 * K * args.steps / sec_rank / 1e9 / peak_fp32,
+                "note": "frac counts the ALGORITHMIC operations of SURVEY.md section 8(d) (5 per voxel); the "
+                        "kernel sums each 8-channel block as a polynomial (3.4 per voxel) and skips blocks that "
+                        "are exactly zero, so it executes fewer: ncu has the FP32 pipe ~51 % busy "
+                        "(profiles/r01_fused_kernel_ncu.md)",
                 "mufu_ops_per_eval_direct": int(mufu_per_eval),
                 "mufu_frac_if_direct": mufu_per_eval * K * args.steps / sec_rank / 1e9 / peak_mufu,
                 "kernel_ms_avg": statistics.mean(ms), "kernel_ms_min": min(ms)}
