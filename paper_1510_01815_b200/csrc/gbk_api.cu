@@ -284,7 +284,6 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   // launch shape: P pixels per thread in the voxel loop, threads per block
   const int n_ext = (dp.tile_w + 2 * r_p_max) * (dp.tile_h + 2 * r_p_max);
   p->fl.smem_bytes = (int)smem;
-  p->fl.pixels_per_thread = 4;
   // 256 threads: three blocks of a whole-field config-3 tile are resident per SM (70.7 KB and
   // <= 85 registers x 256 threads each), so their phases overlap (measured best of 128..384)
   auto threads_for = [&](const DevProblem& q) {

@@ -103,10 +103,9 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->rt = rt;
   rc->nl2e_inv_r0 = -1.4426950408889634f / r0;
   rc->step = s * dp.dv;
-  rc->q = exp2f(-2.0f * rc->step * rc->step);
   rc->m2step = -2.0f * rc->step;
   rc->mstep2 = -rc->step * rc->step;
-  rc->use_rec = rc->step <= kRecMaxStep ? 1 : 0;
+  rc->use_poly = rc->step <= kPolyMaxStep ? 1 : 0;
   rc->r_clamp = fmaf(13.0f * rc->step, rc->step, fmaf(10.4f, rc->step, 0.5f));
   rc->inv_bstep = 1.0f / ((float)kChanBlock * rc->step);
   rc->k1 = -s * vrot_scale;                                  // d0 = k1 * f(r) * cos(theta) + k0
@@ -601,7 +600,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
     u64 s0[kPairs], s1[kPairs], s2[kPairs];
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) s0[j] = s1[j] = s2[j] = pk(0.f, 0.f);
-    if (rc.use_rec) {
+    if (rc.use_poly) {
       // With d_c = d0 + c step the line is g_c = 2^-(d_c^2), so g_{c+1} = g_c r_c with
       // r_c = 2^-(2 d_c step + step^2) and r_{c+1} = r_c q, q = 2^-(2 step^2) a row constant.
       // Block polynomial (exact in exact arithmetic): within a block of kChanBlock = 8 channels
@@ -720,7 +719,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     const float sigma0 = a.params[k * GBK_P + 7];
     const float s_ = 1.0f / (sigma0 * 1.1774100225154747f);
     const float step = s_ * dp.dv;
-    const bool poly = step <= kRecMaxStep;        // false for NaN: the row is out of domain anyway
+    const bool poly = step <= kPolyMaxStep;        // false for NaN: the row is out of domain anyway
     for (int c = tid; c < dp.nvx_pad; c += nthreads) {
       const float4 w = dp.chan_tab[c];
       sm.chan[c] = w;

@@ -14,7 +14,7 @@ constexpr int kMaxFastPsfN = 15; // largest PSF image side of the register-tiled
 constexpr int kMaxLsfR = 64;    // largest LSF tap radius, channels
 constexpr int kVBlock = 8;      // output rows per thread in the vertical pass
 constexpr int kChanBlock = 8;   // channels summed by one block polynomial of the voxel loop (gbk_fused.cu)
-constexpr float kRecMaxStep = 0.8f;  // the block polynomial is used for step <= this (sigma0/dv >= 1.06)
+constexpr float kPolyMaxStep = 0.8f;  // the block polynomial is used for step <= this (sigma0/dv >= 1.06)
 
 // Everything the kernels need to know about a problem; passed by value (__grid_constant__).
 struct DevProblem {
@@ -59,10 +59,9 @@ struct RowConst {
   float inv_rt, rt;
   float nl2e_inv_r0;  // -log2(e)/r0
   float step;         // s * dv with s = 1/(sigma0 sqrt(2 ln 2)): exp(-dv^2/(2 sigma0^2)) = 2^-(s dv)^2
-  float q;            // 2^(-2 step^2): ratio of consecutive line ratios (recurrence of the voxel loop)
   float m2step;       // -2 step
   float mstep2;       // -step^2
-  int use_rec;        // step <= kRecMaxStep: the multiplicative recurrence is safe
+  int use_poly;       // step <= kPolyMaxStep: the block polynomial is safe
   float r_clamp;      // upper clamp of log2 r_0 in the block polynomial (gbk_fused.cu, voxel loop)
   float inv_bstep;    // 1 / (kChanBlock * step): blocks per unit of the line-centre offset d
   float k1;           // -s * V_t sin i (* 2/pi for the arctan curve)
@@ -78,7 +77,6 @@ struct RowConst {
 struct FusedLaunch {
   int threads;
   int smem_bytes;
-  int pixels_per_thread;  // P of the voxel loop
 };
 
 cudaError_t launch_fused(const DevProblem& dp, const EvalArgs& a, const FusedLaunch& fl,
