@@ -357,6 +357,7 @@ __device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const Eva
     }
     const int pix0 = (ty0 + y0) * dp.nx + tx0 + x;
     const bool second = x + 1 < tw;
+    float acc = 0.0f;     // per item, so the sum stays in a register (chi itself is long-lived and spills)
 #pragma unroll
     for (int m = 0; m < BY; ++m)
       if (y0 + m < th) {
@@ -365,10 +366,11 @@ __device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const Eva
         upk(res[0][m], s0a, s0b);
         upk(res[1][m], s1a, s1b);
         upk(res[2][m], s2a, s2b);
-        chi += spaxel_finish<OUT>(dp, a, rc, k, pix, load_obs(dp, rc, pix), s0a, s1a, s2a);
+        acc += spaxel_finish<OUT>(dp, a, rc, k, pix, load_obs(dp, rc, pix), s0a, s1a, s2a);
         if (second)
-          chi += spaxel_finish<OUT>(dp, a, rc, k, pix + 1, load_obs(dp, rc, pix + 1), s0b, s1b, s2b);
+          acc += spaxel_finish<OUT>(dp, a, rc, k, pix + 1, load_obs(dp, rc, pix + 1), s0b, s1b, s2b);
       }
+    chi += acc;
   }
   return chi;
 }
