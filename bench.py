@@ -324,7 +324,7 @@ def run_ours(args, ranks) -> None:
                 "achieved": achieved, "peak": peak_fp32, "unit": "Gop/s", "frac": achieved / peak_fp32,
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed capture
                 # profiles/r01_fused_kernel_ncu.md (config 3 only; not measured live)
-                "traffic": 335360 if cfg == 3 else None, "traffic_unit": "bytes per launch",
+                "traffic": 327424 if cfg == 3 else None, "traffic_unit": "bytes per launch",
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
                 "ops_per_eval": int(fp32_per_eval),
                 "ops_how": "algorithmic FP32 lane-ops: 5/ext voxel + 45/ext sample + 3 maps x (2 x taps separable | taps^2 image)/fine pixel + 12/spaxel",
