@@ -325,7 +325,13 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   GBK_CUDA_P(cudaMemcpy(p->psf_r, psf_r.data(), sizeof(int) * n_psf, cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->obs, obs.data(), sizeof(float4) * obs.size(), cudaMemcpyHostToDevice));
   dp.chan_tab = p->chan_tab, dp.psf_taps = p->psf_taps, dp.psf_r = p->psf_r, dp.obs = p->obs;
-  GBK_CUDA_P(fused_prepare(p->fl));
+  {
+    // opt in to the device's largest dynamic shared memory once and for all: the attribute belongs
+    // to the kernel, not to this problem, and a later problem with a smaller tile must not lower it
+    FusedLaunch cap = p->fl;
+    cap.smem_bytes = (int)smem_cap;
+    GBK_CUDA_P(fused_prepare(cap));
+  }
   GBK_CUDA_P(fused_occupancy(p->fl, &p->blocks_per_sm));
   auto rounds_for = [&](const DevProblem& q, const FusedLaunch& f) {
     const int ne = (q.tile_w + 2 * r_p_max) * (q.tile_h + 2 * r_p_max);

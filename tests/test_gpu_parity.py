@@ -507,3 +507,24 @@ def test_random_shapes_and_kernels(oracle, torch_cuda, gbk, seed):
         d["tile_w"], d["tile_h"] = int(rng.integers(1, nx + 1)), int(rng.integers(1, ny + 1))
     got = _gpu_eval(torch_cuda, gbk, d, rows)
     pu.compare(ref, got, rows, True, f"random case {seed}: {kw} image={image} tile={d.get('tile_w')},{d.get('tile_h')}")
+
+
+def test_two_problems_with_different_tiles_coexist(oracle, torch_cuda, gbk):
+    """The dynamic shared-memory opt-in is a property of the kernel: creating a second problem with
+    a smaller tile must not break launches of the first, larger one."""
+    torch = torch_cuda
+    w_big, g_big, obs_big, true_big, rng = _tiny_case(oracle, nx=64, ny=64, nv=40)     # > 48 KB tile
+    w_small, g_small, obs_small, true_small, _ = _tiny_case(oracle)
+    rows_big = _rows_near(w_big, true_big, rng, 4)
+    rows_small = _rows_near(w_small, true_small, rng, 4)
+    with gbk.Problem(**pu.gbk_desc(w_big, obs_big, tile_w=64, tile_h=64)) as big:
+        assert big.info.smem_bytes > 48 * 1024
+        with gbk.Problem(**pu.gbk_desc(w_small, obs_small)) as small:
+            a = small.eval(torch.from_numpy(rows_small).cuda())["chi2"].cpu().numpy()
+            b = big.eval(torch.from_numpy(rows_big).cuda())["chi2"].cpu().numpy()      # after the small one
+    ref_b = oracle.eval_rows(g_big, obs_big.vobs[0], obs_big.verr[0], obs_big.sobs[0], obs_big.serr[0],
+                             obs_big.mask[0], rows_big)
+    ref_a = oracle.eval_rows(g_small, obs_small.vobs[0], obs_small.verr[0], obs_small.sobs[0],
+                             obs_small.serr[0], obs_small.mask[0], rows_small)
+    pu.compare(ref_b, {"chi2": b}, rows_big, False, "big after small")
+    pu.compare(ref_a, {"chi2": a}, rows_small, False, "small")
