@@ -16,7 +16,9 @@
  * Plain C, no torch types.  Every pointer says whether it is HOST or DEVICE
  * memory.  No function throws or aborts; all return GBK_OK or an error code
  * and leave a message for gbk_last_error().  There is NO CPU fallback: without
- * a CUDA device every compute call returns GBK_ERR_CUDA.
+ * a CUDA device every compute call returns GBK_ERR_CUDA.  Calls make the problem's device current
+ * for their duration and restore the caller's device; a problem must not be used by two host
+ * threads at the same time (its scratch buffers grow on demand).
  *
  * Model row (GBK_P = 10 floats):
  *   [0] x_o, [1] y_o    kinematic centre, data pixels (pixel j is centred on j)

@@ -223,7 +223,8 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   // ---- device and tiling ---------------------------------------------------------------
   int dev = d->device;
   if (dev < 0) GBK_CUDA(cudaGetDevice(&dev));
-  GBK_CUDA(cudaSetDevice(dev));
+  DeviceGuard guard(dev);
+  GBK_CUDA(guard.status);
   cudaDeviceProp prop;
   GBK_CUDA(cudaGetDeviceProperties(&prop, dev));
   const size_t smem_cap = prop.sharedMemPerBlockOptin;
@@ -411,7 +412,8 @@ extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t
   if (int rc = check_cube_model(p)) return rc;
   if (K == 0) return GBK_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  GBK_CUDA(cudaSetDevice(p->device));
+  DeviceGuard guard(p->device);
+  GBK_CUDA(guard.status);
   // tiling: the level with the fewest (waves of blocks) x (voxel-loop passes per block); ties go
   // to the larger tile (less halo work, and one tile needs no second kernel)
   size_t lv = 0;
@@ -441,7 +443,8 @@ extern "C" int gbk_eval_vfield_batch(gbk_problem* p, const float* params, const 
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
   if (K == 0) return GBK_OK;
-  GBK_CUDA(cudaSetDevice(p->device));
+  DeviceGuard guard(p->device);
+  GBK_CUDA(guard.status);
   EvalArgs a{params, gal_index, (long long)K, chi2, nullptr, vmap, nullptr, resid, nullptr};
   GBK_CUDA(launch_vfield(p->dp, a, (cudaStream_t)cuda_stream));
   return GBK_OK;
@@ -453,7 +456,8 @@ extern "C" int gbk_eval_batch_host(gbk_problem* p, const float* params, const in
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
   if (K == 0) return GBK_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  GBK_CUDA(cudaSetDevice(p->device));
+  DeviceGuard guard(p->device);
+  GBK_CUDA(guard.status);
   if (K > p->st_cap) {
     cudaFree(p->st_params), cudaFree(p->st_gal), cudaFree(p->st_chi2);
     p->st_params = nullptr, p->st_gal = nullptr, p->st_chi2 = nullptr, p->st_cap = 0;
@@ -480,7 +484,8 @@ extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
   if (int rc = check_cube_model(p)) return rc;
   if (K == 0) return GBK_OK;
-  GBK_CUDA(cudaSetDevice(p->device));
+  DeviceGuard guard(p->device);
+  GBK_CUDA(guard.status);
   // scratch: two cubes + one contribution map per row, for a chunk of rows (<= 2 GiB, grown lazily)
   const size_t per_row = unfused_bytes_per_row(p->dp);
   const long long cap_rows = std::max<long long>(1, (long long)((size_t(2) << 30) / per_row));

@@ -160,7 +160,8 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
   if (n_rows_d > (double)(1 << 24)) return fail(GBK_ERR_ARG, "nodes^n_axes exceeds 2^24 rows");
   const int n_rows = (int)n_rows_d;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  DRV_CUDA(cudaSetDevice(info.device));
+  DeviceGuard guard(info.device);
+  DRV_CUDA(guard.status);
 
   Buf<float> rows, chi2, best_v;
   Buf<int> best_i, gal_idx;
@@ -338,7 +339,8 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
     return GBK_OK;
   }
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  DRV_CUDA(cudaSetDevice(info.device));
+  DeviceGuard guard(info.device);
+  DRV_CUDA(guard.status);
   const int n = n_free, M = (info.strategy == GBK_STRATEGY_VFIELD ? 1 : 2) * info.nx * info.ny;
   const int n_tri = n * (n + 1) / 2, n_terms = n_tri + n + 1;
   // fits per chunk: the residual buffer of a chunk stays below 1 GiB
@@ -517,7 +519,8 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
   DRV_TRY(check_box(n_free, free_param, lo, hi));
   if (gal < 0 || gal >= info.n_gal) return fail(GBK_ERR_ARG, "gal out of range");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  DRV_CUDA(cudaSetDevice(info.device));
+  DeviceGuard guard(info.device);
+  DRV_CUDA(guard.status);
   const int n = n_free, cap = std::max(n_live, batch);
   Buf<float> rows, chi2;
   Buf<int> gidx;

@@ -94,6 +94,22 @@ cudaError_t launch_unfused(const DevProblem& dp, const EvalArgs& a, const float*
 // velocity-field strategy (gbk_vfield.cu): EvalArgs.m1 = velocity maps, EvalArgs.resid = [K][ny][nx]
 cudaError_t launch_vfield(const DevProblem& dp, const EvalArgs& a, cudaStream_t st);
 
+// Makes `device` current for the scope and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  cudaError_t status = cudaSuccess;
+  explicit DeviceGuard(int device) {
+    status = cudaGetDevice(&prev);
+    if (status == cudaSuccess && prev != device) status = cudaSetDevice(device);
+    else if (status == cudaSuccess) prev = -1;   // nothing to restore
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 // error reporting shared by the translation units (message read by gbk_last_error)
 int fail(int code, const char* fmt, ...);
 void clear_error();
