@@ -528,3 +528,20 @@ def test_two_problems_with_different_tiles_coexist(oracle, torch_cuda, gbk):
                              obs_small.serr[0], obs_small.mask[0], rows_small)
     pu.compare(ref_b, {"chi2": b}, rows_big, False, "big after small")
     pu.compare(ref_a, {"chi2": a}, rows_small, False, "small")
+
+
+@pytest.mark.parametrize("nv,dv,sig", [(400, 5.0, 40.0), (333, 4.0, 4.5), (16, 120.0, 130.0), (9, 60.0, 20.0)])
+def test_many_and_few_channels(oracle, torch_cuda, gbk, nv, dv, sig):
+    """Bands of many fine channels (hundreds of blocks of the voxel loop, lines many channels wide),
+    of very few coarse ones, and odd channel counts (padding of the last block)."""
+    w, g, obs, true, rng = _tiny_case(oracle, nx=12, ny=10, nv=nv, dv=dv, sigma0=sig, lsf_sigma=0.7 * dv)
+    true = true.copy()
+    true[wl.IX_SIG] = sig
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = _rows_near(w, true, rng, 6)
+    rows[:, wl.IX_SIG] = sig * np.array([1.0, 0.8, 1.3, 1.0, 2.0, 0.6], dtype=np.float32)
+    rows[3, wl.IX_VSYS] += 0.4 * nv * dv          # most of the line outside the band
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    got = _gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows)
+    print("channels", nv, dv, sig, pu.compare(ref, got, rows, True, f"nv={nv} dv={dv} sigma0={sig}"))
