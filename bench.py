@@ -255,7 +255,7 @@ def run_ours(args, ranks) -> None:
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB of L2
     stream = torch.cuda.current_stream()
     st = stream.cuda_stream
-    launches_per_step = 1 if info.tiles_x * info.tiles_y == 1 else 2
+    launches_per_step = 1          # one fused kernel per batch, tiled or not
 
     def step(i):
         gbk.gbk_eval_batch(prob.handle, dev_batches[i % len(dev_batches)], None, K, chi2, stream=st)

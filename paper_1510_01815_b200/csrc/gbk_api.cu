@@ -77,6 +77,8 @@ struct gbk_problem {
   int* psf_r = nullptr;
   float4* obs = nullptr;
   float* partial = nullptr;
+  unsigned* tile_count = nullptr;   // [count_cap] zeroed at allocation, self-resetting afterwards
+  long long count_cap = 0;
   long long partial_cap = 0;    // floats
   // staging for gbk_eval_batch_host
   float* st_params = nullptr;
@@ -98,6 +100,7 @@ extern "C" int gbk_destroy(gbk_problem* p) {
   cudaFree(p->psf_r);
   cudaFree(p->obs);
   cudaFree(p->partial);
+  cudaFree(p->tile_count);
   cudaFree(p->st_params);
   cudaFree(p->st_gal);
   cudaFree(p->st_chi2);
@@ -432,7 +435,14 @@ extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t
     GBK_CUDA(cudaMalloc(&p->partial, sizeof(float) * (size_t)need));
     p->partial_cap = need;
   }
-  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, p->partial};
+  if (need > 0 && K > p->count_cap) {
+    if (p->tile_count) GBK_CUDA(cudaFree(p->tile_count));
+    p->tile_count = nullptr, p->count_cap = 0;
+    GBK_CUDA(cudaMalloc(&p->tile_count, sizeof(unsigned) * (size_t)K));
+    GBK_CUDA(cudaMemset(p->tile_count, 0, sizeof(unsigned) * (size_t)K));
+    p->count_cap = K;
+  }
+  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, p->partial, p->tile_count};
   GBK_CUDA(launch_fused(dp, a, p->levels[lv].fl, st));
   return GBK_OK;
 }
@@ -445,7 +455,7 @@ extern "C" int gbk_eval_vfield_batch(gbk_problem* p, const float* params, const 
   if (K == 0) return GBK_OK;
   DeviceGuard guard(p->device);
   GBK_CUDA(guard.status);
-  EvalArgs a{params, gal_index, (long long)K, chi2, nullptr, vmap, nullptr, resid, nullptr};
+  EvalArgs a{params, gal_index, (long long)K, chi2, nullptr, vmap, nullptr, resid, nullptr, nullptr};
   GBK_CUDA(launch_vfield(p->dp, a, (cudaStream_t)cuda_stream));
   return GBK_OK;
 }
@@ -496,7 +506,7 @@ extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const
     GBK_CUDA(cudaMalloc(&p->uf_scratch, per_row * (size_t)want));
     p->uf_rows = want;
   }
-  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, nullptr};
+  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, nullptr, nullptr};
   GBK_CUDA(launch_unfused(p->dp, a, p->lsf_taps, p->uf_scratch, p->uf_rows, p->sm_count,
                           (cudaStream_t)cuda_stream));
   return GBK_OK;

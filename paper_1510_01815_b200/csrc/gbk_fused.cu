@@ -1,4 +1,4 @@
-// Fused hot path of libgbk for sm_100a: one thread block = (parameter row k, spatial tile).
+// Fused hot path of libgbk for sm_100a: one thread block = (parameter row k, spatial tile); one launch per batch.
 //
 // What one block does (steps a1..a9 of SURVEY.md section 8(a); PAPER.md = arXiv:1510.01815):
 //   a1  row constants from the 10 parameters (eq. 1-8)
@@ -807,21 +807,24 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     float tot = 0.0f;
     for (int w = 0; w < (nthreads >> 5); ++w) tot += sm.red[w];
     if (!(tot < f_inf())) tot = f_inf();
-    if (dp.ntiles == 1)
+    if (dp.ntiles == 1) {
       a.chi2[k] = tot;
-    else
+    } else {
+      // the block that finishes a row's last tile adds the row's partials in tile order: one launch,
+      // and still the same sum whichever block comes last
       a.partial[bid] = tot;
+      __threadfence();
+      if (atomicAdd(&a.tile_count[k], 1u) == (unsigned)dp.ntiles - 1u) {
+        __threadfence();
+        const volatile float* part = a.partial + k * dp.ntiles;
+        float sum = 0.0f;
+        for (int t = 0; t < dp.ntiles; ++t) sum += part[t];
+        if (!(sum < f_inf())) sum = f_inf();
+        a.chi2[k] = sum;
+        a.tile_count[k] = 0u;     // ready for the next launch
+      }
+    }
   }
-}
-
-__global__ void finish_kernel(const float* __restrict__ partial, int ntiles, long long K,
-                              float* __restrict__ chi2) {
-  const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= K) return;
-  float tot = 0.0f;
-  for (int t = 0; t < ntiles; ++t) tot += partial[k * ntiles + t];   // fixed order
-  if (!(tot < __int_as_float(0x7f800000))) tot = __int_as_float(0x7f800000);
-  chi2[k] = tot;
 }
 
 }  // namespace
@@ -851,14 +854,7 @@ cudaError_t launch_fused(const DevProblem& dp, const EvalArgs& a, const FusedLau
     fused_kernel<true><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
   else
     fused_kernel<false><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  if (dp.ntiles > 1) {
-    const int th = 128;
-    finish_kernel<<<(unsigned)((a.K + th - 1) / th), th, 0, st>>>(a.partial, dp.ntiles, a.K, a.chi2);
-    e = cudaGetLastError();
-  }
-  return e;
+  return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------- pipe probes ------------

@@ -48,6 +48,7 @@ struct EvalArgs {
   float *m0, *m1, *m2;      // [K][ny][nx] or null
   float* resid;             // [K][2][ny][nx] or null
   float* partial;           // [K][ntiles] cross-tile scratch (ntiles > 1)
+  unsigned* tile_count;     // [K] tiles of a row finished so far (self-resetting; ntiles > 1)
 };
 
 // Per-row constants (a1 of SURVEY.md section 8(a)), computed once per block.
