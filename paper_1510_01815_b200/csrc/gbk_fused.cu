@@ -50,6 +50,7 @@ struct Smem {
   float* spare;     // tile_h x ews (register-tiled image-PSF pass only)
   float4* chan;     // nvx_pad
   u64* coef;        // nvx_pad / 8 blocks x 3 moments x 8 packed coefficients of the block polynomial
+  u64* coefb;       // the same for the polynomial anchored at the block's last channel
   float* taps;      // round_up4(psf_stride)
   RowConst* rc;
   float* red;       // 32
@@ -61,7 +62,8 @@ __device__ __forceinline__ Smem carve(const DevProblem& dp, unsigned char* raw) 
   s.spare = s.maps + 3 * dp.ehs * dp.ews;
   s.chan = reinterpret_cast<float4*>(s.spare + dp.spare_plane);
   s.coef = reinterpret_cast<u64*>(s.chan + dp.nvx_pad);
-  s.taps = reinterpret_cast<float*>(s.coef + 3 * dp.nvx_pad);
+  s.coefb = s.coef + 3 * dp.nvx_pad;
+  s.taps = reinterpret_cast<float*>(s.coefb + 3 * dp.nvx_pad);
   s.rc = reinterpret_cast<RowConst*>(s.taps + taps_floats(dp));
   s.red = reinterpret_cast<float*>(s.rc + 1);
   return s;
@@ -608,48 +610,80 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       // Block polynomial (exact in exact arithmetic): within a block of kChanBlock = 8 channels
       // starting at cb, g_j = g_0 r_0^j q^(j(j-1)/2), so the block's contribution to S_m is
       //   g_0 * sum_j C_m[cb + j] r_0^j,   C_m[c] = w_m[c] q^(j(j-1)/2)  (row table, see prologue):
-      // two ex2 (g_0, r_0) and three degree-7 Horner chains per pixel and block -- 3.4 FP32
-      // instructions per voxel instead of 5 for the channel-by-channel recurrence, and no ex2 per
-      // voxel.  r_0 is clamped to 2^r_clamp: beyond it every voxel of the block is below 2^-27 of
-      // the line peak, and the Horner chain cannot overflow.
-      const u64 m2s = pk1(rc.m2step), ms2 = pk1(rc.mstep2);
-      const float rcl = rc.r_clamp;
+      // two ex2 (anchor, ratio) and three degree-7 Horner chains per pixel and block -- 3.4 FP32
+      // instructions per voxel instead of 5, and no ex2 per voxel.  The anchor must be the block's
+      // LARGEST voxel, or the sum of a block on the far wing of a line loses its relative accuracy
+      // (and a ratio > 1 to the 7th power overflows): blocks the lines of the whole warp item are
+      // leaving use the first channel as anchor (ratio r_0 <= 2^14.6), blocks they are approaching
+      // use the last one with the mirrored table (g_{7-i} = g_7 rho^i q^(i(i-1)/2),
+      // rho = 2^(2 d_7 step - step^2)), and the rare block where the item's lines do both is summed
+      // voxel by voxel.
       const int nblk = dp.nvx_pad / kChanBlock;
-      // Blocks that can hold a non-zero g_0 for some pixel of this warp item: |d_0 + 8 b step| < 11.4
-      // (2^-(11.4^2) is far below the flush threshold 2^-126).  A conservative window; the exact
-      // vote below still decides block by block.  NaN offsets give the full range, infinite ones
-      // an empty one (every g is 0 then).
-      float wlo = 3.0e38f, whi = -3.0e38f;
+      // how far past the anchor a line centre may lie: the anchor 2^-(A^2) must stay a normal number
+      // (A <= 10.5) and (2^(2 A step))^7 times a coefficient <= 2^23 must not overflow (A step <= 7.3)
+      const float kAnchorMargin = fminf(10.5f, 7.3f / rc.step);
+      float dmin = 3.0e38f, dmax = -3.0e38f;   // line-centre offsets of this lane's pixels at channel 0
 #pragma unroll
       for (int j = 0; j < kPairs; ++j) {
         float da, db;
         upk(d0[j], da, db);
-        wlo = fminf(wlo, fminf((-11.4f - da) * rc.inv_bstep, (-11.4f - db) * rc.inv_bstep));
-        whi = fmaxf(whi, fmaxf((11.4f - da) * rc.inv_bstep, (11.4f - db) * rc.inv_bstep));
-        if (da != da || db != db) wlo = -3.0e38f, whi = 3.0e38f;
+        dmin = fminf(dmin, fminf(da, db));
+        dmax = fmaxf(dmax, fmaxf(da, db));
       }
-      const int b_lo = __reduce_min_sync(0xffffffffu, (int)fminf(fmaxf(floorf(wlo), 0.0f), (float)nblk));
-      const int b_hi = __reduce_max_sync(0xffffffffu, (int)fmaxf(fminf(ceilf(whi), (float)(nblk - 1)), -1.0f));
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        dmin = fminf(dmin, __shfl_xor_sync(0xffffffffu, dmin, off));
+        dmax = fmaxf(dmax, __shfl_xor_sync(0xffffffffu, dmax, off));
+      }
+      // Blocks with a voxel that is not flushed to zero for some pixel of the item: |d| < 11.4
+      // somewhere in the block (2^-(11.4^2) is far below 2^-126).  Conservative; infinite offsets give
+      // an empty range (every g is 0 then).
+      const float span = (float)(kChanBlock - 1) * rc.step;
+      const int b_lo = (int)fminf(fmaxf(floorf((-11.4f - span - dmax) * rc.inv_bstep), 0.0f), (float)nblk);
+      const int b_hi = (int)fmaxf(fminf(ceilf((11.4f - dmin) * rc.inv_bstep), (float)(nblk - 1)), -1.0f);
       for (int b = b_lo; b <= b_hi; ++b) {
+        const float first = (float)(b * kChanBlock) * rc.step;          // offset of the block's first channel
+        const bool fwd = dmin + first >= -kAnchorMargin;                 // all lines centred before ~6 past the start
+        const bool bwd = dmax + first + span <= kAnchorMargin;           // all lines centred after ~6 before the end
+        if (!fwd && !bwd) {
+          // lines of this item on both sides of the block: plain sum over its 8 channels
+#pragma unroll
+          for (int cc = 0; cc < kChanBlock; ++cc) {
+            const float4 w = sm.chan[b * kChanBlock + cc];
+#pragma unroll
+            for (int j = 0; j < kPairs; ++j) {
+              const u64 d = fma2(pk1(w.x), st2, d0[j]);
+              float ea, eb;
+              upk(mul2(d, d), ea, eb);
+              const u64 gv = pk(ex2_approx(-ea), ex2_approx(-eb));
+              s0[j] = fma2(pk1(w.y), gv, s0[j]);
+              s1[j] = fma2(pk1(w.z), gv, s1[j]);
+              s2[j] = fma2(pk1(w.w), gv, s2[j]);
+            }
+          }
+          continue;
+        }
+        // anchor: first channel and ratio r_0 (fwd), or last channel and ratio rho (bwd)
+        const float anchor = fwd ? first : first + span;
+        const u64 slope = pk1(fwd ? rc.m2step : -rc.m2step), ms2 = pk1(rc.mstep2);
         u64 g[kPairs], r[kPairs];
-        const float cf = (float)(b * kChanBlock);
 #pragma unroll
         for (int j = 0; j < kPairs; ++j) {
-          const u64 d = fma2(pk1(cf), st2, d0[j]);
+          const u64 d = fma2(pk1(anchor), pk1(1.0f), d0[j]);
           float ea, eb, ra, rb;
           upk(mul2(d, d), ea, eb);
-          upk(fma2(d, m2s, ms2), ra, rb);
+          upk(fma2(d, slope, ms2), ra, rb);
           g[j] = pk(ex2_approx(-ea), ex2_approx(-eb));
-          r[j] = pk(ex2_approx(fminf(ra, rcl)), ex2_approx(fminf(rb, rcl)));
+          r[j] = pk(ex2_approx(fminf(ra, 15.0f)), ex2_approx(fminf(rb, 15.0f)));   // <= 2^14.6 unless garbage
         }
-        // A block whose g_0 has flushed to zero for every pixel of the warp contributes exactly
-        // g_0 * P = 0 to all three sums (P is finite by the clamp): skipping it is bit-identical.
-        // That is the part of the band further than ~13 sigma_0 from the line of all 128 pixels.
+        // The anchor is the largest voxel of the block for every pixel here (up to the margin), so a
+        // block whose anchors have all flushed to zero contributes exactly 0: skipping is bit-identical.
         u64 any_g = g[0];
 #pragma unroll
         for (int j = 1; j < kPairs; ++j) any_g |= g[j];
         if (!__any_sync(0xffffffffu, any_g != 0ull)) continue;
-        const ulonglong2* C = reinterpret_cast<const ulonglong2*>(sm.coef + b * (3 * kChanBlock));
+        const ulonglong2* C =
+            reinterpret_cast<const ulonglong2*>((fwd ? sm.coef : sm.coefb) + b * (3 * kChanBlock));
 #pragma unroll
         for (int m = 0; m < 3; ++m) {
           u64 c[kChanBlock];
@@ -732,6 +766,12 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
         dst[0] = pk1(w.y * f);
         dst[kChanBlock] = pk1(w.z * f);
         dst[2 * kChanBlock] = pk1(w.w * f);
+        const int i = kChanBlock - 1 - j;            // the same channel counted from the block's end
+        const float fb = exp2f(-step * step * (float)(i * (i - 1)));
+        dst = sm.coefb + (c >> 3) * (3 * kChanBlock) + i;
+        dst[0] = pk1(w.y * fb);
+        dst[kChanBlock] = pk1(w.z * fb);
+        dst[2 * kChanBlock] = pk1(w.w * fb);
       }
     }
   }
@@ -831,7 +871,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
 
 size_t fused_smem_bytes(const DevProblem& dp) {
   return sizeof(float) * (3 * (size_t)dp.ehs * dp.ews + dp.spare_plane) + sizeof(float4) * dp.nvx_pad +
-         sizeof(u64) * 3 * dp.nvx_pad + sizeof(float) * taps_floats(dp) + sizeof(RowConst) + sizeof(float) * 32;
+         sizeof(u64) * 6 * dp.nvx_pad + sizeof(float) * taps_floats(dp) + sizeof(RowConst) + sizeof(float) * 32;
 }
 
 cudaError_t fused_prepare(const FusedLaunch& fl) {

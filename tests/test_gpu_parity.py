@@ -459,7 +459,10 @@ def test_eval_batch_in_a_cuda_graph(oracle, torch_cuda, gbk):
     pu.compare(ref, {"chi2": got_b[:16]}, rows_b[:16], False, "graph replay")
 
 
-@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("GBK_FUZZ_CASES", "24"))))
+# seeds 431 and 589: lines centred outside a short band (far-wing spaxels, m0 ~ 1e-15 I) once lost their
+# relative accuracy to the clamped block polynomial
+@pytest.mark.parametrize("seed", sorted(set(range(int(__import__("os").environ.get("GBK_FUZZ_CASES", "24"))))
+                                        | {431, 589}))
 def test_random_shapes_and_kernels(oracle, torch_cuda, gbk, seed):
     """Seeded random problems: odd grid sizes, any up-sampling, Gaussian or image PSFs of any small
     size (symmetric or not), delta or wide LSFs, explicit or automatic tiles, both rotation curves,
