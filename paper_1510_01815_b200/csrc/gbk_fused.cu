@@ -108,7 +108,6 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->m2step = -2.0f * rc->step;
   rc->mstep2 = -rc->step * rc->step;
   rc->use_poly = rc->step <= kPolyMaxStep ? 1 : 0;
-  rc->r_clamp = fmaf(13.0f * rc->step, rc->step, fmaf(10.4f, rc->step, 0.5f));
   rc->inv_bstep = 1.0f / ((float)kChanBlock * rc->step);
   rc->k1 = -s * vrot_scale;                                  // d0 = k1 * f(r) * cos(theta) + k0
   rc->k0 = s * dp.vrel_first - s * (v[4] - dp.v_center);

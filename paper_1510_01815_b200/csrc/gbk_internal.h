@@ -63,7 +63,6 @@ struct RowConst {
   float m2step;       // -2 step
   float mstep2;       // -step^2
   int use_poly;       // step <= kPolyMaxStep: the block polynomial is safe
-  float r_clamp;      // upper clamp of log2 r_0 in the block polynomial (gbk_fused.cu, voxel loop)
   float inv_bstep;    // 1 / (kChanBlock * step): blocks per unit of the line-centre offset d
   float k1;           // -s * V_t sin i (* 2/pi for the arctan curve)
   float k0;           // s * (velocity of extended channel 0 - V_sys): the line-centre offset of a
