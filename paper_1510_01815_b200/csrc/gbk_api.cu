@@ -72,7 +72,7 @@ struct gbk_problem {
   int sm_count = 0, blocks_per_sm = 0;
   long long ext_voxels = 0;
   // device allocations owned by the problem
-  float4* chan_tab = nullptr;
+  double* chan_w = nullptr;
   float* psf_taps = nullptr;
   int* psf_r = nullptr;
   float4* obs = nullptr;
@@ -95,7 +95,7 @@ extern "C" const char* gbk_last_error(void) { return g_err; }
 
 extern "C" int gbk_destroy(gbk_problem* p) {
   if (!p) return GBK_OK;
-  cudaFree(p->chan_tab);
+  cudaFree(p->chan_w);
   cudaFree(p->psf_taps);
   cudaFree(p->psf_r);
   cudaFree(p->obs);
@@ -140,8 +140,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   // w_q[c] = sum over in-band channels k of L[k - ch] * v'_k^q, ch = c - r_v,
   // v'_k = (k - (nv-1)/2) dv  (velocities relative to v_center).
   const int nvx_pad = (nvx + kChanBlock - 1) / kChanBlock * kChanBlock;
-  std::vector<float4> chan(nvx_pad);
-  for (int c = nvx; c < nvx_pad; ++c) chan[c] = make_float4((float)c, 0.f, 0.f, 0.f);  // weightless padding
+  std::vector<double> chan(3 * (size_t)nvx_pad, 0.0);   // weightless padding channels past nvx
   for (int c = 0; c < nvx; ++c) {
     const int ch = c - r_v;
     double w[3] = {0, 0, 0};
@@ -152,7 +151,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
       w[1] += L * v;
       w[2] += L * v * v;
     }
-    chan[c] = make_float4((float)c, (float)w[0], (float)w[1], (float)w[2]);
+    chan[3 * c] = w[0], chan[3 * c + 1] = w[1], chan[3 * c + 2] = w[2];
   }
 
   // ---- PSF sets ------------------------------------------------------------------------
@@ -247,6 +246,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   dp.r_p_max = r_p_max, dp.psf_stride = psf_stride;
   dp.dv = d->dv, dp.v_center = d->v_center;
   dp.vrel_first = (float)((-(double)r_v - 0.5 * (d->nv - 1)) * (double)d->dv);
+  dp.vhalf = (float)(0.5 * (d->nv - 1) * (double)d->dv);
   dp.inv_u = 1.0f / (float)d->u, dp.inv_u2 = 1.0f / ((float)d->u * (float)d->u);
 
   auto set_tile = [&](int tws, int ths) {   // in spaxels
@@ -315,7 +315,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
       return bail(fail(e_ == cudaErrorMemoryAllocation ? GBK_ERR_ALLOC : GBK_ERR_CUDA, "%s: %s", \
                        #expr, cudaGetErrorString(e_)));                                        \
   } while (0)
-  GBK_CUDA_P(cudaMalloc(&p->chan_tab, sizeof(float4) * nvx_pad));
+  GBK_CUDA_P(cudaMalloc(&p->chan_w, sizeof(double) * chan.size()));
   GBK_CUDA_P(cudaMalloc(&p->psf_taps, sizeof(float) * psf_taps.size()));
   GBK_CUDA_P(cudaMalloc(&p->psf_r, sizeof(int) * n_psf));
   GBK_CUDA_P(cudaMalloc(&p->obs, sizeof(float4) * obs.size()));
@@ -324,11 +324,11 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     GBK_CUDA_P(cudaMalloc(&p->lsf_taps, sizeof(float) * lsf_f.size()));
     GBK_CUDA_P(cudaMemcpy(p->lsf_taps, lsf_f.data(), sizeof(float) * lsf_f.size(), cudaMemcpyHostToDevice));
   }
-  GBK_CUDA_P(cudaMemcpy(p->chan_tab, chan.data(), sizeof(float4) * nvx_pad, cudaMemcpyHostToDevice));
+  GBK_CUDA_P(cudaMemcpy(p->chan_w, chan.data(), sizeof(double) * chan.size(), cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->psf_taps, psf_taps.data(), sizeof(float) * psf_taps.size(), cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->psf_r, psf_r.data(), sizeof(int) * n_psf, cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->obs, obs.data(), sizeof(float4) * obs.size(), cudaMemcpyHostToDevice));
-  dp.chan_tab = p->chan_tab, dp.psf_taps = p->psf_taps, dp.psf_r = p->psf_r, dp.obs = p->obs;
+  dp.chan_w = p->chan_w, dp.psf_taps = p->psf_taps, dp.psf_r = p->psf_r, dp.obs = p->obs;
   {
     // opt in to the device's largest dynamic shared memory once and for all: the attribute belongs
     // to the kernel, not to this problem, and a later problem with a smaller tile must not lower it

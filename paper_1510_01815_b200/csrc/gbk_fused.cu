@@ -51,6 +51,7 @@ struct Smem {
   float4* chan;     // nvx_pad
   u64* coef;        // nvx_pad / 8 blocks x 3 moments x 8 packed coefficients of the block polynomial
   u64* coefb;       // the same for the polynomial anchored at the block's last channel
+  RowConstD* rcd;   // FP64 row constants (precise rows only)
   float* taps;      // round_up4(psf_stride)
   RowConst* rc;
   float* red;       // 32
@@ -63,14 +64,16 @@ __device__ __forceinline__ Smem carve(const DevProblem& dp, unsigned char* raw) 
   s.chan = reinterpret_cast<float4*>(s.spare + dp.spare_plane);
   s.coef = reinterpret_cast<u64*>(s.chan + dp.nvx_pad);
   s.coefb = s.coef + 3 * dp.nvx_pad;
-  s.taps = reinterpret_cast<float*>(s.coefb + 3 * dp.nvx_pad);
+  s.rcd = reinterpret_cast<RowConstD*>(s.coefb + 3 * dp.nvx_pad);
+  s.taps = reinterpret_cast<float*>(s.rcd + 1);
   s.rc = reinterpret_cast<RowConst*>(s.taps + taps_floats(dp));
   s.red = reinterpret_cast<float*>(s.rc + 1);
   return s;
 }
 
 // ---------------------------------------------------------------------------------- a1 ------
-__device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long k, RowConst* rc) {
+__device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long k, RowConst* rc,
+                              RowConstD* rd) {
   const float* p = a.params + k * GBK_P;
   float v[GBK_P];
   bool finite = true;
@@ -111,9 +114,35 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->inv_bstep = 1.0f / ((float)kChanBlock * rc->step);
   rc->k1 = -s * vrot_scale;                                  // d0 = k1 * f(r) * cos(theta) + k0
   rc->k0 = s * dp.vrel_first - s * (v[4] - dp.v_center);
+  rc->v_ref = fminf(fmaxf(v[4] - dp.v_center, -dp.vhalf), dp.vhalf);
   const float line_amp = dp.dv / (sigma0 * 2.5066282746310002f) * dp.inv_u2;  // sqrt(2 pi)
   rc->amp = i0 * line_amp;
   rc->dark_s0 = 1e-30f / line_amp;
+  // Precise rows: d0 ranges over k0 -+ |k1| sup f; the line of a sample is centred
+  // at offset -d0 from extended channel 0, the extended band ends at (nvx - 1) step.  A line centred
+  // further than kPreciseMargin outside the band shows only its far wing, where the voxel values need
+  // d to ~1e-6: those rows take the FP64 geometry.  (A non-finite test value is a row that is out of
+  // domain anyway.)
+  const float fsup = dp.rc_model == GBK_RC_ARCTAN ? 1.5707963267948966f : 1.0f;
+  const float tmax = fabsf(rc->k1) * fsup * 1.0001f + 1e-3f;
+  const float band = (float)(dp.nvx - 1) * rc->step;
+  rc->precise = (rc->k0 + tmax > kPreciseMargin || rc->k0 - tmax < -(band + kPreciseMargin)) ? 1 : 0;
+  rc->step_lo = 0.0f;
+  if (rc->precise && rc->valid) {
+    double dsp, dcp, dsi, dci;
+    sincospi((double)v[2] * (1.0 / 180.0), &dsp, &dcp);
+    sincospi((double)v[3] * (1.0 / 180.0), &dsi, &dci);
+    const double sd = 1.0 / ((double)sigma0 * 1.1774100225154747);
+    const double stepd = sd * (double)dp.dv;
+    rc->step_lo = (float)(stepd - (double)rc->step);
+    rd->xo = v[0], rd->yo = v[1];
+    rd->nsp = -dsp, rd->cp = dcp;
+    rd->ncp_ci = -dcp / dci, rd->nsp_ci = -dsp / dci;
+    rd->inv_rt = 1.0 / (double)rt, rd->rt = rt;
+    rd->k1 = -sd * (dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134 : 1.0) * (double)v[5] * dsi;
+    const double vrel_first = (-(double)dp.r_v - 0.5 * (double)(dp.nv - 1)) * (double)dp.dv;
+    rd->k0 = sd * (vrel_first - ((double)v[4] - (double)dp.v_center));
+  }
 }
 
 // ---------------------------------------------------------------------------- a7, a8, a9 ----
@@ -132,7 +161,7 @@ __device__ __forceinline__ float spaxel_finish(const DevProblem& dp, const EvalA
   const float var = fmaf(-m1r, m1r, S2 * inv);
   float m2 = sqrt_approx(fmaxf(var, 0.0f));                     // fmaxf drops a NaN var: m1r carries it
   const bool unmasked = ob.y > 0.0f;
-  float t = (m1r - ob.x) * ob.y;
+  float t = (m1r + (rc.v_ref - ob.x)) * ob.y;
   float s = (m2 - ob.z) * ob.w;
   float contrib = fmaf(t, t, s * s);
   const bool bad = !(contrib < f_inf());                        // NaN or Inf moments
@@ -144,7 +173,7 @@ __device__ __forceinline__ float spaxel_finish(const DevProblem& dp, const EvalA
     const size_t npix = (size_t)dp.nx * dp.ny;
     const size_t o = (size_t)k * npix + pix;
     if (a.m0) a.m0[o] = rc.amp * S0;
-    if (a.m1) a.m1[o] = m1r + dp.v_center;
+    if (a.m1) a.m1[o] = m1r + (rc.v_ref + dp.v_center);
     if (a.m2) a.m2[o] = m2;
     if (a.resid) {
       a.resid[2 * (size_t)k * npix + pix] = t;
@@ -571,8 +600,36 @@ __device__ __forceinline__ u64 pair_geometry(const DevProblem& dp, const RowCons
   return fma2(mul2(f, pk1(rc.k1)), cos_t, pk1(rc.k0));               // eq. 8 -> line centre
 }
 
+// Precise rows (RowConst::precise): eq. 1-4, 6 (or the ramp) and 8 of ONE fine sample in FP64.  Returns
+// the line-centre offset d0 as a float pair hi + lo and the brightness I/I0 (FP32 is enough for that).
+__device__ __noinline__ void sample_geometry_f64(int rc_model, const RowConstD* rdp, float nl2e_inv_r0,
+                                                 double x, double y, float* hi, float* lo,
+                                                 float* bright) {
+  const RowConstD rd = *rdp;
+  const double dx = x - rd.xo, dy = y - rd.yo;
+  const double xe = rd.nsp * dx + rd.cp * dy;                       // eq. 1
+  const double yd = rd.ncp_ci * dx + rd.nsp_ci * dy;                // eq. 2 / cos i
+  const double r2 = xe * xe + yd * yd;                              // eq. 3
+  double r = 0.0, cos_t = 0.0;                                      // r = 0: cos(theta) := 0 (A8)
+  if (r2 > 0.0) {
+    r = sqrt(r2);
+    cos_t = xe / r;                                                 // eq. 4
+  }
+  *bright = ex2_approx((float)r * nl2e_inv_r0);                     // eq. 5 / I0
+  const double q = r * rd.inv_rt;
+  const double f = rc_model == GBK_RC_ARCTAN ? atan(q) : fmin(q, 1.0);   // eq. 6 without (2/pi) V_t; ramp
+  const double d0 = rd.k1 * f * cos_t + rd.k0;                      // eq. 8 -> line centre
+  const float h = (float)d0;
+  *hi = h;
+  *lo = (float)(d0 - (double)h);
+}
+
 // The voxel loop: a warp takes items of 32 lanes x kPairs pixel pairs, evaluates the Gaussian line
 // of each pixel at every extended channel and accumulates the three LSF-folded weighted sums.
+// PRECISE (rows whose lines may be centred outside the band, RowConst::precise): the geometry is
+// evaluated in FP64 and the line offset is carried as hi + lo, with the channel offsets c * step
+// compensated likewise, so that d at the voxels that matter (|d| < 12) is good to ~5e-7.
+template <bool PRECISE>
 __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst& rc, const Smem& sm,
                                             int tx0, int ty0, int EW, int EH, int R, int tid,
                                             int nthreads) {
@@ -585,9 +642,9 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
   const int map_stride = dp.ehs * dp.ews;
   const float inv_u = dp.inv_u;
   const int nvx = dp.nvx;
-  const u64 st2 = pk1(rc.step);
+  const u64 st2 = pk1(rc.step), st2_lo = pk1(rc.step_lo);
   for (int item = warp; item < nitems; item += nwarps) {
-    u64 d0[kPairs], In[kPairs];
+    u64 d0[kPairs], d0lo[kPairs], In[kPairs];
     int sidx[kPairs];
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) {
@@ -595,10 +652,20 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       const int pic = min(pi, npairs - 1);
       const int ey = div_fast(pic, magic), ex = (pic - ey * ppr) << 1;
       sidx[j] = pi < npairs ? ey * dp.ews + ex : -1;
-      const float gx = (float)(tx0 + ex - R), gy = (float)(ty0 + ey - R);
-      const float xa = (gx + 0.5f) * inv_u - 0.5f, xb = (gx + 1.5f) * inv_u - 0.5f;
-      const float y = (gy + 0.5f) * inv_u - 0.5f;
-      d0[j] = pair_geometry(dp, rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo, In[j]);
+      if (PRECISE) {
+        const double inv_ud = 1.0 / (double)dp.u;
+        const double xa = ((double)(tx0 + ex - R) + 0.5) * inv_ud - 0.5, y = ((double)(ty0 + ey - R) + 0.5) * inv_ud - 0.5;
+        float ha, la, ba, hb, lb, bb;
+        sample_geometry_f64(dp.rc_model, sm.rcd, rc.nl2e_inv_r0, xa, y, &ha, &la, &ba);
+        sample_geometry_f64(dp.rc_model, sm.rcd, rc.nl2e_inv_r0, xa + inv_ud, y, &hb, &lb, &bb);
+        d0[j] = pk(ha, hb), d0lo[j] = pk(la, lb), In[j] = pk(ba, bb);
+      } else {
+        const float gx = (float)(tx0 + ex - R), gy = (float)(ty0 + ey - R);
+        const float xa = (gx + 0.5f) * inv_u - 0.5f, xb = (gx + 1.5f) * inv_u - 0.5f;
+        const float y = (gy + 0.5f) * inv_u - 0.5f;
+        d0[j] = pair_geometry(dp, rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo, In[j]);
+        d0lo[j] = 0ull;
+      }
     }
     u64 s0[kPairs], s1[kPairs], s2[kPairs];
 #pragma unroll
@@ -651,7 +718,8 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
             const float4 w = sm.chan[b * kChanBlock + cc];
 #pragma unroll
             for (int j = 0; j < kPairs; ++j) {
-              const u64 d = fma2(pk1(w.x), st2, d0[j]);
+              u64 d = fma2(pk1(w.x), st2, d0[j]);
+              if (PRECISE) d = add2(d, fma2(pk1(w.x), st2_lo, d0lo[j]));
               float ea, eb;
               upk(mul2(d, d), ea, eb);
               const u64 gv = pk(ex2_approx(-ea), ex2_approx(-eb));
@@ -665,10 +733,18 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
         // anchor: first channel and ratio r_0 (fwd), or last channel and ratio rho (bwd)
         const float anchor = fwd ? first : first + span;
         const u64 slope = pk1(fwd ? rc.m2step : -rc.m2step), ms2 = pk1(rc.mstep2);
+        // PRECISE: the anchor offset n * step as a float pair (n * step_hi is not exact in FP32)
+        const float nchan = (float)(b * kChanBlock + (fwd ? 0 : kChanBlock - 1));
+        const float anchor_hi = nchan * rc.step;
+        const float anchor_lo = fmaf(nchan, rc.step, -anchor_hi) + nchan * rc.step_lo;
         u64 g[kPairs], r[kPairs];
 #pragma unroll
         for (int j = 0; j < kPairs; ++j) {
-          const u64 d = fma2(pk1(anchor), pk1(1.0f), d0[j]);
+          u64 d;
+          if (PRECISE)
+            d = add2(add2(pk1(anchor_hi), d0[j]), add2(pk1(anchor_lo), d0lo[j]));
+          else
+            d = fma2(pk1(anchor), pk1(1.0f), d0[j]);
           float ea, eb, ra, rb;
           upk(mul2(d, d), ea, eb);
           upk(fma2(d, slope, ms2), ra, rb);
@@ -708,7 +784,8 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
         const float4 w = sm.chan[c];
 #pragma unroll
         for (int j = 0; j < kPairs; ++j) {
-          const u64 d = fma2(pk1(w.x), st2, d0[j]);
+          u64 d = fma2(pk1(w.x), st2, d0[j]);
+          if (PRECISE) d = add2(d, fma2(pk1(w.x), st2_lo, d0lo[j]));
           float ea, eb;
           upk(mul2(d, d), ea, eb);
           const u64 g = pk(ex2_approx(-ea), ex2_approx(-eb));        // Gaussian line
@@ -732,6 +809,15 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
   }
 }
 
+// Out of line: precise rows are rare, and the FP64 path must not weigh on the register allocation of
+// the common one.
+__device__ __noinline__ void voxel_phase_precise(const DevProblem& dp, unsigned char* smem_raw, int tx0,
+                                                 int ty0, int EW, int EH, int R, int tid, int nthreads) {
+  const Smem sm = carve(dp, smem_raw);
+  const RowConst rc = *sm.rc;
+  voxel_phase<true>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads);
+}
+
 // ------------------------------------------------------------------------------ the kernel ---
 template <bool OUT>
 __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
@@ -747,7 +833,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   const int tw = min(dp.tile_w, dp.fw - tx0), th = min(dp.tile_h, dp.fh - ty0);
   const int map_stride = dp.ehs * dp.ews;
 
-  if (tid == 0) row_constants(dp, a, k, sm.rc);
+  if (tid == 0) row_constants(dp, a, k, sm.rc, sm.rcd);
   {
     // Channel table, and the coefficients of the block polynomial of this row (voxel loop below):
     // C_m[c] = w_m[c] q^(j(j-1)/2), j = c mod 8, q = 2^(-2 step^2), stored as (C, C) pairs.
@@ -755,8 +841,13 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     const float s_ = 1.0f / (sigma0 * 1.1774100225154747f);
     const float step = s_ * dp.dv;
     const bool poly = step <= kPolyMaxStep;        // false for NaN: the row is out of domain anyway
+    // the row's moment weights: the problem's w_q about v_center shifted to v_ref (RowConst::v_ref) in FP64,
+    //   w1' = w1 - v_ref w0,   w2' = w2 - 2 v_ref w1 + v_ref^2 w0
+    const double vr = (double)fminf(fmaxf(a.params[k * GBK_P + 4] - dp.v_center, -dp.vhalf), dp.vhalf);
     for (int c = tid; c < dp.nvx_pad; c += nthreads) {
-      const float4 w = dp.chan_tab[c];
+      const double w0 = dp.chan_w[3 * c], w1 = dp.chan_w[3 * c + 1], w2 = dp.chan_w[3 * c + 2];
+      const float4 w = make_float4((float)c, (float)w0, (float)(w1 - vr * w0),
+                                   (float)(w2 - vr * (2.0 * w1 - vr * w0)));
       sm.chan[c] = w;
       if (poly) {
         const int j = c & (kChanBlock - 1);
@@ -802,7 +893,10 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   } else {
     const int R = rc.r_p;
     const int EW = tw + 2 * R, EH = th + 2 * R;
-    voxel_phase(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads);
+    if (rc.precise)
+      voxel_phase_precise(dp, smem_raw, tx0, ty0, EW, EH, R, tid, nthreads);
+    else
+      voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads);
     __syncthreads();
     // ------------------------------------------------------------------ a5 .. a9 ---------
     if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {
@@ -870,7 +964,8 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
 
 size_t fused_smem_bytes(const DevProblem& dp) {
   return sizeof(float) * (3 * (size_t)dp.ehs * dp.ews + dp.spare_plane) + sizeof(float4) * dp.nvx_pad +
-         sizeof(u64) * 6 * dp.nvx_pad + sizeof(float) * taps_floats(dp) + sizeof(RowConst) + sizeof(float) * 32;
+         sizeof(u64) * 6 * dp.nvx_pad + sizeof(RowConstD) + sizeof(float) * taps_floats(dp) + sizeof(RowConst) +
+         sizeof(float) * 32;
 }
 
 cudaError_t fused_prepare(const FusedLaunch& fl) {

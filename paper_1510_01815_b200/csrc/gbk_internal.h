@@ -34,7 +34,9 @@ struct DevProblem {
   float dv, v_center;
   float vrel_first;         // velocity of extended channel 0 relative to v_center
   float inv_u, inv_u2;
-  const float4* chan_tab;   // [nvx] {channel index as float, w0, w1, w2}: LSF-folded moment weights
+  float vhalf;              // velocity of the last in-band channel relative to v_center, (nv-1)/2 dv
+  const double* chan_w;     // [nvx_pad][3] LSF-folded moment weights w0, w1, w2 about v_center (FP64:
+                            // every row shifts them to its own reference velocity, RowConst::v_ref)
   const float* psf_taps;    // [n_psf][psf_stride]: Gaussian 1-D taps, or flipped PSF image
   const int* psf_r;         // [n_psf] tap radius of each PSF set
   const float4* obs;        // [n_gal][ny][nx] {vobs - v_center, 1/E_v (0 = masked), sobs, 1/E_s}
@@ -67,12 +69,32 @@ struct RowConst {
   float k1;           // -s * V_t sin i (* 2/pi for the arctan curve)
   float k0;           // s * (velocity of extended channel 0 - V_sys): the line-centre offset of a
                       // sample from extended channel 0 is  d0 = k1 * f(r/r_t) * cos(theta) + k0
+  float v_ref;        // reference velocity of the row's moment sums S1, S2, relative to v_center: V_sys
+                      // clamped to the band, so the FP32 cancellation in m2^2 = S2/S0 - m1^2 involves the
+                      // distance of the line from V_sys (or from the band edge) and not from v_center
   float amp;          // I0 * dv / (sigma0 sqrt(2 pi) u^2): scales the S0 block sum to m0
   float dark_s0;      // S0 block sums below this are model-dark (m0 < 1e-30 I0)
   int valid;
   int r_p;            // PSF radius of this row's data set
   int psf_set, gal;
+  int precise;        // some line of this row may be centred outside the extended band by more than
+                      // kPreciseMargin: the voxel loop takes the FP64-geometry path
+  float step_lo;      // step = step + step_lo to FP64 accuracy (precise rows only)
 };
+
+// The row constants of the geometry in FP64, filled for precise rows only (see RowConst::precise):
+// the far wing of a line, 2^-(d^2) at |d| ~ 9, turns an error of d into 2 d ln2 = 12 times that
+// relative error of the voxel, so d must be known to ~1e-6 there while the line-centre offset itself
+// reaches hundreds -- beyond FP32, which carries the product V_t sin i atan(r/r_t) cos(theta) / sigma_0
+// to ~3e-7 relative at best.
+struct RowConstD {
+  double xo, yo;
+  double nsp, cp, ncp_ci, nsp_ci;   // as in RowConst
+  double inv_rt, rt;
+  double k1, k0;                    // d0 = k1 * f(r/r_t) * cos(theta) + k0
+};
+
+constexpr float kPreciseMargin = 2.5f;   // in units of the line offset d (1.18 sigma_0 each)
 
 struct FusedLaunch {
   int threads;
