@@ -67,6 +67,13 @@ __device__ __forceinline__ int div_fast(int n, unsigned magic) {
   return magic ? (int)__umulhi((unsigned)n, magic) : n;
 }
 
+// Order-preserving map float -> int (and back: it is an involution), for redux.sync min / max.
+__device__ __forceinline__ int ordered_key(float f) {
+  const int i = __float_as_int(f);
+  return i ^ ((i >> 31) & 0x7fffffff);
+}
+__device__ __forceinline__ float ordered_float(int k) { return __int_as_float(k ^ ((k >> 31) & 0x7fffffff)); }
+
 __device__ __forceinline__ float f_inf() { return __int_as_float(0x7f800000); }
 __device__ __forceinline__ float f_nan() { return __int_as_float(0x7fc00000); }
 

@@ -39,6 +39,14 @@ constexpr int kMaxThreads = 256;
 constexpr int kMinBlocks = 3;
 constexpr int kVBlockX = 4;      // output rows per thread in the x-packed vertical pass (divides kVBlock)
 constexpr int kPairs = 2;        // pixel pairs per lane in the voxel loop (4 pixels per thread)
+#ifndef GBK_STRIP_PAIRS
+#define GBK_STRIP_PAIRS 8
+#endif
+#ifndef GBK_TRUNC_D
+#define GBK_TRUNC_D 6.5f
+#endif
+constexpr int kStripPairs = GBK_STRIP_PAIRS;  // width of a strip of the voxel loop in pixel pairs (power of two)
+constexpr float kTruncD = GBK_TRUNC_D;        // lines centred in the band are summed out to |d| < this
 
 // floats of the PSF tap area: image taps of the register-tiled pass are stored as (w, w) pairs
 __host__ __device__ __forceinline__ int taps_floats(const DevProblem& dp) {
@@ -49,8 +57,8 @@ struct Smem {
   float* maps;      // 3 x ehs x ews
   float* spare;     // tile_h x ews (register-tiled image-PSF pass only)
   float4* chan;     // nvx_pad
-  u64* coef;        // nvx_pad / 8 blocks x 3 moments x 8 packed coefficients of the block polynomial
-  u64* coefb;       // the same for the polynomial anchored at the block's last channel
+  float* coef;      // nvx_pad / 8 blocks x 3 moments x 8 coefficients of the block polynomial
+  float* coefb;     // the same for the polynomial anchored at the block's last channel
   RowConstD* rcd;   // FP64 row constants (precise rows only)
   float* taps;      // round_up4(psf_stride)
   RowConst* rc;
@@ -62,7 +70,7 @@ __device__ __forceinline__ Smem carve(const DevProblem& dp, unsigned char* raw) 
   s.maps = reinterpret_cast<float*>(raw);
   s.spare = s.maps + 3 * dp.ehs * dp.ews;
   s.chan = reinterpret_cast<float4*>(s.spare + dp.spare_plane);
-  s.coef = reinterpret_cast<u64*>(s.chan + dp.nvx_pad);
+  s.coef = reinterpret_cast<float*>(s.chan + dp.nvx_pad);
   s.coefb = s.coef + 3 * dp.nvx_pad;
   s.rcd = reinterpret_cast<RowConstD*>(s.coefb + 3 * dp.nvx_pad);
   s.taps = reinterpret_cast<float*>(s.rcd + 1);
@@ -115,6 +123,9 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->k1 = -s * vrot_scale;                                  // d0 = k1 * f(r) * cos(theta) + k0
   rc->k0 = s * dp.vrel_first - s * (v[4] - dp.v_center);
   rc->v_ref = fminf(fmaxf(v[4] - dp.v_center, -dp.vhalf), dp.vhalf);
+  rc->anchor_margin = fminf(10.5f, 7.3f / rc->step);
+  rc->cen_lo = (float)dp.r_v * rc->step;                      // line centres inside the band proper:
+  rc->cen_hi = (float)(dp.r_v + dp.nv - 1) * rc->step;        // -d0 in [cen_lo, cen_hi]
   const float line_amp = dp.dv / (sigma0 * 2.5066282746310002f) * dp.inv_u2;  // sqrt(2 pi)
   rc->amp = i0 * line_amp;
   rc->dark_s0 = 1e-30f / line_amp;
@@ -624,6 +635,117 @@ __device__ __noinline__ void sample_geometry_f64(int rc_model, const RowConstD* 
   *lo = (float)(d0 - (double)h);
 }
 
+// ---- pieces of the voxel loop -------------------------------------------------------------
+// With d_c = d0 + c step the line is g_c = 2^-(d_c^2), so g_{c+1} = g_c r_c with
+// r_c = 2^-(2 d_c step + step^2) and r_{c+1} = r_c q, q = 2^-(2 step^2) a row constant.
+// Block polynomial (exact in exact arithmetic): within a block of kChanBlock = 8 channels starting at
+// cb, g_j = g_0 r_0^j q^(j(j-1)/2), so the block's contribution to S_m is
+//   g_0 * sum_j C_m[cb + j] r_0^j,   C_m[c] = w_m[c] q^(j(j-1)/2)  (row table, see the prologue):
+// two ex2 (anchor, ratio) and three degree-7 Horner chains per pixel and block -- 3.4 FP32 lane-ops
+// per voxel instead of 5, and no ex2 per voxel.  The anchor must be the block's LARGEST voxel, or the
+// sum of a block on the far wing of a line loses its relative accuracy (and a ratio > 1 to the 7th
+// power overflows): blocks the lines of the whole warp item are leaving are anchored at their first
+// channel (FWD, ratio r_0 <= 2^14.6), blocks they are approaching at their last one with the mirrored
+// table (g_{7-i} = g_7 rho^i q^(i(i-1)/2), rho = 2^(2 d_7 step - step^2)), and the rare block where the
+// item's lines do both is summed voxel by voxel.
+struct VoxelAcc {
+  u64 d0[kPairs], d0lo[kPairs];              // line-centre offset at extended channel 0 (hi, lo)
+  u64 s0[kPairs], s1[kPairs], s2[kPairs];    // the three weighted sums
+};
+
+template <bool PRECISE, bool FWD>
+__device__ __forceinline__ void poly_block(const RowConst& rc, const Smem& sm, int b, VoxelAcc& v) {
+  const float nchan = (float)(b * kChanBlock + (FWD ? 0 : kChanBlock - 1));   // the anchor channel
+  const float anchor_hi = nchan * rc.step;
+  const u64 slope = pk1(FWD ? rc.m2step : -rc.m2step), ms2 = pk1(rc.mstep2);
+  u64 g[kPairs], r[kPairs];
+#pragma unroll
+  for (int j = 0; j < kPairs; ++j) {
+    u64 d;
+    if (PRECISE) {   // n * step as a float pair (n * step_hi is not exact in FP32)
+      const float anchor_lo = fmaf(nchan, rc.step, -anchor_hi) + nchan * rc.step_lo;
+      d = add2(add2(pk1(anchor_hi), v.d0[j]), add2(pk1(anchor_lo), v.d0lo[j]));
+    } else {
+      d = add2(pk1(anchor_hi), v.d0[j]);
+    }
+    float ea, eb, ra, rb;
+    upk(mul2(d, d), ea, eb);
+    upk(fma2(d, slope, ms2), ra, rb);
+    g[j] = pk(ex2_approx(-ea), ex2_approx(-eb));
+    r[j] = pk(ex2_approx(fminf(ra, 15.0f)), ex2_approx(fminf(rb, 15.0f)));   // <= 2^14.6 unless garbage
+  }
+  // The anchor is the largest voxel of the block for every pixel here (up to the margin), so a block
+  // whose anchors have all flushed to zero contributes exactly 0: skipping is bit-identical.
+  u64 any_g = g[0];
+#pragma unroll
+  for (int j = 1; j < kPairs; ++j) any_g |= g[j];
+  if (!__any_sync(0xffffffffu, any_g != 0ull)) return;
+  // scalar coefficients: FFMA2 takes a broadcast FP32 operand, so no (C, C) pairs are needed
+  const float4* C = reinterpret_cast<const float4*>((FWD ? sm.coef : sm.coefb) + b * (3 * kChanBlock));
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    float c[kChanBlock];
+#pragma unroll
+    for (int i = 0; i < kChanBlock / 4; ++i) {
+      const float4 t = C[m * (kChanBlock / 4) + i];
+      c[4 * i] = t.x, c[4 * i + 1] = t.y, c[4 * i + 2] = t.z, c[4 * i + 3] = t.w;
+    }
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) {
+      u64 P = pk1(c[kChanBlock - 1]);
+#pragma unroll
+      for (int i = kChanBlock - 2; i >= 0; --i) P = fma2(P, r[j], pk1(c[i]));
+      if (m == 0) v.s0[j] = fma2(g[j], P, v.s0[j]);
+      if (m == 1) v.s1[j] = fma2(g[j], P, v.s1[j]);
+      if (m == 2) v.s2[j] = fma2(g[j], P, v.s2[j]);
+    }
+  }
+}
+
+// One channel summed directly: the Gaussian line of PAPER.md:199 by one ex2 per voxel.
+template <bool PRECISE>
+__device__ __forceinline__ void direct_channel(const RowConst& rc, const float4 w, VoxelAcc& v) {
+#pragma unroll
+  for (int j = 0; j < kPairs; ++j) {
+    u64 d = fma2(pk1(w.x), pk1(rc.step), v.d0[j]);
+    if (PRECISE) d = add2(d, fma2(pk1(w.x), pk1(rc.step_lo), v.d0lo[j]));
+    float ea, eb;
+    upk(mul2(d, d), ea, eb);
+    const u64 g = pk(ex2_approx(-ea), ex2_approx(-eb));
+    v.s0[j] = fma2(pk1(w.y), g, v.s0[j]);
+    v.s1[j] = fma2(pk1(w.z), g, v.s1[j]);
+    v.s2[j] = fma2(pk1(w.w), g, v.s2[j]);
+  }
+}
+
+// Pair index of a tile -> extended pixel: the pairs are walked strip by strip (kStripPairs pairs wide,
+// row-major inside a strip), so that the 64 pairs of a warp item form a compact patch (16 x 8 pixels)
+// instead of 1.7 rows of the tile: the line centres of a patch lie close together, so the window of
+// channel blocks the item has to look at is hardly wider than that of a single line.
+struct StripMap {
+  int ppr, EH, full, nfull, wlast;
+  unsigned magic_full, magic_last;
+};
+__device__ __forceinline__ StripMap strip_map(int EW, int EH) {
+  StripMap m;
+  m.ppr = (EW + 1) >> 1, m.EH = EH;
+  m.full = kStripPairs * EH;
+  m.nfull = m.ppr / kStripPairs;
+  m.wlast = m.ppr - m.nfull * kStripPairs;      // pairs per row of the last, narrower strip (0: none)
+  m.magic_full = div_magic(m.full);
+  m.magic_last = div_magic(m.wlast > 0 ? m.wlast : 1);
+  return m;
+}
+__device__ __forceinline__ void strip_pixel(const StripMap& m, int pi, int& ey, int& ex) {
+  const int s = min(div_fast(pi, m.magic_full), m.nfull);
+  const int rem = pi - s * m.full;
+  const bool last = s == m.nfull;
+  const int y = last ? div_fast(rem, m.magic_last) : rem / kStripPairs;
+  const int w = last ? m.wlast : kStripPairs;
+  ey = y;
+  ex = (s * kStripPairs + rem - y * w) << 1;
+}
+
 // The voxel loop: a warp takes items of 32 lanes x kPairs pixel pairs, evaluates the Gaussian line
 // of each pixel at every extended channel and accumulates the three LSF-folded weighted sums.
 // PRECISE (rows whose lines may be centred outside the band, RowConst::precise): the geometry is
@@ -633,178 +755,95 @@ template <bool PRECISE>
 __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst& rc, const Smem& sm,
                                             int tx0, int ty0, int EW, int EH, int R, int tid,
                                             int nthreads) {
-  const int ppr = (EW + 1) >> 1;                  // pixel pairs per extended row
-  const int npairs = ppr * EH;
-  const unsigned magic = div_magic(ppr);
+  const StripMap smap = strip_map(EW, EH);
+  const int npairs = smap.ppr * EH;
   const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
   constexpr int kPerItem = 32 * kPairs;
   const int nitems = (npairs + kPerItem - 1) / kPerItem;
   const int map_stride = dp.ehs * dp.ews;
   const float inv_u = dp.inv_u;
-  const int nvx = dp.nvx;
-  const u64 st2 = pk1(rc.step), st2_lo = pk1(rc.step_lo);
   for (int item = warp; item < nitems; item += nwarps) {
-    u64 d0[kPairs], d0lo[kPairs], In[kPairs];
+    VoxelAcc v;
+    u64 In[kPairs];
     int sidx[kPairs];
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) {
       const int pi = item * kPerItem + j * 32 + lane;
-      const int pic = min(pi, npairs - 1);
-      const int ey = div_fast(pic, magic), ex = (pic - ey * ppr) << 1;
+      int ey, ex;
+      strip_pixel(smap, min(pi, npairs - 1), ey, ex);
       sidx[j] = pi < npairs ? ey * dp.ews + ex : -1;
       if (PRECISE) {
         const double inv_ud = 1.0 / (double)dp.u;
-        const double xa = ((double)(tx0 + ex - R) + 0.5) * inv_ud - 0.5, y = ((double)(ty0 + ey - R) + 0.5) * inv_ud - 0.5;
+        const double xa = ((double)(tx0 + ex - R) + 0.5) * inv_ud - 0.5;
+        const double y = ((double)(ty0 + ey - R) + 0.5) * inv_ud - 0.5;
         float ha, la, ba, hb, lb, bb;
         sample_geometry_f64(dp.rc_model, sm.rcd, rc.nl2e_inv_r0, xa, y, &ha, &la, &ba);
         sample_geometry_f64(dp.rc_model, sm.rcd, rc.nl2e_inv_r0, xa + inv_ud, y, &hb, &lb, &bb);
-        d0[j] = pk(ha, hb), d0lo[j] = pk(la, lb), In[j] = pk(ba, bb);
+        v.d0[j] = pk(ha, hb), v.d0lo[j] = pk(la, lb), In[j] = pk(ba, bb);
       } else {
         const float gx = (float)(tx0 + ex - R), gy = (float)(ty0 + ey - R);
         const float xa = (gx + 0.5f) * inv_u - 0.5f, xb = (gx + 1.5f) * inv_u - 0.5f;
         const float y = (gy + 0.5f) * inv_u - 0.5f;
-        d0[j] = pair_geometry(dp, rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo, In[j]);
-        d0lo[j] = 0ull;
+        v.d0[j] = pair_geometry(dp, rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo, In[j]);
+        v.d0lo[j] = 0ull;
       }
+      v.s0[j] = v.s1[j] = v.s2[j] = pk(0.f, 0.f);
     }
-    u64 s0[kPairs], s1[kPairs], s2[kPairs];
+    // range of the line-centre offsets of the item's 128 pixels (at extended channel 0)
+    float dmin = 3.0e38f, dmax = -3.0e38f;
 #pragma unroll
-    for (int j = 0; j < kPairs; ++j) s0[j] = s1[j] = s2[j] = pk(0.f, 0.f);
+    for (int j = 0; j < kPairs; ++j) {
+      float da, db;
+      upk(v.d0[j], da, db);
+      dmin = fminf(dmin, fminf(da, db));
+      dmax = fmaxf(dmax, fmaxf(da, db));
+    }
+    dmin = ordered_float(__reduce_min_sync(0xffffffffu, ordered_key(dmin)));
+    dmax = ordered_float(__reduce_max_sync(0xffffffffu, ordered_key(dmax)));
+    // How far from its centre a line is summed.  A voxel with |d| >= 11.4 is flushed to zero by
+    // ex2.approx.ftz (2^-(11.4^2) is far below 2^-126), so 11.4 loses nothing.  A line CENTRED IN THE
+    // BAND (all 128 of the item) has a voxel of weight >= 1/2 within half a channel of its centre, so
+    // what lies beyond |d| = kTruncD = 6.5 (7.7 sigma_0) is below 2^-42 = 2e-13 of its sum -- six
+    // orders of magnitude under the FP32 rounding of the sums -- and is left out, like the PSF and LSF
+    // taps beyond 4 sigma (A10), only a million times more conservatively.  Lines centred near or
+    // beyond a band edge keep the full extent: there the far wing is all a spaxel sees.
+    const bool centred = -dmax >= rc.cen_lo && -dmin <= rc.cen_hi;
+    const float D = centred ? kTruncD : 11.4f;
     if (rc.use_poly) {
-      // With d_c = d0 + c step the line is g_c = 2^-(d_c^2), so g_{c+1} = g_c r_c with
-      // r_c = 2^-(2 d_c step + step^2) and r_{c+1} = r_c q, q = 2^-(2 step^2) a row constant.
-      // Block polynomial (exact in exact arithmetic): within a block of kChanBlock = 8 channels
-      // starting at cb, g_j = g_0 r_0^j q^(j(j-1)/2), so the block's contribution to S_m is
-      //   g_0 * sum_j C_m[cb + j] r_0^j,   C_m[c] = w_m[c] q^(j(j-1)/2)  (row table, see prologue):
-      // two ex2 (anchor, ratio) and three degree-7 Horner chains per pixel and block -- 3.4 FP32
-      // instructions per voxel instead of 5, and no ex2 per voxel.  The anchor must be the block's
-      // LARGEST voxel, or the sum of a block on the far wing of a line loses its relative accuracy
-      // (and a ratio > 1 to the 7th power overflows): blocks the lines of the whole warp item are
-      // leaving use the first channel as anchor (ratio r_0 <= 2^14.6), blocks they are approaching
-      // use the last one with the mirrored table (g_{7-i} = g_7 rho^i q^(i(i-1)/2),
-      // rho = 2^(2 d_7 step - step^2)), and the rare block where the item's lines do both is summed
-      // voxel by voxel.
       const int nblk = dp.nvx_pad / kChanBlock;
+      const float span = (float)(kChanBlock - 1) * rc.step;
+      // blocks with a voxel |d| < D for some pixel of the item (infinite offsets give an empty range)
+      const int b_lo = min(max(__float2int_rd((-D - span - dmax) * rc.inv_bstep), 0), nblk);
+      const int b_hi = max(min(__float2int_ru((D - dmin) * rc.inv_bstep), nblk) - 1, -1);
       // how far past the anchor a line centre may lie: the anchor 2^-(A^2) must stay a normal number
       // (A <= 10.5) and (2^(2 A step))^7 times a coefficient <= 2^23 must not overflow (A step <= 7.3)
-      const float kAnchorMargin = fminf(10.5f, 7.3f / rc.step);
-      float dmin = 3.0e38f, dmax = -3.0e38f;   // line-centre offsets of this lane's pixels at channel 0
+      const float A = rc.anchor_margin;
+      // FWD is safe from block b_f on (every line centred at most A past the block's first channel),
+      // the mirrored anchor up to block b_b (every line centred at most A before its last channel)
+      const int b_f = min(max(__float2int_ru((-A - dmin) * rc.inv_bstep), b_lo), b_hi + 1);
+      const int b_b = max(min(__float2int_rd((A - span - dmax) * rc.inv_bstep), b_f - 1), b_lo - 1);
+      for (int b = b_lo; b <= b_b; ++b) poly_block<PRECISE, false>(rc, sm, b, v);
+      for (int b = b_b + 1; b < b_f; ++b)        // lines of this item on both sides of the block
 #pragma unroll
-      for (int j = 0; j < kPairs; ++j) {
-        float da, db;
-        upk(d0[j], da, db);
-        dmin = fminf(dmin, fminf(da, db));
-        dmax = fmaxf(dmax, fmaxf(da, db));
-      }
-#pragma unroll
-      for (int off = 16; off > 0; off >>= 1) {
-        dmin = fminf(dmin, __shfl_xor_sync(0xffffffffu, dmin, off));
-        dmax = fmaxf(dmax, __shfl_xor_sync(0xffffffffu, dmax, off));
-      }
-      // Blocks with a voxel that is not flushed to zero for some pixel of the item: |d| < 11.4
-      // somewhere in the block (2^-(11.4^2) is far below 2^-126).  Conservative; infinite offsets give
-      // an empty range (every g is 0 then).
-      const float span = (float)(kChanBlock - 1) * rc.step;
-      const int b_lo = (int)fminf(fmaxf(floorf((-11.4f - span - dmax) * rc.inv_bstep), 0.0f), (float)nblk);
-      const int b_hi = (int)fmaxf(fminf(ceilf((11.4f - dmin) * rc.inv_bstep), (float)(nblk - 1)), -1.0f);
-      for (int b = b_lo; b <= b_hi; ++b) {
-        const float first = (float)(b * kChanBlock) * rc.step;          // offset of the block's first channel
-        const bool fwd = dmin + first >= -kAnchorMargin;                 // all lines centred before ~6 past the start
-        const bool bwd = dmax + first + span <= kAnchorMargin;           // all lines centred after ~6 before the end
-        if (!fwd && !bwd) {
-          // lines of this item on both sides of the block: plain sum over its 8 channels
-#pragma unroll
-          for (int cc = 0; cc < kChanBlock; ++cc) {
-            const float4 w = sm.chan[b * kChanBlock + cc];
-#pragma unroll
-            for (int j = 0; j < kPairs; ++j) {
-              u64 d = fma2(pk1(w.x), st2, d0[j]);
-              if (PRECISE) d = add2(d, fma2(pk1(w.x), st2_lo, d0lo[j]));
-              float ea, eb;
-              upk(mul2(d, d), ea, eb);
-              const u64 gv = pk(ex2_approx(-ea), ex2_approx(-eb));
-              s0[j] = fma2(pk1(w.y), gv, s0[j]);
-              s1[j] = fma2(pk1(w.z), gv, s1[j]);
-              s2[j] = fma2(pk1(w.w), gv, s2[j]);
-            }
-          }
-          continue;
-        }
-        // anchor: first channel and ratio r_0 (fwd), or last channel and ratio rho (bwd)
-        const float anchor = fwd ? first : first + span;
-        const u64 slope = pk1(fwd ? rc.m2step : -rc.m2step), ms2 = pk1(rc.mstep2);
-        // PRECISE: the anchor offset n * step as a float pair (n * step_hi is not exact in FP32)
-        const float nchan = (float)(b * kChanBlock + (fwd ? 0 : kChanBlock - 1));
-        const float anchor_hi = nchan * rc.step;
-        const float anchor_lo = fmaf(nchan, rc.step, -anchor_hi) + nchan * rc.step_lo;
-        u64 g[kPairs], r[kPairs];
-#pragma unroll
-        for (int j = 0; j < kPairs; ++j) {
-          u64 d;
-          if (PRECISE)
-            d = add2(add2(pk1(anchor_hi), d0[j]), add2(pk1(anchor_lo), d0lo[j]));
-          else
-            d = fma2(pk1(anchor), pk1(1.0f), d0[j]);
-          float ea, eb, ra, rb;
-          upk(mul2(d, d), ea, eb);
-          upk(fma2(d, slope, ms2), ra, rb);
-          g[j] = pk(ex2_approx(-ea), ex2_approx(-eb));
-          r[j] = pk(ex2_approx(fminf(ra, 15.0f)), ex2_approx(fminf(rb, 15.0f)));   // <= 2^14.6 unless garbage
-        }
-        // The anchor is the largest voxel of the block for every pixel here (up to the margin), so a
-        // block whose anchors have all flushed to zero contributes exactly 0: skipping is bit-identical.
-        u64 any_g = g[0];
-#pragma unroll
-        for (int j = 1; j < kPairs; ++j) any_g |= g[j];
-        if (!__any_sync(0xffffffffu, any_g != 0ull)) continue;
-        const ulonglong2* C =
-            reinterpret_cast<const ulonglong2*>((fwd ? sm.coef : sm.coefb) + b * (3 * kChanBlock));
-#pragma unroll
-        for (int m = 0; m < 3; ++m) {
-          u64 c[kChanBlock];
-#pragma unroll
-          for (int i = 0; i < kChanBlock / 2; ++i) {
-            const ulonglong2 v = C[m * (kChanBlock / 2) + i];
-            c[2 * i] = v.x, c[2 * i + 1] = v.y;
-          }
-#pragma unroll
-          for (int j = 0; j < kPairs; ++j) {
-            u64 P = c[kChanBlock - 1];
-#pragma unroll
-            for (int i = kChanBlock - 2; i >= 0; --i) P = fma2(P, r[j], c[i]);
-            if (m == 0) s0[j] = fma2(g[j], P, s0[j]);
-            if (m == 1) s1[j] = fma2(g[j], P, s1[j]);
-            if (m == 2) s2[j] = fma2(g[j], P, s2[j]);
-          }
-        }
-      }
+        for (int cc = 0; cc < kChanBlock; ++cc) direct_channel<PRECISE>(rc, sm.chan[b * kChanBlock + cc], v);
+      for (int b = b_f; b <= b_hi; ++b) poly_block<PRECISE, true>(rc, sm, b, v);
     } else {
+      const float inv_step = rc.inv_bstep * (float)kChanBlock;
+      const int c_lo = min(max(__float2int_rd((-D - dmax) * inv_step), 0), dp.nvx);
+      const int c_hi = max(min(__float2int_ru((D - dmin) * inv_step), dp.nvx) - 1, -1);
 #pragma unroll 4
-      for (int c = 0; c < nvx; ++c) {
-        const float4 w = sm.chan[c];
-#pragma unroll
-        for (int j = 0; j < kPairs; ++j) {
-          u64 d = fma2(pk1(w.x), st2, d0[j]);
-          if (PRECISE) d = add2(d, fma2(pk1(w.x), st2_lo, d0lo[j]));
-          float ea, eb;
-          upk(mul2(d, d), ea, eb);
-          const u64 g = pk(ex2_approx(-ea), ex2_approx(-eb));        // Gaussian line
-          s0[j] = fma2(pk1(w.y), g, s0[j]);
-          s1[j] = fma2(pk1(w.z), g, s1[j]);
-          s2[j] = fma2(pk1(w.w), g, s2[j]);
-        }
-      }
+      for (int c = c_lo; c <= c_hi; ++c) direct_channel<PRECISE>(rc, sm.chan[c], v);
     }
 #pragma unroll
     for (int j = 0; j < kPairs; ++j)
       if (sidx[j] >= 0) {
-        float2 v;
-        upk(mul2(s0[j], In[j]), v.x, v.y);
-        *reinterpret_cast<float2*>(sm.maps + sidx[j]) = v;
-        upk(mul2(s1[j], In[j]), v.x, v.y);
-        *reinterpret_cast<float2*>(sm.maps + map_stride + sidx[j]) = v;
-        upk(mul2(s2[j], In[j]), v.x, v.y);
-        *reinterpret_cast<float2*>(sm.maps + 2 * map_stride + sidx[j]) = v;
+        float2 o;
+        upk(mul2(v.s0[j], In[j]), o.x, o.y);
+        *reinterpret_cast<float2*>(sm.maps + sidx[j]) = o;
+        upk(mul2(v.s1[j], In[j]), o.x, o.y);
+        *reinterpret_cast<float2*>(sm.maps + map_stride + sidx[j]) = o;
+        upk(mul2(v.s2[j], In[j]), o.x, o.y);
+        *reinterpret_cast<float2*>(sm.maps + 2 * map_stride + sidx[j]) = o;
       }
   }
 }
@@ -852,16 +891,16 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
       if (poly) {
         const int j = c & (kChanBlock - 1);
         const float f = exp2f(-step * step * (float)(j * (j - 1)));
-        u64* dst = sm.coef + (c >> 3) * (3 * kChanBlock) + j;
-        dst[0] = pk1(w.y * f);
-        dst[kChanBlock] = pk1(w.z * f);
-        dst[2 * kChanBlock] = pk1(w.w * f);
+        float* dst = sm.coef + (c >> 3) * (3 * kChanBlock) + j;
+        dst[0] = w.y * f;
+        dst[kChanBlock] = w.z * f;
+        dst[2 * kChanBlock] = w.w * f;
         const int i = kChanBlock - 1 - j;            // the same channel counted from the block's end
         const float fb = exp2f(-step * step * (float)(i * (i - 1)));
         dst = sm.coefb + (c >> 3) * (3 * kChanBlock) + i;
-        dst[0] = pk1(w.y * fb);
-        dst[kChanBlock] = pk1(w.z * fb);
-        dst[2 * kChanBlock] = pk1(w.w * fb);
+        dst[0] = w.y * fb;
+        dst[kChanBlock] = w.z * fb;
+        dst[2 * kChanBlock] = w.w * fb;
       }
     }
   }
@@ -964,7 +1003,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
 
 size_t fused_smem_bytes(const DevProblem& dp) {
   return sizeof(float) * (3 * (size_t)dp.ehs * dp.ews + dp.spare_plane) + sizeof(float4) * dp.nvx_pad +
-         sizeof(u64) * 6 * dp.nvx_pad + sizeof(RowConstD) + sizeof(float) * taps_floats(dp) + sizeof(RowConst) +
+         sizeof(float) * 6 * dp.nvx_pad + sizeof(RowConstD) + sizeof(float) * taps_floats(dp) + sizeof(RowConst) +
          sizeof(float) * 32;
 }
 

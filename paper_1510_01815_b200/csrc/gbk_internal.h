@@ -72,6 +72,8 @@ struct RowConst {
   float v_ref;        // reference velocity of the row's moment sums S1, S2, relative to v_center: V_sys
                       // clamped to the band, so the FP32 cancellation in m2^2 = S2/S0 - m1^2 involves the
                       // distance of the line from V_sys (or from the band edge) and not from v_center
+  float anchor_margin;   // how far past a block's anchor a line centre may lie (gbk_fused.cu, voxel loop)
+  float cen_lo, cen_hi;  // offsets (from extended channel 0) of the first and last in-band channel
   float amp;          // I0 * dv / (sigma0 sqrt(2 pi) u^2): scales the S0 block sum to m0
   float dark_s0;      // S0 block sums below this are model-dark (m0 < 1e-30 I0)
   int valid;
