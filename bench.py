@@ -13,8 +13,12 @@ quoted on.  Prints ONE JSON line on rank 0.
              launching stream, L2 flushed between timed launches, max over ranks
   e2e        the same through gbk_eval_batch_host: HOST (pinned) params in, HOST chi^2 out, copies
              inside the timed region (wall clock around a blocking call)
-  roofline   the fused kernel against the SM arithmetic pipe that bounds it (FP32 FMA pipe, "alu")
+  roofline   the fused kernel against the SM arithmetic pipe that bounds it (FP32 FMA pipe, "alu"):
+             `frac` by the algorithmic count of SURVEY.md section 8(d), `frac_executed` by the work the
+             kernel reports through gbk_eval_batch_counted in this very run
   cpu_baseline   the CPU oracle (oracle/, untouched) on a bounded sample of the same rows
+  configs    all five BASELINE.json configs at their own K: device ms per launch (median of >= 20,
+             L2 flushed), evals/s, tiling, op counts and fractions, the oracle beside each
 
 The oracle is executed only by the cpu_baseline leg and by --impl reference.  Nothing here reads
 /root/reference.  All inputs are seeded and synthetic (paper_1510_01815_b200/workloads.py).
@@ -162,6 +166,8 @@ def oracle_case(cfg: int):
     """Workload, oracle grid, observation (clean maps from the ORACLE here) and batches."""
     from oracle import gbk_oracle as oracle
     w = wl.config(cfg)
+    if cfg == 5:      # one galaxy of the survey at the mean PSF FWHM (the GPU leg mixes 1000 of them)
+        w = w.scaled(psf_fwhm=2.75)
     rng = wl.rng_for(cfg, 100)
     true = true_row_for(cfg, w, rng)
     g = oracle_grid(oracle, w)
@@ -177,11 +183,12 @@ def time_oracle(cfg: int, rows_per_step: int, steps: int, warmup: int, threads: 
     o = obs
     call = lambda rows: oracle.eval_rows(g, o.vobs[0], o.verr[0], o.sobs[0], o.serr[0], o.mask[0],
                                          rows, nthreads=threads)
+    take = lambda b, n: b[:n] if len(b) >= n else np.resize(b, (n, b.shape[1]))   # K < sample: rows repeated
     for i in range(warmup):
-        call(batches[i % len(batches)][:max(1, min(rows_per_step, threads))])
+        call(take(batches[i % len(batches)], max(1, min(rows_per_step, threads))))
     t0 = time.perf_counter()
     for i in range(steps):
-        call(batches[i % len(batches)][:rows_per_step])
+        call(take(batches[i % len(batches)], rows_per_step))
     dt = time.perf_counter() - t0
     return {"value": rows_per_step * steps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
             "seconds": dt,
@@ -234,6 +241,168 @@ def measure_pipe_peaks(gbk, torch, sm_count: int) -> dict:
     return out
 
 
+def psf_radius(w: wl.Workload, fwhm: float) -> int:
+    """Tap radius the library derives for a Gaussian PSF (include/gbk.h: R = ceil(4 sigma_fine))."""
+    if w.psf_kind == wl.PSF_IMAGE:
+        return w.psf_n // 2
+    if fwhm <= 0:
+        return 0
+    return int(np.ceil(4.0 * w.u * float(np.float32(fwhm)) / (2.0 * np.sqrt(2.0 * np.log(2.0)))))
+
+
+def ext_samples_per_eval(info, w: wl.Workload, R: int) -> int:
+    """Extended fine samples a row of PSF radius R evaluates: sum over its tiles of (tw+2R)(th+2R)."""
+    tw, th, fw, fh = info.tile_w * w.u, info.tile_h * w.u, w.nx * w.u, w.ny * w.u
+    tot = 0
+    for ty in range(info.tiles_y):
+        for tx in range(info.tiles_x):
+            tot += (min(tw, fw - tx * tw) + 2 * R) * (min(th, fh - ty * th) + 2 * R)
+    return tot
+
+
+def op_counts(info, w: wl.Workload, radii: np.ndarray) -> dict:
+    """Algorithmic FP32 lane-ops per evaluation: 5 per extended voxel, 45 per
+    extended sample, 3 maps x (2 x taps separable | taps^2 image) per fine pixel, 12 per spaxel --
+    averaged over the PSF radii of the batch's rows."""
+    nvx = info.nv + 2 * info.r_v
+    fine = (w.u * w.nx) * (w.u * w.ny)
+    tot = 0.0
+    samples = 0.0
+    for R in np.unique(radii):
+        share = float(np.mean(radii == R))
+        ns = ext_samples_per_eval(info, w, int(R))
+        taps = 2 * int(R) + 1
+        psf = taps * taps if w.psf_kind == wl.PSF_IMAGE else 2 * taps
+        tot += share * (5.0 * ns * nvx + 45.0 * ns + 3.0 * psf * fine + 12.0 * w.nx * w.ny)
+        samples += share * ns
+    return {"ops_per_eval": tot, "ext_samples_per_eval": samples, "ext_voxels_per_eval": samples * nvx}
+
+
+def executed_ops(counters: np.ndarray, K: int, nominal: dict, info, w: wl.Workload) -> float:
+    """FP32 lane-ops per evaluation the kernel executed, from its own work counters: a polynomial
+    block costs 27 per pixel and 8 channels (three degree-7 Horner chains, the g0 P products and the
+    restart), a directly summed channel 5 per voxel, the geometry 45 per sample of every warp item
+    (128 samples, padding lanes included); PSF passes and moments as in the algorithmic count."""
+    items, poly, direct = (float(counters[i]) for i in range(3))
+    nvx = info.nv + 2 * info.r_v
+    rest = nominal["ops_per_eval"] - 5.0 * nominal["ext_voxels_per_eval"] - 45.0 * nominal["ext_samples_per_eval"]
+    return (poly * 128 * 27 + direct * 128 * 5 + items * 128 * 45) / K + rest
+
+
+def build_case(gbk, torch, cfg: int, rank: int = 0) -> dict:
+    """Problem, batches and PSF radii of BASELINE.json config `cfg` at its own K (seeded, synthetic;
+    clean maps from the CUDA path itself)."""
+    w = wl.config(cfg)
+    rng = wl.rng_for(cfg, 100 + rank)
+    if cfg == 5:   # the 1000-galaxy survey: own PSF per galaxy, per-spaxel errors, LM-shaped slots
+        n = w.n_gal
+        fwhms = wl.galaxy_fwhms(w, rng)
+        trues = wl.draw_rows(w, rng, n)
+        shp = (n, w.ny, w.nx)
+        blank = wl.Observed(np.zeros(shp, np.float32), np.ones(shp, np.float32), np.zeros(shp, np.float32),
+                            np.ones(shp, np.float32), np.zeros(shp, np.uint8))
+        d = desc_for(w, blank)
+        d.update(n_gal=n, psf_fwhm=fwhms, psf_per_gal=True)
+        gi = torch.arange(n, dtype=torch.int32, device="cuda")
+        with gbk.Problem(**d) as prob:
+            o = prob.eval(torch.from_numpy(trues).cuda(), gi, want_maps=True)
+            torch.cuda.synchronize()
+            m0, m1, m2 = (o[k].cpu().numpy().astype(np.float64) for k in ("m0", "m1", "m2"))
+        obs = wl.observe(w, m0, m1, m2, rng)
+        d = desc_for(w, obs)
+        d.update(n_gal=n, psf_fwhm=fwhms, psf_per_gal=True)
+        slots = w.K // 8                                  # 2048 LM slots of base + 7 differences
+        gal = (np.arange(slots) % n).astype(np.int32)
+        batches = []
+        for _ in range(2):
+            starts = trues[gal].astype(np.float64)
+            b = wl.box(w)
+            free7 = [wl.IX_XO, wl.IX_YO, wl.IX_PA, wl.IX_INC, wl.IX_VSYS, wl.IX_VT, wl.IX_RT]
+            starts[:, free7] += 0.05 * (b[free7, 1] - b[free7, 0]) * rng.uniform(-1, 1, (slots, 7))
+            starts[:, wl.IX_INC] = np.clip(starts[:, wl.IX_INC], 20.0, 80.0)
+            starts[:, wl.IX_RT] = np.clip(starts[:, wl.IX_RT], 1.0, 8.0)
+            batches.append(np.concatenate([wl.lm_rows(w, r) for r in starts]).astype(np.float32))
+        gal_rows = np.repeat(gal, 8)
+        radii = np.asarray([psf_radius(w, f) for f in fwhms])[gal_rows]
+        return dict(cfg=cfg, w=w, desc=d, batches=batches, gal=gal_rows, radii=radii, true=trues[0],
+                    what=f"{n} galaxies with their own PSF (R 3..7), {slots} LM slots x 8 rows, gal_index mixed")
+    true = true_row_for(cfg, w, rng)
+    obs = observation_from_gpu(gbk, torch, w, true, rng)
+    if cfg == 1:
+        batches = [wl.cfg1_trial_row()]
+        what = "the trial row (K = 1), chi2 only"
+    elif cfg == 2:
+        batches = [wl.lm_rows(w, r) for r in wl.draw_rows(w, rng, 4)]
+        what = "one LM iteration: base row + 7 forward differences (K = 8)"
+    elif cfg == 3:
+        batches = batch_rows(cfg, w, true, rng, 4)
+        what = "nested-grid levels 0-3 cycled (K = 8^4), chi2 only"
+    else:
+        batches = batch_rows(cfg, w, true, rng, 4)
+        what = "K = 256 rows uniform in the prior box (nested-sampling batch), chi2 only"
+    K = batches[0].shape[0]
+    radii = np.full(K, psf_radius(w, w.psf_fwhm))
+    return dict(cfg=cfg, w=w, desc=desc_for(w, obs), batches=batches, gal=None, radii=radii, true=true,
+                what=what)
+
+
+def time_case(gbk, torch, case: dict, launches: int, flush, sm_max_mhz: float, tile=(0, 0)) -> dict:
+    """Device time per launch of one config: CUDA events on the launching stream around every launch,
+    L2 flushed in between; then one counted launch for the executed-work fraction."""
+    w = case["w"]
+    with gbk.Problem(**case["desc"], tile_w=tile[0], tile_h=tile[1]) as prob:
+        info = prob.info
+        dev = [torch.from_numpy(b).cuda() for b in case["batches"]]
+        gal = None if case["gal"] is None else torch.from_numpy(case["gal"]).cuda()
+        K = dev[0].shape[0]
+        chi2 = torch.empty(K, dtype=torch.float32, device="cuda")
+        stream = torch.cuda.current_stream()
+        st = stream.cuda_stream
+        for i in range(3):
+            flush.zero_()
+            gbk.gbk_eval_batch(prob.handle, dev[i % len(dev)], gal, K, chi2, stream=st)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+              for _ in range(launches)]
+        for i in range(launches):
+            flush.zero_()
+            ev[i][0].record(stream)
+            gbk.gbk_eval_batch(prob.handle, dev[i % len(dev)], gal, K, chi2, stream=st)
+            ev[i][1].record(stream)
+        torch.cuda.synchronize()
+        ms = [a.elapsed_time(b) for a, b in ev]
+        counters = torch.zeros(gbk.GBK_N_COUNTERS, dtype=torch.int64, device="cuda")
+        gbk.gbk_eval_batch_counted(prob.handle, dev[0], gal, K, chi2, counters, stream=st)
+        torch.cuda.synchronize()
+        cnt = counters.cpu().numpy()
+        # which tiling the library picked for this K (levels are chosen per call)
+        nominal = op_counts(info, w, case["radii"])
+    med = statistics.median(ms)
+    peak = info.sm_count * FP32_LANES_PER_SM_CLK * sm_max_mhz * 1e6 / 1e9
+    ex = executed_ops(cnt, K, nominal, info, w)
+    out = {"workload": f"config {case['cfg']}: {w.nx}x{w.ny} spaxels x {w.nv} channels, u={w.u}; {case['what']}",
+           "K": K, "launches": launches, "ms_per_launch_median": med, "ms_per_launch_min": min(ms),
+           "evals_per_s": K / (med * 1e-3), "ext_voxels_per_s": nominal["ext_voxels_per_eval"] * K / (med * 1e-3),
+           "tile_of_large_batches": [info.tile_w, info.tile_h], "block_threads": info.block_threads,
+           "ops_per_eval": int(nominal["ops_per_eval"]),
+           "frac": nominal["ops_per_eval"] * K / (med * 1e-3) / 1e9 / peak,
+           "ops_executed_per_eval": int(ex), "frac_executed": ex * K / (med * 1e-3) / 1e9 / peak,
+           "voxel_loop": {"warp_items": int(cnt[0]), "poly_blocks": int(cnt[1]), "direct_channels": int(cnt[2]),
+                          "precise_items": int(cnt[3])},
+           "checksum": float(chi2[torch.isfinite(chi2)].double().sum().item())}
+    if K * max(info.tiles_x * info.tiles_y, 1) < info.sm_count:
+        out["note"] = "launch-latency-bound: fewer thread blocks than SMs at the tile of large batches; " \
+                      "the library picks smaller tiles for such K"
+    return out
+
+
+def oracle_for_config(cfg: int, cores: int) -> dict:
+    """The oracle's evals/s on a bounded sample of config `cfg` (a few CPU-seconds)."""
+    rows = {1: 4 * cores, 2: cores, 3: 8 * cores, 4: cores, 5: 4 * cores}[cfg]
+    r = time_oracle(cfg, rows, 1, 0, cores)
+    return {"oracle_evals_per_s": r["value"], "oracle_cores": cores, "oracle_sample": r["sample"]}
+
+
 def run_ours(args, ranks) -> None:
     import torch
     from paper_1510_01815_b200 import dist, gbk
@@ -242,15 +411,13 @@ def run_ours(args, ranks) -> None:
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(ranks.local_rank)
     cfg = args.config
-    w = wl.config(cfg)
-    rng = wl.rng_for(cfg, 100 + ranks.rank)     # every rank its own galaxy: weak scaling
-    true = true_row_for(cfg, w, rng)
-    obs = observation_from_gpu(gbk, torch, w, true, rng)
-    batches = batch_rows(cfg, w, true, rng, 4)
+    case = build_case(gbk, torch, cfg, ranks.rank)     # every rank its own galaxy: weak scaling
+    w, batches = case["w"], case["batches"]
     K = batches[0].shape[0]
-    prob = gbk.Problem(**desc_for(w, obs), tile_w=args.tile[0], tile_h=args.tile[1])
+    prob = gbk.Problem(**case["desc"], tile_w=args.tile[0], tile_h=args.tile[1])
     info = prob.info
     dev_batches = [torch.from_numpy(b).cuda() for b in batches]
+    gal = None if case["gal"] is None else torch.from_numpy(case["gal"]).cuda()
     chi2 = torch.empty(K, dtype=torch.float32, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB of L2
     stream = torch.cuda.current_stream()
@@ -258,7 +425,7 @@ def run_ours(args, ranks) -> None:
     launches_per_step = 1          # one fused kernel per batch, tiled or not
 
     def step(i):
-        gbk.gbk_eval_batch(prob.handle, dev_batches[i % len(dev_batches)], None, K, chi2, stream=st)
+        gbk.gbk_eval_batch(prob.handle, dev_batches[i % len(dev_batches)], gal, K, chi2, stream=st)
 
     sampler = ClockSampler(ranks.local_rank)
     sampler.start()
@@ -280,7 +447,6 @@ def run_ours(args, ranks) -> None:
         ev[i][1].record(stream)
     torch.cuda.synchronize()
     dist.barrier(ranks)
-    t_end = time.perf_counter()
     ms = [a.elapsed_time(b) for a, b in ev]
     sec_rank = sum(ms) * 1e-3
     checksum = float(chi2[torch.isfinite(chi2)].sum().item())
@@ -288,84 +454,108 @@ def run_ours(args, ranks) -> None:
 
     # ---- end to end through the host entry: pinned host params in, host chi^2 out ----------
     host_batches = [torch.from_numpy(b).pin_memory() for b in batches]
+    host_gal = None if case["gal"] is None else torch.from_numpy(case["gal"]).pin_memory()
     host_chi2 = torch.empty(K, dtype=torch.float32).pin_memory()
     for i in range(3):
-        gbk.gbk_eval_batch_host(prob.handle, host_batches[i % len(host_batches)], None, K, host_chi2, st)
+        gbk.gbk_eval_batch_host(prob.handle, host_batches[i % len(host_batches)], host_gal, K, host_chi2, st)
     dist.barrier(ranks)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for i in range(args.steps):
-        gbk.gbk_eval_batch_host(prob.handle, host_batches[i % len(host_batches)], None, K, host_chi2, st)
+        gbk.gbk_eval_batch_host(prob.handle, host_batches[i % len(host_batches)], host_gal, K, host_chi2, st)
     torch.cuda.synchronize()
     e2e_rank = time.perf_counter() - t0
     t_end = time.perf_counter()
     e2e_value, _ = dist.aggregate_throughput(ranks, K * args.steps, e2e_rank)
     clocks = sampler.stop(t_warm, t_end)
     same = bool(np.array_equal(host_chi2.numpy(),
-                               _chi2_of(gbk, prob, dev_batches[(args.steps - 1) % len(dev_batches)], K, torch)))
+                               _chi2_of(gbk, prob, dev_batches[(args.steps - 1) % len(dev_batches)], gal, K, torch)))
 
-    # ---- roofline of the dominant kernel (the fused kernel: the only one at one tile) ------
+    # ---- roofline of the dominant kernel (the fused kernel: the only one of the step) -------
+    nominal = op_counts(info, w, case["radii"])
+    counters = torch.zeros(gbk.GBK_N_COUNTERS, dtype=torch.int64, device="cuda")
+    for b in dev_batches:                                         # the same batches the timed steps cycle
+        gbk.gbk_eval_batch_counted(prob.handle, b, gal, K, chi2, counters, stream=st)
+    torch.cuda.synchronize()
+    cnt = counters.cpu().numpy()
+    executed = executed_ops(cnt, K * len(dev_batches), nominal, info, w)
     nvx = info.nv + 2 * info.r_v
-    ext_samples = info.ext_voxels_per_eval // nvx
-    mufu_per_eval = info.ext_voxels_per_eval + 3 * ext_samples
-    taps = 2 * info.r_p_max + 1
-    psf_fma = (taps * taps if w.psf_kind == wl.PSF_IMAGE else 2 * taps)       # per map and fine pixel
-    fp32_per_eval = 5 * info.ext_voxels_per_eval + 45 * ext_samples \
-        + 3 * psf_fma * (info.u * info.nx) * (info.u * info.ny) + 12 * info.nx * info.ny
+    mufu_per_eval = nominal["ext_voxels_per_eval"] + 3 * nominal["ext_samples_per_eval"]
     sm_max = (clocks.get("sm_max_mhz") or 1965.0)
-    # The voxel loop sums the Gaussian line over blocks of 8 channels as a polynomial in the line
-    # ratio (one MUFU.EX2 pair per pixel and block, no ex2 per voxel), so the binding pipe is the
-    # FP32 FMA pipe (quote the fraction against that pipe); the MUFU figures
-    # are kept beside it for the direct-evaluation count.
+    # The voxel loop sums the Gaussian line over blocks of 8 channels as a polynomial in the line ratio
+    # (two MUFU.EX2 per pixel and block, no ex2 per voxel), so the binding pipe is the FP32 FMA pipe
+    # (quote the fraction against that pipe); the MUFU figures of a direct
+    # evaluation are kept beside it.
     peak_fp32 = info.sm_count * FP32_LANES_PER_SM_CLK * sm_max * 1e6 / 1e9           # G lane-op/s
     peak_mufu = info.sm_count * MUFU_LANES_PER_SM_CLK * sm_max * 1e6 / 1e9
-    achieved = fp32_per_eval * K * args.steps / sec_rank / 1e9
+    evals_per_s_rank = K * args.steps / sec_rank
+    achieved = nominal["ops_per_eval"] * evals_per_s_rank / 1e9
     roofline = {"bound": "alu", "pipe": "FP32 FMA pipe, 128 lanes/clk/SM (FFMA2 = 2 lanes x 2 clk)",
                 "achieved": achieved, "peak": peak_fp32, "unit": "Gop/s", "frac": achieved / peak_fp32,
-                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed capture
-                # profiles/r01_fused_kernel_ncu.md (config 3 only; not measured live)
-                "traffic": 327424 if cfg == 3 else None, "traffic_unit": "bytes per launch",
+                "traffic": None,
+                "traffic_source": "not measured live; dram__bytes of one launch are in profiles/ (ncu --set full): "
+                                  "~0.3 MB per launch of 4096 rows, irrelevant to an ALU-bound kernel",
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
-                "ops_per_eval": int(fp32_per_eval),
-                "ops_how": "algorithmic FP32 lane-ops: 5/ext voxel + 45/ext sample + 3 maps x (2 x taps separable | taps^2 image)/fine pixel + 12/spaxel",
-                # what the kernel executes AT MOST: the block polynomial needs 27 FP32 lane-ops per
-                # pixel and 8-channel block (3.4 per voxel) where the algorithmic count above has 5 per
-                # voxel, and blocks whose line has flushed to exactly 0 for a whole warp are skipped
-                # (bit-identical; data-dependent, about a third of the blocks on this workload), so
-                # `frac` (algorithmic work / time / peak, as the contract defines it) says how fast the
-                # method's work gets done, not how busy the FP32 pipe is: ncu has the pipe at ~60 %.
-                "ops_executed_max_per_eval": int(fp32_per_eval - (5.0 - 27.0 / 8.0) * info.ext_voxels_per_eval),
-                "frac_executed_max": (fp32_per_eval - (5.0 - 27.0 / 8.0) * info.ext_voxels_per_eval)
-                * K * args.steps / sec_rank / 1e9 / peak_fp32,
-                "note": "frac counts the ALGORITHMIC operations of SURVEY.md section 8(d) (5 per voxel); the "
-                        "kernel sums each 8-channel block as a polynomial (3.4 per voxel) and skips blocks that "
-                        "are exactly zero, so it executes fewer: ncu has the FP32 pipe ~51 % busy "
-                        "(profiles/r01_fused_kernel_ncu.md)",
+                "ops_per_eval": int(nominal["ops_per_eval"]),
+                "ops_how": "ALGORITHMIC FP32 lane-ops of SURVEY.md 8(d): 5/ext voxel + 45/ext sample + 3 maps x "
+                           "(2 x taps separable | taps^2 image)/fine pixel + 12/spaxel",
+                "ops_executed_per_eval": int(executed),
+                "achieved_executed": executed * evals_per_s_rank / 1e9,
+                "frac_executed": executed * evals_per_s_rank / 1e9 / peak_fp32,
+                "executed_how": "counted by the kernel in this run (gbk_eval_batch_counted on the timed batches): "
+                                "27 lane-ops per pixel and executed 8-channel polynomial block, 5 per directly summed "
+                                "voxel, 45 per sample of every warp item; PSF passes and moments as in ops_per_eval",
+                "voxel_loop": {"warp_items": int(cnt[0]), "poly_blocks": int(cnt[1]),
+                               "direct_channels": int(cnt[2]), "precise_items": int(cnt[3]),
+                               "channels_summed_per_sample": float((cnt[1] * 8 + cnt[2]) / max(cnt[0], 1)),
+                               "extended_channels": int(nvx)},
+                "note": "frac follows the contract (algorithmic work of SURVEY.md 8(d) / time / peak): it says how fast "
+                        "the method's nominal work gets done and can exceed what the pipe executes, because the kernel "
+                        "sums a line only where it is non-negligible (lines centred in the band: |d| < 6.5, i.e. beyond "
+                        "7.7 sigma_0 left out, < 2^-42 of the sum) and as a block polynomial (27 lane-ops per 8 voxels "
+                        "instead of 40).  frac_executed is the FP32 work actually executed / time / peak, the figure to "
+                        "compare with ncu's FMA-pipe utilisation in profiles/",
                 "mufu_ops_per_eval_direct": int(mufu_per_eval),
-                "mufu_frac_if_direct": mufu_per_eval * K * args.steps / sec_rank / 1e9 / peak_mufu,
+                "mufu_frac_if_direct": mufu_per_eval * evals_per_s_rank / 1e9 / peak_mufu,
                 "kernel_ms_avg": statistics.mean(ms), "kernel_ms_median": statistics.median(ms),
                 "kernel_ms_min": min(ms)}
     if ranks.is_main:
         pk = measure_pipe_peaks(gbk, torch, info.sm_count)
         roofline.update(pk)
         roofline["frac_of_measured"] = achieved / pk["ffma_gops_measured"]
+        roofline["frac_executed_of_measured"] = roofline["achieved_executed"] / pk["ffma_gops_measured"]
         if clocks.get("sm_mhz"):
             roofline["frac_at_sampled_clock"] = achieved / (peak_fp32 * clocks["sm_mhz"] / sm_max)
 
     cpu = None
+    cores = host_cores()
     if ranks.is_main and ranks.world == 1 and not args.no_cpu_baseline:
-        cores = host_cores()
         cpu = time_oracle(cfg, args.cpu_rows or 32 * cores, 1, 1, cores)
         one = time_oracle(cfg, 24, 1, 1, 1)          # the paper's single-thread column
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
         cpu["value_1_thread"] = one["value"]
         cpu["sample_1_thread"] = one["sample"]
+        cpu["note"] = ("the parity oracle as it stands: the paper's definition written out literally in FP64 (materialised "
+                       "cube, direct non-separable PSF sum per channel, gcc -O2, OpenMP over rows only) -- a correctness "
+                       "reference, NOT a tuned CPU implementation; the GPU/oracle ratio says nothing about kernel quality")
 
-    unfused = time_unfused(gbk, torch, prob, dev_batches[0], K, info) \
+    # ---- all five configs at their own K (rank 0; outside the timed region) -----------------
+    configs = None
+    if ranks.is_main and not args.no_configs:
+        configs = {}
+        for c in (1, 2, 3, 4, 5):
+            cc = case if c == cfg else build_case(gbk, torch, c, ranks.rank)
+            entry = time_case(gbk, torch, cc, max(20, args.config_launches), flush, sm_max,
+                              tile=args.tile if c == cfg else (0, 0))
+            if ranks.world == 1 and not args.no_cpu_baseline:
+                entry.update(oracle_for_config(c, cores))
+            configs[f"cfg{c}"] = entry
+
+    unfused = time_unfused(gbk, torch, prob, dev_batches[0], gal, K, info) \
         if (ranks.is_main and not args.no_fits) else None
-    vfield = time_vfield(gbk, torch, prob, dev_batches[0], K, info, sm_max) \
+    vfield = time_vfield(gbk, torch, prob, dev_batches[0], gal, K, info, sm_max) \
         if (ranks.is_main and not args.no_fits) else None
-    fits = time_fits(gbk, torch, prob, w, true) if (ranks.is_main and cfg == 3 and not args.no_fits) else None
+    fits = time_fits(gbk, torch, prob, w, case["true"]) if (ranks.is_main and cfg == 3 and not args.no_fits) else None
     if ranks.is_main:
         core_vox = w.nx * w.ny * w.nv * w.u * w.u
         line = {
@@ -374,18 +564,19 @@ def run_ours(args, ranks) -> None:
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": f"config {cfg}: {w.nx}x{w.ny} spaxels x {w.nv} channels, u={w.u}, "
-                                   f"K={K} rows per launch (nested-grid levels 0-3 cycled), chi2 only",
+                                   f"K={K} rows per launch; {case['what']}",
                        "rows_per_launch": K, "l2": "flushed between timed launches (256 MiB memset)",
                        "tile": [info.tile_w, info.tile_h], "block_threads": info.block_threads,
                        "smem_bytes": info.smem_bytes, "blocks_per_sm": info.blocks_per_sm,
-                       "ext_voxels_per_eval": int(info.ext_voxels_per_eval),
+                       "ext_voxels_per_eval": int(nominal["ext_voxels_per_eval"]),
                        "parallelism": f"rows sharded, {ranks.world} rank(s), no collective"},
-            "voxels_per_s": value * core_vox, "ext_voxels_per_s": value * info.ext_voxels_per_eval,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": K * wl.P * 4,
+            "voxels_per_s": value * core_vox, "ext_voxels_per_s": value * nominal["ext_voxels_per_eval"],
+            "e2e": {"value": e2e_value, "unit": UNIT,
+                    "h2d_bytes_per_step": K * wl.P * 4 + (K * 4 if case["gal"] is not None else 0),
                     "d2h_bytes_per_step": K * 4, "matches_device_path": same},
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu, "checksum": checksum,
-            "fits": fits, "unfused": unfused, "vfield": vfield,
+            "configs": configs, "fits": fits, "unfused": unfused, "vfield": vfield,
         }
         print(json.dumps(line), flush=True)
     prob.close()
@@ -487,18 +678,18 @@ def time_survey(gbk, torch) -> dict:
             "note": "noisy data (N(0,E), E~U[3,15] km/s): the thresholds are the paper's for noise-free mocks"}
 
 
-def time_unfused(gbk, torch, prob, params, K: int, info, reps: int = 5) -> dict:
+def time_unfused(gbk, torch, prob, params, gal, K: int, info, reps: int = 5) -> dict:
     """The unfused comparison path (one kernel per pipeline step, FP32 cube in HBM) on the same
     batch: evals/s and achieved HBM GB/s = algorithmic bytes / device time, against the measured copy
     bandwidth of MEASURED_PEAKS.json (outside the timed region; rank 0)."""
     chi = torch.empty(K, dtype=torch.float32, device="cuda")
     st = torch.cuda.current_stream().cuda_stream
-    gbk.gbk_eval_batch_unfused(prob.handle, params, None, K, chi, stream=st)      # warm-up + scratch
+    gbk.gbk_eval_batch_unfused(prob.handle, params, gal, K, chi, stream=st)      # warm-up + scratch
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(reps):
-        gbk.gbk_eval_batch_unfused(prob.handle, params, None, K, chi, stream=st)
+        gbk.gbk_eval_batch_unfused(prob.handle, params, gal, K, chi, stream=st)
     e1.record()
     torch.cuda.synchronize()
     sec = e0.elapsed_time(e1) * 1e-3 / reps
@@ -514,7 +705,7 @@ def time_unfused(gbk, torch, prob, params, K: int, info, reps: int = 5) -> dict:
             "unit_bw": "GB/s", "frac": gbs / peak}
 
 
-def time_vfield(gbk, torch, prob, params, K: int, info, sm_max_mhz: float, reps: int = 20) -> dict:
+def time_vfield(gbk, torch, prob, params, gal, K: int, info, sm_max_mhz: float, reps: int = 20) -> dict:
     """The paper's other strategy (velocity-field modelling) on the same batch:
     gbk_eval_vfield_batch, chi^2 only.  27 FP32 lane-ops per spaxel and row (eq. 1-4, 6, 8, residual,
     square-accumulate); bound by the FP32 pipe / issue, not by memory (the observation is read from
@@ -522,12 +713,12 @@ def time_vfield(gbk, torch, prob, params, K: int, info, sm_max_mhz: float, reps:
     chi = torch.empty(K, dtype=torch.float32, device="cuda")
     st = torch.cuda.current_stream().cuda_stream
     for _ in range(3):
-        gbk.gbk_eval_vfield_batch(prob.handle, params, None, K, chi, stream=st)
+        gbk.gbk_eval_vfield_batch(prob.handle, params, gal, K, chi, stream=st)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(reps):
-        gbk.gbk_eval_vfield_batch(prob.handle, params, None, K, chi, stream=st)
+        gbk.gbk_eval_vfield_batch(prob.handle, params, gal, K, chi, stream=st)
     e1.record()
     torch.cuda.synchronize()
     sec = e0.elapsed_time(e1) * 1e-3 / reps
@@ -539,9 +730,9 @@ def time_vfield(gbk, torch, prob, params, K: int, info, sm_max_mhz: float, reps:
             "note": "back-to-back launches on a warm L2 (64 KB observation, 160 KB parameters)"}
 
 
-def _chi2_of(gbk, prob, params, K, torch):
+def _chi2_of(gbk, prob, params, gal, K, torch):
     out = torch.empty(K, dtype=torch.float32, device="cuda")
-    gbk.gbk_eval_batch(prob.handle, params, None, K, out, stream=torch.cuda.current_stream().cuda_stream)
+    gbk.gbk_eval_batch(prob.handle, params, gal, K, out, stream=torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
     return out.cpu().numpy()
 
@@ -557,6 +748,8 @@ def main() -> None:
     ap.add_argument("--ref-rows", type=int, default=0, help="rows per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fits", action="store_true", help="skip the wall-time-to-fit legs")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config table (configs 1-5)")
+    ap.add_argument("--config-launches", type=int, default=25, help="timed launches per config of the table")
     ap.add_argument("--tile", type=int, nargs=2, default=(0, 0), metavar=("W", "H"),
                     help="spatial tile in spaxels (default 0 0 = the library's automatic tiling)")
     args = ap.parse_args()

@@ -17,8 +17,16 @@
  * memory.  No function throws or aborts; all return GBK_OK or an error code
  * and leave a message for gbk_last_error().  There is NO CPU fallback: without
  * a CUDA device every compute call returns GBK_ERR_CUDA.  Calls make the problem's device current
- * for their duration and restore the caller's device; a problem must not be used by two host
- * threads at the same time (its scratch buffers grow on demand).
+ * for their duration and restore the caller's device.
+ *
+ * Streams and threads.  The eval calls are asynchronous on the caller's stream.  The only state they
+ * share is a small scratch (cross-tile chi^2 partials of tiled launches, staging of the host entry)
+ * that the problem keeps PER STREAM: launches of one problem on different streams may overlap, from
+ * one host thread or several (the scratch table is guarded by a mutex).  Launches on the SAME stream
+ * are ordered by the stream and share that stream's scratch.  A CUDA graph captured from a stream
+ * uses that stream's scratch: do not replay it while other work of the same problem and stream is in
+ * flight elsewhere.  The scratch grows (cudaMalloc, which synchronises) the first time a stream sees
+ * a larger batch; gbk_reserve sizes it up front, which is REQUIRED before a stream capture.
  *
  * Model row (GBK_P = 10 floats):
  *   [0] x_o, [1] y_o    kinematic centre, data pixels (pixel j is centred on j)
@@ -138,8 +146,9 @@ int gbk_set_strategy(gbk_problem *p, int32_t strategy);
 /*
  * The hot path (PAPER.md:63-66 steps 1-3 for K rows), fused: the model cube is
  * never written to memory.  Asynchronous on `cuda_stream`; never synchronises
- * or allocates except to grow the cross-tile scratch when K grows (first call
- * with a larger K).
+ * or allocates except to grow that stream's cross-tile scratch (see gbk_reserve).
+ * Errors: GBK_ERR_ARG (NULL arguments, K < 0, K x tiles beyond the grid limit, scratch growth
+ * needed during a stream capture), GBK_ERR_UNSUPPORTED, GBK_ERR_ALLOC, GBK_ERR_CUDA.
  *   params     DEVICE [K][GBK_P] float32, row-major
  *   gal_index  DEVICE [K] int32 in [0, n_gal), or NULL (all rows use data set 0)
  *   chi2       DEVICE [K] float32, required (eq. 11)
@@ -154,6 +163,27 @@ int gbk_set_strategy(gbk_problem *p, int32_t strategy);
 int gbk_eval_batch(gbk_problem *p, const float *params, const int32_t *gal_index, int64_t K,
                    float *chi2, float *m0, float *m1, float *m2, float *resid,
                    void *cuda_stream);
+
+/*
+ * gbk_eval_batch (chi^2 only) that also COUNTS the work the voxel loop executes, for the roofline
+ * of bench.py: `counters` is a DEVICE array of GBK_N_COUNTERS uint64 the kernel adds to (the caller
+ * zeroes it).  Units: one warp item = 128 fine samples (32 lanes x 2 pixel pairs); a polynomial block
+ * = 8 channels of one warp item summed as a polynomial (1024 voxels); a direct channel = 1 channel of
+ * one warp item by one ex2 per voxel (128 voxels).  The counting costs a few atomics per thread block,
+ * so timings are taken with gbk_eval_batch.
+ */
+enum { GBK_CNT_ITEMS = 0, GBK_CNT_POLY_BLOCKS = 1, GBK_CNT_DIRECT_CHANNELS = 2, GBK_CNT_PRECISE_ITEMS = 3,
+       GBK_N_COUNTERS = 4 };
+int gbk_eval_batch_counted(gbk_problem *p, const float *params, const int32_t *gal_index, int64_t K,
+                           float *chi2, uint64_t *counters, void *cuda_stream);
+
+/*
+ * Sizes the scratch that `cuda_stream` needs for batches of up to K_max rows (any tiling the library
+ * may choose for them) and for gbk_eval_batch_host, so that later eval calls on that stream neither
+ * allocate nor synchronise.  Needed before capturing eval calls into a CUDA graph: an eval call that
+ * would have to grow the scratch during a capture returns GBK_ERR_ARG instead.
+ */
+int gbk_reserve(gbk_problem *p, int64_t K_max, void *cuda_stream);
 
 /*
  * Comparison path, same contract: one kernel per step of the paper's pipeline

@@ -6,6 +6,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -76,15 +77,20 @@ struct gbk_problem {
   float* psf_taps = nullptr;
   int* psf_r = nullptr;
   float4* obs = nullptr;
-  float* partial = nullptr;
-  unsigned* tile_count = nullptr;   // [count_cap] zeroed at allocation, self-resetting afterwards
-  long long count_cap = 0;
-  long long partial_cap = 0;    // floats
-  // staging for gbk_eval_batch_host
-  float* st_params = nullptr;
-  int32_t* st_gal = nullptr;
-  float* st_chi2 = nullptr;
-  long long st_cap = 0;
+  // Scratch of the eval calls, one set per CUDA stream the problem has been used on, so that
+  // launches issued on different streams may overlap (they never share a buffer).
+  struct StreamScratch {
+    cudaStream_t stream = nullptr;
+    float* partial = nullptr;         // [partial_cap] cross-tile chi^2 partials (tiled launches)
+    unsigned* tile_count = nullptr;   // [count_cap] zeroed at allocation, self-resetting afterwards
+    long long partial_cap = 0, count_cap = 0;
+    float* st_params = nullptr;       // staging of gbk_eval_batch_host
+    int32_t* st_gal = nullptr;
+    float* st_chi2 = nullptr;
+    long long st_cap = 0;
+  };
+  std::vector<StreamScratch*> scratch;
+  std::mutex mu;                      // guards `scratch` (lookup and growth)
   // scratch of the unfused path
   float* uf_scratch = nullptr;
   long long uf_rows = 0;        // rows the scratch holds
@@ -99,11 +105,11 @@ extern "C" int gbk_destroy(gbk_problem* p) {
   cudaFree(p->psf_taps);
   cudaFree(p->psf_r);
   cudaFree(p->obs);
-  cudaFree(p->partial);
-  cudaFree(p->tile_count);
-  cudaFree(p->st_params);
-  cudaFree(p->st_gal);
-  cudaFree(p->st_chi2);
+  for (gbk_problem::StreamScratch* sc : p->scratch) {
+    cudaFree(sc->partial), cudaFree(sc->tile_count);
+    cudaFree(sc->st_params), cudaFree(sc->st_gal), cudaFree(sc->st_chi2);
+    delete sc;
+  }
   cudaFree(p->uf_scratch);
   cudaFree(p->lsf_taps);
   delete p;
@@ -402,23 +408,12 @@ static int check_eval_args(gbk_problem* p, const float* params, int64_t K, float
   if (!p) return fail(GBK_ERR_ARG, "null problem");
   if (K < 0) return fail(GBK_ERR_ARG, "K must be >= 0");
   if (K > 0 && (!params || !chi2)) return fail(GBK_ERR_ARG, "params and chi2 are required");
-  if (K * (int64_t)p->dp.ntiles > 0x7fffffffLL)   // smaller tilings are only used for small K
-    return fail(GBK_ERR_ARG, "K * tiles exceeds the grid limit");
   return GBK_OK;
 }
 
-extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
-                              float* chi2, float* m0, float* m1, float* m2, float* resid,
-                              void* cuda_stream) {
-  g_err[0] = 0;
-  if (int rc = check_eval_args(p, params, K, chi2)) return rc;
-  if (int rc = check_cube_model(p)) return rc;
-  if (K == 0) return GBK_OK;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  DeviceGuard guard(p->device);
-  GBK_CUDA(guard.status);
-  // tiling: the level with the fewest (waves of blocks) x (voxel-loop passes per block); ties go
-  // to the larger tile (less halo work, and one tile needs no second kernel)
+// The tiling level a batch of K rows runs on: the one with the fewest (waves of blocks) x
+// (voxel-loop passes per block); ties go to the larger tile (less halo work).
+static size_t pick_level(const gbk_problem* p, int64_t K) {
   size_t lv = 0;
   long long best_cost = 0;
   for (size_t i = 0; i < p->levels.size(); ++i) {
@@ -427,22 +422,112 @@ extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t
     const long long cost = ((long long)K * L.dp.ntiles + slots - 1) / slots * L.rounds;
     if (i == 0 || cost < best_cost) best_cost = cost, lv = i;
   }
+  return lv;
+}
+
+static gbk_problem::StreamScratch* scratch_of(gbk_problem* p, cudaStream_t st) {
+  for (gbk_problem::StreamScratch* sc : p->scratch)
+    if (sc->stream == st) return sc;
+  gbk_problem::StreamScratch* sc = new (std::nothrow) gbk_problem::StreamScratch;
+  if (!sc) return nullptr;
+  sc->stream = st;
+  p->scratch.push_back(sc);
+  return sc;
+}
+
+// Grows the cross-tile scratch of a stream to `need` partials and `rows` counters.  Never during a
+// stream capture: allocation is illegal there, so the caller has to gbk_reserve beforehand.
+static int grow_tile_scratch(gbk_problem::StreamScratch* sc, long long need, long long rows, cudaStream_t st) {
+  if (need <= sc->partial_cap && rows <= sc->count_cap) return GBK_OK;
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  GBK_CUDA(cudaStreamIsCapturing(st, &cap));
+  if (cap != cudaStreamCaptureStatusNone)
+    return fail(GBK_ERR_ARG, "the stream is being captured and the cross-tile scratch is too small: call "
+                             "gbk_reserve(problem, K, stream) before the capture");
+  if (need > sc->partial_cap) {
+    if (sc->partial) GBK_CUDA(cudaFree(sc->partial));   // waits for launches that still use it
+    sc->partial = nullptr, sc->partial_cap = 0;
+    GBK_CUDA(cudaMalloc(&sc->partial, sizeof(float) * (size_t)need));
+    sc->partial_cap = need;
+  }
+  if (rows > sc->count_cap) {
+    if (sc->tile_count) GBK_CUDA(cudaFree(sc->tile_count));
+    sc->tile_count = nullptr, sc->count_cap = 0;
+    GBK_CUDA(cudaMalloc(&sc->tile_count, sizeof(unsigned) * (size_t)rows));
+    GBK_CUDA(cudaMemsetAsync(sc->tile_count, 0, sizeof(unsigned) * (size_t)rows, st));
+    sc->count_cap = rows;
+  }
+  return GBK_OK;
+}
+
+extern "C" int gbk_reserve(gbk_problem* p, int64_t K_max, void* cuda_stream) {
+  g_err[0] = 0;
+  if (!p) return fail(GBK_ERR_ARG, "null problem");
+  if (K_max < 0) return fail(GBK_ERR_ARG, "K_max must be >= 0");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DeviceGuard guard(p->device);
+  GBK_CUDA(guard.status);
+  // the largest K x tiles any batch of up to K_max rows asks for (the tiling depends on K)
+  long long need = 0, rows = 0;
+  for (int64_t K = 1; K <= K_max; ++K) {
+    const int ntiles = p->levels[pick_level(p, K)].dp.ntiles;
+    if (ntiles > 1) need = std::max(need, (long long)K * ntiles), rows = K;
+  }
+  std::lock_guard<std::mutex> lock(p->mu);
+  gbk_problem::StreamScratch* sc = scratch_of(p, st);
+  if (!sc) return fail(GBK_ERR_ALLOC, "out of host memory");
+  if (int rc = grow_tile_scratch(sc, need, rows, st)) return rc;
+  if (K_max > sc->st_cap) {
+    cudaFree(sc->st_params), cudaFree(sc->st_gal), cudaFree(sc->st_chi2);
+    sc->st_params = nullptr, sc->st_gal = nullptr, sc->st_chi2 = nullptr, sc->st_cap = 0;
+    GBK_CUDA(cudaMalloc(&sc->st_params, sizeof(float) * GBK_P * (size_t)K_max));
+    GBK_CUDA(cudaMalloc(&sc->st_gal, sizeof(int32_t) * (size_t)K_max));
+    GBK_CUDA(cudaMalloc(&sc->st_chi2, sizeof(float) * (size_t)K_max));
+    sc->st_cap = K_max;
+  }
+  return GBK_OK;
+}
+
+static int eval_batch_impl(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
+                           float* chi2, float* m0, float* m1, float* m2, float* resid,
+                           unsigned long long* counters, void* cuda_stream);
+
+extern "C" int gbk_eval_batch(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
+                              float* chi2, float* m0, float* m1, float* m2, float* resid,
+                              void* cuda_stream) {
+  return eval_batch_impl(p, params, gal_index, K, chi2, m0, m1, m2, resid, nullptr, cuda_stream);
+}
+
+extern "C" int gbk_eval_batch_counted(gbk_problem* p, const float* params, const int32_t* gal_index,
+                                      int64_t K, float* chi2, uint64_t* counters, void* cuda_stream) {
+  if (!counters) return fail(GBK_ERR_ARG, "counters is required");
+  return eval_batch_impl(p, params, gal_index, K, chi2, nullptr, nullptr, nullptr, nullptr,
+                         reinterpret_cast<unsigned long long*>(counters), cuda_stream);
+}
+
+static int eval_batch_impl(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
+                           float* chi2, float* m0, float* m1, float* m2, float* resid,
+                           unsigned long long* counters, void* cuda_stream) {
+  g_err[0] = 0;
+  if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  if (int rc = check_cube_model(p)) return rc;
+  if (K == 0) return GBK_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DeviceGuard guard(p->device);
+  GBK_CUDA(guard.status);
+  const size_t lv = pick_level(p, K);
   const DevProblem& dp = p->levels[lv].dp;
-  const long long need = dp.ntiles > 1 ? (long long)K * dp.ntiles : 0;
-  if (need > p->partial_cap) {
-    if (p->partial) GBK_CUDA(cudaFree(p->partial));   // synchronises; only when K grows
-    p->partial = nullptr, p->partial_cap = 0;
-    GBK_CUDA(cudaMalloc(&p->partial, sizeof(float) * (size_t)need));
-    p->partial_cap = need;
+  if (K * (int64_t)dp.ntiles > 0x7fffffffLL) return fail(GBK_ERR_ARG, "K * tiles exceeds the grid limit");
+  float* partial = nullptr;
+  unsigned* tile_count = nullptr;
+  if (dp.ntiles > 1) {
+    std::lock_guard<std::mutex> lock(p->mu);
+    gbk_problem::StreamScratch* sc = scratch_of(p, st);
+    if (!sc) return fail(GBK_ERR_ALLOC, "out of host memory");
+    if (int rc = grow_tile_scratch(sc, (long long)K * dp.ntiles, K, st)) return rc;
+    partial = sc->partial, tile_count = sc->tile_count;
   }
-  if (need > 0 && K > p->count_cap) {
-    if (p->tile_count) GBK_CUDA(cudaFree(p->tile_count));
-    p->tile_count = nullptr, p->count_cap = 0;
-    GBK_CUDA(cudaMalloc(&p->tile_count, sizeof(unsigned) * (size_t)K));
-    GBK_CUDA(cudaMemset(p->tile_count, 0, sizeof(unsigned) * (size_t)K));
-    p->count_cap = K;
-  }
-  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, p->partial, p->tile_count};
+  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, partial, tile_count, counters};
   GBK_CUDA(launch_fused(dp, a, p->levels[lv].fl, st));
   return GBK_OK;
 }
@@ -455,7 +540,7 @@ extern "C" int gbk_eval_vfield_batch(gbk_problem* p, const float* params, const 
   if (K == 0) return GBK_OK;
   DeviceGuard guard(p->device);
   GBK_CUDA(guard.status);
-  EvalArgs a{params, gal_index, (long long)K, chi2, nullptr, vmap, nullptr, resid, nullptr, nullptr};
+  EvalArgs a{params, gal_index, (long long)K, chi2, nullptr, vmap, nullptr, resid, nullptr, nullptr, nullptr};
   GBK_CUDA(launch_vfield(p->dp, a, (cudaStream_t)cuda_stream));
   return GBK_OK;
 }
@@ -468,21 +553,21 @@ extern "C" int gbk_eval_batch_host(gbk_problem* p, const float* params, const in
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(p->device);
   GBK_CUDA(guard.status);
-  if (K > p->st_cap) {
-    cudaFree(p->st_params), cudaFree(p->st_gal), cudaFree(p->st_chi2);
-    p->st_params = nullptr, p->st_gal = nullptr, p->st_chi2 = nullptr, p->st_cap = 0;
-    GBK_CUDA(cudaMalloc(&p->st_params, sizeof(float) * GBK_P * (size_t)K));
-    GBK_CUDA(cudaMalloc(&p->st_gal, sizeof(int32_t) * (size_t)K));
-    GBK_CUDA(cudaMalloc(&p->st_chi2, sizeof(float) * (size_t)K));
-    p->st_cap = K;
+  gbk_problem::StreamScratch* sc;
+  {
+    std::lock_guard<std::mutex> lock(p->mu);
+    sc = scratch_of(p, st);
   }
-  GBK_CUDA(cudaMemcpyAsync(p->st_params, params, sizeof(float) * GBK_P * (size_t)K, cudaMemcpyHostToDevice, st));
+  if (!sc) return fail(GBK_ERR_ALLOC, "out of host memory");
+  if (K > sc->st_cap)
+    if (int rc = gbk_reserve(p, K, cuda_stream)) return rc;
+  GBK_CUDA(cudaMemcpyAsync(sc->st_params, params, sizeof(float) * GBK_P * (size_t)K, cudaMemcpyHostToDevice, st));
   if (gal_index)
-    GBK_CUDA(cudaMemcpyAsync(p->st_gal, gal_index, sizeof(int32_t) * (size_t)K, cudaMemcpyHostToDevice, st));
-  if (int rc = gbk_eval_batch(p, p->st_params, gal_index ? p->st_gal : nullptr, K, p->st_chi2, nullptr,
+    GBK_CUDA(cudaMemcpyAsync(sc->st_gal, gal_index, sizeof(int32_t) * (size_t)K, cudaMemcpyHostToDevice, st));
+  if (int rc = gbk_eval_batch(p, sc->st_params, gal_index ? sc->st_gal : nullptr, K, sc->st_chi2, nullptr,
                               nullptr, nullptr, nullptr, cuda_stream))
     return rc;
-  GBK_CUDA(cudaMemcpyAsync(chi2, p->st_chi2, sizeof(float) * (size_t)K, cudaMemcpyDeviceToHost, st));
+  GBK_CUDA(cudaMemcpyAsync(chi2, sc->st_chi2, sizeof(float) * (size_t)K, cudaMemcpyDeviceToHost, st));
   GBK_CUDA(cudaStreamSynchronize(st));
   return GBK_OK;
 }
@@ -506,7 +591,7 @@ extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const
     GBK_CUDA(cudaMalloc(&p->uf_scratch, per_row * (size_t)want));
     p->uf_rows = want;
   }
-  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, nullptr, nullptr};
+  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, nullptr, nullptr, nullptr};
   GBK_CUDA(launch_unfused(p->dp, a, p->lsf_taps, p->uf_scratch, p->uf_rows, p->sm_count,
                           (cudaStream_t)cuda_stream));
   return GBK_OK;

@@ -654,7 +654,7 @@ struct VoxelAcc {
 };
 
 template <bool PRECISE, bool FWD>
-__device__ __forceinline__ void poly_block(const RowConst& rc, const Smem& sm, int b, VoxelAcc& v) {
+__device__ __forceinline__ bool poly_block(const RowConst& rc, const Smem& sm, int b, VoxelAcc& v) {
   const float nchan = (float)(b * kChanBlock + (FWD ? 0 : kChanBlock - 1));   // the anchor channel
   const float anchor_hi = nchan * rc.step;
   const u64 slope = pk1(FWD ? rc.m2step : -rc.m2step), ms2 = pk1(rc.mstep2);
@@ -679,7 +679,7 @@ __device__ __forceinline__ void poly_block(const RowConst& rc, const Smem& sm, i
   u64 any_g = g[0];
 #pragma unroll
   for (int j = 1; j < kPairs; ++j) any_g |= g[j];
-  if (!__any_sync(0xffffffffu, any_g != 0ull)) return;
+  if (!__any_sync(0xffffffffu, any_g != 0ull)) return false;
   // scalar coefficients: FFMA2 takes a broadcast FP32 operand, so no (C, C) pairs are needed
   const float4* C = reinterpret_cast<const float4*>((FWD ? sm.coef : sm.coefb) + b * (3 * kChanBlock));
 #pragma unroll
@@ -700,6 +700,7 @@ __device__ __forceinline__ void poly_block(const RowConst& rc, const Smem& sm, i
       if (m == 2) v.s2[j] = fma2(g[j], P, v.s2[j]);
     }
   }
+  return true;
 }
 
 // One channel summed directly: the Gaussian line of PAPER.md:199 by one ex2 per voxel.
@@ -754,8 +755,9 @@ __device__ __forceinline__ void strip_pixel(const StripMap& m, int pi, int& ey, 
 template <bool PRECISE>
 __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst& rc, const Smem& sm,
                                             int tx0, int ty0, int EW, int EH, int R, int tid,
-                                            int nthreads) {
+                                            int nthreads, unsigned long long* counters) {
   const StripMap smap = strip_map(EW, EH);
+  int n_poly = 0, n_direct = 0, n_items = 0;     // work counters of this warp (gbk_eval_batch_counted)
   const int npairs = smap.ppr * EH;
   const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
   constexpr int kPerItem = 32 * kPairs;
@@ -822,18 +824,22 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       // the mirrored anchor up to block b_b (every line centred at most A before its last channel)
       const int b_f = min(max(__float2int_ru((-A - dmin) * rc.inv_bstep), b_lo), b_hi + 1);
       const int b_b = max(min(__float2int_rd((A - span - dmax) * rc.inv_bstep), b_f - 1), b_lo - 1);
-      for (int b = b_lo; b <= b_b; ++b) poly_block<PRECISE, false>(rc, sm, b, v);
-      for (int b = b_b + 1; b < b_f; ++b)        // lines of this item on both sides of the block
+      for (int b = b_lo; b <= b_b; ++b) n_poly += poly_block<PRECISE, false>(rc, sm, b, v) ? 1 : 0;
+      for (int b = b_b + 1; b < b_f; ++b) {      // lines of this item on both sides of the block
 #pragma unroll
         for (int cc = 0; cc < kChanBlock; ++cc) direct_channel<PRECISE>(rc, sm.chan[b * kChanBlock + cc], v);
-      for (int b = b_f; b <= b_hi; ++b) poly_block<PRECISE, true>(rc, sm, b, v);
+        n_direct += kChanBlock;
+      }
+      for (int b = b_f; b <= b_hi; ++b) n_poly += poly_block<PRECISE, true>(rc, sm, b, v) ? 1 : 0;
     } else {
       const float inv_step = rc.inv_bstep * (float)kChanBlock;
       const int c_lo = min(max(__float2int_rd((-D - dmax) * inv_step), 0), dp.nvx);
       const int c_hi = max(min(__float2int_ru((D - dmin) * inv_step), dp.nvx) - 1, -1);
 #pragma unroll 4
       for (int c = c_lo; c <= c_hi; ++c) direct_channel<PRECISE>(rc, sm.chan[c], v);
+      n_direct += max(c_hi - c_lo + 1, 0);
     }
+    ++n_items;
 #pragma unroll
     for (int j = 0; j < kPairs; ++j)
       if (sidx[j] >= 0) {
@@ -846,15 +852,22 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
         *reinterpret_cast<float2*>(sm.maps + 2 * map_stride + sidx[j]) = o;
       }
   }
+  if (counters && lane == 0) {
+    atomicAdd(&counters[GBK_CNT_ITEMS], (unsigned long long)n_items);
+    atomicAdd(&counters[GBK_CNT_POLY_BLOCKS], (unsigned long long)n_poly);
+    atomicAdd(&counters[GBK_CNT_DIRECT_CHANNELS], (unsigned long long)n_direct);
+    if (PRECISE) atomicAdd(&counters[GBK_CNT_PRECISE_ITEMS], (unsigned long long)n_items);
+  }
 }
 
 // Out of line: precise rows are rare, and the FP64 path must not weigh on the register allocation of
 // the common one.
 __device__ __noinline__ void voxel_phase_precise(const DevProblem& dp, unsigned char* smem_raw, int tx0,
-                                                 int ty0, int EW, int EH, int R, int tid, int nthreads) {
+                                                 int ty0, int EW, int EH, int R, int tid, int nthreads,
+                                                 unsigned long long* counters) {
   const Smem sm = carve(dp, smem_raw);
   const RowConst rc = *sm.rc;
-  voxel_phase<true>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads);
+  voxel_phase<true>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, counters);
 }
 
 // ------------------------------------------------------------------------------ the kernel ---
@@ -933,9 +946,9 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     const int R = rc.r_p;
     const int EW = tw + 2 * R, EH = th + 2 * R;
     if (rc.precise)
-      voxel_phase_precise(dp, smem_raw, tx0, ty0, EW, EH, R, tid, nthreads);
+      voxel_phase_precise(dp, smem_raw, tx0, ty0, EW, EH, R, tid, nthreads, a.counters);
     else
-      voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads);
+      voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, a.counters);
     __syncthreads();
     // ------------------------------------------------------------------ a5 .. a9 ---------
     if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {

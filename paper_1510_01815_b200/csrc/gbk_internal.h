@@ -51,6 +51,7 @@ struct EvalArgs {
   float* resid;             // [K][2][ny][nx] or null
   float* partial;           // [K][ntiles] cross-tile scratch (ntiles > 1)
   unsigned* tile_count;     // [K] tiles of a row finished so far (self-resetting; ntiles > 1)
+  unsigned long long* counters;  // [GBK_N_COUNTERS] work counters (gbk_eval_batch_counted) or null
 };
 
 // Per-row constants (a1 of SURVEY.md section 8(a)), computed once per block.

@@ -21,9 +21,11 @@ GBK_RC_ARCTAN, GBK_RC_RAMP, GBK_RC_EPINAT = 0, 1, 2
 GBK_STRATEGY_CUBE, GBK_STRATEGY_VFIELD = 0, 1
 GBK_PSF_GAUSSIAN, GBK_PSF_IMAGE = 0, 1
 
-EXPORTS = (
-    "gbk_create_problem", "gbk_get_info", "gbk_eval_batch", "gbk_eval_batch_unfused",
-    "gbk_eval_batch_host", "gbk_destroy", "gbk_last_error", "gbk_probe_pipe",
+EXPORTS = (   # every symbol include/gbk.h declares (tests/test_abi_and_dist.py checks them all)
+    "gbk_create_problem", "gbk_get_info", "gbk_set_strategy", "gbk_reserve", "gbk_eval_batch",
+    "gbk_eval_batch_counted",
+    "gbk_eval_batch_unfused", "gbk_eval_vfield_batch", "gbk_eval_batch_host", "gbk_destroy",
+    "gbk_last_error", "gbk_probe_pipe", "gbk_fit_ng", "gbk_fit_lm", "gbk_fit_ns",
 )
 
 
@@ -91,6 +93,10 @@ def lib():
             f = getattr(L, name)
             f.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp]
             f.restype = C.c_int
+        L.gbk_eval_batch_counted.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp]
+        L.gbk_eval_batch_counted.restype = C.c_int
+        L.gbk_reserve.argtypes = [vp, C.c_int64, vp]
+        L.gbk_reserve.restype = C.c_int
         L.gbk_set_strategy.argtypes = [vp, C.c_int32]
         L.gbk_set_strategy.restype = C.c_int
         L.gbk_eval_vfield_batch.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp]
@@ -197,6 +203,20 @@ def gbk_eval_batch(handle, params, gal_index, K, chi2, m0=None, m1=None, m2=None
 def gbk_eval_batch_unfused(handle, params, gal_index, K, chi2, m0=None, m1=None, m2=None,
                            resid=None, stream=0):
     gbk_eval_batch(handle, params, gal_index, K, chi2, m0, m1, m2, resid, stream, unfused=True)
+
+
+GBK_CNT_ITEMS, GBK_CNT_POLY_BLOCKS, GBK_CNT_DIRECT_CHANNELS, GBK_CNT_PRECISE_ITEMS, GBK_N_COUNTERS = range(5)
+
+
+def gbk_eval_batch_counted(handle, params, gal_index, K, chi2, counters, stream=0):
+    """gbk_eval_batch (chi^2 only) adding the voxel loop's work counts to `counters` (device int64 [4])."""
+    _check(lib().gbk_eval_batch_counted(handle, _ptr(params), _ptr(gal_index), int(K), _ptr(chi2),
+                                        _ptr(counters), stream or None))
+
+
+def gbk_reserve(handle, K_max: int, stream=0):
+    """Sizes the scratch of `stream` for batches of up to K_max rows (required before a capture)."""
+    _check(lib().gbk_reserve(handle, int(K_max), stream or None))
 
 
 def gbk_set_strategy(handle, strategy: int):

@@ -56,6 +56,7 @@ def test_library_exports_every_declared_symbol(libgbk):
     for n in names:
         assert hasattr(raw, n), f"libgbk.so does not export {n}"
         assert hasattr(libgbk, n), f"the Python binding has no function named {n}"
+    assert sorted(libgbk.EXPORTS) == names          # the binding's list is the header's, nothing less
 
 
 def test_binding_struct_layout_follows_the_header(libgbk):

@@ -495,6 +495,49 @@ def test_eval_batch_in_a_cuda_graph(oracle, torch_cuda, gbk):
     pu.compare(ref, {"chi2": got_b[:16]}, rows_b[:16], False, "graph replay")
 
 
+def test_two_streams_overlap_on_one_problem_and_capture_needs_reserve(oracle, torch_cuda, gbk):
+    """Multi-tile launches of ONE problem on two streams at the same time: each stream has its own
+    cross-tile scratch, so the results are those of sequential launches (bit for bit).  Growing the
+    scratch during a stream capture is refused with GBK_ERR_ARG; after gbk_reserve the capture works."""
+    torch = torch_cuda
+    w, g, obs, true, rng = _tiny_case(oracle, nx=40, ny=36)
+    Ka, Kb = 700, 900
+    rows_a, rows_b = _rows_near(w, true, rng, Ka), _rows_near(w, true, rng, Kb)
+    with gbk.Problem(**pu.gbk_desc(w, obs, tile_w=8, tile_h=6)) as prob:        # 35 tiles per row
+        pa, pb = torch.from_numpy(rows_a).cuda(), torch.from_numpy(rows_b).cuda()
+        seq_a = prob.eval(pa)["chi2"].cpu().numpy()
+        seq_b = prob.eval(pb)["chi2"].cpu().numpy()
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        ca = torch.empty(Ka, dtype=torch.float32, device="cuda")
+        cb = torch.empty(Kb, dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        for rep in range(6):                          # several rounds in flight on both streams
+            gbk.gbk_eval_batch(prob.handle, pa, None, Ka, ca, stream=s1.cuda_stream)
+            gbk.gbk_eval_batch(prob.handle, pb, None, Kb, cb, stream=s2.cuda_stream)
+        torch.cuda.synchronize()
+        assert np.array_equal(ca.cpu().numpy(), seq_a) and np.array_equal(cb.cpu().numpy(), seq_b)
+        # capture on a fresh stream whose scratch has never been sized
+        s3 = torch.cuda.Stream()
+        graph = torch.cuda.CUDAGraph()
+        with pytest.raises(gbk.GbkError) as e:
+            with torch.cuda.graph(graph, stream=s3):
+                gbk.gbk_eval_batch(prob.handle, pa, None, Ka, ca, stream=s3.cuda_stream)
+        assert e.value.code == gbk.GBK_ERR_ARG and "gbk_reserve" in str(e.value)
+        torch.cuda.synchronize()
+        s4 = torch.cuda.Stream()
+        gbk.gbk_reserve(prob.handle, Ka, s4.cuda_stream)
+        s4.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s4):
+            gbk.gbk_eval_batch(prob.handle, pa, None, Ka, ca, stream=s4.cuda_stream)
+        ca.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(ca.cpu().numpy(), seq_a)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows_a[:8])
+    pu.compare(ref, {"chi2": seq_a[:8]}, rows_a[:8], False, "two streams")
+
+
 # seeds 431 and 589: lines centred outside a short band (far-wing spaxels, m0 ~ 1e-15 I) once lost their
 # relative accuracy to the clamped block polynomial; seed 2313: a spaxel that sees only the far wing
 # (m0 ~ 1e-24 I) was 1.36e-4 off in m0 while the line offset was carried in FP32 (DESIGN.md section 6)
