@@ -251,6 +251,8 @@ typedef struct {
   int32_t iterations;  /* NG: levels; LM: largest iteration count over the fits; NS: batches  */
   int32_t converged;   /* fits that met their stopping rule                                   */
   float ms_total;      /* wall clock of the call, ms                                          */
+  int32_t failed;      /* LM: fits that could not iterate (start row out of domain, a finite-   */
+                       /* difference row out of domain, singular or non-finite normal equations) */
 } gbk_fit_stats;
 
 /*
@@ -269,15 +271,23 @@ int gbk_fit_ng(gbk_problem *p, const float *base_row, int32_t gal, int32_t n_axe
 
 /*
  * Levenberg-Marquardt for n_fits independent fits at once (config 5: one fit
- * per galaxy; config 2: n_fits = 1).  Per iteration ONE batch of n_active*(n_free+1) rows (base +
- * forward differences of rel_step x box width, backward at the upper bound) with weighted
- * residuals, J^T J and J^T r reduced on the device, the damped normal equations
- * solved on the host, and ONE batch of n_active*4 trial rows (four damping factors) for chi^2.
- * Parameters are clipped to [lo, hi].  A fit stops when the relative chi^2 decrease of an accepted
- * step is < ftol, when no damping factor up to 1e10 lowers chi^2, or after max_iter iterations.
+ * per galaxy; config 2: n_fits = 1), device-resident: the state of every fit stays in
+ * device memory and the host reads back one integer (fits still active) every four iterations.  Per
+ * iteration ONE batch of n_listed*(n_free+1) rows (base + forward differences of rel_step x box
+ * width, backward at the upper bound, doubled until the step is representable) with weighted
+ * residuals, J^T J and J^T r reduced in FP64, the damped normal equations
+ * (A + lambda diag A) x = -g solved by Cholesky for four damping factors lambda x {0.1, 1, 10, 100},
+ * and ONE batch of n_listed*4 trial rows for chi^2.  The best trial that lowers chi^2 is accepted
+ * (lambda <- max(1e-9, 0.3 x its factor x lambda)), else lambda <- 1e4 lambda.  Parameters are
+ * clipped to [lo, hi].  A fit stops when the relative chi^2 decrease of an accepted step is < ftol
+ * (converged), when no damping factor up to 1e10 lowers chi^2 (converged: stationary as far as LM can
+ * tell), after max_iter iterations, or as FAILED when it cannot iterate: the start row or a
+ * difference row is out of domain (chi^2 = +INF), or the normal equations are singular or not finite
+ * for every damping factor.  Failed fits are counted in stats->failed, never in stats->converged.
  *   start_rows [n_fits][GBK_P], gal [n_fits] or NULL (all 0), free_param/lo/hi [n_free]
  *   fit_rows [n_fits][GBK_P], fit_chi2 [n_fits], fit_iters [n_fits] or NULL
  * A fit whose start row has chi^2 = +INF is returned unchanged with chi^2 = +INF.
+ * stats->evals counts the rows evaluated for fits that were active.
  */
 int gbk_fit_lm(gbk_problem *p, int32_t n_fits, const float *start_rows, const int32_t *gal,
                int32_t n_free, const int32_t *free_param, const float *lo, const float *hi,

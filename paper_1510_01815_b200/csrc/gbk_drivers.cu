@@ -9,6 +9,8 @@
 
 #include <algorithm>
 #include <chrono>
+#include <mutex>
+#include <new>
 #include <vector>
 
 #include "gbk_internal.h"
@@ -29,22 +31,71 @@ namespace {
     if (int rc_ = (expr)) return rc_; \
   } while (0)
 
-// Device / pinned-host buffer pair that frees itself (the drivers allocate per call, off the hot path).
+// Workspace of the drivers: ONE device block and ONE pinned host block per device, kept across calls
+// (cudaMallocHost alone costs ~0.1 ms per buffer, more than a small fit) and carved into typed
+// buffers by Buf::alloc.  The drivers block until their fit is done and hold the lock meanwhile.
+struct Workspace {
+  int device = -1;
+  char* d = nullptr;
+  char* h = nullptr;
+  size_t d_cap = 0, h_cap = 0, d_used = 0, h_used = 0;
+};
+std::mutex g_ws_mu;
+std::vector<Workspace*> g_ws;
+
+Workspace* workspace_for(int device) {
+  for (Workspace* w : g_ws)
+    if (w->device == device) return w;
+  Workspace* w = new (std::nothrow) Workspace;
+  if (w) w->device = device, g_ws.push_back(w);
+  return w;
+}
+
+// Sizes are requested first (plan = true: only adds up), then the blocks are grown if needed, then
+// the same sequence of alloc calls hands out the pointers.
+struct Arena {
+  Workspace* ws;
+  bool plan = true;
+  size_t d_need = 0, h_need = 0;
+  explicit Arena(Workspace* w) : ws(w) {}
+  static size_t up(size_t n) { return (n + 255) & ~size_t(255); }
+  cudaError_t commit() {
+    cudaError_t e = cudaSuccess;
+    if (d_need > ws->d_cap) {
+      cudaFree(ws->d);
+      ws->d = nullptr, ws->d_cap = 0;
+      e = cudaMalloc(&ws->d, d_need);
+      if (e != cudaSuccess) return e;
+      ws->d_cap = d_need;
+    }
+    if (h_need > ws->h_cap) {
+      cudaFreeHost(ws->h);
+      ws->h = nullptr, ws->h_cap = 0;
+      e = cudaMallocHost(&ws->h, h_need);
+      if (e != cudaSuccess) return e;
+      ws->h_cap = h_need;
+    }
+    ws->d_used = ws->h_used = 0;
+    plan = false;
+    return e;
+  }
+};
+
 template <typename T>
 struct Buf {
   T* d = nullptr;
   T* h = nullptr;
   size_t n = 0;
-  ~Buf() {
-    cudaFree(d);
-    cudaFreeHost(h);
-  }
-  cudaError_t alloc(size_t count, bool host = true, bool dev = true) {
+  void alloc(Arena& ar, size_t count, bool host = true, bool dev = true) {
     n = count;
-    cudaError_t e = cudaSuccess;
-    if (dev) e = cudaMalloc(&d, sizeof(T) * std::max<size_t>(count, 1));
-    if (e == cudaSuccess && host) e = cudaMallocHost(&h, sizeof(T) * std::max<size_t>(count, 1));
-    return e;
+    const size_t bytes = Arena::up(sizeof(T) * std::max<size_t>(count, 1));
+    if (ar.plan) {
+      if (dev) ar.d_need += bytes;
+      if (host) ar.h_need += bytes;
+      return;
+    }
+    if (dev) d = reinterpret_cast<T*>(ar.ws->d + ar.ws->d_used), ar.ws->d_used += bytes;
+    if (host) h = reinterpret_cast<T*>(ar.ws->h + ar.ws->h_used), ar.ws->h_used += bytes;
   }
   cudaError_t to_device(size_t count, cudaStream_t st) {
     return cudaMemcpyAsync(d, h, sizeof(T) * count, cudaMemcpyHostToDevice, st);
@@ -163,14 +214,21 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
   DeviceGuard guard(info.device);
   DRV_CUDA(guard.status);
 
+  std::lock_guard<std::mutex> ws_lock(g_ws_mu);
+  Workspace* ws = workspace_for(info.device);
+  if (!ws) return fail(GBK_ERR_ALLOC, "out of host memory");
+  Arena ar(ws);
   Buf<float> rows, chi2, best_v;
   Buf<int> best_i, gal_idx;
-  DRV_CUDA(rows.alloc((size_t)n_rows * GBK_P, false));
-  DRV_CUDA(chi2.alloc(n_rows, false));
-  DRV_CUDA(best_v.alloc(1));
-  DRV_CUDA(best_i.alloc(1));
+  for (int pass = 0; pass < 2; ++pass) {
+    rows.alloc(ar, (size_t)n_rows * GBK_P, false);
+    chi2.alloc(ar, n_rows, false);
+    best_v.alloc(ar, 1);
+    best_i.alloc(ar, 1);
+    if (gal != 0) gal_idx.alloc(ar, n_rows);
+    if (pass == 0) DRV_CUDA(ar.commit());
+  }
   if (gal != 0) {
-    DRV_CUDA(gal_idx.alloc(n_rows));
     std::fill(gal_idx.h, gal_idx.h + n_rows, gal);
     DRV_CUDA(gal_idx.to_device(n_rows, st));
   }
@@ -226,15 +284,80 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
 }
 
 // ------------------------------------------------------------------ Levenberg-Marquardt ----
+// Device-resident (PAPER.md:758 names a GPU-only LM as future work):
+// the state of every fit (row, chi^2, damping factor, status) lives in device memory, and one
+// iteration is six launches on the caller's stream with no host round trip between them --
+//   lm_jacobian_rows   base + n one-sided difference rows per listed fit
+//   gbk_eval_batch     their chi^2 and weighted residuals
+//   lm_normal_kernel   J^T J, J^T r in FP64
+//   lm_trial_rows      the damped 7x7 Cholesky solves (four damping factors per fit), trial rows
+//   gbk_eval_batch     chi^2 of the trial rows
+//   lm_update          accept / reject, damping update, stopping rules, count of fits still active
+// The host reads back ONE integer (fits still active) every kLmReadback iterations, and compacts the
+// list of fits when it has shrunk; fits that stop in between cost an out-of-domain row per slot (a
+// thread block that exits at once).
 namespace {
 
-// One block per (term, fit).  Terms: n(n+1)/2 entries of J^T J (upper triangle, row-major),
-// n entries of J^T r, and r.r; J_a = (r_a - r_0) / h_a from the forward-difference rows.
-// resid: [n_fits][n+1][M]; h: [n_fits][n]; out: [n_fits][n_terms] (double).
-__global__ void lm_normal_kernel(const float* __restrict__ resid, const float* __restrict__ h, int n,
-                                 int M, double* __restrict__ out) {
+enum { LM_ACTIVE = 0, LM_CONVERGED = 1, LM_STALLED = 2, LM_FAILED = 3, LM_MAXITER = 4, LM_BAD_START = 5 };
+constexpr int kLmTrials = 4;
+constexpr int kLmReadback = 4;
+__constant__ double kLmFactor[kLmTrials] = {0.1, 1.0, 10.0, 100.0};
+
+struct LmSetup {
+  int n, M, n_terms, max_iter;
+  int free_param[GBK_P];
+  float lo[GBK_P], hi[GBK_P];
+  float rel_step, ftol;
+};
+
+struct LmState {         // device arrays, one entry per fit
+  float* row;            // [n_fits][GBK_P]
+  double* chi2;          // chi^2 of `row` (+inf until evaluated)
+  double* lambda;
+  int* iters;
+  int* status;
+  int* gal;
+  float* hstep;          // [n_fits][n] finite-difference steps actually taken (FP32)
+  unsigned long long* evals;   // [1] rows evaluated for fits that were active
+};
+
+// One thread per (slot, r): row r of the slot's Jacobian batch.  r = 0 is the base row.
+__global__ void lm_jacobian_rows(const __grid_constant__ LmSetup su, const LmState stt, const int* __restrict__ list,
+                                 int n_list, float* __restrict__ rows, int* __restrict__ gidx) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int slot = t / (su.n + 1), r = t - slot * (su.n + 1);
+  if (slot >= n_list) return;
+  const int f = list[slot];
+  float row[GBK_P];
+#pragma unroll
+  for (int j = 0; j < GBK_P; ++j) row[j] = stt.row[(size_t)f * GBK_P + j];
+  gidx[t] = stt.gal[f];
+  if (stt.status[f] != LM_ACTIVE) {
+    row[0] = __int_as_float(0x7fc00000);          // finished: an out-of-domain row costs next to nothing
+  } else if (r > 0) {
+    const int a = r - 1, j = su.free_param[a];
+    float h = su.rel_step * (su.hi[a] - su.lo[a]);
+    float moved = row[j] + h;
+    for (int k = 0; k < 30 && moved == row[j]; ++k) h *= 2.0f, moved = row[j] + h;   // a step below one ulp
+    if (moved > su.hi[a]) h = -h, moved = row[j] + h;                                  // backward at the wall
+    stt.hstep[(size_t)f * su.n + a] = moved - row[j];   // the step actually taken in FP32 (0: see lm_trial_rows)
+    row[j] = moved;
+  } else {
+    atomicAdd(stt.evals, (unsigned long long)(su.n + 1));
+  }
+#pragma unroll
+  for (int j = 0; j < GBK_P; ++j) rows[(size_t)t * GBK_P + j] = row[j];
+}
+
+// One block per (term, slot).  Terms: n(n+1)/2 entries of J^T J (upper triangle, row-major),
+// n entries of J^T r, and r.r; J_a = (r_a - r_0) / h_a from the one-sided difference rows.
+// resid: [n_list][n+1][M]; out: [n_list][n_terms] (double).
+__global__ void lm_normal_kernel(const float* __restrict__ resid, const LmState stt, const int* __restrict__ list,
+                                 int n, int M, double* __restrict__ out) {
   const int n_tri = n * (n + 1) / 2, n_terms = n_tri + n + 1;
-  const int term = blockIdx.x, fit = blockIdx.y;
+  const int term = blockIdx.x, slot = blockIdx.y;
+  const int f = list[slot];
+  if (stt.status[f] != LM_ACTIVE) return;
   int a = -1, b = -1;   // a = b = -1: r.r;  b = -1: (J^T r)_a
   if (term < n_tri) {
     int t = term;
@@ -244,7 +367,7 @@ __global__ void lm_normal_kernel(const float* __restrict__ resid, const float* _
   } else if (term < n_tri + n) {
     a = term - n_tri;
   }
-  const float* r0 = resid + (size_t)fit * (n + 1) * M;
+  const float* r0 = resid + (size_t)slot * (n + 1) * M;
   const float* ra = a >= 0 ? r0 + (size_t)(a + 1) * M : r0;
   const float* rb = b >= 0 ? r0 + (size_t)(b + 1) * M : r0;
   double acc = 0.0;
@@ -263,14 +386,14 @@ __global__ void lm_normal_kernel(const float* __restrict__ resid, const float* _
   }
   if (threadIdx.x == 0) {
     double v = red[0];
-    if (a >= 0) v /= (double)h[(size_t)fit * n + a];
-    if (b >= 0) v /= (double)h[(size_t)fit * n + b];
-    out[(size_t)fit * n_terms + term] = v;
+    if (a >= 0) v /= (double)stt.hstep[(size_t)f * n + a];
+    if (b >= 0) v /= (double)stt.hstep[(size_t)f * n + b];
+    out[(size_t)slot * n_terms + term] = v;
   }
 }
 
 // Solves (A + lambda diag(A)) x = -g by Cholesky (A symmetric, upper triangle packed row-major).
-bool solve_damped(int n, const double* tri, const double* g, double lambda, double* x) {
+__device__ bool solve_damped(int n, const double* tri, const double* g, double lambda, double* x) {
   double L[GBK_P][GBK_P];
   int t = 0;
   for (int a = 0; a < n; ++a)
@@ -305,15 +428,112 @@ bool solve_damped(int n, const double* tri, const double* g, double lambda, doub
   return true;
 }
 
-constexpr int kLmTrials = 4;
-const double kLmFactor[kLmTrials] = {0.1, 1.0, 10.0, 100.0};
-
-struct LmFit {
+// One thread per (slot, trial): books the base chi^2 of the Jacobian batch, applies the stopping
+// rules that need no trial (bad start, iteration limit, unusable Jacobian), and writes the trial row
+// of damping factor lambda x kLmFactor[trial].  jac_chi2: [n_list][n+1]; normal: [n_list][n_terms].
+__global__ void lm_trial_rows(const __grid_constant__ LmSetup su, const LmState stt, const int* __restrict__ list,
+                              int n_list, const float* __restrict__ jac_chi2, const double* __restrict__ normal,
+                              float* __restrict__ rows, int* __restrict__ gidx) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int slot = t / kLmTrials, trial = t - slot * kLmTrials;
+  if (slot >= n_list) return;
+  const int f = list[slot], n = su.n;
   float row[GBK_P];
-  double chi2 = INFINITY, lambda = 1e-3;
-  int iters = 0, gal = 0;
-  bool active = true, converged = false;
-};
+#pragma unroll
+  for (int j = 0; j < GBK_P; ++j) row[j] = stt.row[(size_t)f * GBK_P + j];
+  gidx[t] = stt.gal[f];
+  int status = stt.status[f];
+  if (status == LM_ACTIVE) {
+    const float* c = jac_chi2 + (size_t)slot * (n + 1);
+    const double base = c[0];
+    bool jac_ok = true;           // every difference row in domain and every step non-zero
+    for (int a = 0; a < n; ++a) jac_ok = jac_ok && isfinite(c[a + 1]) && stt.hstep[(size_t)f * n + a] != 0.0f;
+    if (!isfinite(base)) status = stt.iters[f] == 0 ? LM_BAD_START : LM_FAILED;
+    else if (stt.iters[f] >= su.max_iter) status = LM_MAXITER;
+    else if (!jac_ok) status = LM_FAILED;
+    const double* nm = normal + (size_t)slot * su.n_terms;
+    double dx[GBK_P];
+    bool solved = false;
+    if (status == LM_ACTIVE) {
+      solved = solve_damped(n, nm, nm + n * (n + 1) / 2, stt.lambda[f] * kLmFactor[trial], dx);
+      if (solved)
+        for (int a = 0; a < n; ++a) {
+          const int j = su.free_param[a];
+          row[j] = (float)fmin((double)su.hi[a], fmax((double)su.lo[a], (double)row[j] + dx[a]));
+        }
+    }
+    if (trial == 0) {             // one thread per slot writes the state
+      if (isfinite(base) || stt.iters[f] == 0) stt.chi2[f] = base;
+      if (status == LM_ACTIVE) atomicAdd(stt.evals, (unsigned long long)kLmTrials);
+      else stt.status[f] = status;
+    }
+    if (status == LM_ACTIVE && !solved) row[0] = __int_as_float(0x7fc00000);   // this factor gives no step
+  }
+  if (status != LM_ACTIVE) row[0] = __int_as_float(0x7fc00000);
+#pragma unroll
+  for (int j = 0; j < GBK_P; ++j) rows[(size_t)t * GBK_P + j] = row[j];
+}
+
+// One thread per slot: best of the four trials, accept / reject, damping update, stopping rules.
+__global__ void lm_update(const __grid_constant__ LmSetup su, const LmState stt, const int* __restrict__ list,
+                          int n_list, const float* __restrict__ trial_rows, const float* __restrict__ trial_chi2,
+                          int* __restrict__ n_active) {
+  const int slot = blockIdx.x * blockDim.x + threadIdx.x;
+  if (slot >= n_list) return;
+  const int f = list[slot];
+  if (stt.status[f] != LM_ACTIVE) return;
+  int best = -1, n_finite = 0;
+  double best_chi = stt.chi2[f];
+  for (int t = 0; t < kLmTrials; ++t) {
+    const double c = trial_chi2[(size_t)slot * kLmTrials + t];
+    n_finite += isfinite(c) ? 1 : 0;
+    if (c < best_chi) best_chi = c, best = t;
+  }
+  stt.iters[f] += 1;
+  int status = LM_ACTIVE;
+  if (best >= 0) {
+    const double rel = (stt.chi2[f] - best_chi) / stt.chi2[f];
+    for (int j = 0; j < GBK_P; ++j)
+      stt.row[(size_t)f * GBK_P + j] = trial_rows[((size_t)slot * kLmTrials + best) * GBK_P + j];
+    stt.lambda[f] = fmax(1e-9, stt.lambda[f] * kLmFactor[best] * 0.3);
+    stt.chi2[f] = best_chi;
+    if (rel < (double)su.ftol) status = LM_CONVERGED;
+  } else {
+    stt.lambda[f] *= 1e4;
+    // no downhill step up to the largest damping: a stationary point of chi^2 as far as LM can tell --
+    // unless no trial was ever evaluated (singular or non-finite normal equations): that is a failure
+    if (stt.lambda[f] > 1e10) status = n_finite > 0 ? LM_STALLED : LM_FAILED;
+  }
+  if (status != LM_ACTIVE) stt.status[f] = status;
+  else atomicAdd(n_active, 1);
+}
+
+// Stable compaction of the list of fits to those still active (one block; lists are short).
+__global__ void lm_compact(const LmState stt, const int* __restrict__ list, int n_list, int* __restrict__ out) {
+  __shared__ int base;
+  __shared__ int warp_tot[32];
+  if (threadIdx.x == 0) base = 0;
+  __syncthreads();
+  for (int i0 = 0; i0 < n_list; i0 += blockDim.x) {
+    const int i = i0 + threadIdx.x;
+    const int f = i < n_list ? list[i] : -1;
+    const bool keep = f >= 0 && stt.status[f] == LM_ACTIVE;
+    const unsigned m = __ballot_sync(0xffffffffu, keep);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) warp_tot[w] = __popc(m);
+    __syncthreads();
+    int off = base;
+    for (int k = 0; k < w; ++k) off += warp_tot[k];
+    if (keep) out[off + __popc(m & ((1u << lane) - 1u))] = f;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int tot = 0;
+      for (int k = 0; k < (int)(blockDim.x >> 5); ++k) tot += warp_tot[k];
+      base += tot;
+    }
+    __syncthreads();
+  }
+}
 
 }  // namespace
 
@@ -341,132 +561,117 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(info.device);
   DRV_CUDA(guard.status);
-  const int n = n_free, M = (info.strategy == GBK_STRATEGY_VFIELD ? 1 : 2) * info.nx * info.ny;
-  const int n_tri = n * (n + 1) / 2, n_terms = n_tri + n + 1;
+  LmSetup su{};
+  su.n = n_free, su.M = (info.strategy == GBK_STRATEGY_VFIELD ? 1 : 2) * info.nx * info.ny;
+  su.n_terms = su.n * (su.n + 1) / 2 + su.n + 1, su.max_iter = max_iter;
+  su.rel_step = rel_step, su.ftol = ftol;
+  for (int a = 0; a < su.n; ++a) su.free_param[a] = free_param[a], su.lo[a] = lo[a], su.hi[a] = hi[a];
+  const int n = su.n;
   // fits per chunk: the residual buffer of a chunk stays below 1 GiB
-  const size_t resid_per_fit = sizeof(float) * (size_t)(n + 1) * M;
+  const size_t resid_per_fit = sizeof(float) * (size_t)(n + 1) * su.M;
   const int chunk = (int)std::max<size_t>(1, std::min<size_t>(n_fits, (size_t(1) << 30) / resid_per_fit));
   const int rows_per_fit = std::max(n + 1, kLmTrials);
-  Buf<float> rows, chi2, resid, hstep;
-  Buf<int> gidx;
-  Buf<double> normal;
-  DRV_CUDA(rows.alloc((size_t)chunk * rows_per_fit * GBK_P));
-  DRV_CUDA(chi2.alloc((size_t)chunk * rows_per_fit));
-  DRV_CUDA(gidx.alloc((size_t)chunk * rows_per_fit));
-  DRV_CUDA(resid.alloc((size_t)chunk * (n + 1) * M, false));
-  DRV_CUDA(hstep.alloc((size_t)chunk * n));
-  DRV_CUDA(normal.alloc((size_t)chunk * n_terms));
-
-  std::vector<LmFit> fits(n_fits);
-  for (int f = 0; f < n_fits; ++f) {
-    memcpy(fits[f].row, start_rows + (size_t)f * GBK_P, sizeof(float) * GBK_P);
-    fits[f].gal = gal ? gal[f] : 0;
-    for (int a = 0; a < n; ++a)   // start inside the box
-      fits[f].row[free_param[a]] = std::min(hi[a], std::max(lo[a], fits[f].row[free_param[a]]));
-    if (!finite_row(fits[f].row)) fits[f].active = false;
+  std::lock_guard<std::mutex> ws_lock(g_ws_mu);
+  Workspace* ws = workspace_for(info.device);
+  if (!ws) return fail(GBK_ERR_ALLOC, "out of host memory");
+  Arena ar(ws);
+  Buf<float> rows, chi2, resid, state_row, hstep;
+  Buf<int> gidx, list_a, list_b, iters, status, galb, n_active;
+  Buf<double> normal, state_chi2, lambda;
+  Buf<unsigned long long> evals;
+  for (int pass = 0; pass < 2; ++pass) {
+    rows.alloc(ar, (size_t)chunk * rows_per_fit * GBK_P, false);
+    chi2.alloc(ar, (size_t)chunk * rows_per_fit, false);
+    gidx.alloc(ar, (size_t)chunk * rows_per_fit, false);
+    resid.alloc(ar, (size_t)chunk * (n + 1) * su.M, false);
+    normal.alloc(ar, (size_t)chunk * su.n_terms, false);
+    hstep.alloc(ar, (size_t)n_fits * n, false);
+    state_row.alloc(ar, (size_t)n_fits * GBK_P);
+    state_chi2.alloc(ar, n_fits);
+    lambda.alloc(ar, n_fits);
+    iters.alloc(ar, n_fits);
+    status.alloc(ar, n_fits);
+    galb.alloc(ar, n_fits);
+    list_a.alloc(ar, chunk);
+    list_b.alloc(ar, chunk, false);
+    n_active.alloc(ar, kLmReadback + 1);
+    evals.alloc(ar, 1);
+    if (pass == 0) DRV_CUDA(ar.commit());
   }
+  for (int f = 0; f < n_fits; ++f) {
+    float* row = state_row.h + (size_t)f * GBK_P;
+    memcpy(row, start_rows + (size_t)f * GBK_P, sizeof(float) * GBK_P);
+    for (int a = 0; a < n; ++a)   // start inside the box
+      row[free_param[a]] = std::min(hi[a], std::max(lo[a], row[free_param[a]]));
+    state_chi2.h[f] = INFINITY, lambda.h[f] = 1e-3, iters.h[f] = 0;
+    status.h[f] = finite_row(row) ? LM_ACTIVE : LM_BAD_START;
+    galb.h[f] = gal ? gal[f] : 0;
+  }
+  evals.h[0] = 0;
+  DRV_CUDA(state_row.to_device((size_t)n_fits * GBK_P, st));
+  DRV_CUDA(state_chi2.to_device(n_fits, st));
+  DRV_CUDA(lambda.to_device(n_fits, st));
+  DRV_CUDA(iters.to_device(n_fits, st));
+  DRV_CUDA(status.to_device(n_fits, st));
+  DRV_CUDA(galb.to_device(n_fits, st));
+  DRV_CUDA(evals.to_device(1, st));
+  DRV_TRY(gbk_reserve(p, (int64_t)chunk * rows_per_fit, cuda_stream));
+  const LmState stt{state_row.d, state_chi2.d, lambda.d, iters.d, status.d, galb.d, hstep.d, evals.d};
 
   for (int c0 = 0; c0 < n_fits; c0 += chunk) {
     const int c1 = std::min(n_fits, c0 + chunk);
-    for (int iter = 0;; ++iter) {
-      std::vector<int> act;
-      for (int f = c0; f < c1; ++f)
-        if (fits[f].active) act.push_back(f);
-      if (act.empty()) break;
-      const int na = (int)act.size();
-      // ---- Jacobian batch: base + n one-sided differences per active fit ----
-      for (int i = 0; i < na; ++i) {
-        const LmFit& ft = fits[act[i]];
-        for (int r = 0; r <= n; ++r) {
-          float* row = rows.h + ((size_t)i * (n + 1) + r) * GBK_P;
-          memcpy(row, ft.row, sizeof(float) * GBK_P);
-          gidx.h[(size_t)i * (n + 1) + r] = ft.gal;
-          if (r > 0) {
-            const int a = r - 1, j = free_param[a];
-            float h = rel_step * (hi[a] - lo[a]);
-            if (row[j] + h > hi[a]) h = -h;
-            const float moved = row[j] + h;
-            hstep.h[(size_t)i * n + a] = moved - row[j];   // the step actually taken in FP32
-            row[j] = moved;
-          }
-        }
+    int n_list = 0;
+    for (int f = c0; f < c1; ++f)
+      if (status.h[f] == LM_ACTIVE) list_a.h[n_list++] = f;
+    if (n_list == 0) continue;
+    DRV_CUDA(list_a.to_device(n_list, st));
+    int* list = list_a.d;
+    int* spare = list_b.d;
+    // every fit stops after at most max_iter + 1 iterations (the last one only books chi^2)
+    for (int it = 0; n_list > 0 && it <= max_iter + kLmReadback; it += kLmReadback) {
+      DRV_CUDA(cudaMemsetAsync(n_active.d, 0, sizeof(int) * (kLmReadback + 1), st));
+      for (int sub = 0; sub < kLmReadback; ++sub) {
+        const int kj = n_list * (n + 1), kt = n_list * kLmTrials;
+        lm_jacobian_rows<<<(kj + 127) / 128, 128, 0, st>>>(su, stt, list, n_list, rows.d, gidx.d);
+        DRV_CUDA(cudaGetLastError());
+        DRV_TRY(eval_rows(p, info, rows.d, gidx.d, kj, chi2.d, resid.d, cuda_stream));
+        lm_normal_kernel<<<dim3(su.n_terms, n_list), 256, 0, st>>>(resid.d, stt, list, n, su.M, normal.d);
+        DRV_CUDA(cudaGetLastError());
+        lm_trial_rows<<<(kt + 127) / 128, 128, 0, st>>>(su, stt, list, n_list, chi2.d, normal.d, rows.d, gidx.d);
+        DRV_CUDA(cudaGetLastError());
+        // the Jacobian chi^2 are consumed by lm_trial_rows before this launch overwrites them (stream order)
+        DRV_TRY(eval_rows(p, info, rows.d, gidx.d, kt, chi2.d, nullptr, cuda_stream));
+        lm_update<<<(n_list + 127) / 128, 128, 0, st>>>(su, stt, list, n_list, rows.d, chi2.d, n_active.d + sub);
+        DRV_CUDA(cudaGetLastError());
+        fs.launches += 2;
       }
-      const int kj = na * (n + 1);
-      DRV_CUDA(rows.to_device((size_t)kj * GBK_P, st));
-      DRV_CUDA(gidx.to_device(kj, st));
-      DRV_CUDA(hstep.to_device((size_t)na * n, st));
-      DRV_TRY(eval_rows(p, info, rows.d, gidx.d, kj, chi2.d, resid.d, cuda_stream));
-      lm_normal_kernel<<<dim3(n_terms, na), 256, 0, st>>>(resid.d, hstep.d, n, M, normal.d);
-      DRV_CUDA(cudaGetLastError());
-      DRV_CUDA(normal.to_host((size_t)na * n_terms, st));
-      DRV_CUDA(chi2.to_host(kj, st));
+      DRV_CUDA(n_active.to_host(kLmReadback, st));
       DRV_CUDA(cudaStreamSynchronize(st));
-      fs.evals += kj, fs.launches += 1;
-      // ---- trial rows: four damping factors per fit ----
-      std::vector<int> live;   // indices into act with a usable base row
-      for (int i = 0; i < na; ++i) {
-        LmFit& ft = fits[act[i]];
-        ft.chi2 = chi2.h[(size_t)i * (n + 1)];
-        if (!isfinite(ft.chi2) || iter >= max_iter) {
-          ft.active = false;
-          continue;
-        }
-        live.push_back(i);
-      }
-      const int nl = (int)live.size();
-      if (nl == 0) continue;
-      for (int q = 0; q < nl; ++q) {
-        const int i = live[q];
-        const LmFit& ft = fits[act[i]];
-        const double* nm = normal.h + (size_t)i * n_terms;
-        for (int t = 0; t < kLmTrials; ++t) {
-          float* row = rows.h + ((size_t)q * kLmTrials + t) * GBK_P;
-          memcpy(row, ft.row, sizeof(float) * GBK_P);
-          gidx.h[(size_t)q * kLmTrials + t] = ft.gal;
-          double dx[GBK_P];
-          if (solve_damped(n, nm, nm + n_tri, ft.lambda * kLmFactor[t], dx))
-            for (int a = 0; a < n; ++a) {
-              const int j = free_param[a];
-              row[j] = (float)std::min<double>(hi[a], std::max<double>(lo[a], (double)row[j] + dx[a]));
-            }
-        }
-      }
-      const int kt = nl * kLmTrials;
-      DRV_CUDA(rows.to_device((size_t)kt * GBK_P, st));
-      DRV_CUDA(gidx.to_device(kt, st));
-      DRV_TRY(eval_rows(p, info, rows.d, gidx.d, kt, chi2.d, nullptr, cuda_stream));
-      DRV_CUDA(chi2.to_host(kt, st));
-      DRV_CUDA(cudaStreamSynchronize(st));
-      fs.evals += kt, fs.launches += 1;
-      for (int q = 0; q < nl; ++q) {
-        LmFit& ft = fits[act[live[q]]];
-        int best = -1;
-        double best_chi = ft.chi2;
-        for (int t = 0; t < kLmTrials; ++t) {
-          const double c = chi2.h[(size_t)q * kLmTrials + t];
-          if (c < best_chi) best_chi = c, best = t;
-        }
-        ft.iters += 1;
-        if (best >= 0) {
-          const double rel = (ft.chi2 - best_chi) / ft.chi2;
-          memcpy(ft.row, rows.h + ((size_t)q * kLmTrials + best) * GBK_P, sizeof(float) * GBK_P);
-          ft.lambda = std::max(1e-9, ft.lambda * kLmFactor[best] * 0.3);
-          ft.chi2 = best_chi;
-          if (rel < (double)ftol) ft.active = false, ft.converged = true;
-        } else {
-          ft.lambda *= 1e4;
-          if (ft.lambda > 1e10) ft.active = false, ft.converged = true;   // no downhill step left
-        }
+      const int left = n_active.h[kLmReadback - 1];
+      if (left == 0) break;
+      if (left < n_list - n_list / 4 || left <= 64) {     // the list has shrunk: drop the finished fits
+        lm_compact<<<1, 1024, 0, st>>>(stt, list, n_list, spare);
+        DRV_CUDA(cudaGetLastError());
+        std::swap(list, spare);
+        n_list = left;
       }
     }
   }
+  DRV_CUDA(state_row.to_host((size_t)n_fits * GBK_P, st));
+  DRV_CUDA(state_chi2.to_host(n_fits, st));
+  DRV_CUDA(iters.to_host(n_fits, st));
+  DRV_CUDA(status.to_host(n_fits, st));
+  DRV_CUDA(evals.to_host(1, st));
+  DRV_CUDA(cudaStreamSynchronize(st));
   for (int f = 0; f < n_fits; ++f) {
-    memcpy(fit_rows + (size_t)f * GBK_P, fits[f].row, sizeof(float) * GBK_P);
-    fit_chi2[f] = (float)fits[f].chi2;
-    if (fit_iters) fit_iters[f] = fits[f].iters;
-    fs.iterations = std::max(fs.iterations, fits[f].iters);
-    fs.converged += fits[f].converged ? 1 : 0;
+    memcpy(fit_rows + (size_t)f * GBK_P, state_row.h + (size_t)f * GBK_P, sizeof(float) * GBK_P);
+    fit_chi2[f] = (float)state_chi2.h[f];
+    if (fit_iters) fit_iters[f] = iters.h[f];
+    fs.iterations = std::max(fs.iterations, iters.h[f]);
+    fs.converged += (status.h[f] == LM_CONVERGED || status.h[f] == LM_STALLED) ? 1 : 0;
+    fs.failed += (status.h[f] == LM_FAILED || status.h[f] == LM_BAD_START) ? 1 : 0;
   }
+  fs.evals = (int64_t)evals.h[0];
   fs.ms_total = clock.ms();
   if (stats) *stats = fs;
   return GBK_OK;
@@ -522,11 +727,18 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
   DeviceGuard guard(info.device);
   DRV_CUDA(guard.status);
   const int n = n_free, cap = std::max(n_live, batch);
+  std::lock_guard<std::mutex> ws_lock(g_ws_mu);
+  Workspace* ws = workspace_for(info.device);
+  if (!ws) return fail(GBK_ERR_ALLOC, "out of host memory");
+  Arena ar(ws);
   Buf<float> rows, chi2;
   Buf<int> gidx;
-  DRV_CUDA(rows.alloc((size_t)cap * GBK_P));
-  DRV_CUDA(chi2.alloc(cap));
-  DRV_CUDA(gidx.alloc(cap));
+  for (int pass = 0; pass < 2; ++pass) {
+    rows.alloc(ar, (size_t)cap * GBK_P);
+    chi2.alloc(ar, cap);
+    gidx.alloc(ar, cap);
+    if (pass == 0) DRV_CUDA(ar.commit());
+  }
   std::fill(gidx.h, gidx.h + cap, gal);
   DRV_CUDA(gidx.to_device(cap, st));
   Xoshiro rng(seed);

@@ -68,7 +68,7 @@ class gbk_problem_info(C.Structure):
 class gbk_fit_stats(C.Structure):
     _fields_ = [
         ("evals", C.c_int64), ("launches", C.c_int32), ("iterations", C.c_int32),
-        ("converged", C.c_int32), ("ms_total", C.c_float),
+        ("converged", C.c_int32), ("ms_total", C.c_float), ("failed", C.c_int32),
     ]
 
 
@@ -336,6 +336,11 @@ class Problem:
 
     def __exit__(self, *exc):
         self.close()
+
+    def set_strategy(self, strategy: int):
+        """gbk_set_strategy, keeping `info` (which reports the strategy) up to date."""
+        gbk_set_strategy(self.handle, strategy)
+        self.info = gbk_get_info(self.handle)
 
     def eval_vfield(self, params, gal_index=None, want_maps=False, want_resid=False, stream=None):
         """Velocity-field strategy: torch CUDA float32 [K, 10] -> dict(chi2[, vmap][, resid])."""
