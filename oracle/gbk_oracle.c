@@ -57,19 +57,29 @@
 #endif
 
 #define GBKO_P 10 /* xo, yo, pa_deg, inc_deg, vsys, vt, rt, sigma0, r0, i0 */
+#define GBKO_P_EPINAT 12 /* ... + a, g: the slopes of eq. 7 */
 #define GBKO_PI 3.14159265358979323846
 
 typedef struct {
   int32_t nx, ny, nv;  /* observed grid: spaxels and channels              */
   int32_t u;           /* spatial up-sampling factor        */
   double v_center, dv; /* A2                                               */
-  int32_t rc_model;    /* 0 = arctan (eq. 6), 1 = linear ramp (A7)         */
+  int32_t rc_model;    /* 0 = arctan (eq. 6), 1 = linear ramp (A7), 2 = Epinat (eq. 7): rows of 12 */
   int32_t psf_n;       /* odd side of the PSF image on the fine grid       */
   const double *psf;   /* [psf_n*psf_n], row-major (y, x), sum = 1         */
   int32_t lsf_n;       /* odd length of the LSF taps (channels)            */
   const double *lsf;   /* [lsf_n], sum = 1                                 */
   int32_t halo_zero;   /* A6 switch, unit tests only                       */
+  /* "User-specified intensity model" (reading A22 of DESIGN.md): when tab_n > 0 the
+   * radial profile of eq. 5 is replaced by I(r) = I0 * T(r / r0), T tabulated at x_j = j * tab_dx,
+   * j = 0..tab_n-1, linear interpolation between nodes, T = tab[tab_n-1] beyond the last node.   */
+  int32_t tab_n;
+  const double *tab;
+  double tab_dx;
 } gbko_grid;
+
+/* Parameters per row: 12 with the Epinat curve, else 10.                      */
+int gbko_row_len(int rc_model) { return rc_model == 2 ? GBKO_P_EPINAT : GBKO_P; }
 
 /* ---------------------------------------------------------------- taps -- */
 
@@ -137,6 +147,24 @@ int gbko_row_valid(const double *p) {
   return 1;
 }
 
+/* The same for a row of the given rotation curve: the Epinat slopes a = p[10],
+ * g = p[11] must be finite and > 0 as well.                                   */
+int gbko_row_valid_rc(const double *p, int rc_model) {
+  if (!gbko_row_valid(p)) return 0;
+  if (rc_model == 2 && (!isfinite(p[10]) || !isfinite(p[11]) || !(p[10] > 0.0) || !(p[11] > 0.0)))
+    return 0;
+  return 1;
+}
+
+/* Tabulated radial profile T(x), x = r / r0 (see gbko_grid).                 */
+double gbko_table_profile(const double *tab, int n, double dx, double x) {
+  const double t = x / dx;
+  if (!(t < (double)(n - 1))) return tab[n - 1];
+  const int j = (int)floor(t);
+  const double f = t - (double)j;
+  return tab[j] + f * (tab[j + 1] - tab[j]);
+}
+
 /* One sky position (x, y): eq. 1-4 (deprojection), eq. 5 (brightness),
  * eq. 6 or the ramp (rotation curve), eq. 8 (line-of-sight velocity).
  * PAPER.md:84-96, 110, 120, 143.                                           */
@@ -157,8 +185,8 @@ void gbko_disc_point(const double *p, int rc_model, double x, double y, double *
     vrot = (2.0 / GBKO_PI) * vt * atan(r / rt);         /* eq. 6 */
   else if (rc_model == 1)
     vrot = vt * fmin(r / rt, 1.0);                      /* A7 */
-  else                                                  /* eq. 7, velocity-field */
-    vrot = vt * pow(r / rt, p[8]) / (1.0 + pow(r / rt, p[7]));   /* strategy only: a = p[7], g = p[8] */
+  else                                                  /* eq. 7: a = p[10], g = p[11] */
+    vrot = vt * pow(r / rt, p[11]) / (1.0 + pow(r / rt, p[10]));
   *I_out = I;
   *vlos_out = vsys + vrot * si * cos_theta;             /* eq. 8 */
 }
@@ -193,8 +221,15 @@ void gbko_model_cube(const gbko_grid *g, const double *p, double *cube) {
       const int fa = a - Rp, fb = b - Rp;
       const int in_field = fa >= 0 && fa < g->u * g->nx && fb >= 0 && fb < g->u * g->ny;
       double I, vlos;
-      gbko_disc_point(p, g->rc_model, gbko_fine_coord(fa, g->u), gbko_fine_coord(fb, g->u), &I,
-                      &vlos);
+      const double xs = gbko_fine_coord(fa, g->u), ys = gbko_fine_coord(fb, g->u);
+      gbko_disc_point(p, g->rc_model, xs, ys, &I, &vlos);
+      if (g->tab_n > 0) {          /* user-specified profile instead of eq. 5: I0 * T(r / r0) */
+        const double pa = p[2] * GBKO_PI / 180.0, inc = p[3] * GBKO_PI / 180.0;
+        const double xe = -(xs - p[0]) * sin(pa) + (ys - p[1]) * cos(pa);   /* eq. 1 */
+        const double ye = -(xs - p[0]) * cos(pa) - (ys - p[1]) * sin(pa);   /* eq. 2 */
+        const double r = sqrt(xe * xe + (ye / cos(inc)) * (ye / cos(inc))); /* eq. 3 */
+        I = p[9] * gbko_table_profile(g->tab, g->tab_n, g->tab_dx, r / p[8]);
+      }
       for (int c = 0; c < ec; ++c) {
         const int ch = c - Rv;
         const int in_band = ch >= 0 && ch < g->nv;
@@ -323,7 +358,7 @@ double gbko_chi2(const double *m0, const double *m1, const double *m2, const flo
  * An out-of-domain row fills the maps with NaN and returns 1.              */
 int gbko_model_maps(const gbko_grid *g, const double *p, double *m0, double *m1, double *m2) {
   const size_t npix = (size_t)g->nx * g->ny;
-  if (!gbko_row_valid(p)) {
+  if (!gbko_row_valid_rc(p, g->rc_model)) {
     for (size_t q = 0; q < npix; ++q) m0[q] = m1[q] = m2[q] = NAN;
     return 1;
   }
@@ -353,8 +388,8 @@ int gbko_model_maps(const gbko_grid *g, const double *p, double *m0, double *m1,
   return rc;
 }
 
-/* K parameter rows (float32 at the boundary, promoted to double) against one
- * observed data set.  Outputs (any may be NULL except chi2):
+/* K parameter rows (float32 at the boundary, promoted to double; gbko_row_len
+ * floats each) against one observed data set.  Outputs (any may be NULL except chi2):
  *   chi2[K]; m0,m1,m2[K][ny][nx]; resid[K][2][ny][nx].
  * nthreads <= 0 uses the OpenMP default.  Returns 0 or -1.                  */
 int gbko_eval_rows(const gbko_grid *g, const float *vobs, const float *verr, const float *sobs,
@@ -368,10 +403,11 @@ int gbko_eval_rows(const gbko_grid *g, const float *vobs, const float *verr, con
 #else
   (void)nthreads;
 #endif
+  const int P = gbko_row_len(g->rc_model);
 #pragma omp parallel for schedule(dynamic, 1)
   for (int64_t k = 0; k < K; ++k) {
-    double p[GBKO_P];
-    for (int j = 0; j < GBKO_P; ++j) p[j] = (double)params[k * GBKO_P + j];
+    double p[GBKO_P_EPINAT];
+    for (int j = 0; j < P; ++j) p[j] = (double)params[k * P + j];
     double *a0 = (double *)malloc(sizeof(double) * npix * 3);
     if (!a0) {
       fail = 1;
@@ -403,8 +439,9 @@ int gbko_eval_rows(const gbko_grid *g, const float *vobs, const float *verr, con
  * no PSF, no LSF (the paper skips steps 2.2.2-2.2.5), then the
  * velocity residual and the first term of eq. 11 only
  * (no dispersion map is modelled).  Only the seven kinematic
- * parameters p[0..6] are used (plus a = p[7], g = p[8] with the Epinat curve,
- * rc_model 2, eq. 7); a row is out of domain when one of them is not finite,
+ * parameters p[0..6] are used (plus a = p[10], g = p[11] of the 12-float rows
+ * of the Epinat curve, rc_model 2, eq. 7); a row is out of domain when one of
+ * them is not finite,
  * r_t <= 0, |cos i| < 1e-6, or a <= 0 or g <= 0 (chi2 = +INF, NaN maps).
  * Outputs: chi2[K]; vmap[K][ny][nx] and resid[K][ny][nx] may be NULL.        */
 int gbko_vfield_rows(const gbko_grid *g, const float *vobs, const float *verr, const uint8_t *mask,
@@ -416,21 +453,20 @@ int gbko_vfield_rows(const gbko_grid *g, const float *vobs, const float *verr, c
 #else
   (void)nthreads;
 #endif
+  const int P = gbko_row_len(g->rc_model);
 #pragma omp parallel for schedule(dynamic, 16)
   for (int64_t k = 0; k < K; ++k) {
-    double p[GBKO_P];
+    double p[GBKO_P_EPINAT];
     int ok = 1;
-    for (int j = 0; j < GBKO_P; ++j) p[j] = (double)params[k * GBKO_P + j];
+    for (int j = 0; j < P; ++j) p[j] = (double)params[k * P + j];
     for (int j = 0; j < 7; ++j)
       if (!isfinite(p[j])) ok = 0;
     if (ok && (!(p[6] > 0.0) || fabs(cos(p[3] * GBKO_PI / 180.0)) < 1e-6)) ok = 0;
-    if (g->rc_model == 2) {               /* Epinat curve: the slopes a = p[7], g = p[8] must be > 0 */
-      if (!isfinite(p[7]) || !isfinite(p[8]) || !(p[7] > 0.0) || !(p[8] > 0.0)) ok = 0;
-      if (!ok) p[7] = 1.0, p[8] = 1.0;
-    } else {
-      p[7] = 1.0, p[8] = 1.0;             /* unused by eq. 8; keep the brightness finite */
+    if (g->rc_model == 2) {               /* Epinat curve: the slopes a = p[10], g = p[11] must be > 0 */
+      if (!isfinite(p[10]) || !isfinite(p[11]) || !(p[10] > 0.0) || !(p[11] > 0.0)) ok = 0;
+      if (!ok) p[10] = 1.0, p[11] = 1.0;
     }
-    p[9] = 1.0;
+    p[7] = 1.0, p[8] = 1.0, p[9] = 1.0;   /* sigma0, r0, I0 are not part of eq. 8; keep the brightness finite */
     double sum = 0.0;
     for (size_t q = 0; q < npix; ++q) {
       const int iy = (int)(q / (size_t)g->nx), ix = (int)(q % (size_t)g->nx);

@@ -21,7 +21,12 @@ _SRC = os.path.join(_HERE, "gbk_oracle.c")
 _LIB = os.path.join(_HERE, "libgbk_oracle.so")
 
 P = 10  # xo, yo, pa_deg, inc_deg, vsys, vt, rt, sigma0, r0, i0
-RC_ARCTAN, RC_RAMP = 0, 1
+P_EPINAT = 12  # ... + a, g (eq. 7)
+RC_ARCTAN, RC_RAMP, RC_EPINAT = 0, 1, 2
+
+
+def row_len(rc_model: int) -> int:
+    return P_EPINAT if rc_model == RC_EPINAT else P
 
 
 def build(force: bool = False) -> str:
@@ -42,6 +47,7 @@ class _Grid(C.Structure):
         ("rc_model", C.c_int32), ("psf_n", C.c_int32), ("psf", C.POINTER(C.c_double)),
         ("lsf_n", C.c_int32), ("lsf", C.POINTER(C.c_double)),
         ("halo_zero", C.c_int32),
+        ("tab_n", C.c_int32), ("tab", C.POINTER(C.c_double)), ("tab_dx", C.c_double),
     ]
 
 
@@ -64,6 +70,10 @@ def lib():
         L.gbko_psf_moffat_image.restype = C.c_int
         L.gbko_row_valid.argtypes = [dp]
         L.gbko_row_valid.restype = C.c_int
+        L.gbko_row_valid_rc.argtypes = [dp, C.c_int]
+        L.gbko_row_valid_rc.restype = C.c_int
+        L.gbko_table_profile.argtypes = [dp, C.c_int, C.c_double, C.c_double]
+        L.gbko_table_profile.restype = C.c_double
         L.gbko_disc_point.argtypes = [dp, C.c_int, C.c_double, C.c_double, dp, dp]
         L.gbko_disc_point.restype = None
         L.gbko_channel_velocity.argtypes = [gp, C.c_int]
@@ -159,15 +169,24 @@ class Grid:
     psf: np.ndarray = field(default_factory=lambda: np.ones((1, 1)))
     lsf: np.ndarray = field(default_factory=lambda: np.ones(1))
     halo_zero: bool = False
+    tab: np.ndarray | None = None      # tabulated radial profile T(x_j), x_j = j * tab_dx
+    tab_dx: float = 0.0
 
     def c(self) -> _Grid:
         self._psf = _c64(self.psf)
         self._lsf = _c64(self.lsf)
         assert self._psf.ndim == 2 and self._psf.shape[0] == self._psf.shape[1]
         assert self._psf.shape[0] % 2 == 1 and self._lsf.size % 2 == 1
+        self._tab = None if self.tab is None else _c64(self.tab)
+        assert self._tab is None or (self._tab.size >= 2 and self.tab_dx > 0)
         return _Grid(self.nx, self.ny, self.nv, self.u, self.v_center, self.dv, self.rc_model,
                      self._psf.shape[0], _dp(self._psf), self._lsf.size, _dp(self._lsf),
-                     1 if self.halo_zero else 0)
+                     1 if self.halo_zero else 0,
+                     0 if self._tab is None else self._tab.size, _dp(self._tab), float(self.tab_dx))
+
+    @property
+    def P(self) -> int:
+        return row_len(self.rc_model)
 
     @property
     def ext_shape(self):
@@ -186,8 +205,20 @@ def row_valid(p) -> bool:
     return bool(lib().gbko_row_valid(_dp(p)))
 
 
+def row_valid_rc(p, rc_model: int) -> bool:
+    p = _c64(p)
+    assert p.size >= row_len(rc_model)
+    return bool(lib().gbko_row_valid_rc(_dp(p), int(rc_model)))
+
+
+def table_profile(tab, dx: float, x: float) -> float:
+    tab = _c64(tab)
+    return float(lib().gbko_table_profile(_dp(tab), tab.size, float(dx), float(x)))
+
+
 def disc_point(p, rc_model: int, x: float, y: float):
     p = _c64(p)
+    assert p.size >= row_len(rc_model)
     I, v = C.c_double(), C.c_double()
     lib().gbko_disc_point(_dp(p), int(rc_model), float(x), float(y), C.byref(I), C.byref(v))
     return I.value, v.value
@@ -257,6 +288,7 @@ def chi2(m0, m1, m2, vobs, verr, sobs=None, serr=None, mask=None, dark_level=0.0
 def model_maps(grid: Grid, p):
     """Steps 1-5 for one row -> (m0, m1, m2), float64 [ny, nx]."""
     p = _c64(p)
+    assert p.size == grid.P
     g = grid.c()
     m0, m1, m2 = (np.empty((grid.ny, grid.nx), dtype=np.float64) for _ in range(3))
     if lib().gbko_model_maps(C.byref(g), _dp(p), _dp(m0), _dp(m1), _dp(m2)) < 0:
@@ -267,7 +299,7 @@ def model_maps(grid: Grid, p):
 def eval_rows(grid: Grid, vobs, verr, sobs, serr, mask, params, want_maps=False,
               want_resid=False, nthreads: int = 0):
     """K float32 rows against one data set -> dict(chi2[, m0, m1, m2][, resid])."""
-    params = np.ascontiguousarray(params, dtype=np.float32).reshape(-1, P)
+    params = np.ascontiguousarray(params, dtype=np.float32).reshape(-1, grid.P)
     K = params.shape[0]
     vobs, verr, sobs, serr = _c32(vobs), _c32(verr), _c32(sobs), _c32(serr)
     mask = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
@@ -291,7 +323,7 @@ def eval_rows(grid: Grid, vobs, verr, sobs, serr, mask, params, want_maps=False,
 def vfield_rows(grid: Grid, vobs, verr, mask, params, want_maps=False, want_resid=False,
                 nthreads: int = 0):
     """Velocity-field strategy: K rows -> dict(chi2[, vmap][, resid])."""
-    params = np.ascontiguousarray(params, dtype=np.float32).reshape(-1, P)
+    params = np.ascontiguousarray(params, dtype=np.float32).reshape(-1, grid.P)
     K = params.shape[0]
     vobs, verr = _c32(vobs), _c32(verr)
     mask = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)

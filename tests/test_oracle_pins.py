@@ -462,8 +462,9 @@ def test_golden_hand_values_file(oracle):
                 continue
             tok = line.split()
             rc = {"arctan": 0, "ramp": 1, "epinat": 2}[tok[0]]
-            p = [float(t) for t in tok[1:11]]
-            x, y, I_want, v_want = (float(t) for t in tok[11:15])
+            npar = oracle.row_len(rc)                      # 12 columns for the Epinat curve (a, g last)
+            p = [float(t) for t in tok[1:1 + npar]]
+            x, y, I_want, v_want = (float(t) for t in tok[1 + npar:5 + npar])
             I, v = oracle.disc_point(p, rc, x, y)
             assert I == pytest.approx(I_want, rel=1e-9), line
             assert v == pytest.approx(v_want, abs=1e-7), line
@@ -489,8 +490,9 @@ def test_vfield_map_equals_the_golden_hand_values(oracle):
                 continue
             tok = line.split()
             rc = {"arctan": 0, "ramp": 1, "epinat": 2}[tok[0]]
-            p = np.array([float(t) for t in tok[1:11]], dtype=np.float32)
-            x, y, _, v_want = (float(t) for t in tok[11:15])
+            npar = oracle.row_len(rc)
+            p = np.array([float(t) for t in tok[1:1 + npar]], dtype=np.float32)
+            x, y, _, v_want = (float(t) for t in tok[1 + npar:5 + npar])
             if x < 0 or y < 0 or x != int(x) or y != int(y):
                 continue
             g = _vf_grid(oracle, 20, 20, rc)
@@ -541,15 +543,90 @@ def test_vfield_epinat_plateaus_and_domain(oracle):
     g = _vf_grid(oracle, 400, 1, rc=2)
     z = np.zeros((1, 400), np.float32)
     def curve(a, gg):
-        p = np.array([[0.0, 0.0, 90.0, 90.0 - 1e-3, 0.0, 100.0, 2.0, a, gg, 0.0]], dtype=np.float32)
+        p = np.array([[0.0, 0.0, 90.0, 90.0 - 1e-3, 0.0, 100.0, 2.0, np.nan, np.nan, np.nan, a, gg]],
+                     dtype=np.float32)                  # sigma_0, r_0, I_0 are not part of eq. 8
         # PA = 90: x_e = -(x - x_o); i ~ 90: sin i = 1 -> v(x) = -V_rot(|x|) on this row
         return -oracle.vfield_rows(g, z, z + 1, None, p, want_maps=True)["vmap"][0, 0]
     flat, rising, falling = curve(1.5, 1.5), curve(1.0, 1.5), curve(1.5, 1.0)
     assert flat[-1] == pytest.approx(100.0, rel=2e-3) and flat[2] == pytest.approx(50.0, rel=1e-9)
     assert rising[-1] > rising[200] > 100.0 and falling[-1] < falling[200] < falling[4]
-    p = np.array([[0.0, 0.0, 0.0, 30.0, 0.0, 100.0, 2.0, 1.0, 1.0, 0.0]], dtype=np.float32)
+    p = np.array([[0.0, 0.0, 0.0, 30.0, 0.0, 100.0, 2.0, 40.0, 4.0, 1.0, 1.0, 1.0]], dtype=np.float32)
     assert np.isfinite(oracle.vfield_rows(g, z, z + 1, None, p)["chi2"][0])
-    for j, bad in ((7, 0.0), (8, 0.0), (7, -1.0), (8, np.nan)):
+    for j, bad in ((10, 0.0), (11, 0.0), (10, -1.0), (11, np.nan)):
         q = p.copy()
         q[0, j] = bad
         assert np.isinf(oracle.vfield_rows(g, z, z + 1, None, q)["chi2"][0]), (j, bad)
+
+
+# ------------------------- Epinat curve and a tabulated profile in the cube ----
+
+def test_cube_with_the_epinat_curve_delta_kernels(oracle):
+    """Eq. 7 inside the intensity-cube strategy: with delta PSF and LSF the m1 map
+    is eq. 8 with V_rot = V_t q^g / (1 + q^a), q = r / r_t -- written out here for every spaxel -- m2
+    is sigma_0 and m0 the exponential disc of eq. 5; a = g = 1 at r = r_t gives V_t / 2 by hand."""
+    g = oracle.Grid(nx=17, ny=15, nv=160, u=1, v_center=0.0, dv=12.0, rc_model=oracle.RC_EPINAT,
+                    psf=np.ones((1, 1)), lsf=np.ones(1))
+    xo, yo, pa, inc, vsys, vt, rt, sig, r0, i0, a, gg = 8.0, 7.0, 0.0, 30.0, 7.0, 200.0, 3.0, 40.0, 4.0, 2.5, 1.7, 0.8
+    p = np.array([xo, yo, pa, inc, vsys, vt, rt, sig, r0, i0, a, gg])
+    m0, m1, m2 = oracle.model_maps(g, p)
+    yy, xx = np.mgrid[0:15, 0:17].astype(float)
+    xe = (yy - yo)                                    # PA = 0: eq. 1 gives x_e = y - y_o
+    ye = -(xx - xo)                                   # eq. 2
+    r = np.sqrt(xe ** 2 + (ye / np.cos(np.radians(inc))) ** 2)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        cos_t = np.where(r > 0, xe / r, 0.0)
+    q = r / rt
+    v = vsys + vt * q ** gg / (1.0 + q ** a) * np.sin(np.radians(inc)) * cos_t
+    assert np.max(np.abs(m1 - v)) < 1e-6
+    assert np.max(np.abs(m2 - sig)) < 1e-6
+    assert np.max(np.abs(m0 / (i0 * np.exp(-r / r0)) - 1.0)) < 1e-8
+    p1 = p.copy()
+    p1[10:] = 1.0
+    _, m1b, _ = oracle.model_maps(g, p1)
+    assert m1b[10, 8] == pytest.approx(7.0 + 100.0 * 0.5, abs=1e-6)      # (x, y) = (8, 10): r = r_t, on the major axis
+    for j, bad in ((10, 0.0), (11, -2.0), (10, np.nan)):                    # slopes must be finite and > 0
+        pb = p.copy()
+        pb[j] = bad
+        assert not oracle.row_valid_rc(pb, oracle.RC_EPINAT)
+        assert np.isnan(oracle.model_maps(g, pb)[0]).all()
+
+
+def test_tabulated_profile_by_hand(oracle):
+    """The tabulated radial profile (reading A22): linear interpolation between the
+    nodes x_j = j dx, the last value beyond them."""
+    tab = np.array([4.0, 2.0, 1.0, 0.25])
+    assert oracle.table_profile(tab, 0.5, 0.0) == 4.0
+    assert oracle.table_profile(tab, 0.5, 0.25) == pytest.approx(3.0)           # half way 4 -> 2
+    assert oracle.table_profile(tab, 0.5, 0.5) == 2.0
+    assert oracle.table_profile(tab, 0.5, 1.2) == pytest.approx(1.0 - 0.4 * 0.75)   # 40 % of the way 1 -> 0.25
+    assert oracle.table_profile(tab, 0.5, 1.5) == 0.25
+    assert oracle.table_profile(tab, 0.5, 7.0) == 0.25
+
+
+def test_cube_with_a_tabulated_intensity_profile(oracle):
+    """I(r) = I_0 T(r / r_0) replaces eq. 5 in the cube: (1) a constant table gives a uniform disc,
+    m0 = I_0 c; (2) a table of exp(-x) on a fine mesh reproduces the exponential model to the
+    interpolation error dx^2/8; (3) a linear table gives hand-computable m0 at spaxels of known r;
+    the velocity and dispersion maps do not depend on the profile when the kernels are deltas."""
+    base = dict(nx=13, ny=11, nv=128, u=1, v_center=0.0, dv=15.0, rc_model=0, psf=np.ones((1, 1)),
+                lsf=np.ones(1))
+    p = np.array([6.0, 5.0, 0.0, 60.0, 3.0, 150.0, 2.0, 35.0, 3.0, 1.5])
+    g_exp = oracle.Grid(**base)
+    m0e, m1e, m2e = oracle.model_maps(g_exp, p)
+    # (1) uniform disc
+    m0, m1, m2 = oracle.model_maps(oracle.Grid(**base, tab=np.array([0.7, 0.7]), tab_dx=1.0), p)
+    assert np.max(np.abs(m0 / (1.5 * 0.7) - 1.0)) < 1e-8
+    assert np.max(np.abs(m1 - m1e)) < 1e-9 and np.max(np.abs(m2 - m2e)) < 1e-9
+    # (2) exp(-x) on a mesh of 0.01 out to x = 12
+    dx = 0.01
+    tab = np.exp(-dx * np.arange(1201))
+    m0, _, _ = oracle.model_maps(oracle.Grid(**base, tab=tab, tab_dx=dx), p)
+    rel = np.abs(m0 / m0e - 1.0)
+    assert rel.max() < 1.3 * dx * dx / 8.0 and rel.max() > 0.0       # chord above a convex curve: <= dx^2/8
+    # (3) T(x) = 1 - x/4 on [0, 4] (two nodes), 0 beyond is not reached here: r_0 = 3, r <= 12
+    m0, _, _ = oracle.model_maps(oracle.Grid(**base, tab=np.array([1.0, 0.0]), tab_dx=4.0), p)
+    # PA = 0, i = 60: spaxel (x, y) = (6, 8) lies on the major axis at r = 3 => x = 1, T = 0.75;
+    # spaxel (8, 5) lies on the minor axis: r = 2 / cos 60 = 4 => x = 4/3, T = 2/3
+    assert m0[8, 6] == pytest.approx(1.5 * 0.75, rel=1e-8)
+    assert m0[5, 8] == pytest.approx(1.5 * (1.0 - (4.0 / 3.0) / 4.0), rel=1e-8)
+    assert m0[5, 6] == pytest.approx(1.5, rel=1e-8)                      # the centre: r = 0
