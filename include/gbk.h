@@ -28,14 +28,18 @@
  * flight elsewhere.  The scratch grows (cudaMalloc, which synchronises) the first time a stream sees
  * a larger batch; gbk_reserve sizes it up front, which is REQUIRED before a stream capture.
  *
- * Model row (GBK_P = 10 floats):
+ * Model row (GBK_P = 10 floats; GBK_P_EPINAT = 12 with the Epinat rotation curve):
  *   [0] x_o, [1] y_o    kinematic centre, data pixels (pixel j is centred on j)
  *   [2] PA   degrees    position angle (eq. 1-2)
  *   [3] i    degrees    inclination (eq. 3)
  *   [4] V_sys km/s      systemic velocity (eq. 8)
  *   [5] V_t  km/s, [6] r_t px   rotation curve (eq. 6; or ramp)
  *   [7] sigma_0 km/s    intrinsic dispersion
- *   [8] r_0 px, [9] I_0 exponential disc (eq. 5)
+ *   [8] r_0 px, [9] I_0 exponential disc (eq. 5), or the scale length and
+ *                       amplitude of a tabulated profile (gbk_problem_desc.intensity_table)
+ *   [10] a, [11] g      GBK_RC_EPINAT only: the slopes of eq. 7, both > 0
+ * Every array of rows at this boundary is [K][row_stride] with row_stride = gbk_problem_info.row_stride
+ * (GBK_P, or GBK_P_EPINAT for a GBK_RC_EPINAT problem).
  *
  * Out-of-domain rows are not errors: a row with a non-finite parameter,
  * sigma_0 <= 0, r_0 <= 0, r_t <= 0, I_0 <= 0 or |cos i| < 1e-6, or with an
@@ -52,14 +56,14 @@ extern "C" {
 #endif
 
 #define GBK_P 10
+#define GBK_P_EPINAT 12 /* GBK_P + the Epinat slopes a, g */
+#define GBK_P_MAX 12
 
 enum { GBK_OK = 0, GBK_ERR_ARG = 1, GBK_ERR_ALLOC = 2, GBK_ERR_CUDA = 3, GBK_ERR_UNSUPPORTED = 4 };
 enum { GBK_RC_ARCTAN = 0, GBK_RC_RAMP = 1, GBK_RC_EPINAT = 2 };
 /* eq. 6; V_t*min(r/r_t,1); eq. 7: V_t q^g/(1+q^a), q = r/r_t.
- * GBK_RC_EPINAT is the curve the paper pairs with velocity-field modelling and is
- * available with gbk_eval_vfield_batch only: its slopes travel in the row slots that strategy does
- * not use, [7] = a > 0 and [8] = g > 0 (the cube strategy would need 12 parameters per row:
- * gbk_eval_batch and gbk_eval_batch_unfused return GBK_ERR_UNSUPPORTED for it). */
+ * GBK_RC_EPINAT is the curve the paper pairs with velocity-field modelling; its rows
+ * have GBK_P_EPINAT = 12 floats, the slopes in [10] = a > 0 and [11] = g > 0, for BOTH strategies. */
 enum { GBK_PSF_GAUSSIAN = 0, GBK_PSF_IMAGE = 1 }; /* eq. 9; image */
 
 typedef struct gbk_problem gbk_problem; /* opaque; owns device copies of the observation */
@@ -102,6 +106,11 @@ typedef struct {
                           /* batches too small to fill the GPU (chi^2 then differs between    */
                           /* batch sizes by summation order only, ~1e-7 relative)             */
   int32_t device;       /* CUDA device ordinal; < 0 = the current device                   */
+  const float *intensity_table; /* NULL: the exponential disc of eq. 5.  Else a "user-specified      */
+  int32_t intensity_n;          /* intensity model": I(r) = I_0 T(r / r_0) with T      */
+  float intensity_dx;           /* tabulated at x_j = j * intensity_dx, j = 0 .. intensity_n - 1      */
+                                /* (>= 2 finite values >= 0, dx > 0), linear interpolation between   */
+                                /* nodes, the last value beyond them; cube strategy only             */
 } gbk_problem_desc;
 
 /* What gbk_create_problem decided (for tests, benchmarks and op counting). */
@@ -120,6 +129,7 @@ typedef struct {
   int32_t strategy;       /* GBK_STRATEGY_* the host drivers evaluate with (gbk_set_strategy) */
   int64_t unfused_bytes_per_eval; /* algorithmic HBM bytes of gbk_eval_batch_unfused per row:   */
                           /* every intermediate array written once and read once per consumer */
+  int32_t row_stride;     /* floats per parameter row: GBK_P, or GBK_P_EPINAT                  */
 } gbk_problem_info;
 
 /*
@@ -138,7 +148,8 @@ int gbk_get_info(const gbk_problem *p, gbk_problem_info *info);
  * Which of the paper's two modelling strategies the host drivers gbk_fit_* evaluate
  * rows with: the intensity-cube strategy (gbk_eval_batch, the default) or the velocity-field
  * strategy (gbk_eval_vfield_batch; residual vectors are then ny*nx long instead of 2*ny*nx).
- * GBK_RC_EPINAT problems start as GBK_STRATEGY_VFIELD.  The eval calls themselves ignore it.
+ * GBK_RC_EPINAT problems start as GBK_STRATEGY_VFIELD (the paper's pairing), all others
+ * as GBK_STRATEGY_CUBE.  The eval calls themselves ignore it.
  */
 enum { GBK_STRATEGY_CUBE = 0, GBK_STRATEGY_VFIELD = 1 };
 int gbk_set_strategy(gbk_problem *p, int32_t strategy);
@@ -149,7 +160,7 @@ int gbk_set_strategy(gbk_problem *p, int32_t strategy);
  * or allocates except to grow that stream's cross-tile scratch (see gbk_reserve).
  * Errors: GBK_ERR_ARG (NULL arguments, K < 0, K x tiles beyond the grid limit, scratch growth
  * needed during a stream capture), GBK_ERR_UNSUPPORTED, GBK_ERR_ALLOC, GBK_ERR_CUDA.
- *   params     DEVICE [K][GBK_P] float32, row-major
+ *   params     DEVICE [K][row_stride] float32, row-major
  *   gal_index  DEVICE [K] int32 in [0, n_gal), or NULL (all rows use data set 0)
  *   chi2       DEVICE [K] float32, required (eq. 11)
  *   m0,m1,m2   DEVICE [K][ny][nx] float32 each, any may be NULL: flux (sum over
@@ -201,9 +212,10 @@ int gbk_eval_batch_unfused(gbk_problem *p, const float *params, const int32_t *g
  * PSF, no LSF, no up-sampling (the paper skips steps 2.2.2-2.2.5) -- then the
  * velocity residual and the first term of eq. 11 only.  Uses the
  * problem's vobs / verr / mask and rc_model; of a row only x_o, y_o, PA, i, V_sys, V_t, r_t are
- * read, plus a = row[7], g = row[8] with GBK_RC_EPINAT (a row is out of domain, chi2 = +INF, when
- * one of those is not finite, r_t <= 0, |cos i| < 1e-6, or a <= 0 or g <= 0).  Asynchronous on `cuda_stream`, no allocation.
- *   params DEVICE [K][GBK_P]; gal_index DEVICE [K] or NULL; chi2 DEVICE [K], required
+ * read, plus a = row[10], g = row[11] with GBK_RC_EPINAT (a row is out of domain, chi2 = +INF, when
+ * one of those is not finite, r_t <= 0, |cos i| < 1e-6, or a <= 0 or g <= 0).  Asynchronous on
+ * `cuda_stream`, no allocation.
+ *   params DEVICE [K][row_stride]; gal_index DEVICE [K] or NULL; chi2 DEVICE [K], required
  *   vmap   DEVICE [K][ny][nx] or NULL: the model velocity field
  *   resid  DEVICE [K][ny][nx] or NULL: (model - vobs) / verr, 0 where masked
  */
@@ -262,7 +274,8 @@ typedef struct {
  * and nodes c + (j - (nodes-1)/2) h; c = box centre at level 0, then the best node of the level
  * before.  An axis on PA (index 2) whose box spans >= 360 degrees wraps; any other axis is shifted
  * to stay inside its box.  Ties in chi^2 take the lowest flat index (axis 0 slowest).
- * nodes^n_axes <= 2^24.  best_row [GBK_P] and best_chi2 [1] receive the final level's best node.
+ * nodes^n_axes <= 2^24.  base_row and best_row are [row_stride]; best_chi2 [1] receives the chi^2 of the
+ * final level's best node.
  */
 int gbk_fit_ng(gbk_problem *p, const float *base_row, int32_t gal, int32_t n_axes,
                const int32_t *axis_param, const float *axis_lo, const float *axis_hi, int32_t nodes,
@@ -284,8 +297,8 @@ int gbk_fit_ng(gbk_problem *p, const float *base_row, int32_t gal, int32_t n_axe
  * tell), after max_iter iterations, or as FAILED when it cannot iterate: the start row or a
  * difference row is out of domain (chi^2 = +INF), or the normal equations are singular or not finite
  * for every damping factor.  Failed fits are counted in stats->failed, never in stats->converged.
- *   start_rows [n_fits][GBK_P], gal [n_fits] or NULL (all 0), free_param/lo/hi [n_free]
- *   fit_rows [n_fits][GBK_P], fit_chi2 [n_fits], fit_iters [n_fits] or NULL
+ *   start_rows [n_fits][row_stride], gal [n_fits] or NULL (all 0), free_param/lo/hi [n_free]
+ *   fit_rows [n_fits][row_stride], fit_chi2 [n_fits], fit_iters [n_fits] or NULL
  * A fit whose start row has chi^2 = +INF is returned unchanged with chi^2 = +INF.
  * stats->evals counts the rows evaluated for fits that were active.
  */
@@ -303,7 +316,7 @@ int gbk_fit_lm(gbk_problem *p, int32_t n_fits, const float *start_rows, const in
  * the current worst live point replaces it (prior volume X_i = exp(-i/n_live), evidence by the
  * simple rule Z += L_i (X_{i-1} - X_i)).
  * Stops when L_max X_i < tol x Z or after max_batches.  Outputs: the best row, its chi^2, the
- * posterior-mean row and ln Z.  `seed` seeds the driver's own generator (xoshiro256**).
+ * posterior-mean row (base_row, best_row, mean_row: [row_stride]) and ln Z.  `seed` seeds the driver's own generator (xoshiro256**).
  */
 int gbk_fit_ns(gbk_problem *p, const float *base_row, int32_t gal, int32_t n_free,
                const int32_t *free_param, const float *lo, const float *hi, int32_t n_live,

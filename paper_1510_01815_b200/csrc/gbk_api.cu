@@ -74,6 +74,7 @@ struct gbk_problem {
   long long ext_voxels = 0;
   // device allocations owned by the problem
   double* chan_w = nullptr;
+  float* tab = nullptr;         // tabulated intensity profile
   float* psf_taps = nullptr;
   int* psf_r = nullptr;
   float4* obs = nullptr;
@@ -102,6 +103,7 @@ extern "C" const char* gbk_last_error(void) { return g_err; }
 extern "C" int gbk_destroy(gbk_problem* p) {
   if (!p) return GBK_OK;
   cudaFree(p->chan_w);
+  cudaFree(p->tab);
   cudaFree(p->psf_taps);
   cudaFree(p->psf_r);
   cudaFree(p->obs);
@@ -134,6 +136,13 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   if (d->psf_kind != GBK_PSF_GAUSSIAN && d->psf_kind != GBK_PSF_IMAGE)
     return fail(GBK_ERR_ARG, "unknown psf_kind %d", d->psf_kind);
   if (!isfinite(d->lsf_sigma)) return fail(GBK_ERR_ARG, "lsf_sigma must be finite");
+  if (d->intensity_table) {
+    if (d->intensity_n < 2 || d->intensity_n > (1 << 20) || !(d->intensity_dx > 0.f) || !isfinite(d->intensity_dx))
+      return fail(GBK_ERR_ARG, "intensity_table needs 2 <= intensity_n <= 2^20 and intensity_dx > 0");
+    for (int j = 0; j < d->intensity_n; ++j)
+      if (!isfinite(d->intensity_table[j]) || d->intensity_table[j] < 0.f)
+        return fail(GBK_ERR_ARG, "intensity_table[%d] must be finite and >= 0", j);
+  }
 
   const int n_psf = d->psf_per_gal ? d->n_gal : 1;
   const size_t npix = (size_t)d->nx * d->ny;
@@ -248,6 +257,9 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   dp.fw = d->u * d->nx, dp.fh = d->u * d->ny;
   dp.r_v = r_v, dp.nvx = nvx, dp.nvx_pad = nvx_pad;
   dp.rc_model = d->rc_model, dp.psf_kind = d->psf_kind;
+  dp.row_stride = d->rc_model == GBK_RC_EPINAT ? GBK_P_EPINAT : GBK_P;
+  dp.tab_n = d->intensity_table ? d->intensity_n : 0;
+  dp.tab_inv_dx = d->intensity_table ? 1.0f / d->intensity_dx : 0.0f;
   dp.has_disp = d->sobs ? 1 : 0, dp.psf_per_gal = d->psf_per_gal ? 1 : 0;
   dp.r_p_max = r_p_max, dp.psf_stride = psf_stride;
   dp.dv = d->dv, dp.v_center = d->v_center;
@@ -331,6 +343,11 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     GBK_CUDA_P(cudaMemcpy(p->lsf_taps, lsf_f.data(), sizeof(float) * lsf_f.size(), cudaMemcpyHostToDevice));
   }
   GBK_CUDA_P(cudaMemcpy(p->chan_w, chan.data(), sizeof(double) * chan.size(), cudaMemcpyHostToDevice));
+  if (d->intensity_table) {
+    GBK_CUDA_P(cudaMalloc(&p->tab, sizeof(float) * (size_t)d->intensity_n));
+    GBK_CUDA_P(cudaMemcpy(p->tab, d->intensity_table, sizeof(float) * (size_t)d->intensity_n, cudaMemcpyHostToDevice));
+  }
+  dp.tab = p->tab;
   GBK_CUDA_P(cudaMemcpy(p->psf_taps, psf_taps.data(), sizeof(float) * psf_taps.size(), cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->psf_r, psf_r.data(), sizeof(int) * n_psf, cudaMemcpyHostToDevice));
   GBK_CUDA_P(cudaMemcpy(p->obs, obs.data(), sizeof(float4) * obs.size(), cudaMemcpyHostToDevice));
@@ -367,6 +384,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
   p->d.vobs = p->d.verr = p->d.sobs = p->d.serr = nullptr;
   p->d.mask = nullptr;
   p->d.psf_fwhm = p->d.psf_image = nullptr;
+  p->d.intensity_table = nullptr;
   *out = p;
   return GBK_OK;
 }
@@ -384,6 +402,7 @@ extern "C" int gbk_get_info(const gbk_problem* p, gbk_problem_info* info) {
   info->device = p->device;
   info->strategy = p->strategy;
   info->unfused_bytes_per_eval = (int64_t)unfused_algorithmic_bytes_per_row(p->dp);
+  info->row_stride = dp.row_stride;
   return GBK_OK;
 }
 
@@ -392,15 +411,7 @@ extern "C" int gbk_set_strategy(gbk_problem* p, int32_t strategy) {
   if (!p) return fail(GBK_ERR_ARG, "null problem");
   if (strategy != GBK_STRATEGY_CUBE && strategy != GBK_STRATEGY_VFIELD)
     return fail(GBK_ERR_ARG, "unknown strategy %d", strategy);
-  if (strategy == GBK_STRATEGY_CUBE && p->dp.rc_model == GBK_RC_EPINAT)
-    return fail(GBK_ERR_UNSUPPORTED, "the Epinat curve is available with the velocity-field strategy only");
   p->strategy = strategy;
-  return GBK_OK;
-}
-
-static int check_cube_model(const gbk_problem* p) {
-  if (p && p->dp.rc_model == GBK_RC_EPINAT)
-    return fail(GBK_ERR_UNSUPPORTED, "the Epinat curve is available with gbk_eval_vfield_batch only");
   return GBK_OK;
 }
 
@@ -480,7 +491,7 @@ extern "C" int gbk_reserve(gbk_problem* p, int64_t K_max, void* cuda_stream) {
   if (K_max > sc->st_cap) {
     cudaFree(sc->st_params), cudaFree(sc->st_gal), cudaFree(sc->st_chi2);
     sc->st_params = nullptr, sc->st_gal = nullptr, sc->st_chi2 = nullptr, sc->st_cap = 0;
-    GBK_CUDA(cudaMalloc(&sc->st_params, sizeof(float) * GBK_P * (size_t)K_max));
+    GBK_CUDA(cudaMalloc(&sc->st_params, sizeof(float) * GBK_P_MAX * (size_t)K_max));
     GBK_CUDA(cudaMalloc(&sc->st_gal, sizeof(int32_t) * (size_t)K_max));
     GBK_CUDA(cudaMalloc(&sc->st_chi2, sizeof(float) * (size_t)K_max));
     sc->st_cap = K_max;
@@ -510,7 +521,6 @@ static int eval_batch_impl(gbk_problem* p, const float* params, const int32_t* g
                            unsigned long long* counters, void* cuda_stream) {
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
-  if (int rc = check_cube_model(p)) return rc;
   if (K == 0) return GBK_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(p->device);
@@ -561,7 +571,7 @@ extern "C" int gbk_eval_batch_host(gbk_problem* p, const float* params, const in
   if (!sc) return fail(GBK_ERR_ALLOC, "out of host memory");
   if (K > sc->st_cap)
     if (int rc = gbk_reserve(p, K, cuda_stream)) return rc;
-  GBK_CUDA(cudaMemcpyAsync(sc->st_params, params, sizeof(float) * GBK_P * (size_t)K, cudaMemcpyHostToDevice, st));
+  GBK_CUDA(cudaMemcpyAsync(sc->st_params, params, sizeof(float) * p->dp.row_stride * (size_t)K, cudaMemcpyHostToDevice, st));
   if (gal_index)
     GBK_CUDA(cudaMemcpyAsync(sc->st_gal, gal_index, sizeof(int32_t) * (size_t)K, cudaMemcpyHostToDevice, st));
   if (int rc = gbk_eval_batch(p, sc->st_params, gal_index ? sc->st_gal : nullptr, K, sc->st_chi2, nullptr,
@@ -577,7 +587,6 @@ extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const
                                       float* resid, void* cuda_stream) {
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
-  if (int rc = check_cube_model(p)) return rc;
   if (K == 0) return GBK_OK;
   DeviceGuard guard(p->device);
   GBK_CUDA(guard.status);

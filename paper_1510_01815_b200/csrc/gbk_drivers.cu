@@ -121,16 +121,16 @@ int eval_rows(gbk_problem* p, const gbk_problem_info& info, const float* rows, c
   return gbk_eval_batch(p, rows, gal, K, chi2, nullptr, nullptr, nullptr, resid, stream);
 }
 
-bool finite_row(const float* r) {
-  for (int j = 0; j < GBK_P; ++j)
+bool finite_row(const float* r, int S) {
+  for (int j = 0; j < S; ++j)
     if (!isfinite(r[j])) return false;
   return true;
 }
 
-int check_box(int n, const int32_t* idx, const float* lo, const float* hi) {
-  if (n < 1 || n > GBK_P || !idx || !lo || !hi) return fail(GBK_ERR_ARG, "bad parameter box");
+int check_box(int n, const int32_t* idx, const float* lo, const float* hi, int S) {
+  if (n < 1 || n > S || !idx || !lo || !hi) return fail(GBK_ERR_ARG, "bad parameter box");
   for (int a = 0; a < n; ++a) {
-    if (idx[a] < 0 || idx[a] >= GBK_P) return fail(GBK_ERR_ARG, "parameter index %d out of range", idx[a]);
+    if (idx[a] < 0 || idx[a] >= S) return fail(GBK_ERR_ARG, "parameter index %d out of range", idx[a]);
     if (!isfinite(lo[a]) || !isfinite(hi[a]) || !(hi[a] > lo[a]))
       return fail(GBK_ERR_ARG, "box of parameter %d is empty or not finite", idx[a]);
     for (int b = 0; b < a; ++b)
@@ -143,19 +143,19 @@ int check_box(int n, const int32_t* idx, const float* lo, const float* hi) {
 constexpr int kNgMaxAxes = 6, kNgMaxNodes = 32;
 
 struct NgAxes {
-  int n_axes, nodes;
+  int n_axes, nodes, S;       // S: floats per row
   int param[kNgMaxAxes];
   float value[kNgMaxAxes][kNgMaxNodes];
-  float base[GBK_P];
+  float base[GBK_P_MAX];
 };
 
 // Row r of the level: flat index with axis 0 slowest.
 __global__ void ng_rows_kernel(const __grid_constant__ NgAxes ax, int n_rows, float* __restrict__ rows) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= n_rows) return;
-  float row[GBK_P];
+  float row[GBK_P_MAX];
 #pragma unroll
-  for (int j = 0; j < GBK_P; ++j) row[j] = ax.base[j];
+  for (int j = 0; j < GBK_P_MAX; ++j) row[j] = ax.base[j];
   int rem = r;
   for (int a = ax.n_axes - 1; a >= 0; --a) {
     const int j = rem % ax.nodes;
@@ -163,7 +163,8 @@ __global__ void ng_rows_kernel(const __grid_constant__ NgAxes ax, int n_rows, fl
     row[ax.param[a]] = ax.value[a][j];
   }
 #pragma unroll
-  for (int j = 0; j < GBK_P; ++j) rows[(size_t)r * GBK_P + j] = row[j];
+  for (int j = 0; j < GBK_P_MAX; ++j)
+    if (j < ax.S) rows[(size_t)r * ax.S + j] = row[j];
 }
 
 // Smallest chi^2 and its lowest index (NaN never wins; +INF only if everything is +INF).
@@ -204,7 +205,7 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
   if (!base_row || !best_row || !best_chi2) return fail(GBK_ERR_ARG, "null argument");
   if (n_axes > kNgMaxAxes || nodes < 2 || nodes > kNgMaxNodes || levels < 1 || levels > 30)
     return fail(GBK_ERR_ARG, "need n_axes <= %d, 2 <= nodes <= %d, 1 <= levels <= 30", kNgMaxAxes, kNgMaxNodes);
-  DRV_TRY(check_box(n_axes, axis_param, axis_lo, axis_hi));
+  DRV_TRY(check_box(n_axes, axis_param, axis_lo, axis_hi, info.row_stride));
   if (gal < 0 || gal >= info.n_gal) return fail(GBK_ERR_ARG, "gal out of range");
   double n_rows_d = 1.0;
   for (int a = 0; a < n_axes; ++a) n_rows_d *= nodes;
@@ -221,7 +222,7 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
   Buf<float> rows, chi2, best_v;
   Buf<int> best_i, gal_idx;
   for (int pass = 0; pass < 2; ++pass) {
-    rows.alloc(ar, (size_t)n_rows * GBK_P, false);
+    rows.alloc(ar, (size_t)n_rows * GBK_P_MAX, false);
     chi2.alloc(ar, n_rows, false);
     best_v.alloc(ar, 1);
     best_i.alloc(ar, 1);
@@ -235,8 +236,9 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
 
   NgAxes ax;
   memset(&ax, 0, sizeof(ax));
-  ax.n_axes = n_axes, ax.nodes = nodes;
-  memcpy(ax.base, base_row, sizeof(float) * GBK_P);
+  const int S = info.row_stride;
+  ax.n_axes = n_axes, ax.nodes = nodes, ax.S = S;
+  memcpy(ax.base, base_row, sizeof(float) * S);
   double centre[kNgMaxAxes];
   for (int a = 0; a < n_axes; ++a) {
     ax.param[a] = axis_param[a];
@@ -274,7 +276,7 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
     }
     fs.evals += n_rows, fs.launches += 1, fs.iterations += 1;
   }
-  memcpy(best_row, base_row, sizeof(float) * GBK_P);
+  memcpy(best_row, base_row, sizeof(float) * S);
   for (int a = 0; a < n_axes; ++a) best_row[axis_param[a]] = (float)centre[a];
   *best_chi2 = best_v.h[0];
   fs.converged = isfinite(best_v.h[0]) ? 1 : 0;
@@ -304,14 +306,14 @@ constexpr int kLmReadback = 4;
 __constant__ double kLmFactor[kLmTrials] = {0.1, 1.0, 10.0, 100.0};
 
 struct LmSetup {
-  int n, M, n_terms, max_iter;
-  int free_param[GBK_P];
-  float lo[GBK_P], hi[GBK_P];
+  int n, M, n_terms, max_iter, S;   // S: floats per row
+  int free_param[GBK_P_MAX];
+  float lo[GBK_P_MAX], hi[GBK_P_MAX];
   float rel_step, ftol;
 };
 
 struct LmState {         // device arrays, one entry per fit
-  float* row;            // [n_fits][GBK_P]
+  float* row;            // [n_fits][S]
   double* chi2;          // chi^2 of `row` (+inf until evaluated)
   double* lambda;
   int* iters;
@@ -328,9 +330,9 @@ __global__ void lm_jacobian_rows(const __grid_constant__ LmSetup su, const LmSta
   const int slot = t / (su.n + 1), r = t - slot * (su.n + 1);
   if (slot >= n_list) return;
   const int f = list[slot];
-  float row[GBK_P];
+  float row[GBK_P_MAX];
 #pragma unroll
-  for (int j = 0; j < GBK_P; ++j) row[j] = stt.row[(size_t)f * GBK_P + j];
+  for (int j = 0; j < GBK_P_MAX; ++j) row[j] = j < su.S ? stt.row[(size_t)f * su.S + j] : 0.0f;
   gidx[t] = stt.gal[f];
   if (stt.status[f] != LM_ACTIVE) {
     row[0] = __int_as_float(0x7fc00000);          // finished: an out-of-domain row costs next to nothing
@@ -346,7 +348,8 @@ __global__ void lm_jacobian_rows(const __grid_constant__ LmSetup su, const LmSta
     atomicAdd(stt.evals, (unsigned long long)(su.n + 1));
   }
 #pragma unroll
-  for (int j = 0; j < GBK_P; ++j) rows[(size_t)t * GBK_P + j] = row[j];
+  for (int j = 0; j < GBK_P_MAX; ++j)
+    if (j < su.S) rows[(size_t)t * su.S + j] = row[j];
 }
 
 // One block per (term, slot).  Terms: n(n+1)/2 entries of J^T J (upper triangle, row-major),
@@ -394,7 +397,7 @@ __global__ void lm_normal_kernel(const float* __restrict__ resid, const LmState 
 
 // Solves (A + lambda diag(A)) x = -g by Cholesky (A symmetric, upper triangle packed row-major).
 __device__ bool solve_damped(int n, const double* tri, const double* g, double lambda, double* x) {
-  double L[GBK_P][GBK_P];
+  double L[GBK_P_MAX][GBK_P_MAX];
   int t = 0;
   for (int a = 0; a < n; ++a)
     for (int b = a; b < n; ++b, ++t) L[a][b] = L[b][a] = tri[t];
@@ -413,7 +416,7 @@ __device__ bool solve_damped(int n, const double* tri, const double* g, double l
       L[i][j] = s / L[j][j];
     }
   }
-  double y[GBK_P];
+  double y[GBK_P_MAX];
   for (int i = 0; i < n; ++i) {
     double s = -g[i];
     for (int k = 0; k < i; ++k) s -= L[i][k] * y[k];
@@ -438,9 +441,9 @@ __global__ void lm_trial_rows(const __grid_constant__ LmSetup su, const LmState 
   const int slot = t / kLmTrials, trial = t - slot * kLmTrials;
   if (slot >= n_list) return;
   const int f = list[slot], n = su.n;
-  float row[GBK_P];
+  float row[GBK_P_MAX];
 #pragma unroll
-  for (int j = 0; j < GBK_P; ++j) row[j] = stt.row[(size_t)f * GBK_P + j];
+  for (int j = 0; j < GBK_P_MAX; ++j) row[j] = j < su.S ? stt.row[(size_t)f * su.S + j] : 0.0f;
   gidx[t] = stt.gal[f];
   int status = stt.status[f];
   if (status == LM_ACTIVE) {
@@ -452,7 +455,7 @@ __global__ void lm_trial_rows(const __grid_constant__ LmSetup su, const LmState 
     else if (stt.iters[f] >= su.max_iter) status = LM_MAXITER;
     else if (!jac_ok) status = LM_FAILED;
     const double* nm = normal + (size_t)slot * su.n_terms;
-    double dx[GBK_P];
+    double dx[GBK_P_MAX];
     bool solved = false;
     if (status == LM_ACTIVE) {
       solved = solve_damped(n, nm, nm + n * (n + 1) / 2, stt.lambda[f] * kLmFactor[trial], dx);
@@ -471,7 +474,8 @@ __global__ void lm_trial_rows(const __grid_constant__ LmSetup su, const LmState 
   }
   if (status != LM_ACTIVE) row[0] = __int_as_float(0x7fc00000);
 #pragma unroll
-  for (int j = 0; j < GBK_P; ++j) rows[(size_t)t * GBK_P + j] = row[j];
+  for (int j = 0; j < GBK_P_MAX; ++j)
+    if (j < su.S) rows[(size_t)t * su.S + j] = row[j];
 }
 
 // One thread per slot: best of the four trials, accept / reject, damping update, stopping rules.
@@ -493,8 +497,8 @@ __global__ void lm_update(const __grid_constant__ LmSetup su, const LmState stt,
   int status = LM_ACTIVE;
   if (best >= 0) {
     const double rel = (stt.chi2[f] - best_chi) / stt.chi2[f];
-    for (int j = 0; j < GBK_P; ++j)
-      stt.row[(size_t)f * GBK_P + j] = trial_rows[((size_t)slot * kLmTrials + best) * GBK_P + j];
+    for (int j = 0; j < su.S; ++j)
+      stt.row[(size_t)f * su.S + j] = trial_rows[((size_t)slot * kLmTrials + best) * su.S + j];
     stt.lambda[f] = fmax(1e-9, stt.lambda[f] * kLmFactor[best] * 0.3);
     stt.chi2[f] = best_chi;
     if (rel < (double)su.ftol) status = LM_CONVERGED;
@@ -550,7 +554,7 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
     return fail(GBK_ERR_ARG, "null argument");
   if (!(rel_step > 0.f) || !isfinite(rel_step) || max_iter < 0 || !(ftol >= 0.f))
     return fail(GBK_ERR_ARG, "need rel_step > 0, max_iter >= 0, ftol >= 0");
-  DRV_TRY(check_box(n_free, free_param, lo, hi));
+  DRV_TRY(check_box(n_free, free_param, lo, hi, info.row_stride));
   for (int f = 0; f < n_fits; ++f)
     if (gal && (gal[f] < 0 || gal[f] >= info.n_gal)) return fail(GBK_ERR_ARG, "gal[%d] out of range", f);
   gbk_fit_stats fs{};
@@ -564,7 +568,8 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
   LmSetup su{};
   su.n = n_free, su.M = (info.strategy == GBK_STRATEGY_VFIELD ? 1 : 2) * info.nx * info.ny;
   su.n_terms = su.n * (su.n + 1) / 2 + su.n + 1, su.max_iter = max_iter;
-  su.rel_step = rel_step, su.ftol = ftol;
+  su.rel_step = rel_step, su.ftol = ftol, su.S = info.row_stride;
+  const int S = su.S;
   for (int a = 0; a < su.n; ++a) su.free_param[a] = free_param[a], su.lo[a] = lo[a], su.hi[a] = hi[a];
   const int n = su.n;
   // fits per chunk: the residual buffer of a chunk stays below 1 GiB
@@ -580,13 +585,13 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
   Buf<double> normal, state_chi2, lambda;
   Buf<unsigned long long> evals;
   for (int pass = 0; pass < 2; ++pass) {
-    rows.alloc(ar, (size_t)chunk * rows_per_fit * GBK_P, false);
+    rows.alloc(ar, (size_t)chunk * rows_per_fit * S, false);
     chi2.alloc(ar, (size_t)chunk * rows_per_fit, false);
     gidx.alloc(ar, (size_t)chunk * rows_per_fit, false);
     resid.alloc(ar, (size_t)chunk * (n + 1) * su.M, false);
     normal.alloc(ar, (size_t)chunk * su.n_terms, false);
     hstep.alloc(ar, (size_t)n_fits * n, false);
-    state_row.alloc(ar, (size_t)n_fits * GBK_P);
+    state_row.alloc(ar, (size_t)n_fits * S);
     state_chi2.alloc(ar, n_fits);
     lambda.alloc(ar, n_fits);
     iters.alloc(ar, n_fits);
@@ -599,16 +604,16 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
     if (pass == 0) DRV_CUDA(ar.commit());
   }
   for (int f = 0; f < n_fits; ++f) {
-    float* row = state_row.h + (size_t)f * GBK_P;
-    memcpy(row, start_rows + (size_t)f * GBK_P, sizeof(float) * GBK_P);
+    float* row = state_row.h + (size_t)f * S;
+    memcpy(row, start_rows + (size_t)f * S, sizeof(float) * S);
     for (int a = 0; a < n; ++a)   // start inside the box
       row[free_param[a]] = std::min(hi[a], std::max(lo[a], row[free_param[a]]));
     state_chi2.h[f] = INFINITY, lambda.h[f] = 1e-3, iters.h[f] = 0;
-    status.h[f] = finite_row(row) ? LM_ACTIVE : LM_BAD_START;
+    status.h[f] = finite_row(row, S) ? LM_ACTIVE : LM_BAD_START;
     galb.h[f] = gal ? gal[f] : 0;
   }
   evals.h[0] = 0;
-  DRV_CUDA(state_row.to_device((size_t)n_fits * GBK_P, st));
+  DRV_CUDA(state_row.to_device((size_t)n_fits * S, st));
   DRV_CUDA(state_chi2.to_device(n_fits, st));
   DRV_CUDA(lambda.to_device(n_fits, st));
   DRV_CUDA(iters.to_device(n_fits, st));
@@ -657,14 +662,14 @@ extern "C" int gbk_fit_lm(gbk_problem* p, int32_t n_fits, const float* start_row
       }
     }
   }
-  DRV_CUDA(state_row.to_host((size_t)n_fits * GBK_P, st));
+  DRV_CUDA(state_row.to_host((size_t)n_fits * S, st));
   DRV_CUDA(state_chi2.to_host(n_fits, st));
   DRV_CUDA(iters.to_host(n_fits, st));
   DRV_CUDA(status.to_host(n_fits, st));
   DRV_CUDA(evals.to_host(1, st));
   DRV_CUDA(cudaStreamSynchronize(st));
   for (int f = 0; f < n_fits; ++f) {
-    memcpy(fit_rows + (size_t)f * GBK_P, state_row.h + (size_t)f * GBK_P, sizeof(float) * GBK_P);
+    memcpy(fit_rows + (size_t)f * S, state_row.h + (size_t)f * S, sizeof(float) * S);
     fit_chi2[f] = (float)state_chi2.h[f];
     if (fit_iters) fit_iters[f] = iters.h[f];
     fs.iterations = std::max(fs.iterations, iters.h[f]);
@@ -721,12 +726,12 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
   if (!base_row || !best_row || !best_chi2) return fail(GBK_ERR_ARG, "null argument");
   if (n_live < 2 || batch < 1 || max_batches < 0 || !(enlarge >= 0.f) || !(tol > 0.f))
     return fail(GBK_ERR_ARG, "need n_live >= 2, batch >= 1, max_batches >= 0, enlarge >= 0, tol > 0");
-  DRV_TRY(check_box(n_free, free_param, lo, hi));
+  DRV_TRY(check_box(n_free, free_param, lo, hi, info.row_stride));
   if (gal < 0 || gal >= info.n_gal) return fail(GBK_ERR_ARG, "gal out of range");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(info.device);
   DRV_CUDA(guard.status);
-  const int n = n_free, cap = std::max(n_live, batch);
+  const int n = n_free, cap = std::max(n_live, batch), S = info.row_stride;
   std::lock_guard<std::mutex> ws_lock(g_ws_mu);
   Workspace* ws = workspace_for(info.device);
   if (!ws) return fail(GBK_ERR_ALLOC, "out of host memory");
@@ -734,7 +739,7 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
   Buf<float> rows, chi2;
   Buf<int> gidx;
   for (int pass = 0; pass < 2; ++pass) {
-    rows.alloc(ar, (size_t)cap * GBK_P);
+    rows.alloc(ar, (size_t)cap * S);
     chi2.alloc(ar, cap);
     gidx.alloc(ar, cap);
     if (pass == 0) DRV_CUDA(ar.commit());
@@ -745,7 +750,7 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
   gbk_fit_stats fs{};
 
   auto evaluate = [&](int k) -> int {   // rows.h[0..k) -> chi2.h[0..k)
-    DRV_CUDA(rows.to_device((size_t)k * GBK_P, st));
+    DRV_CUDA(rows.to_device((size_t)k * S, st));
     DRV_TRY(eval_rows(p, info, rows.d, gidx.d, k, chi2.d, nullptr, cuda_stream));
     DRV_CUDA(chi2.to_host(k, st));
     DRV_CUDA(cudaStreamSynchronize(st));
@@ -753,15 +758,15 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
     return GBK_OK;
   };
   auto draw = [&](float* row, const double* blo, const double* bhi) {
-    memcpy(row, base_row, sizeof(float) * GBK_P);
+    memcpy(row, base_row, sizeof(float) * S);
     for (int a = 0; a < n; ++a) row[free_param[a]] = (float)(blo[a] + (bhi[a] - blo[a]) * rng.uniform());
   };
 
   // live points from the whole prior box
   std::vector<double> plo(lo, lo + n), phi(hi, hi + n);
-  std::vector<float> live((size_t)n_live * GBK_P);
+  std::vector<float> live((size_t)n_live * S);
   std::vector<double> live_lnl(n_live);
-  for (int i = 0; i < n_live; ++i) draw(rows.h + (size_t)i * GBK_P, plo.data(), phi.data());
+  for (int i = 0; i < n_live; ++i) draw(rows.h + (size_t)i * S, plo.data(), phi.data());
   DRV_TRY(evaluate(n_live));
   memcpy(live.data(), rows.h, sizeof(float) * live.size());
   for (int i = 0; i < n_live; ++i) live_lnl[i] = isfinite(chi2.h[i]) ? -0.5 * (double)chi2.h[i] : -INFINITY;
@@ -781,26 +786,26 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
     for (int a = 0; a < n; ++a) {
       double mn = INFINITY, mx = -INFINITY;
       for (int i = 0; i < n_live; ++i) {
-        const double v = live[(size_t)i * GBK_P + free_param[a]];
+        const double v = live[(size_t)i * S + free_param[a]];
         mn = std::min(mn, v), mx = std::max(mx, v);
       }
       const double pad = 0.5 * enlarge * (mx - mn) + 1e-6 * (phi[a] - plo[a]);
       blo[a] = std::max(plo[a], mn - pad), bhi[a] = std::min(phi[a], mx + pad);
     }
-    double mu[GBK_P], Lc[GBK_P][GBK_P], scale = 0.0;
+    double mu[GBK_P_MAX], Lc[GBK_P_MAX][GBK_P_MAX], scale = 0.0;
     bool ellipsoid = n_live > 2 * n;
     if (ellipsoid) {
-      double cov[GBK_P][GBK_P] = {};
+      double cov[GBK_P_MAX][GBK_P_MAX] = {};
       for (int a = 0; a < n; ++a) {
         mu[a] = 0.0;
         for (int i = 0; i < n_live; ++i)
-          mu[a] += (live[(size_t)i * GBK_P + free_param[a]] - plo[a]) / (phi[a] - plo[a]);
+          mu[a] += (live[(size_t)i * S + free_param[a]] - plo[a]) / (phi[a] - plo[a]);
         mu[a] /= n_live;
       }
       for (int i = 0; i < n_live; ++i) {
-        double dlt[GBK_P];
+        double dlt[GBK_P_MAX];
         for (int a = 0; a < n; ++a)
-          dlt[a] = (live[(size_t)i * GBK_P + free_param[a]] - plo[a]) / (phi[a] - plo[a]) - mu[a];
+          dlt[a] = (live[(size_t)i * S + free_param[a]] - plo[a]) / (phi[a] - plo[a]) - mu[a];
         for (int a = 0; a < n; ++a)
           for (int c = 0; c <= a; ++c) cov[a][c] += dlt[a] * dlt[c] / (n_live - 1);
       }
@@ -820,9 +825,9 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
       }
       if (ellipsoid) {                                       // largest Mahalanobis distance of a live point
         for (int i = 0; i < n_live; ++i) {
-          double y[GBK_P], d2 = 0.0;
+          double y[GBK_P_MAX], d2 = 0.0;
           for (int a = 0; a < n; ++a) {
-            double t = (live[(size_t)i * GBK_P + free_param[a]] - plo[a]) / (phi[a] - plo[a]) - mu[a];
+            double t = (live[(size_t)i * S + free_param[a]] - plo[a]) / (phi[a] - plo[a]) - mu[a];
             for (int q = 0; q < a; ++q) t -= Lc[a][q] * y[q];
             y[a] = t / Lc[a][a];
             d2 += y[a] * y[a];
@@ -833,15 +838,15 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
       }
     }
     for (int i = 0; i < batch; ++i) {
-      float* row = rows.h + (size_t)i * GBK_P;
+      float* row = rows.h + (size_t)i * S;
       if (!ellipsoid) {
         draw(row, blo.data(), bhi.data());
         continue;
       }
-      memcpy(row, base_row, sizeof(float) * GBK_P);
+      memcpy(row, base_row, sizeof(float) * S);
       for (int attempt = 0;; ++attempt) {
         // uniform in the unit n-ball: Gaussian direction, radius U^(1/n)
-        double z[GBK_P], nrm = 0.0;
+        double z[GBK_P_MAX], nrm = 0.0;
         for (int a = 0; a < n; a += 2) {
           const double u1 = std::max(rng.uniform(), 1e-300), u2 = rng.uniform();
           const double rr = sqrt(-2.0 * log(u1));
@@ -877,10 +882,10 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
       const double x_prev = -(double)n_dead / n_live, x_now = -(double)(n_dead + 1) / n_live;
       const double lnw = x_prev + log1p(-exp(x_now - x_prev));
       dead_lnl.push_back(live_lnl[worst]), dead_lnw.push_back(lnw);
-      for (int a = 0; a < n; ++a) dead_x.push_back(live[(size_t)worst * GBK_P + free_param[a]]);
+      for (int a = 0; a < n; ++a) dead_x.push_back(live[(size_t)worst * S + free_param[a]]);
       lnz = log_add(lnz, live_lnl[worst] + lnw);
       ++n_dead;
-      memcpy(&live[(size_t)worst * GBK_P], rows.h + (size_t)i * GBK_P, sizeof(float) * GBK_P);
+      memcpy(&live[(size_t)worst * S], rows.h + (size_t)i * S, sizeof(float) * S);
       live_lnl[worst] = lnl;
       const double lmax = *std::max_element(live_lnl.begin(), live_lnl.end());
       if (lmax + x_now < lnz + log((double)tol)) done = true;   // what is left cannot change Z by > tol
@@ -890,16 +895,16 @@ extern "C" int gbk_fit_ns(gbk_problem* p, const float* base_row, int32_t gal, in
   const double ln_rest = -(double)n_dead / n_live - log((double)n_live);
   for (int i = 0; i < n_live; ++i) {
     dead_lnl.push_back(live_lnl[i]), dead_lnw.push_back(ln_rest);
-    for (int a = 0; a < n; ++a) dead_x.push_back(live[(size_t)i * GBK_P + free_param[a]]);
+    for (int a = 0; a < n; ++a) dead_x.push_back(live[(size_t)i * S + free_param[a]]);
     lnz = log_add(lnz, live_lnl[i] + ln_rest);
   }
   int best = 0;
   for (int j = 1; j < n_live; ++j)
     if (live_lnl[j] > live_lnl[best]) best = j;
-  memcpy(best_row, &live[(size_t)best * GBK_P], sizeof(float) * GBK_P);
+  memcpy(best_row, &live[(size_t)best * S], sizeof(float) * S);
   *best_chi2 = live_lnl[best] == -INFINITY ? INFINITY : (float)(-2.0 * live_lnl[best]);
   if (mean_row) {
-    memcpy(mean_row, base_row, sizeof(float) * GBK_P);
+    memcpy(mean_row, base_row, sizeof(float) * S);
     std::vector<double> acc(n, 0.0);
     for (size_t i = 0; i < dead_lnl.size(); ++i) {
       const double w = exp(dead_lnl[i] + dead_lnw[i] - lnz);

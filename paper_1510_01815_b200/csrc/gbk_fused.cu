@@ -82,19 +82,21 @@ __device__ __forceinline__ Smem carve(const DevProblem& dp, unsigned char* raw) 
 // ---------------------------------------------------------------------------------- a1 ------
 __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long k, RowConst* rc,
                               RowConstD* rd) {
-  const float* p = a.params + k * GBK_P;
-  float v[GBK_P];
+  const float* p = a.params + k * dp.row_stride;
+  float v[GBK_P_MAX];
   bool finite = true;
 #pragma unroll
-  for (int j = 0; j < GBK_P; ++j) {
-    v[j] = p[j];
+  for (int j = 0; j < GBK_P_MAX; ++j) {
+    v[j] = j < dp.row_stride ? p[j] : 1.0f;
     finite = finite && isfinite(v[j]);
   }
   float sp, cp, si, ci;
   sincospif(v[2] * (1.0f / 180.0f), &sp, &cp);
   sincospif(v[3] * (1.0f / 180.0f), &si, &ci);
   const float sigma0 = v[7], r0 = v[8], rt = v[6], i0 = v[9];
-  const bool ok = finite && sigma0 > 0.f && r0 > 0.f && rt > 0.f && i0 > 0.f && !(fabsf(ci) < 1e-6f);
+  const bool ok = finite && sigma0 > 0.f && r0 > 0.f && rt > 0.f && i0 > 0.f && !(fabsf(ci) < 1e-6f) &&
+                  (dp.rc_model != GBK_RC_EPINAT || (v[10] > 0.f && v[11] > 0.f));
+  rc->ea = v[10], rc->eg = v[11];
   int gal = a.gal_index ? a.gal_index[k] : 0;
   const bool gal_ok = gal >= 0 && gal < dp.n_gal;
   if (!gal_ok) gal = 0;
@@ -115,6 +117,7 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->inv_rt = 1.0f / rt;
   rc->rt = rt;
   rc->nl2e_inv_r0 = -1.4426950408889634f / r0;
+  rc->tab_scale = dp.tab_inv_dx / r0;
   rc->step = s * dp.dv;
   rc->m2step = -2.0f * rc->step;
   rc->mstep2 = -rc->step * rc->step;
@@ -134,7 +137,15 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   // further than kPreciseMargin outside the band shows only its far wing, where the voxel values need
   // d to ~1e-6: those rows take the FP64 geometry.  (A non-finite test value is a row that is out of
   // domain anyway.)
-  const float fsup = dp.rc_model == GBK_RC_ARCTAN ? 1.5707963267948966f : 1.0f;
+  float fsup = dp.rc_model == GBK_RC_ARCTAN ? 1.5707963267948966f : 1.0f;
+  if (dp.rc_model == GBK_RC_EPINAT && v[11] > v[10]) {
+    // q^g / (1 + q^a) <= max(1, q^(g - a)): bounded by the largest deprojected radius of the extended field
+    const float R = (float)dp.r_p_max * dp.inv_u + 1.0f;
+    const float ax = fmaxf(fabsf(v[0] + R), fabsf((float)dp.nx + R - v[0]));
+    const float ay = fmaxf(fabsf(v[1] + R), fabsf((float)dp.ny + R - v[1]));
+    const float qmax = sqrtf(ax * ax + ay * ay) * fabsf(inv_ci) / rt;
+    fsup = fmaxf(1.0f, powf(qmax, v[11] - v[10]));
+  }
   const float tmax = fabsf(rc->k1) * fsup * 1.0001f + 1e-3f;
   const float band = (float)(dp.nvx - 1) * rc->step;
   rc->precise = (rc->k0 + tmax > kPreciseMargin || rc->k0 - tmax < -(band + kPreciseMargin)) ? 1 : 0;
@@ -151,6 +162,8 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
     rd->ncp_ci = -dcp / dci, rd->nsp_ci = -dsp / dci;
     rd->inv_rt = 1.0 / (double)rt, rd->rt = rt;
     rd->k1 = -sd * (dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134 : 1.0) * (double)v[5] * dsi;
+    rd->ea = v[10], rd->eg = v[11];
+    rd->tab_scale = (double)dp.tab_inv_dx / (double)r0;
     const double vrel_first = (-(double)dp.r_v - 0.5 * (double)(dp.nv - 1)) * (double)dp.dv;
     rd->k0 = sd * (vrel_first - ((double)v[4] - (double)dp.v_center));
   }
@@ -578,6 +591,31 @@ __device__ __forceinline__ float separable_phase(const DevProblem& dp, const Eva
 // Geometry of one horizontally adjacent pixel pair (dx = x - x_o of both, dy = y - y_o shared):
 // returns the line-centre offsets d0 (in units of 1/s, from extended channel 0) and writes the
 // brightness I/I0 of both.
+// Tabulated radial profile at table position t = (r / r0) / mesh: linear interpolation between the
+// nodes, the last value beyond them.
+__device__ __forceinline__ float table_profile(const float* tab, int n, float t) {
+  const float tc = fminf(t, (float)(n - 1));
+  const int j = min((int)tc, n - 2);
+  const float lo = __ldg(tab + j), hi = __ldg(tab + j + 1);
+  return fmaf(tc - (float)j, hi - lo, lo);
+}
+
+__device__ __forceinline__ u64 table_profile2(const float* tab, int n, u64 t) {
+  float ta, tb;
+  upk(t, ta, tb);
+  return pk(table_profile(tab, n, ta), table_profile(tab, n, tb));
+}
+__device__ __forceinline__ u64 epinat_factor2(u64 q, float ea, float eg) {
+  float qa, qb, na, nb, da, db;
+  upk(q, qa, qb);
+  const u64 lq = pk(lg2_approx(qa), lg2_approx(qb));                 // q = 0: -inf -> q^g = q^a = 0
+  upk(mul2(lq, pk1(eg)), na, nb);
+  upk(mul2(lq, pk1(ea)), da, db);
+  return mul2(pk(ex2_approx(na), ex2_approx(nb)),
+              pk(rcp_approx(1.0f + ex2_approx(da)), rcp_approx(1.0f + ex2_approx(db))));
+}
+
+template <bool GENERAL>
 __device__ __forceinline__ u64 pair_geometry(const DevProblem& dp, const RowConst& rc, u64 dx,
                                              float dy, u64& brightness) {
   const u64 xe = fma2(pk1(rc.nsp), dx, pk1(dy * rc.cp));            // eq. 1
@@ -589,12 +627,18 @@ __device__ __forceinline__ u64 pair_geometry(const DevProblem& dp, const RowCons
   const u64 rs = pk(r2a > 1e-30f ? rsqrt_approx(r2a) : 0.0f, r2b > 1e-30f ? rsqrt_approx(r2b) : 0.0f);
   const u64 r = mul2(r2, rs);
   const u64 cos_t = mul2(xe, rs);                                    // eq. 4
-  float ea, eb;
-  upk(mul2(r, pk1(rc.nl2e_inv_r0)), ea, eb);
-  brightness = pk(ex2_approx(ea), ex2_approx(eb));                   // eq. 5 / I0
+  if (GENERAL && dp.tab_n > 0) {                                     // tabulated T(r / r0)
+    brightness = table_profile2(dp.tab, dp.tab_n, mul2(r, pk1(rc.tab_scale)));
+  } else {
+    float ea, eb;
+    upk(mul2(r, pk1(rc.nl2e_inv_r0)), ea, eb);
+    brightness = pk(ex2_approx(ea), ex2_approx(eb));                 // eq. 5 / I0
+  }
   const u64 q = mul2(r, pk1(rc.inv_rt));
   u64 f;
-  if (dp.rc_model == GBK_RC_ARCTAN) {                                // eq. 6 without (2/pi) V_t
+  if (GENERAL && dp.rc_model == GBK_RC_EPINAT) {                     // eq. 7 without V_t: q^g / (1 + q^a)
+    f = epinat_factor2(q, rc.ea, rc.eg);
+  } else if (dp.rc_model == GBK_RC_ARCTAN) {                         // eq. 6 without (2/pi) V_t
     float qa, qb, ia, ib;
     upk(q, qa, qb);
     upk(mul2(rs, pk1(rc.rt)), ia, ib);                               // 1/q = r_t / r
@@ -611,11 +655,24 @@ __device__ __forceinline__ u64 pair_geometry(const DevProblem& dp, const RowCons
   return fma2(mul2(f, pk1(rc.k1)), cos_t, pk1(rc.k0));               // eq. 8 -> line centre
 }
 
+// The less common models (Epinat curve, tabulated profile) take ONE out-of-line call per pixel pair, so
+// that they do not weigh on the register allocation of the headline path (arctan / ramp, exponential disc).
+struct PairGeom {
+  u64 d0, brightness;
+};
+__device__ __noinline__ PairGeom pair_geometry_general(const DevProblem& dp, const RowConst* rcp, u64 dx, float dy) {
+  const RowConst rc = *rcp;
+  PairGeom g;
+  g.d0 = pair_geometry<true>(dp, rc, dx, dy, g.brightness);
+  return g;
+}
+
 // Precise rows (RowConst::precise): eq. 1-4, 6 (or the ramp) and 8 of ONE fine sample in FP64.  Returns
 // the line-centre offset d0 as a float pair hi + lo and the brightness I/I0 (FP32 is enough for that).
-__device__ __noinline__ void sample_geometry_f64(int rc_model, const RowConstD* rdp, float nl2e_inv_r0,
+__device__ __noinline__ void sample_geometry_f64(const DevProblem& dp, const RowConstD* rdp, float nl2e_inv_r0,
                                                  double x, double y, float* hi, float* lo,
                                                  float* bright) {
+  const int rc_model = dp.rc_model;
   const RowConstD rd = *rdp;
   const double dx = x - rd.xo, dy = y - rd.yo;
   const double xe = rd.nsp * dx + rd.cp * dy;                       // eq. 1
@@ -626,9 +683,19 @@ __device__ __noinline__ void sample_geometry_f64(int rc_model, const RowConstD* 
     r = sqrt(r2);
     cos_t = xe / r;                                                 // eq. 4
   }
-  *bright = ex2_approx((float)r * nl2e_inv_r0);                     // eq. 5 / I0
+  if (dp.tab_n > 0) {                                               // tabulated T(r / r0)
+    const double tc = fmin(r * rd.tab_scale, (double)(dp.tab_n - 1));
+    const int j = min((int)tc, dp.tab_n - 2);
+    const double t0 = (double)__ldg(dp.tab + j), t1 = (double)__ldg(dp.tab + j + 1);
+    *bright = (float)(t0 + (tc - (double)j) * (t1 - t0));
+  } else {
+    *bright = ex2_approx((float)r * nl2e_inv_r0);                   // eq. 5 / I0
+  }
   const double q = r * rd.inv_rt;
-  const double f = rc_model == GBK_RC_ARCTAN ? atan(q) : fmin(q, 1.0);   // eq. 6 without (2/pi) V_t; ramp
+  double f;
+  if (rc_model == GBK_RC_ARCTAN) f = atan(q);                       // eq. 6 without (2/pi) V_t
+  else if (rc_model == GBK_RC_RAMP) f = fmin(q, 1.0);               // ramp (A7)
+  else f = q > 0.0 ? pow(q, rd.eg) / (1.0 + pow(q, rd.ea)) : 0.0;   // eq. 7 without V_t
   const double d0 = rd.k1 * f * cos_t + rd.k0;                      // eq. 8 -> line centre
   const float h = (float)d0;
   *hi = h;
@@ -757,6 +824,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
                                             int tx0, int ty0, int EW, int EH, int R, int tid,
                                             int nthreads, unsigned long long* counters) {
   const StripMap smap = strip_map(EW, EH);
+  const bool general = dp.rc_model == GBK_RC_EPINAT || dp.tab_n > 0;
   int n_poly = 0, n_direct = 0, n_items = 0;     // work counters of this warp (gbk_eval_batch_counted)
   const int npairs = smap.ppr * EH;
   const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
@@ -779,14 +847,19 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
         const double xa = ((double)(tx0 + ex - R) + 0.5) * inv_ud - 0.5;
         const double y = ((double)(ty0 + ey - R) + 0.5) * inv_ud - 0.5;
         float ha, la, ba, hb, lb, bb;
-        sample_geometry_f64(dp.rc_model, sm.rcd, rc.nl2e_inv_r0, xa, y, &ha, &la, &ba);
-        sample_geometry_f64(dp.rc_model, sm.rcd, rc.nl2e_inv_r0, xa + inv_ud, y, &hb, &lb, &bb);
+        sample_geometry_f64(dp, sm.rcd, rc.nl2e_inv_r0, xa, y, &ha, &la, &ba);
+        sample_geometry_f64(dp, sm.rcd, rc.nl2e_inv_r0, xa + inv_ud, y, &hb, &lb, &bb);
         v.d0[j] = pk(ha, hb), v.d0lo[j] = pk(la, lb), In[j] = pk(ba, bb);
       } else {
         const float gx = (float)(tx0 + ex - R), gy = (float)(ty0 + ey - R);
         const float xa = (gx + 0.5f) * inv_u - 0.5f, xb = (gx + 1.5f) * inv_u - 0.5f;
         const float y = (gy + 0.5f) * inv_u - 0.5f;
-        v.d0[j] = pair_geometry(dp, rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo, In[j]);
+        if (general) {
+          const PairGeom pg = pair_geometry_general(dp, sm.rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo);
+          v.d0[j] = pg.d0, In[j] = pg.brightness;
+        } else {
+          v.d0[j] = pair_geometry<false>(dp, rc, pk(xa - rc.xo, xb - rc.xo), y - rc.yo, In[j]);
+        }
         v.d0lo[j] = 0ull;
       }
       v.s0[j] = v.s1[j] = v.s2[j] = pk(0.f, 0.f);
@@ -871,7 +944,7 @@ __device__ __noinline__ void voxel_phase_precise(const DevProblem& dp, unsigned 
 }
 
 // ------------------------------------------------------------------------------ the kernel ---
-template <bool OUT>
+template <bool OUT, bool COUNT>
 __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     fused_kernel(const __grid_constant__ DevProblem dp, const __grid_constant__ EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -889,13 +962,13 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   {
     // Channel table, and the coefficients of the block polynomial of this row (voxel loop below):
     // C_m[c] = w_m[c] q^(j(j-1)/2), j = c mod 8, q = 2^(-2 step^2), stored as (C, C) pairs.
-    const float sigma0 = a.params[k * GBK_P + 7];
+    const float sigma0 = a.params[k * dp.row_stride + 7];
     const float s_ = 1.0f / (sigma0 * 1.1774100225154747f);
     const float step = s_ * dp.dv;
     const bool poly = step <= kPolyMaxStep;        // false for NaN: the row is out of domain anyway
     // the row's moment weights: the problem's w_q about v_center shifted to v_ref (RowConst::v_ref) in FP64,
     //   w1' = w1 - v_ref w0,   w2' = w2 - 2 v_ref w1 + v_ref^2 w0
-    const double vr = (double)fminf(fmaxf(a.params[k * GBK_P + 4] - dp.v_center, -dp.vhalf), dp.vhalf);
+    const double vr = (double)fminf(fmaxf(a.params[k * dp.row_stride + 4] - dp.v_center, -dp.vhalf), dp.vhalf);
     for (int c = tid; c < dp.nvx_pad; c += nthreads) {
       const double w0 = dp.chan_w[3 * c], w1 = dp.chan_w[3 * c + 1], w2 = dp.chan_w[3 * c + 2];
       const float4 w = make_float4((float)c, (float)w0, (float)(w1 - vr * w0),
@@ -946,9 +1019,9 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     const int R = rc.r_p;
     const int EW = tw + 2 * R, EH = th + 2 * R;
     if (rc.precise)
-      voxel_phase_precise(dp, smem_raw, tx0, ty0, EW, EH, R, tid, nthreads, a.counters);
+      voxel_phase_precise(dp, smem_raw, tx0, ty0, EW, EH, R, tid, nthreads, COUNT ? a.counters : nullptr);
     else
-      voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, a.counters);
+      voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, COUNT ? a.counters : nullptr);
     __syncthreads();
     // ------------------------------------------------------------------ a5 .. a9 ---------
     if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {
@@ -1021,15 +1094,17 @@ size_t fused_smem_bytes(const DevProblem& dp) {
 }
 
 cudaError_t fused_prepare(const FusedLaunch& fl) {
-  cudaError_t e = cudaFuncSetAttribute(fused_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  cudaError_t e = cudaFuncSetAttribute(fused_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        fl.smem_bytes);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(fused_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  e = cudaFuncSetAttribute(fused_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fl.smem_bytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(fused_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               fl.smem_bytes);
 }
 
 cudaError_t fused_occupancy(const FusedLaunch& fl, int* n) {
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(n, fused_kernel<false>, fl.threads,
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(n, fused_kernel<false, false>, fl.threads,
                                                        fl.smem_bytes);
 }
 
@@ -1037,9 +1112,11 @@ cudaError_t launch_fused(const DevProblem& dp, const EvalArgs& a, const FusedLau
                          cudaStream_t st) {
   const long long nblocks = a.K * dp.ntiles;
   if (a.m0 || a.m1 || a.m2 || a.resid)
-    fused_kernel<true><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
+    fused_kernel<true, false><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
+  else if (a.counters)
+    fused_kernel<false, true><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
   else
-    fused_kernel<false><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
+    fused_kernel<false, false><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
   return cudaGetLastError();
 }
 

@@ -20,6 +20,10 @@ constexpr float kPolyMaxStep = 0.8f;  // the block polynomial is used for step <
 struct DevProblem {
   int nx, ny, nv, u;        // spaxels, channels, up-sampling
   int n_gal;
+  int row_stride;           // floats per parameter row (GBK_P, or GBK_P_EPINAT)
+  int tab_n;                // > 0: tabulated radial profile I(r) = I0 T(r/r0) instead of eq. 5
+  float tab_inv_dx;         // 1 / mesh of the table (in units of r/r0)
+  const float* tab;         // [tab_n]
   int fw, fh;               // fine grid = u*nx, u*ny
   int r_v, nvx;             // LSF radius, nv + 2 r_v extended channels
   int nvx_pad;              // nvx rounded up to kChanBlock; the padding channels have zero weights
@@ -43,7 +47,7 @@ struct DevProblem {
 };
 
 struct EvalArgs {
-  const float* params;      // [K][GBK_P]
+  const float* params;      // [K][row_stride]
   const int32_t* gal_index; // [K] or null
   long long K;
   float* chi2;              // [K]
@@ -62,6 +66,8 @@ struct RowConst {
   float nsp_ci;       // -sin(PA) / cos(i)
   float inv_rt, rt;
   float nl2e_inv_r0;  // -log2(e)/r0
+  float tab_scale;    // 1 / (r0 * table mesh): position in the intensity table per pixel of radius
+  float ea, eg;       // Epinat slopes a, g (eq. 7)
   float step;         // s * dv with s = 1/(sigma0 sqrt(2 ln 2)): exp(-dv^2/(2 sigma0^2)) = 2^-(s dv)^2
   float m2step;       // -2 step
   float mstep2;       // -step^2
@@ -95,6 +101,8 @@ struct RowConstD {
   double nsp, cp, ncp_ci, nsp_ci;   // as in RowConst
   double inv_rt, rt;
   double k1, k0;                    // d0 = k1 * f(r/r_t) * cos(theta) + k0
+  double ea, eg;                    // Epinat slopes
+  double tab_scale;                 // 1 / (r0 * table mesh)
 };
 
 constexpr float kPreciseMargin = 2.5f;   // in units of the line offset d (1.18 sigma_0 each)

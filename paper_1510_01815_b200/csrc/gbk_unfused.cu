@@ -23,15 +23,17 @@ namespace gbk {
 namespace {
 
 struct URow {          // constants of one parameter row (a1)
-  float xo, yo, sp, cp, si, inv_ci, vsys, vt, inv_rt, inv_r0, i0, sigma0;
+  float xo, yo, sp, cp, si, inv_ci, vsys, vt, inv_rt, inv_r0, i0, sigma0, ea, eg;
   int gal, psf_set, r_p, valid;
 };
 
 __device__ URow uf_row(const DevProblem& dp, const float* params, const int32_t* gal_index, long long k) {
-  const float* p = params + k * GBK_P;
+  const float* p = params + k * dp.row_stride;
   URow r;
   bool finite = true;
-  for (int j = 0; j < GBK_P; ++j) finite = finite && isfinite(p[j]);
+  for (int j = 0; j < dp.row_stride; ++j) finite = finite && isfinite(p[j]);
+  r.ea = r.eg = 1.0f;
+  if (dp.rc_model == GBK_RC_EPINAT) r.ea = p[10], r.eg = p[11];
   sincospif(p[2] * (1.0f / 180.0f), &r.sp, &r.cp);
   float ci;
   sincospif(p[3] * (1.0f / 180.0f), &r.si, &ci);
@@ -43,7 +45,8 @@ __device__ URow uf_row(const DevProblem& dp, const float* params, const int32_t*
   r.gal = gal;
   r.psf_set = dp.psf_per_gal ? gal : 0;
   r.r_p = dp.psf_r[r.psf_set];
-  r.valid = finite && gal_ok && p[7] > 0.f && p[8] > 0.f && p[6] > 0.f && p[9] > 0.f && !(fabsf(ci) < 1e-6f);
+  r.valid = finite && gal_ok && p[7] > 0.f && p[8] > 0.f && p[6] > 0.f && p[9] > 0.f && !(fabsf(ci) < 1e-6f) &&
+            r.ea > 0.f && r.eg > 0.f;
   return r;
 }
 
@@ -95,10 +98,19 @@ __global__ void uf_cube_kernel(const __grid_constant__ DevProblem dp, const floa
     const float ye = (-x * r.cp - y * r.sp) * r.inv_ci;                     // eq. 2 / cos i
     const float rad = sqrtf(xe * xe + ye * ye);                             // eq. 3
     const float cos_t = rad > 0.0f ? xe / rad : 0.0f;                       // eq. 4, A8
-    const float bright = r.i0 * expf(-rad * r.inv_r0);                      // eq. 5
+    float bright;
+    if (dp.tab_n > 0) {                                                     // tabulated T(r / r0)
+      const float tc = fminf(rad * r.inv_r0 * dp.tab_inv_dx, (float)(dp.tab_n - 1));
+      const int j = min((int)tc, dp.tab_n - 2);
+      bright = r.i0 * (dp.tab[j] + (tc - (float)j) * (dp.tab[j + 1] - dp.tab[j]));
+    } else {
+      bright = r.i0 * expf(-rad * r.inv_r0);                                // eq. 5
+    }
     const float q = rad * r.inv_rt;
-    const float vrot = dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134f * r.vt * atanf(q)   // eq. 6
-                                                    : r.vt * fminf(q, 1.0f);                   // A7
+    float vrot;
+    if (dp.rc_model == GBK_RC_ARCTAN) vrot = 0.63661977236758134f * r.vt * atanf(q);            // eq. 6
+    else if (dp.rc_model == GBK_RC_RAMP) vrot = r.vt * fminf(q, 1.0f);                          // A7
+    else vrot = q > 0.0f ? r.vt * powf(q, r.eg) / (1.0f + powf(q, r.ea)) : 0.0f;                // eq. 7
     const float vlos = (r.vsys - dp.v_center) + vrot * r.si * cos_t;        // eq. 8, from v_center
     const float amp = bright * dp.dv / (r.sigma0 * 2.5066282746310002f) ; // A3
     const float inv_s = 1.0f / r.sigma0;

@@ -30,7 +30,7 @@ struct VRow {
 };
 
 __device__ void vf_row(const DevProblem& dp, const EvalArgs& a, long long k, VRow* r) {
-  const float* p = a.params + k * GBK_P;
+  const float* p = a.params + k * dp.row_stride;
   bool finite = true;
   float v[7];
 #pragma unroll
@@ -45,8 +45,8 @@ __device__ void vf_row(const DevProblem& dp, const EvalArgs& a, long long k, VRo
   const bool gal_ok = gal >= 0 && gal < dp.n_gal;
   r->gal = gal_ok ? gal : 0;
   r->valid = (finite && gal_ok && v[6] > 0.f && !(fabsf(ci) < 1e-6f)) ? 1 : 0;
-  if (dp.rc_model == GBK_RC_EPINAT) {       // slopes in the row slots eq. 8 does not use
-    const float ea = p[7], eg = p[8];
+  if (dp.rc_model == GBK_RC_EPINAT) {       // slopes a, g of eq. 7: slots 10, 11 of the 12-float row
+    const float ea = p[10], eg = p[11];
     if (!(isfinite(ea) && isfinite(eg) && ea > 0.f && eg > 0.f)) r->valid = 0;
     r->ea = pk1(ea), r->eg = pk1(eg);
   }

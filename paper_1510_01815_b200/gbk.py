@@ -16,6 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgbk.so")
 
 GBK_P = 10
+GBK_P_EPINAT = 12   # GBK_P + the Epinat slopes a, g (eq. 7)
+GBK_P_MAX = 12
 GBK_OK, GBK_ERR_ARG, GBK_ERR_ALLOC, GBK_ERR_CUDA, GBK_ERR_UNSUPPORTED = range(5)
 GBK_RC_ARCTAN, GBK_RC_RAMP, GBK_RC_EPINAT = 0, 1, 2
 GBK_STRATEGY_CUBE, GBK_STRATEGY_VFIELD = 0, 1
@@ -48,6 +50,7 @@ class gbk_problem_desc(C.Structure):
         ("lsf_sigma", C.c_float),
         ("tile_w", C.c_int32), ("tile_h", C.c_int32),
         ("device", C.c_int32),
+        ("intensity_table", C.c_void_p), ("intensity_n", C.c_int32), ("intensity_dx", C.c_float),
     ]
 
 
@@ -62,6 +65,7 @@ class gbk_problem_info(C.Structure):
         ("device", C.c_int32),
         ("strategy", C.c_int32),
         ("unfused_bytes_per_eval", C.c_int64),
+        ("row_stride", C.c_int32),
     ]
 
 
@@ -157,7 +161,8 @@ def _host_f32(a, shape=None):
 def gbk_create_problem(*, nx, ny, nv, u=1, v_center=0.0, dv, rc_model=GBK_RC_ARCTAN, n_gal=1,
                        vobs, verr, sobs=None, serr=None, mask=None,
                        psf_kind=GBK_PSF_GAUSSIAN, psf_fwhm=None, psf_image=None, psf_per_gal=False,
-                       lsf_sigma=0.0, tile_w=0, tile_h=0, device=-1) -> int:
+                       lsf_sigma=0.0, tile_w=0, tile_h=0, device=-1, intensity_table=None,
+                       intensity_dx=0.0) -> int:
     """Returns the opaque handle (an integer address).  Host arrays are copied by the library."""
     shape = (n_gal, ny, nx)
     keep = [_host_f32(vobs, shape), _host_f32(verr, shape), _host_f32(sobs, shape),
@@ -177,10 +182,12 @@ def gbk_create_problem(*, nx, ny, nv, u=1, v_center=0.0, dv, rc_model=GBK_RC_ARC
         psf_n = img.shape[-1]
         if img.size != n_psf * psf_n * psf_n:
             raise ValueError("psf_image has the wrong size")
+    tab = _host_f32(intensity_table)
     d = gbk_problem_desc(nx, ny, nv, u, v_center, dv, rc_model, n_gal,
                          _ptr(keep[0]), _ptr(keep[1]), _ptr(keep[2]), _ptr(keep[3]), _ptr(mk),
                          psf_kind, _ptr(fw), _ptr(img), psf_n, 1 if psf_per_gal else 0,
-                         lsf_sigma, tile_w, tile_h, device)
+                         lsf_sigma, tile_w, tile_h, device,
+                         _ptr(tab), 0 if tab is None else tab.size, intensity_dx)
     out = C.c_void_p()
     _check(lib().gbk_create_problem(C.byref(d), C.byref(out)))
     return out.value
@@ -261,11 +268,16 @@ def _box(params, lo, hi):
     return idx, lo, hi
 
 
+def _stride(handle) -> int:
+    return gbk_get_info(handle).row_stride
+
+
 def gbk_fit_ng(handle, base_row, gal, axis_param, axis_lo, axis_hi, nodes, levels, stream=0):
-    """Nested grids (host arrays in, host results out) -> (best_row [P], best_chi2, stats)."""
-    base = _host_f32(base_row, (GBK_P,))
+    """Nested grids (host arrays in, host results out) -> (best_row [row_stride], best_chi2, stats)."""
+    S = _stride(handle)
+    base = _host_f32(base_row, (S,))
     idx, lo, hi = _box(axis_param, axis_lo, axis_hi)
-    best = np.empty(GBK_P, np.float32)
+    best = np.empty(S, np.float32)
     chi = np.empty(1, np.float32)
     st = gbk_fit_stats()
     _check(lib().gbk_fit_ng(handle, _ptr(base), int(gal), idx.size, _ptr(idx), _ptr(lo), _ptr(hi),
@@ -277,13 +289,14 @@ def gbk_fit_ng(handle, base_row, gal, axis_param, axis_lo, axis_hi, nodes, level
 def gbk_fit_lm(handle, start_rows, gal, free_param, lo, hi, rel_step=1e-3, max_iter=50, ftol=1e-6,
                stream=0):
     """Levenberg-Marquardt for n_fits rows at once -> (fit_rows [n, P], chi2 [n], iters [n], stats)."""
-    start = np.ascontiguousarray(start_rows, dtype=np.float32).reshape(-1, GBK_P)
+    S = _stride(handle)
+    start = np.ascontiguousarray(start_rows, dtype=np.float32).reshape(-1, S)
     n = start.shape[0]
     g = None if gal is None else np.ascontiguousarray(gal, dtype=np.int32)
     if g is not None and g.size != n:
         raise ValueError("gal must have one entry per fit")
     idx, lo, hi = _box(free_param, lo, hi)
-    rows = np.empty((n, GBK_P), np.float32)
+    rows = np.empty((n, S), np.float32)
     chi = np.empty(n, np.float32)
     iters = np.empty(n, np.int32)
     st = gbk_fit_stats()
@@ -296,10 +309,11 @@ def gbk_fit_lm(handle, start_rows, gal, free_param, lo, hi, rel_step=1e-3, max_i
 def gbk_fit_ns(handle, base_row, gal, free_param, lo, hi, n_live=256, batch=256, max_batches=200,
                enlarge=0.2, tol=0.01, seed=1, stream=0):
     """Nested sampling -> dict(best_row, best_chi2, mean_row, log_evidence, stats)."""
-    base = _host_f32(base_row, (GBK_P,))
+    S = _stride(handle)
+    base = _host_f32(base_row, (S,))
     idx, lo, hi = _box(free_param, lo, hi)
-    best = np.empty(GBK_P, np.float32)
-    mean = np.empty(GBK_P, np.float32)
+    best = np.empty(S, np.float32)
+    mean = np.empty(S, np.float32)
     chi = np.empty(1, np.float32)
     lnz = C.c_double()
     st = gbk_fit_stats()
@@ -343,9 +357,10 @@ class Problem:
         self.info = gbk_get_info(self.handle)
 
     def eval_vfield(self, params, gal_index=None, want_maps=False, want_resid=False, stream=None):
-        """Velocity-field strategy: torch CUDA float32 [K, 10] -> dict(chi2[, vmap][, resid])."""
+        """Velocity-field strategy: torch CUDA float32 [K, row_stride] -> dict(chi2[, vmap][, resid])."""
         import torch
         assert params.is_cuda and params.dtype == torch.float32 and params.is_contiguous()
+        assert params.ndim == 2 and params.shape[1] == self.info.row_stride
         K = params.shape[0]
         i = self.info
         out = {"chi2": torch.empty(K, dtype=torch.float32, device=params.device)}
@@ -362,9 +377,10 @@ class Problem:
 
     def eval(self, params, gal_index=None, want_maps=False, want_resid=False, unfused=False,
              stream=None):
-        """params: torch CUDA float32 [K, 10] -> dict of torch tensors (chi2[, m0, m1, m2][, resid])."""
+        """params: torch CUDA float32 [K, row_stride] -> dict of torch tensors (chi2[, m0, m1, m2][, resid])."""
         import torch
         assert params.is_cuda and params.dtype == torch.float32 and params.is_contiguous()
+        assert params.ndim == 2 and params.shape[1] == self.info.row_stride
         K = params.shape[0]
         dev = params.device
         i = self.info

@@ -19,8 +19,9 @@ def f32(x) -> float:
     return float(np.float32(x))
 
 
-def oracle_grid(oracle, w: wl.Workload, fwhm=None):
-    """Oracle Grid for workload w (Gaussian PSF of `fwhm` data pixels, or w's Moffat image)."""
+def oracle_grid(oracle, w: wl.Workload, fwhm=None, tab=None, tab_dx=0.0):
+    """Oracle Grid for workload w (Gaussian PSF of `fwhm` data pixels, or w's Moffat image; `tab`:
+    a tabulated radial intensity profile, float32 values promoted like every other input)."""
     if w.psf_kind == wl.PSF_GAUSSIAN:
         psf = oracle.psf_gaussian_image(f32(w.psf_fwhm if fwhm is None else fwhm), w.u)
     else:
@@ -28,7 +29,9 @@ def oracle_grid(oracle, w: wl.Workload, fwhm=None):
         psf = img / img.sum()
     lsf = oracle.gaussian_taps(f32(w.lsf_sigma) / f32(w.dv) if w.lsf_sigma > 0 else 0.0)
     return oracle.Grid(nx=w.nx, ny=w.ny, nv=w.nv, u=w.u, v_center=f32(w.v_center), dv=f32(w.dv),
-                       rc_model=w.rc_model, psf=psf, lsf=lsf)
+                       rc_model=w.rc_model, psf=psf, lsf=lsf,
+                       tab=None if tab is None else np.asarray(tab, dtype=np.float32).astype(np.float64),
+                       tab_dx=f32(tab_dx))
 
 
 def gbk_desc(w: wl.Workload, obs: wl.Observed, fwhms=None, **extra):
@@ -46,9 +49,9 @@ def gbk_desc(w: wl.Workload, obs: wl.Observed, fwhms=None, **extra):
     return d
 
 
-def single_galaxy_case(oracle, w: wl.Workload, true_row, rng, fwhm=None):
+def single_galaxy_case(oracle, w: wl.Workload, true_row, rng, fwhm=None, tab=None, tab_dx=0.0):
     """Observation of one galaxy: oracle maps of `true_row` + seeded noise / errors / mask."""
-    g = oracle_grid(oracle, w, fwhm)
+    g = oracle_grid(oracle, w, fwhm, tab, tab_dx)
     m0, m1, m2 = oracle.model_maps(g, np.asarray(true_row, dtype=np.float32).astype(np.float64))
     obs = wl.observe(w, m0[None], m1[None], m2[None], rng)
     return g, obs

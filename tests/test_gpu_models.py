@@ -1,0 +1,145 @@
+"""SURVEY.md section 8(f) item 3 on the GPU: the Epinat rotation curve (eq. 7) inside
+the intensity-cube strategy, and a tabulated "user-specified" radial intensity profile (PAPER.md:106,
+reading A22) -- fused and unfused paths against the oracle, at config-1 and config-3 size, element by
+element at BASELINE.json's tolerances (parity_util.compare).
+"""
+import numpy as np
+import pytest
+
+from paper_1510_01815_b200 import workloads as wl
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu tests need a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gbk():
+    from paper_1510_01815_b200 import gbk as g
+    g.lib()
+    return g
+
+
+def _eval(torch, gbk, desc, rows, unfused=False, want_maps=True):
+    with gbk.Problem(**desc) as prob:
+        out = prob.eval(torch.from_numpy(np.ascontiguousarray(rows, dtype=np.float32)).cuda(),
+                        want_maps=want_maps, unfused=unfused)
+        torch.cuda.synchronize()
+        return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+def _epinat_rows(w, rng, K, true12):
+    rows = np.repeat(np.asarray(true12, dtype=np.float64)[None], K, axis=0)
+    b = wl.box(w)
+    width = np.concatenate([b[:, 1] - b[:, 0], [2.0, 2.0]])
+    rows[1:] += 0.1 * width * rng.uniform(-1, 1, (K - 1, 12))
+    rows[:, wl.IX_INC] = np.clip(rows[:, wl.IX_INC], 5.0, 85.0)
+    rows[:, wl.IX_RT] = np.clip(rows[:, wl.IX_RT], 0.5, None)
+    rows[:, 10:] = np.clip(rows[:, 10:], 0.3, 3.0)
+    return rows.astype(np.float32)
+
+
+@pytest.mark.parametrize("cfg,tile", [(1, (0, 0)), (1, (12, 10)), (3, (0, 0))])
+def test_cube_with_the_epinat_curve(oracle, torch_cuda, gbk, cfg, tile):
+    w = wl.config(cfg).scaled(rc_model=wl.RC_EPINAT)
+    rng = wl.rng_for(cfg, 31)
+    true = np.concatenate([wl.cfg1_true_row(rng)[0] if cfg == 1 else wl.draw_rows(w, rng, 1)[0], [1.4, 0.9]])
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = _epinat_rows(w, rng, 10 if cfg == 1 else 6, true)
+    rows[2, 10:] = (0.8, 1.6)           # g > a: the curve keeps rising
+    rows[3, 10:] = (1.0, 1.0)           # the paper's starting slopes
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    desc = pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1])
+    print("epinat cube", cfg, tile, pu.compare(ref, _eval(torch_cuda, gbk, desc, rows), rows, True,
+                                               f"epinat cube cfg{cfg} tile={tile}"))
+    if cfg == 1:
+        print("epinat cube unfused", pu.compare(ref, _eval(torch_cuda, gbk, desc, rows, unfused=True), rows,
+                                                True, "epinat cube unfused"))
+        bad = rows[:3].copy()
+        bad[1, 10] = 0.0
+        bad[2, 11] = np.nan
+        got = _eval(torch_cuda, gbk, desc, bad)
+        assert np.isfinite(got["chi2"][0]) and np.isposinf(got["chi2"][1:]).all()
+        assert np.isnan(got["m1"][1:]).all()
+
+
+def test_epinat_cube_full_launch_and_far_wing(oracle, torch_cuda, gbk):
+    """K = 4096 Epinat rows of config-3 shape in one launch (sampled against the oracle), plus rows whose
+    lines leave a short band (the FP64 geometry path with eq. 7)."""
+    torch = torch_cuda
+    w = wl.config(3).scaled(rc_model=wl.RC_EPINAT)
+    rng = wl.rng_for(3, 32)
+    true = np.concatenate([wl.draw_rows(w, rng, 1)[0], [1.2, 1.0]])
+    g, obs = pu.single_galaxy_case(oracle, w, true, rng)
+    rows = np.concatenate([wl.draw_rows(w, rng, 4096), rng.uniform(0.5, 2.5, (4096, 2)).astype(np.float32)], axis=1)
+    got = _eval(torch, gbk, pu.gbk_desc(w, obs), rows, want_maps=False)
+    pick = rng.choice(4096, size=24, replace=False)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows[pick])
+    print("epinat cfg3 full", pu.compare(ref, {"chi2": got["chi2"][pick]}, rows[pick], False, "epinat cfg3 full"))
+    ws = wl.config(1).scaled(rc_model=wl.RC_EPINAT, nx=18, ny=15, nv=20, dv=10.0, lsf_sigma=6.0, psf_fwhm=1.7)
+    trues = np.array([8.3, 7.1, 140.0, 50.0, 8.0, 180.0, 2.0, 12.0, 3.0, 1.5, 1.3, 0.9], dtype=np.float32)
+    gs, obss = pu.single_galaxy_case(oracle, ws, trues, rng)
+    far = []
+    for nsig in (0.0, 4.0, 8.0, 10.5):
+        for a_, g_ in ((1.3, 0.9), (0.7, 1.8)):
+            r = trues.copy()
+            r[wl.IX_VSYS] = 100.0 + nsig * 12.0
+            r[wl.IX_VT] = 280.0
+            r[10:] = (a_, g_)
+            far.append(r)
+    far = np.stack(far)
+    ref = oracle.eval_rows(gs, obss.vobs[0], obss.verr[0], obss.sobs[0], obss.serr[0], obss.mask[0], far,
+                           want_maps=True)
+    print("epinat far wing", pu.compare(ref, _eval(torch, gbk, pu.gbk_desc(ws, obss), far), far, True,
+                                        "epinat far wing"))
+
+
+def _tables(rng):
+    x = np.arange(0.0, 9.0, 0.05)
+    return [("sersic-like exp(-x^0.7)", np.exp(-x ** 0.7).astype(np.float32), 0.05),
+            ("ring", (np.exp(-0.5 * ((x - 1.5) / 0.6) ** 2) + 0.05 * np.exp(-x / 3)).astype(np.float32), 0.05),
+            ("coarse random", rng.uniform(0.2, 1.0, 7).astype(np.float32), 0.9)]
+
+
+@pytest.mark.parametrize("cfg,tile", [(1, (0, 0)), (1, (9, 16)), (3, (0, 0))])
+def test_cube_with_a_tabulated_intensity_profile(oracle, torch_cuda, gbk, cfg, tile):
+    w = wl.config(cfg)
+    rng = wl.rng_for(cfg, 33)
+    true = wl.cfg1_true_row(rng)[0] if cfg == 1 else wl.draw_rows(w, rng, 1)[0]
+    for name, tab, dx in _tables(rng):
+        g, obs = pu.single_galaxy_case(oracle, w, true, rng, tab=tab, tab_dx=dx)
+        rows = np.repeat(true[None].astype(np.float64), 8 if cfg == 1 else 5, axis=0)
+        b = wl.box(w)
+        rows[1:] += 0.1 * (b[:, 1] - b[:, 0]) * rng.uniform(-1, 1, (rows.shape[0] - 1, wl.P))
+        rows[:, wl.IX_R0] = true[wl.IX_R0] * rng.uniform(0.6, 1.6, rows.shape[0])     # the table's scale length
+        rows[:, wl.IX_INC] = np.clip(rows[:, wl.IX_INC], 5.0, 85.0)
+        rows[:, wl.IX_RT] = np.clip(rows[:, wl.IX_RT], 0.5, None)
+        rows = rows.astype(np.float32)
+        ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                               want_maps=True)
+        desc = pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1], intensity_table=tab, intensity_dx=dx)
+        print("table", name, cfg, tile, pu.compare(ref, _eval(torch_cuda, gbk, desc, rows), rows, True,
+                                                   f"table {name} cfg{cfg} tile={tile}"))
+        if cfg == 1 and tile == (0, 0):
+            print("table unfused", name, pu.compare(ref, _eval(torch_cuda, gbk, desc, rows, unfused=True),
+                                                    rows, True, f"table {name} unfused"))
+
+
+def test_create_rejects_bad_tables(oracle, torch_cuda, gbk):
+    w = wl.config(1)
+    rng = wl.rng_for(1, 34)
+    g, obs = pu.single_galaxy_case(oracle, w, wl.cfg1_true_row(rng)[0], rng)
+    for tab, dx in ((np.array([1.0], np.float32), 1.0), (np.array([1.0, np.nan], np.float32), 1.0),
+                    (np.array([1.0, -0.5], np.float32), 1.0), (np.array([1.0, 0.5], np.float32), 0.0)):
+        with pytest.raises(gbk.GbkError) as e:
+            gbk.Problem(**pu.gbk_desc(w, obs, intensity_table=tab, intensity_dx=dx))
+        assert e.value.code == gbk.GBK_ERR_ARG

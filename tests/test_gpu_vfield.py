@@ -147,29 +147,24 @@ def test_vfield_full_size_sampled_rows(oracle, torch_cuda, gbk):
 
 def test_vfield_epinat_curve(oracle, torch_cuda, gbk):
     """Eq. 7 with the velocity-field strategy, the GHASP model:
-    slopes a, g in row slots 7 and 8; the cube strategy refuses the model."""
+    rows of 12 floats, the slopes a, g in slots 10 and 11."""
     torch = torch_cuda
     w, g, obs, true, rng = _case(oracle, 3, nx=45, ny=38)
     w = w.scaled(rc_model=wl.RC_EPINAT)
     g = pu.oracle_grid(oracle, w)
     K = 64
-    rows = wl.draw_rows(w, rng, K)
-    rows[:, wl.IX_SIG] = rng.uniform(0.5, 2.5, K)      # a
-    rows[:, wl.IX_R0] = rng.uniform(0.5, 2.5, K)       # g
+    rows = np.concatenate([wl.draw_rows(w, rng, K), rng.uniform(0.5, 2.5, (K, 2)).astype(np.float32)], axis=1)
     rows[0, wl.IX_XO], rows[0, wl.IX_YO] = 20.0, 17.0   # r = 0 on a spaxel
-    rows[1, wl.IX_SIG] = 0.0                           # a <= 0: out of domain
-    rows[2, wl.IX_R0] = np.nan
-    rows[3, wl.IX_SIG:wl.IX_R0 + 1] = (1.0, 1.0)       # the paper's initial slopes (PAPER.md:154)
+    rows[1, 10] = 0.0                                  # a <= 0: out of domain
+    rows[2, 11] = np.nan
+    rows[3, 10:] = (1.0, 1.0)                          # the paper's initial slopes (PAPER.md:154)
+    rows[4, wl.IX_SIG] = np.nan                        # sigma_0 is not part of eq. 8: harmless here
     ref = oracle.vfield_rows(g, obs.vobs[0], obs.verr[0], obs.mask[0], rows, want_maps=True,
                              want_resid=True)
     assert np.isinf(ref["chi2"][[1, 2]]).all() and np.isfinite(np.delete(ref["chi2"], [1, 2])).all()
     with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        assert prob.info.row_stride == gbk.GBK_P_EPINAT == 12
         p = torch.from_numpy(rows).cuda()
         out = prob.eval_vfield(p, want_maps=True, want_resid=True)
         got = {k: v.cpu().numpy() for k, v in out.items()}
-        with pytest.raises(gbk.GbkError) as ei:
-            prob.eval(p)
-        assert ei.value.code == gbk.GBK_ERR_UNSUPPORTED
-        with pytest.raises(gbk.GbkError):
-            prob.eval(p, unfused=True)
     print("vfield epinat", _compare(ref, got, "vfield epinat"))
