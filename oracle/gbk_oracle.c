@@ -76,6 +76,8 @@ typedef struct {
   int32_t tab_n;
   const double *tab;
   double tab_dx;
+  int32_t extract;     /* 0: moments (the paper's choice); 1: Gaussian-profile fit of every spectrum  */
+                       /* ("fitting an analytic profile (e.g., Gaussian)"; reading A23)  */
 } gbko_grid;
 
 /* Parameters per row: 12 with the Epinat curve, else 10.                      */
@@ -320,6 +322,99 @@ void gbko_moments(const double *cube, int nv, size_t npix, const double *vel, do
   }
 }
 
+/* Step 5, the alternative the paper describes and times but does not adopt (PAPER.md:228-232,
+ * 493-507, 666-678): fit G(v) = A exp(-(v - mu)^2 / (2 s^2)) to every spectrum by unweighted least
+ * squares; velocity = mu, dispersion = s; m0 stays the plain sum (A4).  Reading A23 of DESIGN.md (the
+ * paper used MPFIT and gives no details): Levenberg-Marquardt on (A, mu, s),
+ *   start   mu = m1, s = max(m2, dv/2), A = m0 dv / (s sqrt(2 pi))   (from the moments)
+ *   step    (J^T J + lambda diag(J^T J)) delta = J^T r,  r_k = C_k - G(v_k), lambda_0 = 1e-3
+ *   accept  when the sum of squares decreases: lambda <- max(lambda/10, 1e-12); else lambda <- 10 lambda
+ *   stop    converged when an accepted step has |delta mu| and |delta s| < 1e-6 dv, or when the sum of
+ *           squares is already <= 1e-28 m0^2 (an exact fit); FAILED (NaN velocity and dispersion: "may
+ *           occasionally fail to converge") after 200 iterations, when lambda exceeds
+ *           1e12, when s leaves (0, 1e3 nv dv) or a value is not finite.
+ * A spectrum with m0 == 0 or non-finite moments gives NaN.                                        */
+void gbko_gaussfit(const double *cube, int nv, size_t npix, const double *vel, double *m0,
+                   double *mu_out, double *s_out) {
+  const double dv = nv > 1 ? vel[1] - vel[0] : 1.0;
+  for (size_t q = 0; q < npix; ++q) {
+    double s0 = 0.0, s1 = 0.0;
+    for (int k = 0; k < nv; ++k) {
+      const double c = cube[(size_t)k * npix + q];
+      s0 += c;
+      s1 += c * vel[k];
+    }
+    const double mean = s1 / s0;
+    double s2 = 0.0;
+    for (int k = 0; k < nv; ++k) {
+      const double d = vel[k] - mean;
+      s2 += cube[(size_t)k * npix + q] * d * d;
+    }
+    m0[q] = s0;
+    mu_out[q] = s_out[q] = NAN;
+    const double var = s2 / s0;
+    if (!(s0 > 0.0) || !isfinite(mean) || !isfinite(var)) continue;
+    double mu = mean, sg = fmax(sqrt(fmax(var, 0.0)), 0.5 * dv);
+    double A = s0 * dv / (sg * sqrt(2.0 * GBKO_PI));
+    double lambda = 1e-3;
+    int done = 0;
+    for (int it = 0; it < 200 && !done; ++it) {
+      /* normal equations at (A, mu, sg) */
+      double JJ[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, Jr[3] = {0, 0, 0}, sse = 0.0;
+      for (int k = 0; k < nv; ++k) {
+        const double d = vel[k] - mu;
+        const double e = exp(-0.5 * d * d / (sg * sg));
+        const double r = cube[(size_t)k * npix + q] - A * e;
+        const double J[3] = {e, A * e * d / (sg * sg), A * e * d * d / (sg * sg * sg)};
+        for (int a = 0; a < 3; ++a) {
+          Jr[a] += J[a] * r;
+          for (int b = 0; b < 3; ++b) JJ[a][b] += J[a] * J[b];
+        }
+        sse += r * r;
+      }
+      if (sse <= 1e-28 * s0 * s0) {
+        done = 1;
+        break;
+      }
+      /* damped solve by Cramer's rule (3 x 3) */
+      double M[3][3];
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) M[a][b] = JJ[a][b] * (a == b ? 1.0 + lambda : 1.0);
+      const double det = M[0][0] * (M[1][1] * M[2][2] - M[1][2] * M[2][1]) -
+                         M[0][1] * (M[1][0] * M[2][2] - M[1][2] * M[2][0]) +
+                         M[0][2] * (M[1][0] * M[2][1] - M[1][1] * M[2][0]);
+      double dl[3];
+      for (int c = 0; c < 3; ++c) {
+        double N[3][3];
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b) N[a][b] = b == c ? Jr[a] : M[a][b];
+        dl[c] = (N[0][0] * (N[1][1] * N[2][2] - N[1][2] * N[2][1]) -
+                 N[0][1] * (N[1][0] * N[2][2] - N[1][2] * N[2][0]) +
+                 N[0][2] * (N[1][0] * N[2][1] - N[1][1] * N[2][0])) / det;
+      }
+      const double A1 = A + dl[0], mu1 = mu + dl[1], sg1 = sg + dl[2];
+      double sse1 = INFINITY;
+      if (isfinite(A1) && isfinite(mu1) && sg1 > 0.0 && sg1 < 1e3 * nv * dv) {
+        sse1 = 0.0;
+        for (int k = 0; k < nv; ++k) {
+          const double d = vel[k] - mu1;
+          const double r = cube[(size_t)k * npix + q] - A1 * exp(-0.5 * d * d / (sg1 * sg1));
+          sse1 += r * r;
+        }
+      }
+      if (sse1 < sse) {
+        A = A1, mu = mu1, sg = sg1;
+        lambda = fmax(lambda / 10.0, 1e-12);
+        if (fabs(dl[1]) < 1e-6 * dv && fabs(dl[2]) < 1e-6 * dv) done = 1;
+      } else {
+        lambda *= 10.0;
+        if (!(lambda <= 1e12)) break;
+      }
+    }
+    if (done) mu_out[q] = mu, s_out[q] = sg;
+  }
+}
+
 /* Step 6 (eq. 11; masks PAPER.md:185): W is pre-folded
  * into serr by the caller; sobs == NULL drops the dispersion term.
  * Optional resid[2][npix] receives the weighted residuals (0 where masked,
@@ -377,7 +472,10 @@ int gbko_model_maps(const gbko_grid *g, const double *p, double *m0, double *m1,
     gbko_conv_psf(c_lsf, g->nv, eh, ew, g->psf, g->psf_n, c_psf);    /* 3 */
     gbko_downsample(c_psf, g->nv, g->ny, g->nx, g->u, c_ds);         /* 4 */
     for (int k = 0; k < g->nv; ++k) vel[k] = gbko_channel_velocity(g, k);
-    gbko_moments(c_ds, g->nv, npix, vel, m0, m1, m2);                /* 5 */
+    if (g->extract == 1)
+      gbko_gaussfit(c_ds, g->nv, npix, vel, m0, m1, m2);             /* 5, Gaussian-fit variant */
+    else
+      gbko_moments(c_ds, g->nv, npix, vel, m0, m1, m2);              /* 5 */
     rc = 0;
   }
   free(cube);

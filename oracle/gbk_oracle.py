@@ -48,6 +48,7 @@ class _Grid(C.Structure):
         ("lsf_n", C.c_int32), ("lsf", C.POINTER(C.c_double)),
         ("halo_zero", C.c_int32),
         ("tab_n", C.c_int32), ("tab", C.POINTER(C.c_double)), ("tab_dx", C.c_double),
+        ("extract", C.c_int32),
     ]
 
 
@@ -90,6 +91,8 @@ def lib():
         L.gbko_downsample.restype = None
         L.gbko_moments.argtypes = [dp, C.c_int, C.c_size_t, dp, dp, dp, dp]
         L.gbko_moments.restype = None
+        L.gbko_gaussfit.argtypes = [dp, C.c_int, C.c_size_t, dp, dp, dp, dp]
+        L.gbko_gaussfit.restype = None
         L.gbko_chi2.argtypes = [dp, dp, dp, fp, fp, fp, fp, u8p, C.c_size_t, C.c_double, dp]
         L.gbko_chi2.restype = C.c_double
         L.gbko_model_maps.argtypes = [gp, dp, dp, dp, dp]
@@ -171,6 +174,7 @@ class Grid:
     halo_zero: bool = False
     tab: np.ndarray | None = None      # tabulated radial profile T(x_j), x_j = j * tab_dx
     tab_dx: float = 0.0
+    extract: int = 0                   # 0: moments; 1: Gaussian-profile fit of every spectrum
 
     def c(self) -> _Grid:
         self._psf = _c64(self.psf)
@@ -182,7 +186,8 @@ class Grid:
         return _Grid(self.nx, self.ny, self.nv, self.u, self.v_center, self.dv, self.rc_model,
                      self._psf.shape[0], _dp(self._psf), self._lsf.size, _dp(self._lsf),
                      1 if self.halo_zero else 0,
-                     0 if self._tab is None else self._tab.size, _dp(self._tab), float(self.tab_dx))
+                     0 if self._tab is None else self._tab.size, _dp(self._tab), float(self.tab_dx),
+                     int(self.extract))
 
     @property
     def P(self) -> int:
@@ -271,6 +276,17 @@ def moments(cube: np.ndarray, vel: np.ndarray):
     m0, m1, m2 = (np.empty(shp, dtype=np.float64) for _ in range(3))
     lib().gbko_moments(_dp(cube), nv, npix, _dp(vel), _dp(m0), _dp(m1), _dp(m2))
     return m0, m1, m2
+
+
+def gaussfit(cube: np.ndarray, vel: np.ndarray):
+    """Gaussian-profile fit of every spectrum -> (m0, mu, sigma); NaN where the fit fails."""
+    cube, vel = _c64(cube), _c64(vel)
+    nv = cube.shape[0]
+    shp = cube.shape[1:]
+    npix = int(np.prod(shp))
+    m0, mu, sg = (np.empty(shp, dtype=np.float64) for _ in range(3))
+    lib().gbko_gaussfit(_dp(cube), nv, npix, _dp(vel), _dp(m0), _dp(mu), _dp(sg))
+    return m0, mu, sg
 
 
 def chi2(m0, m1, m2, vobs, verr, sobs=None, serr=None, mask=None, dark_level=0.0,

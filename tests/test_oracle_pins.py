@@ -630,3 +630,73 @@ def test_cube_with_a_tabulated_intensity_profile(oracle):
     assert m0[8, 6] == pytest.approx(1.5 * 0.75, rel=1e-8)
     assert m0[5, 8] == pytest.approx(1.5 * (1.0 - (4.0 / 3.0) / 4.0), rel=1e-8)
     assert m0[5, 6] == pytest.approx(1.5, rel=1e-8)                      # the centre: r = 0
+
+
+# ---------------- Gaussian-profile extraction ----
+
+def _gauss(v, A, mu, s):
+    return A * np.exp(-0.5 * ((v - mu) / s) ** 2)
+
+
+def test_gaussfit_recovers_an_exact_sampled_gaussian(oracle):
+    """A spectrum that IS a sampled Gaussian is fitted exactly, whether the centre sits on a channel,
+    between channels, or close to the band edge with a third of the line cut off (where the moments
+    are biased: the reason the paper gives for the method's "superior accuracy")."""
+    v = (np.arange(48) - 23.5) * 12.0
+    cases = [(3.0, 6.0, 30.0), (0.7, -41.3, 17.0), (5.0, 100.0, 55.0), (1.0, 250.0, 40.0), (2.0, -275.0, 25.0)]
+    cube = np.stack([_gauss(v, *c) for c in cases], axis=1)[:, None, :]      # [nv, 1, ncase]
+    m0, mu, sg = oracle.gaussfit(cube, v)
+    mm0, m1, m2 = oracle.moments(cube, v)
+    for i, (A, mu_t, s_t) in enumerate(cases):
+        assert mu[0, i] == pytest.approx(mu_t, abs=1e-6) and sg[0, i] == pytest.approx(s_t, abs=1e-6), i
+        assert m0[0, i] == pytest.approx(mm0[0, i], rel=1e-14)              # flux stays the plain sum
+    assert abs(m1[0, 3] - 250.0) > 5.0 and abs(m1[0, 4] + 275.0) > 5.0       # the truncated lines bias the moments
+    assert abs(m1[0, 0] - 6.0) < 1e-6 and abs(m2[0, 0] - 30.0) < 1e-3        # ... not the complete ones
+
+
+def test_gaussfit_minimises_the_sum_of_squares_and_matches_scipy(oracle):
+    """For a spectrum that is NOT a Gaussian (two components, a skewed line) the result is the
+    least-squares Gaussian: the gradient of the sum of squares vanishes there (central differences
+    taken here), and scipy.optimize.least_squares from the same start lands on the same point."""
+    from scipy.optimize import least_squares
+    v = (np.arange(64) - 31.5) * 10.0
+    specs = [_gauss(v, 2.0, -30.0, 25.0) + _gauss(v, 1.2, 40.0, 35.0),
+             _gauss(v, 1.0, 10.0, 20.0) * (1.0 + 0.4 * np.tanh((v - 10.0) / 30.0)),
+             _gauss(v, 3.0, 0.0, 12.0) + 0.02]
+    cube = np.stack(specs, axis=1)[:, None, :]
+    m0, mu, sg = oracle.gaussfit(cube, v)
+    _, m1, m2 = oracle.moments(cube, v)
+    for i, c in enumerate(specs):
+        sse = lambda p: float(np.sum((c - _gauss(v, *p)) ** 2))
+        start = [c.sum() * 10.0 / (max(m2[0, i], 5.0) * np.sqrt(2 * np.pi)), m1[0, i], max(m2[0, i], 5.0)]
+        sol = least_squares(lambda p: c - _gauss(v, *p), start, xtol=1e-14, ftol=1e-14, gtol=1e-14).x
+        assert mu[0, i] == pytest.approx(sol[1], abs=1e-4) and sg[0, i] == pytest.approx(abs(sol[2]), abs=1e-4), i
+        A = np.sum(c * _gauss(v, 1.0, mu[0, i], sg[0, i])) / np.sum(_gauss(v, 1.0, mu[0, i], sg[0, i]) ** 2)
+        p0 = np.array([A, mu[0, i], sg[0, i]])
+        for j, h in ((1, 1e-3), (2, 1e-3)):
+            e = np.zeros(3)
+            e[j] = h
+            grad = (sse(p0 + e) - sse(p0 - e)) / (2 * h)
+            assert abs(grad) < 1e-6 * sse(p0) + 1e-9, (i, j, grad)
+
+
+def test_gaussfit_in_the_pipeline_and_failures(oracle):
+    """extract = 1 in the whole pipeline: with delta kernels and a line well inside the band the fitted
+    velocity is eq. 8 and the fitted dispersion sigma_0 (the spectrum is an exact Gaussian), as with the
+    moments; a dark spectrum (m0 = 0) gives NaN."""
+    kw = dict(nx=9, ny=8, nv=96, u=1, v_center=0.0, dv=12.0, rc_model=0, psf=np.ones((1, 1)), lsf=np.ones(1))
+    p = np.array([4.0, 3.5, 25.0, 50.0, 5.0, 150.0, 2.0, 35.0, 3.0, 1.5])
+    m0a, m1a, m2a = oracle.model_maps(oracle.Grid(**kw), p)
+    m0b, m1b, m2b = oracle.model_maps(oracle.Grid(**kw, extract=1), p)
+    assert np.array_equal(m0a, m0b)
+    assert np.max(np.abs(m1a - m1b)) < 1e-6 and np.max(np.abs(m2b - 35.0)) < 1e-6
+    z = np.zeros((8, 1, 2))
+    m0, mu, sg = oracle.gaussfit(z, np.arange(8.0))
+    assert np.isnan(mu).all() and np.isnan(sg).all() and (m0 == 0).all()
+    # beam smearing: with a wide PSF the two extractions differ near the centre (PAPER.md:672, Fig. 14)
+    psf = oracle.psf_gaussian_image(4.0, 1)
+    g1 = oracle.Grid(**{**kw, "psf": psf})
+    g2 = oracle.Grid(**{**kw, "psf": psf}, extract=1)
+    _, v1, s1 = oracle.model_maps(g1, p)
+    _, v2, s2 = oracle.model_maps(g2, p)
+    assert 0.05 < np.nanmax(np.abs(s1 - s2)) < 20.0
