@@ -130,6 +130,7 @@ typedef struct {
   int64_t unfused_bytes_per_eval; /* algorithmic HBM bytes of gbk_eval_batch_unfused per row:   */
                           /* every intermediate array written once and read once per consumer */
   int32_t row_stride;     /* floats per parameter row: GBK_P, or GBK_P_EPINAT                  */
+  int32_t extraction;     /* GBK_EXTRACT_* (gbk_set_extraction)                                 */
 } gbk_problem_info;
 
 /*
@@ -153,6 +154,20 @@ int gbk_get_info(const gbk_problem *p, gbk_problem_info *info);
  */
 enum { GBK_STRATEGY_CUBE = 0, GBK_STRATEGY_VFIELD = 1 };
 int gbk_set_strategy(gbk_problem *p, int32_t strategy);
+
+/*
+ * How the cube strategy extracts the velocity and dispersion maps from the down-sampled cube
+ * (PAPER.md:228): GBK_EXTRACT_MOMENTS, the first and second moments of every spectrum (the paper's
+ * choice, and the default), or GBK_EXTRACT_GAUSSFIT, a Gaussian profile fitted to every
+ * spectrum (the paper tried it, and compares the two in section
+ * 6.2): unweighted least squares for (A, mu, sigma) by Levenberg-Marquardt started
+ * from the moments, velocity = mu, dispersion = sigma, m0 = the plain sum; a fit that does not
+ * converge gives NaN there and chi2 = +INF if the spaxel is unmasked.  The fit needs the whole
+ * convolved spectrum of every spaxel, which the fused kernel never forms: with GBK_EXTRACT_GAUSSFIT
+ * gbk_eval_batch (and the drivers) run the multi-kernel pipeline of gbk_eval_batch_unfused.
+ */
+enum { GBK_EXTRACT_MOMENTS = 0, GBK_EXTRACT_GAUSSFIT = 1 };
+int gbk_set_extraction(gbk_problem *p, int32_t extraction);
 
 /*
  * The hot path (PAPER.md:63-66 steps 1-3 for K rows), fused: the model cube is

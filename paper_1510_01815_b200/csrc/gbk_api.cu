@@ -70,6 +70,7 @@ struct gbk_problem {
   std::vector<Level> levels;
   int device = 0;
   int strategy = GBK_STRATEGY_CUBE;
+  int extraction = GBK_EXTRACT_MOMENTS;
   int sm_count = 0, blocks_per_sm = 0;
   long long ext_voxels = 0;
   // device allocations owned by the problem
@@ -403,6 +404,7 @@ extern "C" int gbk_get_info(const gbk_problem* p, gbk_problem_info* info) {
   info->strategy = p->strategy;
   info->unfused_bytes_per_eval = (int64_t)unfused_algorithmic_bytes_per_row(p->dp);
   info->row_stride = dp.row_stride;
+  info->extraction = p->extraction;
   return GBK_OK;
 }
 
@@ -412,6 +414,15 @@ extern "C" int gbk_set_strategy(gbk_problem* p, int32_t strategy) {
   if (strategy != GBK_STRATEGY_CUBE && strategy != GBK_STRATEGY_VFIELD)
     return fail(GBK_ERR_ARG, "unknown strategy %d", strategy);
   p->strategy = strategy;
+  return GBK_OK;
+}
+
+extern "C" int gbk_set_extraction(gbk_problem* p, int32_t extraction) {
+  g_err[0] = 0;
+  if (!p) return fail(GBK_ERR_ARG, "null problem");
+  if (extraction != GBK_EXTRACT_MOMENTS && extraction != GBK_EXTRACT_GAUSSFIT)
+    return fail(GBK_ERR_ARG, "unknown extraction %d", extraction);
+  p->extraction = extraction;
   return GBK_OK;
 }
 
@@ -516,12 +527,19 @@ extern "C" int gbk_eval_batch_counted(gbk_problem* p, const float* params, const
                          reinterpret_cast<unsigned long long*>(counters), cuda_stream);
 }
 
+static int eval_unfused_impl(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
+                             float* chi2, float* m0, float* m1, float* m2, float* resid, void* cuda_stream);
+
 static int eval_batch_impl(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
                            float* chi2, float* m0, float* m1, float* m2, float* resid,
                            unsigned long long* counters, void* cuda_stream) {
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
   if (K == 0) return GBK_OK;
+  if (p->extraction == GBK_EXTRACT_GAUSSFIT) {   // needs whole spectra: the multi-kernel pipeline
+    if (counters) return fail(GBK_ERR_UNSUPPORTED, "work counters belong to the fused kernel (moment extraction)");
+    return eval_unfused_impl(p, params, gal_index, K, chi2, m0, m1, m2, resid, cuda_stream);
+  }
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(p->device);
   GBK_CUDA(guard.status);
@@ -588,6 +606,11 @@ extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const
   g_err[0] = 0;
   if (int rc = check_eval_args(p, params, K, chi2)) return rc;
   if (K == 0) return GBK_OK;
+  return eval_unfused_impl(p, params, gal_index, K, chi2, m0, m1, m2, resid, cuda_stream);
+}
+
+static int eval_unfused_impl(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
+                             float* chi2, float* m0, float* m1, float* m2, float* resid, void* cuda_stream) {
   DeviceGuard guard(p->device);
   GBK_CUDA(guard.status);
   // scratch: two cubes + one contribution map per row, for a chunk of rows (<= 2 GiB, grown lazily)
@@ -601,7 +624,7 @@ extern "C" int gbk_eval_batch_unfused(gbk_problem* p, const float* params, const
     p->uf_rows = want;
   }
   EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, nullptr, nullptr, nullptr};
-  GBK_CUDA(launch_unfused(p->dp, a, p->lsf_taps, p->uf_scratch, p->uf_rows, p->sm_count,
+  GBK_CUDA(launch_unfused(p->dp, a, p->lsf_taps, p->uf_scratch, p->uf_rows, p->sm_count, p->extraction,
                           (cudaStream_t)cuda_stream));
   return GBK_OK;
 }

@@ -122,7 +122,7 @@ size_t fused_smem_bytes(const DevProblem& dp);
 size_t unfused_bytes_per_row(const DevProblem& dp);
 double unfused_algorithmic_bytes_per_row(const DevProblem& dp);
 cudaError_t launch_unfused(const DevProblem& dp, const EvalArgs& a, const float* lsf_taps, float* scratch,
-                           long long chunk_rows, int sm_count, cudaStream_t st);
+                           long long chunk_rows, int sm_count, int extraction, cudaStream_t st);
 
 // velocity-field strategy (gbk_vfield.cu): EvalArgs.m1 = velocity maps, EvalArgs.resid = [K][ny][nx]
 cudaError_t launch_vfield(const DevProblem& dp, const EvalArgs& a, cudaStream_t st);

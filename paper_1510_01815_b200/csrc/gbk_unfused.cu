@@ -16,6 +16,7 @@
 
 #include <algorithm>
 
+#include "gbk_device.cuh"
 #include "gbk_internal.h"
 
 namespace gbk {
@@ -50,16 +51,12 @@ __device__ URow uf_row(const DevProblem& dp, const float* params, const int32_t*
   return r;
 }
 
-// Which PSF set a row uses (the convolution kernels need nothing else of the row).
-__device__ __forceinline__ URow uf_row_psf(const DevProblem& dp, const int32_t* gal_index, long long k) {
-  URow r;
-  int gal = gal_index ? gal_index[k] : 0;
-  if (gal < 0 || gal >= dp.n_gal) gal = 0;
-  r.gal = gal;
-  r.psf_set = dp.psf_per_gal ? gal : 0;
-  r.r_p = dp.psf_r[r.psf_set];
-  r.valid = 1;
-  return r;
+// a1 once per row of the chunk (the step kernels read the constants instead of re-deriving them)
+__global__ void uf_rows_kernel(const __grid_constant__ DevProblem dp, const float* __restrict__ params,
+                               const int32_t* __restrict__ gal_index, long long k0, int nrows,
+                               URow* __restrict__ rows) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < nrows) rows[i] = uf_row(dp, params, gal_index, k0 + i);
 }
 
 struct UGeom {         // extended grid of the unfused path
@@ -76,8 +73,7 @@ __host__ __device__ inline UGeom uf_geom(const DevProblem& dp) {
 
 // Step 1: one thread per extended spatial sample evaluates its whole spectrum;
 // consecutive threads <-> consecutive x, so every channel slice is written coalesced.
-__global__ void uf_cube_kernel(const __grid_constant__ DevProblem dp, const float* __restrict__ params,
-                               const int32_t* __restrict__ gal_index, long long k0, int nrows,
+__global__ void uf_cube_kernel(const __grid_constant__ DevProblem dp, const URow* __restrict__ rows, int nrows,
                                float* __restrict__ cube) {
   const UGeom g = uf_geom(dp);
   const long long n = (long long)nrows * g.plane;
@@ -86,7 +82,7 @@ __global__ void uf_cube_kernel(const __grid_constant__ DevProblem dp, const floa
     const int row = (int)(idx / g.plane);
     const int pix = (int)(idx - row * (long long)g.plane);
     const int ey = pix / g.EW, ex = pix - ey * g.EW;
-    const URow r = uf_row(dp, params, gal_index, k0 + row);
+    const URow r = rows[row];
     float* out = cube + (size_t)row * g.cube + pix;
     if (!r.valid) {
       for (int c = 0; c < g.nvx; ++c) out[(size_t)c * g.plane] = 0.0f;
@@ -121,87 +117,205 @@ __global__ void uf_cube_kernel(const __grid_constant__ DevProblem dp, const floa
   }
 }
 
-// Step 2a: LSF along v (direct sum, "valid": nvx -> nv channels).  lsf[j], j = 0..2 r_v.
-__global__ void uf_lsf_kernel(const __grid_constant__ DevProblem dp, const float* __restrict__ lsf,
-                              int nrows, const float* __restrict__ in, float* __restrict__ out) {
+// Step 2a: LSF along v (direct sum, "valid": nvx -> nv channels), lsf[j], j = 0..2 r_v.  A block
+// takes 32 consecutive pixels of one row's plane and walks the channels in pieces of kLsfPiece: the
+// slab [piece + 2 r_v][32] goes through shared memory, so every input value is read from device
+// memory once (128-byte coalesced lines) however many taps use it.
+constexpr int kLsfPiece = 64, kLsfPix = 64;       // channels per piece, pixels per block pass (2 per lane)
+__global__ void __launch_bounds__(256) uf_lsf_kernel(const __grid_constant__ DevProblem dp,
+                                                     const float* __restrict__ lsf, int nrows,
+                                                     const float* __restrict__ in, float* __restrict__ out) {
+  extern __shared__ float slab[];                 // [kLsfPiece + 2 r_v][kLsfPix]
+  __shared__ float taps[2 * kMaxLsfR + 1];
   const UGeom g = uf_geom(dp);
-  const size_t per_row = g.plane * dp.nv;
-  const long long n = (long long)nrows * per_row;
-  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
-       idx += (long long)gridDim.x * blockDim.x) {
-    const int row = (int)(idx / per_row);
-    const size_t rem = idx - row * (long long)per_row;
-    const int c = (int)(rem / g.plane);
-    const size_t pix = rem - c * g.plane;
+  const int ntap = 2 * dp.r_v + 1;
+  for (int j = threadIdx.x; j < ntap; j += blockDim.x) taps[j] = lsf[j];
+  const int lane = threadIdx.x & 31, grp = threadIdx.x >> 5, ngrp = blockDim.x >> 5;
+  const long long nseg = ((long long)g.plane + kLsfPix - 1) / kLsfPix;
+  for (long long job = blockIdx.x; job < (long long)nrows * nseg; job += gridDim.x) {
+    const int row = (int)(job / nseg);
+    const size_t pix = (size_t)(job - (long long)row * nseg) * kLsfPix + lane;
+    const bool live0 = pix < g.plane, live1 = pix + 32 < g.plane;
     const float* src = in + (size_t)row * g.cube + pix;
-    float s = 0.0f;
-    for (int j = -dp.r_v; j <= dp.r_v; ++j)            // out[c] = sum_j L[j] in[c - j]
-      s = fmaf(lsf[j + dp.r_v], src[(size_t)(c + dp.r_v - j) * g.plane], s);
-    out[(size_t)row * g.cube + rem] = s;
+    float* dst = out + (size_t)row * g.cube + pix;
+    for (int c0 = 0; c0 < dp.nv; c0 += kLsfPiece) {
+      const int nc = min(kLsfPiece, dp.nv - c0);
+      __syncthreads();
+#pragma unroll 4
+      for (int c = grp; c < nc + ntap - 1; c += ngrp) {
+        const float* q = src + (size_t)(c0 + c) * g.plane;
+        slab[c * kLsfPix + lane] = live0 ? q[0] : 0.0f;
+        slab[c * kLsfPix + lane + 32] = live1 ? q[32] : 0.0f;
+      }
+      __syncthreads();
+      for (int c = grp; c < nc; c += ngrp) {      // out[c] = sum_j L[j] in[c - j]  (extended index c + r_v - j)
+        float sa = 0.0f, sb = 0.0f;
+        for (int j = 0; j < ntap; ++j) {
+          const float t = taps[j];
+          sa = fmaf(t, slab[(c + ntap - 1 - j) * kLsfPix + lane], sa);
+          sb = fmaf(t, slab[(c + ntap - 1 - j) * kLsfPix + lane + 32], sb);
+        }
+        float* q = dst + (size_t)(c0 + c) * g.plane;
+        if (live0) q[0] = sa;
+        if (live1) q[32] = sb;
+      }
+    }
   }
 }
 
-// Step 2b: one 1-D pass of the separable Gaussian PSF along x (axis = 0) or y (axis = 1), in the
-// extended layout.  The x pass produces columns [R, R + fw); the y pass rows [R, R + fh).
-__global__ void uf_psf1d_kernel(const __grid_constant__ DevProblem dp, const float* __restrict__ params,
-                                const int32_t* __restrict__ gal_index, long long k0, int nrows, int axis,
-                                const float* __restrict__ in, float* __restrict__ out) {
+// Step 2b, separable Gaussian PSF: both 1-D passes in one kernel.  A block takes one tile of one
+// channel of one row: the extended tile (tile + 2R each way) is read once into shared memory, the x
+// pass writes an intermediate (tile width x extended height) there, the y pass writes the fine-grid
+// result to device memory; a thread produces 4 consecutive outputs per pass from 4 + 2R inputs held
+// in registers.  R is the problem's largest tap radius; a data set with a narrower PSF has its taps
+// centred and zero-padded to that radius (the same sums).
+// in: extended layout [row][c][EH][EW]; out: compact [row][c][fh][fw].
+constexpr int kPsfTileW = 64;
+template <int R>
+__global__ void __launch_bounds__(256) uf_psf_sep_kernel(const __grid_constant__ DevProblem dp,
+                                                         const URow* __restrict__ rows, int nrows,
+                                                         const float* __restrict__ in, float* __restrict__ out) {
+  constexpr int kPsfTileH = R <= 8 ? 64 : 32;     // the taller tile has less halo; R > 8 would not fit 48 KB
+  constexpr int IW = (kPsfTileW + 2 * R + 3) & ~3, IH = kPsfTileH + 2 * R;
+  __shared__ __align__(16) float tin[IH][IW];
+  __shared__ float tmid[IH][kPsfTileW + 1];
+  __shared__ float taps[2 * R + 1];
   const UGeom g = uf_geom(dp);
-  const int W = dp.fw, H = axis == 0 ? g.EH : dp.fh;
-  const size_t per_chan = (size_t)W * H, per_row = per_chan * dp.nv;
-  const long long n = (long long)nrows * per_row;
-  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
-       idx += (long long)gridDim.x * blockDim.x) {
-    const int row = (int)(idx / per_row);
-    size_t rem = idx - row * (long long)per_row;
-    const int c = (int)(rem / per_chan);
-    rem -= c * per_chan;
-    const int yy = (int)(rem / W), xx = (int)(rem - (size_t)yy * W);
-    const URow r = uf_row_psf(dp, gal_index, k0 + row);
-    const float* taps = dp.psf_taps + (size_t)r.psf_set * dp.psf_stride;
-    const int ex = xx + g.R, ey = axis == 0 ? yy : yy + g.R;
-    const float* src = in + (size_t)row * g.cube + (size_t)c * g.plane + (size_t)ey * g.EW + ex;
-    const int stride = axis == 0 ? 1 : g.EW;
-    float s = 0.0f;
-    for (int j = -r.r_p; j <= r.r_p; ++j) s = fmaf(taps[j + r.r_p], src[-j * stride], s);
-    out[(size_t)row * g.cube + (size_t)c * g.plane + (size_t)ey * g.EW + ex] = s;
+  const int ntx = (dp.fw + kPsfTileW - 1) / kPsfTileW, nty = (dp.fh + kPsfTileH - 1) / kPsfTileH;
+  const long long per_row = (long long)dp.nv * ntx * nty;
+  for (long long job = blockIdx.x; job < (long long)nrows * per_row; job += gridDim.x) {
+    const int row = (int)(job / per_row);
+    long long rem = job - (long long)row * per_row;
+    const int c = (int)(rem / (ntx * nty));
+    rem -= (long long)c * ntx * nty;
+    const int ty = (int)(rem / ntx), tx = (int)(rem - (long long)ty * ntx);
+    const URow r = rows[row];
+    __syncthreads();
+    if (threadIdx.x < 2 * R + 1) {
+      const int idx = (int)threadIdx.x - (R - r.r_p);
+      taps[threadIdx.x] = idx >= 0 && idx <= 2 * r.r_p ? dp.psf_taps[(size_t)r.psf_set * dp.psf_stride + idx] : 0.0f;
+    }
+    const int x0 = tx * kPsfTileW, y0 = ty * kPsfTileH;
+    const int tw = min(kPsfTileW, dp.fw - x0), th = min(kPsfTileH, dp.fh - y0);
+    const float* src = in + (size_t)row * g.cube + (size_t)c * g.plane + (size_t)y0 * g.EW + x0;
+    if ((g.EW & 3) == 0 && (reinterpret_cast<size_t>(src) & 15) == 0 && tw == kPsfTileW) {
+      for (int i = threadIdx.x; i < (th + 2 * R) * (IW / 4); i += blockDim.x) {   // 16-byte loads
+        const int yy = i / (IW / 4), xx = (i - yy * (IW / 4)) * 4;
+        float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (xx + 3 < tw + 2 * R) {
+          f = *reinterpret_cast<const float4*>(src + (size_t)yy * g.EW + xx);
+        } else {
+          if (xx < tw + 2 * R) f.x = src[(size_t)yy * g.EW + xx];
+          if (xx + 1 < tw + 2 * R) f.y = src[(size_t)yy * g.EW + xx + 1];
+          if (xx + 2 < tw + 2 * R) f.z = src[(size_t)yy * g.EW + xx + 2];
+        }
+        *reinterpret_cast<float4*>(&tin[yy][xx]) = f;
+      }
+    } else {
+      for (int i = threadIdx.x; i < (th + 2 * R) * IW; i += blockDim.x) {
+        const int yy = i / IW, xx = i - yy * IW;
+        tin[yy][xx] = xx < tw + 2 * R ? src[(size_t)yy * g.EW + xx] : 0.0f;
+      }
+    }
+    __syncthreads();
+    // Tap pairs for packed FP32 (FFMA2): an output pair (o[x], o[x+1]) receives from input v[i],
+    // i = 0..2R+1, the pair (f[i], f[i-1]) of flipped taps f[j] = taps[2R - j] (f[-1] = f[2R+1] = 0)
+    // times the broadcast input, i.e. 2R + 2 instructions per two outputs instead of 2 (2R + 1).
+    u64 tp[2 * R + 2];
+#pragma unroll
+    for (int i = 0; i < 2 * R + 2; ++i)
+      tp[i] = pk(i <= 2 * R ? taps[2 * R - i] : 0.0f, i >= 1 ? taps[2 * R - (i - 1)] : 0.0f);
+    constexpr int NX4 = kPsfTileW / 4;
+    for (int i = threadIdx.x; i < (th + 2 * R) * NX4; i += blockDim.x) {      // x pass
+      const int yy = i / NX4, xx = (i - yy * NX4) * 4;
+      float v[4 + 2 * R + 3];
+#pragma unroll
+      for (int q = 0; q < (4 + 2 * R + 3) / 4; ++q) {
+        const float4 f = *reinterpret_cast<const float4*>(&tin[yy][xx + 4 * q]);
+        v[4 * q] = f.x, v[4 * q + 1] = f.y, v[4 * q + 2] = f.z, v[4 * q + 3] = f.w;
+      }
+      u64 o01 = pk(0.f, 0.f), o23 = o01;
+#pragma unroll
+      for (int j = 0; j < 2 * R + 2; ++j) {
+        o01 = fma2(tp[j], pk1(v[j]), o01);
+        o23 = fma2(tp[j], pk1(v[j + 2]), o23);
+      }
+      float o0, o1, o2, o3;
+      upk(o01, o0, o1);
+      upk(o23, o2, o3);
+      tmid[yy][xx] = o0, tmid[yy][xx + 1] = o1, tmid[yy][xx + 2] = o2, tmid[yy][xx + 3] = o3;
+    }
+    __syncthreads();
+    float* dst = out + (size_t)row * g.cube + (size_t)c * dp.fw * dp.fh + (size_t)y0 * dp.fw + x0;
+    const int ny4 = (th + 3) / 4;
+    for (int i = threadIdx.x; i < ny4 * tw; i += blockDim.x) {                // y pass
+      const int yb = i / tw, xx = i - yb * tw, yy = yb * 4;
+      u64 o01 = pk(0.f, 0.f), o23 = o01;
+#pragma unroll
+      for (int j = 0; j < 4 + 2 * R; ++j) {
+        const float vv = yy + j < th + 2 * R ? tmid[yy + j][xx] : 0.0f;
+        if (j < 2 * R + 2) o01 = fma2(tp[j], pk1(vv), o01);
+        if (j >= 2) o23 = fma2(tp[j - 2], pk1(vv), o23);
+      }
+      float o[4];
+      upk(o01, o[0], o[1]);
+      upk(o23, o[2], o[3]);
+#pragma unroll
+      for (int m = 0; m < 4; ++m)
+        if (yy + m < th) dst[(size_t)(yy + m) * dp.fw + xx] = o[m];
+    }
   }
 }
 
-// Step 2b for a general PSF image: direct 2-D sum per voxel.  The image is stored flipped at
-// create, so this correlation is the true convolution (A11).
-__global__ void uf_psf2d_kernel(const __grid_constant__ DevProblem dp, const float* __restrict__ params,
-                                const int32_t* __restrict__ gal_index, long long k0, int nrows,
-                                const float* __restrict__ in, float* __restrict__ out) {
+// Step 2b for a general PSF image: direct 2-D sum from a shared-memory tile.  The image is stored
+// flipped at create, so this correlation is the true convolution (A11).
+constexpr int kImgTile = 32;
+__global__ void __launch_bounds__(256) uf_psf2d_kernel(const __grid_constant__ DevProblem dp,
+                                                       const URow* __restrict__ rows, int nrows,
+                                                       const float* __restrict__ in, float* __restrict__ out) {
+  extern __shared__ float sh[];                   // [(kImgTile + 2R)^2] tile, then [n^2] taps
   const UGeom g = uf_geom(dp);
-  const size_t per_chan = (size_t)dp.fw * dp.fh, per_row = per_chan * dp.nv;
-  const long long n = (long long)nrows * per_row;
-  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
-       idx += (long long)gridDim.x * blockDim.x) {
-    const int row = (int)(idx / per_row);
-    size_t rem = idx - row * (long long)per_row;
-    const int c = (int)(rem / per_chan);
-    rem -= c * per_chan;
-    const int yy = (int)(rem / dp.fw), xx = (int)(rem - (size_t)yy * dp.fw);
-    const URow r = uf_row_psf(dp, gal_index, k0 + row);
-    const int nn = 2 * r.r_p + 1;
-    const float* taps = dp.psf_taps + (size_t)r.psf_set * dp.psf_stride;
-    const float* src = in + (size_t)row * g.cube + (size_t)c * g.plane + (size_t)(yy + g.R - r.r_p) * g.EW +
-                       xx + g.R - r.r_p;
-    float s = 0.0f;
-    for (int ky = 0; ky < nn; ++ky)
-      for (int kx = 0; kx < nn; ++kx) s = fmaf(taps[ky * nn + kx], src[(size_t)ky * g.EW + kx], s);
-    out[(size_t)row * g.cube + (size_t)c * g.plane + (size_t)(yy + g.R) * g.EW + xx + g.R] = s;
+  const int Rm = g.R;
+  const int ntx = (dp.fw + kImgTile - 1) / kImgTile, nty = (dp.fh + kImgTile - 1) / kImgTile;
+  const long long per_row = (long long)dp.nv * ntx * nty;
+  for (long long job = blockIdx.x; job < (long long)nrows * per_row; job += gridDim.x) {
+    const int row = (int)(job / per_row);
+    long long rem = job - (long long)row * per_row;
+    const int c = (int)(rem / (ntx * nty));
+    rem -= (long long)c * ntx * nty;
+    const int ty = (int)(rem / ntx), tx = (int)(rem - (long long)ty * ntx);
+    const URow r = rows[row];
+    const int R = r.r_p, n = 2 * R + 1, iw = kImgTile + 2 * Rm;
+    float* tile = sh;
+    float* taps = sh + iw * iw;
+    const int x0 = tx * kImgTile, y0 = ty * kImgTile;
+    const int tw = min(kImgTile, dp.fw - x0), th = min(kImgTile, dp.fh - y0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < n * n; i += blockDim.x) taps[i] = dp.psf_taps[(size_t)r.psf_set * dp.psf_stride + i];
+    const float* src = in + (size_t)row * g.cube + (size_t)c * g.plane + (size_t)(y0 + Rm - R) * g.EW + x0 + Rm - R;
+    for (int i = threadIdx.x; i < (th + 2 * R) * (tw + 2 * R); i += blockDim.x) {
+      const int yy = i / (tw + 2 * R), xx = i - yy * (tw + 2 * R);
+      tile[yy * iw + xx] = src[(size_t)yy * g.EW + xx];
+    }
+    __syncthreads();
+    float* dst = out + (size_t)row * g.cube + (size_t)c * dp.fw * dp.fh + (size_t)y0 * dp.fw + x0;
+    for (int i = threadIdx.x; i < th * tw; i += blockDim.x) {
+      const int yy = i / tw, xx = i - yy * tw;
+      float sum = 0.0f;
+      for (int ky = 0; ky < n; ++ky)
+        for (int kx = 0; kx < n; ++kx) sum = fmaf(taps[ky * n + kx], tile[(yy + ky) * iw + xx + kx], sum);
+      dst[(size_t)yy * dp.fw + xx] = sum;
+    }
   }
 }
 
 // Steps 3-5: per spaxel, down-sample every channel (mean over the u x u block),
-// moments (two passes over the spectrum, like a plain implementation), residuals against the packed
-// observation, and the spaxel's chi^2 contribution.
-__global__ void uf_moments_kernel(const __grid_constant__ DevProblem dp, const float* __restrict__ params,
-                                  const int32_t* __restrict__ gal_index, long long k0, int nrows,
-                                  const float* __restrict__ cube, float* __restrict__ contrib,
-                                  const EvalArgs a) {
+// moments, residuals against the packed observation, and the spaxel's chi^2 contribution.  One pass
+// over the spectrum: S0, S1, S2 about a reference velocity close to the line (V_sys clamped to the
+// band, as in the fused kernel), then m1 = S1/S0, m2^2 = S2/S0 - m1^2.
+__global__ void uf_moments_kernel(const __grid_constant__ DevProblem dp, const URow* __restrict__ rows,
+                                  long long k0, int nrows, const float* __restrict__ cube,
+                                  float* __restrict__ contrib, const EvalArgs a) {
   const UGeom g = uf_geom(dp);
   const int npix = dp.nx * dp.ny;
   const long long n = (long long)nrows * npix;
@@ -212,35 +326,165 @@ __global__ void uf_moments_kernel(const __grid_constant__ DevProblem dp, const f
     const int pix = (int)(idx - (long long)row * npix);
     const int Y = pix / dp.nx, X = pix - Y * dp.nx;
     const long long k = k0 + row;
-    const URow r = uf_row(dp, params, gal_index, k);
+    const URow r = rows[row];
     const float4 ob = dp.obs[(size_t)r.gal * npix + pix];
     const bool unmasked = ob.y > 0.0f;
     float m0 = nan, m1 = nan, m2 = nan, t = nan, s = nan, c2 = inf;
     if (r.valid) {
-      const float* src = cube + (size_t)row * g.cube + (size_t)(Y * dp.u + g.R) * g.EW + X * dp.u + g.R;
-      const float v_first = -0.5f * (float)(dp.nv - 1) * dp.dv;
-      float s0 = 0.0f, s1 = 0.0f;
-      for (int c = 0; c < dp.nv; ++c) {
-        float blk = 0.0f;
-        for (int dy = 0; dy < dp.u; ++dy)
-          for (int dx = 0; dx < dp.u; ++dx) blk += src[(size_t)c * g.plane + (size_t)dy * g.EW + dx];
-        blk *= dp.inv_u2;
-        s0 += blk;
-        s1 = fmaf(blk, v_first + (float)c * dp.dv, s1);
+      // the convolved cube is compact: [row][c][fh][fw]
+      const size_t cplane = (size_t)dp.fw * dp.fh;
+      const float* src = cube + (size_t)row * g.cube + (size_t)(Y * dp.u) * dp.fw + X * dp.u;
+      const float v_ref = fminf(fmaxf(r.vsys - dp.v_center, -dp.vhalf), dp.vhalf);
+      const float v_first = -dp.vhalf - v_ref;                               // channel 0 from the reference
+      float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f;
+      if (dp.u == 1) {
+#pragma unroll 8
+        for (int c = 0; c < dp.nv; ++c) {
+          const float blk = src[(size_t)c * cplane];
+          const float v = fmaf((float)c, dp.dv, v_first);
+          s0 += blk;
+          s1 = fmaf(blk, v, s1);
+          s2 = fmaf(blk * v, v, s2);
+        }
+      } else {
+        for (int c = 0; c < dp.nv; ++c) {
+          float blk = 0.0f;
+          for (int dy = 0; dy < dp.u; ++dy)
+            for (int dx = 0; dx < dp.u; ++dx) blk += src[(size_t)c * cplane + (size_t)dy * dp.fw + dx];
+          blk *= dp.inv_u2;
+          const float v = fmaf((float)c, dp.dv, v_first);
+          s0 += blk;
+          s1 = fmaf(blk, v, s1);
+          s2 = fmaf(blk * v, v, s2);
+        }
       }
       m0 = s0;
       m1 = s1 / s0;
-      float s2 = 0.0f;
-      for (int c = 0; c < dp.nv; ++c) {
-        float blk = 0.0f;
-        for (int dy = 0; dy < dp.u; ++dy)
-          for (int dx = 0; dx < dp.u; ++dx) blk += src[(size_t)c * g.plane + (size_t)dy * g.EW + dx];
-        blk *= dp.inv_u2;
-        const float d = v_first + (float)c * dp.dv - m1;
-        s2 = fmaf(blk * d, d, s2);
-      }
-      const float var = s2 / s0;
+      const float var = s2 / s0 - m1 * m1;
       m2 = var > 0.0f ? sqrtf(var) : (var == var ? 0.0f : var);            // A5
+      const bool dark = !(m0 >= 1e-30f * r.i0);                             // A15
+      t = (m1 + (v_ref - ob.x)) * ob.y;
+      s = (m2 - ob.z) * ob.w;
+      c2 = fmaf(t, t, s * s);
+      const bool bad = dark || !(c2 < inf);
+      if (dark) m1 = m2 = nan;
+      if (!unmasked) t = s = 0.0f, c2 = 0.0f;
+      else if (bad) t = s = nan, c2 = inf;
+      m1 += v_ref + dp.v_center;
+    } else if (!unmasked) {
+      c2 = inf;   // an out-of-domain row is +INF whatever the mask
+    }
+    contrib[idx] = c2;
+    const size_t o = (size_t)k * npix + pix;
+    if (a.m0) a.m0[o] = m0;
+    if (a.m1) a.m1[o] = m1;
+    if (a.m2) a.m2[o] = m2;
+    if (a.resid) {
+      a.resid[2 * (size_t)k * npix + pix] = t;
+      a.resid[(2 * (size_t)k + 1) * npix + pix] = s;
+    }
+  }
+}
+
+// Steps 3-5 with the Gaussian-profile extraction the paper describes as the alternative to moments
+// (reading A23 of DESIGN.md): per spaxel, down-sample every
+// channel, fit A exp(-(v - mu)^2 / (2 s^2)) to the spectrum by unweighted least squares (Levenberg-
+// Marquardt started from the moments; the 3 x 3 normal equations in FP64), velocity = mu,
+// dispersion = s, m0 = the plain sum; then residuals and the chi^2 contribution as usual.  The fit
+// needs the whole convolved spectrum of a spaxel, so it cannot use the moment-first identity of the
+// fused kernel: it runs on this pipeline only.  A fit that does not converge gives NaN maps and, at an
+// unmasked spaxel, chi^2 = +INF ("may occasionally fail to converge").
+__device__ __forceinline__ float uf_spaxel_channel(const DevProblem& dp, const float* src, size_t cplane, int c) {
+  float blk = 0.0f;
+  for (int dy = 0; dy < dp.u; ++dy)
+    for (int dx = 0; dx < dp.u; ++dx) blk += src[(size_t)c * cplane + (size_t)dy * dp.fw + dx];
+  return blk * dp.inv_u2;
+}
+
+__global__ void uf_gaussfit_kernel(const __grid_constant__ DevProblem dp, const URow* __restrict__ rows,
+                                   long long k0, int nrows, const float* __restrict__ cube,
+                                   float* __restrict__ contrib, const EvalArgs a) {
+  const UGeom g = uf_geom(dp);
+  const int npix = dp.nx * dp.ny, nv = dp.nv;
+  const long long n = (long long)nrows * npix;
+  const float inf = __int_as_float(0x7f800000), nan = __int_as_float(0x7fc00000);
+  const double dv = dp.dv, v_first = -0.5 * (double)(nv - 1) * dv;            // velocities from v_center
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const int row = (int)(idx / npix);
+    const int pix = (int)(idx - (long long)row * npix);
+    const int Y = pix / dp.nx, X = pix - Y * dp.nx;
+    const long long k = k0 + row;
+    const URow r = rows[row];
+    const float4 ob = dp.obs[(size_t)r.gal * npix + pix];
+    const bool unmasked = ob.y > 0.0f;
+    float m0 = nan, m1 = nan, m2 = nan, t = nan, s = nan, c2 = inf;
+    if (r.valid) {
+      const size_t cplane = (size_t)dp.fw * dp.fh;
+      const float* src = cube + (size_t)row * g.cube + (size_t)(Y * dp.u) * dp.fw + X * dp.u;
+      double s0 = 0.0, s1 = 0.0;
+      for (int c = 0; c < nv; ++c) {
+        const double v = uf_spaxel_channel(dp, src, cplane, c);
+        s0 += v;
+        s1 += v * (v_first + c * dv);
+      }
+      const double mean = s1 / s0;
+      double s2 = 0.0;
+      for (int c = 0; c < nv; ++c) {
+        const double d = v_first + c * dv - mean;
+        s2 += (double)uf_spaxel_channel(dp, src, cplane, c) * d * d;
+      }
+      const double var = s2 / s0;
+      m0 = (float)s0;
+      bool done = false;
+      double mu = mean, sg = fmax(sqrt(fmax(var, 0.0)), 0.5 * dv);
+      if (s0 > 0.0 && isfinite(mean) && isfinite(var)) {
+        double A = s0 * dv / (sg * 2.5066282746310002);
+        double lambda = 1e-3;
+        for (int it = 0; it < 200 && !done; ++it) {
+          double j00 = 0, j01 = 0, j02 = 0, j11 = 0, j12 = 0, j22 = 0, r0 = 0, r1 = 0, r2 = 0, sse = 0;
+          const double is2 = 1.0 / (sg * sg);
+          for (int c = 0; c < nv; ++c) {
+            const double d = v_first + c * dv - mu;
+            const double e = exp(-0.5 * d * d * is2);
+            const double res = (double)uf_spaxel_channel(dp, src, cplane, c) - A * e;
+            const double J0 = e, J1 = A * e * d * is2, J2 = J1 * d / sg;
+            j00 += J0 * J0, j01 += J0 * J1, j02 += J0 * J2, j11 += J1 * J1, j12 += J1 * J2, j22 += J2 * J2;
+            r0 += J0 * res, r1 += J1 * res, r2 += J2 * res;
+            sse += res * res;
+          }
+          if (sse <= 1e-28 * s0 * s0) {
+            done = true;
+            break;
+          }
+          // (J^T J + lambda diag) delta = J^T r by Cramer's rule
+          const double a00 = j00 * (1.0 + lambda), a11 = j11 * (1.0 + lambda), a22 = j22 * (1.0 + lambda);
+          const double det = a00 * (a11 * a22 - j12 * j12) - j01 * (j01 * a22 - j12 * j02) + j02 * (j01 * j12 - a11 * j02);
+          const double d0 = (r0 * (a11 * a22 - j12 * j12) - j01 * (r1 * a22 - j12 * r2) + j02 * (r1 * j12 - a11 * r2)) / det;
+          const double d1 = (a00 * (r1 * a22 - j12 * r2) - r0 * (j01 * a22 - j12 * j02) + j02 * (j01 * r2 - r1 * j02)) / det;
+          const double d2 = (a00 * (a11 * r2 - r1 * j12) - j01 * (j01 * r2 - r1 * j02) + r0 * (j01 * j12 - a11 * j02)) / det;
+          const double A1 = A + d0, mu1 = mu + d1, sg1 = sg + d2;
+          double sse1 = INFINITY;
+          if (isfinite(A1) && isfinite(mu1) && sg1 > 0.0 && sg1 < 1e3 * nv * dv) {
+            sse1 = 0.0;
+            const double is21 = 1.0 / (sg1 * sg1);
+            for (int c = 0; c < nv; ++c) {
+              const double d = v_first + c * dv - mu1;
+              const double res = (double)uf_spaxel_channel(dp, src, cplane, c) - A1 * exp(-0.5 * d * d * is21);
+              sse1 += res * res;
+            }
+          }
+          if (sse1 < sse) {
+            A = A1, mu = mu1, sg = sg1;
+            lambda = fmax(lambda / 10.0, 1e-12);
+            if (fabs(d1) < 1e-6 * dv && fabs(d2) < 1e-6 * dv) done = true;
+          } else {
+            lambda *= 10.0;
+            if (!(lambda <= 1e12)) break;
+          }
+        }
+      }
+      if (done) m1 = (float)mu, m2 = (float)sg;
       const bool dark = !(m0 >= 1e-30f * r.i0);                             // A15
       t = (m1 - ob.x) * ob.y;
       s = (m2 - ob.z) * ob.w;
@@ -293,47 +537,68 @@ inline unsigned grid_for(long long n, int threads, int sm_count) {
 
 size_t unfused_bytes_per_row(const DevProblem& dp) {
   const UGeom g = uf_geom(dp);
-  return sizeof(float) * (2 * g.cube + (size_t)dp.nx * dp.ny);
+  return sizeof(float) * (2 * g.cube + (size_t)dp.nx * dp.ny) + sizeof(URow);
 }
 
-// Algorithmic HBM bytes of the unfused pipeline per row (every array written once, read once per
-// consumer).
+// Algorithmic HBM bytes of the unfused pipeline per row: every array written once and read once by
+// the step that consumes it (cube: written, read by the LSF; LSF output: written, read by the PSF
+// kernel; convolved cube: written, read by the extraction kernel, whose second pass over a spectrum
+// comes from cache).
 double unfused_algorithmic_bytes_per_row(const DevProblem& dp) {
   const UGeom g = uf_geom(dp);
-  const double ext = (double)g.cube, lsf = (double)g.plane * dp.nv;
-  const double px = (double)dp.fw * g.EH * dp.nv, fine = (double)dp.fw * dp.fh * dp.nv;
-  double b = ext /*w*/ + ext /*r*/ + lsf /*w*/;
-  if (dp.psf_kind == GBK_PSF_GAUSSIAN) b += lsf + px + px + fine;   // x pass r/w, y pass r/w
-  else b += lsf + fine;
-  b += 2.0 * fine;                                                    // moments: two passes
-  return 4.0 * b;
+  const double ext = (double)g.cube, lsf = (double)g.plane * dp.nv, fine = (double)dp.fw * dp.fh * dp.nv;
+  return 4.0 * (2.0 * ext + 2.0 * lsf + 2.0 * fine);
 }
 
+namespace {
+template <int R>
+void launch_psf_sep(const DevProblem& dp, const URow* rows, int n, unsigned cap, const float* in, float* out,
+                    cudaStream_t st) {
+  const int th = R <= 8 ? 64 : 32;
+  const long long jobs = (long long)n * dp.nv * ((dp.fw + kPsfTileW - 1) / kPsfTileW) * ((dp.fh + th - 1) / th);
+  uf_psf_sep_kernel<R><<<(unsigned)std::min<long long>(jobs, cap), 256, 0, st>>>(dp, rows, n, in, out);
+}
+}  // namespace
+
 cudaError_t launch_unfused(const DevProblem& dp, const EvalArgs& a, const float* lsf_taps, float* scratch,
-                           long long chunk_rows, int sm_count, cudaStream_t st) {
+                           long long chunk_rows, int sm_count, int extraction, cudaStream_t st) {
   const UGeom g = uf_geom(dp);
   const int T = 256, npix = dp.nx * dp.ny;
   float* A = scratch;
   float* B = A + (size_t)chunk_rows * g.cube;
   float* contrib = B + (size_t)chunk_rows * g.cube;
+  URow* rows = reinterpret_cast<URow*>(contrib + (size_t)chunk_rows * npix);
+  const unsigned wide = (unsigned)sm_count * 16;      // block-per-job kernels: grid-stride over the jobs
   for (long long k0 = 0; k0 < a.K; k0 += chunk_rows) {
     const int n = (int)std::min(chunk_rows, a.K - k0);
-    uf_cube_kernel<<<grid_for((long long)n * g.plane, T, sm_count), T, 0, st>>>(dp, a.params, a.gal_index, k0, n, A);
-    uf_lsf_kernel<<<grid_for((long long)n * g.plane * dp.nv, T, sm_count), T, 0, st>>>(dp, lsf_taps, n, A, B);
-    const float* conv;
-    if (dp.psf_kind == GBK_PSF_GAUSSIAN) {
-      uf_psf1d_kernel<<<grid_for((long long)n * dp.fw * g.EH * dp.nv, T, sm_count), T, 0, st>>>(
-          dp, a.params, a.gal_index, k0, n, 0, B, A);
-      uf_psf1d_kernel<<<grid_for((long long)n * dp.fw * dp.fh * dp.nv, T, sm_count), T, 0, st>>>(
-          dp, a.params, a.gal_index, k0, n, 1, A, B);
-      conv = B;
-    } else {
-      uf_psf2d_kernel<<<grid_for((long long)n * dp.fw * dp.fh * dp.nv, T, sm_count), T, 0, st>>>(
-          dp, a.params, a.gal_index, k0, n, B, A);
-      conv = A;
+    uf_rows_kernel<<<(n + 127) / 128, 128, 0, st>>>(dp, a.params, a.gal_index, k0, n, rows);
+    uf_cube_kernel<<<grid_for((long long)n * g.plane, T, sm_count), T, 0, st>>>(dp, rows, n, A);
+    {
+      const long long jobs = (long long)n * (((long long)g.plane + kLsfPix - 1) / kLsfPix);
+      const size_t smem = sizeof(float) * kLsfPix * (kLsfPiece + 2 * dp.r_v);
+      uf_lsf_kernel<<<(unsigned)std::min<long long>(jobs, wide), 256, smem, st>>>(dp, lsf_taps, n, A, B);
     }
-    uf_moments_kernel<<<grid_for((long long)n * npix, 128, sm_count), 128, 0, st>>>(dp, a.params, a.gal_index,
-                                                                                  k0, n, conv, contrib, a);
+    // PSF: B (extended layout) -> A (compact fine-grid layout)
+    if (dp.psf_kind == GBK_PSF_GAUSSIAN) {
+#define GBK_UF_CASE(RR) case RR: launch_psf_sep<RR>(dp, rows, n, wide, B, A, st); break;
+      switch (dp.r_p_max) {
+        GBK_UF_CASE(0) GBK_UF_CASE(1) GBK_UF_CASE(2) GBK_UF_CASE(3) GBK_UF_CASE(4) GBK_UF_CASE(5)
+        GBK_UF_CASE(6) GBK_UF_CASE(7) GBK_UF_CASE(8) GBK_UF_CASE(9) GBK_UF_CASE(10) GBK_UF_CASE(11)
+        GBK_UF_CASE(12) GBK_UF_CASE(13) GBK_UF_CASE(14) GBK_UF_CASE(15) GBK_UF_CASE(16)
+        default: return cudaErrorInvalidValue;
+      }
+#undef GBK_UF_CASE
+    } else {
+      const long long jobs = (long long)n * dp.nv * ((dp.fw + kImgTile - 1) / kImgTile) *
+                             ((dp.fh + kImgTile - 1) / kImgTile);
+      const int iw = kImgTile + 2 * g.R, nn = 2 * g.R + 1;
+      const size_t smem = sizeof(float) * ((size_t)iw * iw + (size_t)nn * nn);
+      uf_psf2d_kernel<<<(unsigned)std::min<long long>(jobs, wide), 256, smem, st>>>(dp, rows, n, B, A);
+    }
+    if (extraction == GBK_EXTRACT_GAUSSFIT)
+      uf_gaussfit_kernel<<<grid_for((long long)n * npix, 128, sm_count), 128, 0, st>>>(dp, rows, k0, n, A, contrib, a);
+    else
+      uf_moments_kernel<<<grid_for((long long)n * npix, 128, sm_count), 128, 0, st>>>(dp, rows, k0, n, A, contrib, a);
     uf_chi2_kernel<<<n, 256, 0, st>>>(contrib, npix, k0, a.chi2);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

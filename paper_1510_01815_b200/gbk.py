@@ -22,9 +22,10 @@ GBK_OK, GBK_ERR_ARG, GBK_ERR_ALLOC, GBK_ERR_CUDA, GBK_ERR_UNSUPPORTED = range(5)
 GBK_RC_ARCTAN, GBK_RC_RAMP, GBK_RC_EPINAT = 0, 1, 2
 GBK_STRATEGY_CUBE, GBK_STRATEGY_VFIELD = 0, 1
 GBK_PSF_GAUSSIAN, GBK_PSF_IMAGE = 0, 1
+GBK_EXTRACT_MOMENTS, GBK_EXTRACT_GAUSSFIT = 0, 1
 
 EXPORTS = (   # every symbol include/gbk.h declares (tests/test_abi_and_dist.py checks them all)
-    "gbk_create_problem", "gbk_get_info", "gbk_set_strategy", "gbk_reserve", "gbk_eval_batch",
+    "gbk_create_problem", "gbk_get_info", "gbk_set_strategy", "gbk_set_extraction", "gbk_reserve", "gbk_eval_batch",
     "gbk_eval_batch_counted",
     "gbk_eval_batch_unfused", "gbk_eval_vfield_batch", "gbk_eval_batch_host", "gbk_destroy",
     "gbk_last_error", "gbk_probe_pipe", "gbk_fit_ng", "gbk_fit_lm", "gbk_fit_ns",
@@ -65,7 +66,7 @@ class gbk_problem_info(C.Structure):
         ("device", C.c_int32),
         ("strategy", C.c_int32),
         ("unfused_bytes_per_eval", C.c_int64),
-        ("row_stride", C.c_int32),
+        ("row_stride", C.c_int32), ("extraction", C.c_int32),
     ]
 
 
@@ -101,6 +102,8 @@ def lib():
         L.gbk_eval_batch_counted.restype = C.c_int
         L.gbk_reserve.argtypes = [vp, C.c_int64, vp]
         L.gbk_reserve.restype = C.c_int
+        L.gbk_set_extraction.argtypes = [vp, C.c_int32]
+        L.gbk_set_extraction.restype = C.c_int
         L.gbk_set_strategy.argtypes = [vp, C.c_int32]
         L.gbk_set_strategy.restype = C.c_int
         L.gbk_eval_vfield_batch.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp]
@@ -231,6 +234,11 @@ def gbk_set_strategy(handle, strategy: int):
     _check(lib().gbk_set_strategy(handle, int(strategy)))
 
 
+def gbk_set_extraction(handle, extraction: int):
+    """Moments (GBK_EXTRACT_MOMENTS) or Gaussian-profile fits (GBK_EXTRACT_GAUSSFIT) for the maps."""
+    _check(lib().gbk_set_extraction(handle, int(extraction)))
+
+
 def gbk_eval_vfield_batch(handle, params, gal_index, K, chi2, vmap=None, resid=None, stream=0):
     """Velocity-field strategy (device buffers; asynchronous on `stream`)."""
     _check(lib().gbk_eval_vfield_batch(handle, _ptr(params), _ptr(gal_index), int(K), _ptr(chi2),
@@ -354,6 +362,10 @@ class Problem:
     def set_strategy(self, strategy: int):
         """gbk_set_strategy, keeping `info` (which reports the strategy) up to date."""
         gbk_set_strategy(self.handle, strategy)
+        self.info = gbk_get_info(self.handle)
+
+    def set_extraction(self, extraction: int):
+        gbk_set_extraction(self.handle, extraction)
         self.info = gbk_get_info(self.handle)
 
     def eval_vfield(self, params, gal_index=None, want_maps=False, want_resid=False, stream=None):

@@ -19,7 +19,7 @@ def f32(x) -> float:
     return float(np.float32(x))
 
 
-def oracle_grid(oracle, w: wl.Workload, fwhm=None, tab=None, tab_dx=0.0):
+def oracle_grid(oracle, w: wl.Workload, fwhm=None, tab=None, tab_dx=0.0, extract=0):
     """Oracle Grid for workload w (Gaussian PSF of `fwhm` data pixels, or w's Moffat image; `tab`:
     a tabulated radial intensity profile, float32 values promoted like every other input)."""
     if w.psf_kind == wl.PSF_GAUSSIAN:
@@ -31,7 +31,7 @@ def oracle_grid(oracle, w: wl.Workload, fwhm=None, tab=None, tab_dx=0.0):
     return oracle.Grid(nx=w.nx, ny=w.ny, nv=w.nv, u=w.u, v_center=f32(w.v_center), dv=f32(w.dv),
                        rc_model=w.rc_model, psf=psf, lsf=lsf,
                        tab=None if tab is None else np.asarray(tab, dtype=np.float32).astype(np.float64),
-                       tab_dx=f32(tab_dx))
+                       tab_dx=f32(tab_dx), extract=extract)
 
 
 def gbk_desc(w: wl.Workload, obs: wl.Observed, fwhms=None, **extra):

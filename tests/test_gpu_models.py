@@ -143,3 +143,56 @@ def test_create_rejects_bad_tables(oracle, torch_cuda, gbk):
         with pytest.raises(gbk.GbkError) as e:
             gbk.Problem(**pu.gbk_desc(w, obs, intensity_table=tab, intensity_dx=dx))
         assert e.value.code == gbk.GBK_ERR_ARG
+
+
+# ------------------------ Gaussian-profile extraction ----
+
+@pytest.mark.parametrize("cfg,kw", [(1, {}), (1, dict(u=2, nx=20, ny=18, nv=48)), (3, {})])
+def test_gaussian_profile_extraction(oracle, torch_cuda, gbk, cfg, kw):
+    """GBK_EXTRACT_GAUSSFIT: velocity and dispersion maps from a Gaussian fitted to every spectrum, through
+    gbk_eval_batch (which then runs the multi-kernel pipeline) against the oracle's extract = 1.  Maps are
+    compared at the unmasked spaxels (the observation's mask keeps m0 >= 1e-3 max); where the oracle's fit
+    fails (NaN) the GPU's must fail too."""
+    torch = torch_cuda
+    w = wl.config(cfg).scaled(**kw)
+    rng = wl.rng_for(cfg, 41)
+    true = wl.cfg1_true_row(rng)[0] if cfg == 1 else wl.draw_rows(w, rng, 1)[0]
+    g = pu.oracle_grid(oracle, w, extract=1)
+    m0, m1, m2 = oracle.model_maps(g, true.astype(np.float64))
+    obs = wl.observe(w, m0[None], m1[None], m2[None], rng)
+    rows = np.repeat(true[None].astype(np.float64), 6 if cfg == 1 else 3, axis=0)
+    b = wl.box(w)
+    rows[1:] += 0.05 * (b[:, 1] - b[:, 0]) * rng.uniform(-1, 1, (rows.shape[0] - 1, wl.P))
+    rows[:, wl.IX_INC] = np.clip(rows[:, wl.IX_INC], 5.0, 85.0)
+    rows[:, wl.IX_RT] = np.clip(rows[:, wl.IX_RT], 0.5, None)
+    rows = rows.astype(np.float32)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
+                           want_maps=True)
+    ref_mom = oracle.eval_rows(pu.oracle_grid(oracle, w), obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0],
+                               obs.mask[0], rows, want_maps=True)
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        prob.set_extraction(gbk.GBK_EXTRACT_GAUSSFIT)
+        assert prob.info.extraction == gbk.GBK_EXTRACT_GAUSSFIT
+        out = prob.eval(torch.from_numpy(rows).cuda(), want_maps=True)
+        torch.cuda.synchronize()
+        got = {k: v.cpu().numpy().astype(np.float64) for k, v in out.items()}
+        prob.set_extraction(gbk.GBK_EXTRACT_MOMENTS)            # and back: the fused kernel again
+        back = prob.eval(torch.from_numpy(rows).cuda(), want_maps=True)
+        mom = {k: v.cpu().numpy().astype(np.float64) for k, v in back.items()}
+    m = obs.mask[0] != 0
+    worst = {}
+    for k in range(rows.shape[0]):
+        assert np.array_equal(np.isnan(ref["m1"][k][m]), np.isnan(got["m1"][k][m]))
+        ok = m & np.isfinite(ref["m1"][k])
+        worst["m0"] = max(worst.get("m0", 0), float(np.max(np.abs(got["m0"][k][ok] / ref["m0"][k][ok] - 1))))
+        worst["m1"] = max(worst.get("m1", 0), float(np.max(np.abs(got["m1"][k][ok] - ref["m1"][k][ok]))))
+        worst["m2"] = max(worst.get("m2", 0), float(np.max(np.abs(got["m2"][k][ok] - ref["m2"][k][ok]))))
+    fin = np.isfinite(ref["chi2"])
+    assert np.array_equal(fin, np.isfinite(got["chi2"]))
+    worst["chi2"] = float(np.max(np.abs(got["chi2"][fin] / ref["chi2"][fin] - 1))) if fin.any() else 0.0
+    print("gaussfit", cfg, kw, worst)
+    assert worst["m0"] <= pu.TOL_M0_REL and worst["m1"] <= pu.TOL_M12_ABS and worst["m2"] <= pu.TOL_M12_ABS
+    assert worst["chi2"] <= pu.TOL_CHI2_REL
+    pu.compare(ref_mom, mom, rows, True, "moments after switching back")
+    # the two extractions are different things: beam smearing separates them (PAPER.md:672)
+    assert np.nanmax(np.abs(ref["m2"][0][m] - ref_mom["m2"][0][m])) > 0.05
