@@ -284,18 +284,23 @@ typedef struct {
 
 /*
  * Nested grids (refinement rule: DESIGN.md reading A19).  `n_axes` parameters
- * (indices axis_param[a] into the row, box [axis_lo[a], axis_hi[a]]) are gridded with `nodes`
- * nodes each, the other parameters stay at base_row.  Level l has spacing h = (hi-lo)/(nodes 2^l)
- * and nodes c + (j - (nodes-1)/2) h; c = box centre at level 0, then the best node of the level
- * before.  An axis on PA (index 2) whose box spans >= 360 degrees wraps; any other axis is shifted
- * to stay inside its box.  Ties in chi^2 take the lowest flat index (axis 0 slowest).
- * nodes^n_axes <= 2^24.  base_row and best_row are [row_stride]; best_chi2 [1] receives the chi^2 of the
- * final level's best node.
+ * (indices axis_param[a] into the row, box [axis_lo[a], axis_hi[a]]) are gridded with axis_nodes[a]
+ * nodes each (the paper uses 7, 11, 11, 5, 5, 5 for PA, r_t, V_t, sigma, a, g), the
+ * other parameters stay at base_row.  Level l has spacing h_a = (hi-lo)/(nodes_a 2^l) and nodes
+ * c + (j - (nodes_a-1)/2) h_a; c = box centre at level 0, then the best node of the level before.  An
+ * axis on PA (index 2) whose box spans >= 360 degrees wraps; any other axis is shifted to stay inside
+ * its box.  Ties in chi^2 take the lowest flat index (axis 0 slowest).  The product of the node counts
+ * is <= 2^24.  Stopping ("until the area of the parameter space under the grid is smaller
+ * than a user-defined accuracy threshold a"; :362: a = 0.01 for r_t, 0.1 otherwise): the level whose
+ * spacing is <= axis_accuracy[a] on EVERY axis is the last one; axis_accuracy == NULL runs exactly
+ * max_levels levels; max_levels always caps the count.  stats->converged is 1 when the thresholds were
+ * reached (or none were given) and the best chi^2 is finite.
+ * base_row and best_row are [row_stride]; best_chi2 [1] receives the chi^2 of the last level's best node.
  */
 int gbk_fit_ng(gbk_problem *p, const float *base_row, int32_t gal, int32_t n_axes,
-               const int32_t *axis_param, const float *axis_lo, const float *axis_hi, int32_t nodes,
-               int32_t levels, float *best_row, float *best_chi2, gbk_fit_stats *stats,
-               void *cuda_stream);
+               const int32_t *axis_param, const float *axis_lo, const float *axis_hi,
+               const int32_t *axis_nodes, const float *axis_accuracy, int32_t max_levels,
+               float *best_row, float *best_chi2, gbk_fit_stats *stats, void *cuda_stream);
 
 /*
  * Levenberg-Marquardt for n_fits independent fits at once (config 5: one fit

@@ -143,7 +143,8 @@ int check_box(int n, const int32_t* idx, const float* lo, const float* hi, int S
 constexpr int kNgMaxAxes = 6, kNgMaxNodes = 32;
 
 struct NgAxes {
-  int n_axes, nodes, S;       // S: floats per row
+  int n_axes, S;              // S: floats per row
+  int nodes[kNgMaxAxes];
   int param[kNgMaxAxes];
   float value[kNgMaxAxes][kNgMaxNodes];
   float base[GBK_P_MAX];
@@ -158,8 +159,8 @@ __global__ void ng_rows_kernel(const __grid_constant__ NgAxes ax, int n_rows, fl
   for (int j = 0; j < GBK_P_MAX; ++j) row[j] = ax.base[j];
   int rem = r;
   for (int a = ax.n_axes - 1; a >= 0; --a) {
-    const int j = rem % ax.nodes;
-    rem /= ax.nodes;
+    const int j = rem % ax.nodes[a];
+    rem /= ax.nodes[a];
     row[ax.param[a]] = ax.value[a][j];
   }
 #pragma unroll
@@ -196,20 +197,25 @@ __global__ void argmin_kernel(const float* __restrict__ chi2, int n, int* __rest
 
 extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, int32_t n_axes,
                           const int32_t* axis_param, const float* axis_lo, const float* axis_hi,
-                          int32_t nodes, int32_t levels, float* best_row, float* best_chi2,
-                          gbk_fit_stats* stats, void* cuda_stream) {
+                          const int32_t* axis_nodes, const float* axis_accuracy, int32_t max_levels,
+                          float* best_row, float* best_chi2, gbk_fit_stats* stats, void* cuda_stream) {
   clear_error();
   Clock clock;
   gbk_problem_info info;
   DRV_TRY(gbk_get_info(p, &info));
-  if (!base_row || !best_row || !best_chi2) return fail(GBK_ERR_ARG, "null argument");
-  if (n_axes > kNgMaxAxes || nodes < 2 || nodes > kNgMaxNodes || levels < 1 || levels > 30)
-    return fail(GBK_ERR_ARG, "need n_axes <= %d, 2 <= nodes <= %d, 1 <= levels <= 30", kNgMaxAxes, kNgMaxNodes);
+  if (!base_row || !best_row || !best_chi2 || !axis_nodes) return fail(GBK_ERR_ARG, "null argument");
+  if (n_axes > kNgMaxAxes || max_levels < 1 || max_levels > 30)
+    return fail(GBK_ERR_ARG, "need n_axes <= %d and 1 <= max_levels <= 30", kNgMaxAxes);
   DRV_TRY(check_box(n_axes, axis_param, axis_lo, axis_hi, info.row_stride));
   if (gal < 0 || gal >= info.n_gal) return fail(GBK_ERR_ARG, "gal out of range");
   double n_rows_d = 1.0;
-  for (int a = 0; a < n_axes; ++a) n_rows_d *= nodes;
-  if (n_rows_d > (double)(1 << 24)) return fail(GBK_ERR_ARG, "nodes^n_axes exceeds 2^24 rows");
+  for (int a = 0; a < n_axes; ++a) {
+    if (axis_nodes[a] < 2 || axis_nodes[a] > kNgMaxNodes)
+      return fail(GBK_ERR_ARG, "need 2 <= axis_nodes <= %d", kNgMaxNodes);
+    if (axis_accuracy && !(axis_accuracy[a] > 0.f)) return fail(GBK_ERR_ARG, "axis_accuracy must be > 0");
+    n_rows_d *= axis_nodes[a];
+  }
+  if (n_rows_d > (double)(1 << 24)) return fail(GBK_ERR_ARG, "the grid exceeds 2^24 rows");
   const int n_rows = (int)n_rows_d;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(info.device);
@@ -233,22 +239,27 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
     std::fill(gal_idx.h, gal_idx.h + n_rows, gal);
     DRV_CUDA(gal_idx.to_device(n_rows, st));
   }
+  DRV_TRY(gbk_reserve(p, n_rows, cuda_stream));
 
   NgAxes ax;
   memset(&ax, 0, sizeof(ax));
   const int S = info.row_stride;
-  ax.n_axes = n_axes, ax.nodes = nodes, ax.S = S;
+  ax.n_axes = n_axes, ax.S = S;
   memcpy(ax.base, base_row, sizeof(float) * S);
   double centre[kNgMaxAxes];
   for (int a = 0; a < n_axes; ++a) {
-    ax.param[a] = axis_param[a];
+    ax.param[a] = axis_param[a], ax.nodes[a] = axis_nodes[a];
     centre[a] = 0.5 * ((double)axis_lo[a] + (double)axis_hi[a]);
   }
   gbk_fit_stats fs{};
-  for (int level = 0; level < levels; ++level) {
+  bool reached = false;
+  for (int level = 0; level < max_levels && !reached; ++level) {
+    reached = axis_accuracy != nullptr;
     for (int a = 0; a < n_axes; ++a) {
+      const int nodes = axis_nodes[a];
       const double lo = axis_lo[a], hi = axis_hi[a];
       const double h = (hi - lo) / ((double)nodes * (double)(1u << level));
+      if (axis_accuracy && h > (double)axis_accuracy[a]) reached = false;   // this level is not the last
       const bool wraps = axis_param[a] == 2 && hi - lo >= 360.0;
       double first = centre[a] - 0.5 * (nodes - 1) * h;
       if (!wraps) {   // shift the whole axis back inside the box
@@ -271,15 +282,16 @@ extern "C" int gbk_fit_ng(gbk_problem* p, const float* base_row, int32_t gal, in
     DRV_CUDA(cudaStreamSynchronize(st));
     int rem = best_i.h[0];
     for (int a = n_axes - 1; a >= 0; --a) {
-      centre[a] = ax.value[a][rem % nodes];
-      rem /= nodes;
+      centre[a] = ax.value[a][rem % axis_nodes[a]];
+      rem /= axis_nodes[a];
     }
     fs.evals += n_rows, fs.launches += 1, fs.iterations += 1;
   }
   memcpy(best_row, base_row, sizeof(float) * S);
   for (int a = 0; a < n_axes; ++a) best_row[axis_param[a]] = (float)centre[a];
   *best_chi2 = best_v.h[0];
-  fs.converged = isfinite(best_v.h[0]) ? 1 : 0;
+  // converged: the accuracy thresholds were reached (or none were asked for) with a finite chi^2
+  fs.converged = (isfinite(best_v.h[0]) && (reached || !axis_accuracy)) ? 1 : 0;
   fs.ms_total = clock.ms();
   if (stats) *stats = fs;
   return GBK_OK;

@@ -118,7 +118,7 @@ def lib():
                                      C.POINTER(C.c_double), vp]
         L.gbk_probe_pipe.restype = C.c_int
         sp = C.POINTER(gbk_fit_stats)
-        L.gbk_fit_ng.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, vp, vp, C.c_int32, C.c_int32, vp,
+        L.gbk_fit_ng.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, vp, vp, vp, vp, C.c_int32, vp,
                                  vp, sp, vp]
         L.gbk_fit_ng.restype = C.c_int
         L.gbk_fit_lm.argtypes = [vp, C.c_int32, vp, vp, C.c_int32, vp, vp, vp, C.c_float, C.c_int32,
@@ -280,16 +280,21 @@ def _stride(handle) -> int:
     return gbk_get_info(handle).row_stride
 
 
-def gbk_fit_ng(handle, base_row, gal, axis_param, axis_lo, axis_hi, nodes, levels, stream=0):
-    """Nested grids (host arrays in, host results out) -> (best_row [row_stride], best_chi2, stats)."""
+def gbk_fit_ng(handle, base_row, gal, axis_param, axis_lo, axis_hi, nodes, levels, accuracy=None, stream=0):
+    """Nested grids (host arrays in, host results out) -> (best_row [row_stride], best_chi2, stats).
+    `nodes`: one count for all axes or one per axis; `levels`: the most levels to run; `accuracy`:
+    per-axis spacing thresholds that end the refinement (None: run exactly `levels` levels)."""
     S = _stride(handle)
     base = _host_f32(base_row, (S,))
     idx, lo, hi = _box(axis_param, axis_lo, axis_hi)
+    nn = np.ascontiguousarray(np.broadcast_to(np.asarray(nodes, dtype=np.int32).reshape(-1), (idx.size,)))
+    acc = None if accuracy is None else np.ascontiguousarray(
+        np.broadcast_to(np.asarray(accuracy, dtype=np.float32).reshape(-1), (idx.size,)))
     best = np.empty(S, np.float32)
     chi = np.empty(1, np.float32)
     st = gbk_fit_stats()
     _check(lib().gbk_fit_ng(handle, _ptr(base), int(gal), idx.size, _ptr(idx), _ptr(lo), _ptr(hi),
-                            int(nodes), int(levels), _ptr(best), _ptr(chi), C.byref(st),
+                            _ptr(nn), _ptr(acc), int(levels), _ptr(best), _ptr(chi), C.byref(st),
                             stream or None))
     return best, float(chi[0]), _stats_dict(st)
 

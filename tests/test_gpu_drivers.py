@@ -82,6 +82,26 @@ def test_nested_grids_follow_rule_a19_and_find_the_truth(oracle, torch_cuda, gbk
     assert np.array_equal(np.delete(best, FREE4), np.delete(true, FREE4))
 
 
+def test_nested_grids_per_axis_nodes_and_accuracy_thresholds(oracle, torch_cuda, gbk):
+    """The paper's configuration: a node count per axis (7 for PA, 11 for r_t and V_t; i
+    fixed) and accuracy thresholds (0.01 for r_t, 0.1 otherwise) that end the refinement."""
+    w0 = wl.config(3).scaled(nx=32, ny=32, nv=48)
+    true = _true_row(w0)
+    w, obs = _case(oracle, 3, true, nx=32, ny=32, nv=48)
+    b = wl.box(w)
+    axes = [wl.IX_PA, wl.IX_RT, wl.IX_VT]
+    nodes, acc = [7, 11, 11], [0.1, 0.01, 0.1]
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        best, chi, st = gbk.gbk_fit_ng(prob.handle, true, 0, axes, b[axes, 0], b[axes, 1], nodes, 30, accuracy=acc)
+        capped = gbk.gbk_fit_ng(prob.handle, true, 0, axes, b[axes, 0], b[axes, 1], nodes, 3, accuracy=acc)[2]
+    width = b[axes, 1] - b[axes, 0]
+    need = max(int(np.ceil(np.log2(width[a] / (nodes[a] * acc[a])))) for a in range(3)) + 1   # first level with h <= a on all axes
+    assert st["iterations"] == need and st["evals"] == need * 7 * 11 * 11 and st["converged"] == 1
+    assert capped["iterations"] == 3 and capped["converged"] == 0             # max_levels hit first
+    assert _pa_diff(best[wl.IX_PA], true[wl.IX_PA]) <= 0.2
+    assert abs(best[wl.IX_RT] - true[wl.IX_RT]) <= 0.02 and abs(best[wl.IX_VT] - true[wl.IX_VT]) <= 0.3
+
+
 def test_levenberg_marquardt_recovers_noise_free_parameters(oracle, torch_cuda, gbk):
     w0 = wl.config(1)
     true = _true_row(w0)
@@ -173,6 +193,8 @@ def test_driver_argument_errors(oracle, torch_cuda, gbk):
     with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
         for call in (
             lambda: gbk.gbk_fit_ng(prob.handle, true, 0, [2, 2], [0, 0], [1, 1], 4, 2),       # twice
+            lambda: gbk.gbk_fit_ng(prob.handle, true, 0, [2], [0.0], [1.0], 1, 2),            # one node
+            lambda: gbk.gbk_fit_ng(prob.handle, true, 0, [2], [0.0], [1.0], 4, 2, accuracy=[0.0]),   # threshold 0
             lambda: gbk.gbk_fit_ng(prob.handle, true, 0, [2], [1.0], [1.0], 4, 2),            # empty box
             lambda: gbk.gbk_fit_ng(prob.handle, true, 5, [2], [0.0], [1.0], 4, 2),            # gal
             lambda: gbk.gbk_fit_lm(prob.handle, true[None], None, [11], [0.0], [1.0]),        # index
