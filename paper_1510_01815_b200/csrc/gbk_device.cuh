@@ -9,6 +9,16 @@ namespace {
 
 typedef unsigned long long u64;  // two packed floats {lo, hi}
 
+// Bounds checks of the shared-memory indexing, compiled in with -DGBK_DEBUG_BOUNDS only (the pool
+// this was developed on has compute-sanitizer closed, so the checks a memcheck run would do are
+// written out at the sites that index with run-time strides): a violation traps, the launch fails
+// and every test that follows reports a CUDA error.
+#ifdef GBK_DEBUG_BOUNDS
+#define GBK_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define GBK_CHECK(cond) do { } while (0)
+#endif
+
 __device__ __forceinline__ u64 pk(float lo, float hi) {
   u64 r;
   asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));

@@ -330,6 +330,8 @@ __device__ __forceinline__ u64 tap_sym(const u64 (&tb)[R + 1], int j) {   // j i
 template <int R>
 __device__ __forceinline__ void hpass_x(float* maps, int map_stride, int ews, int EH, int tw,
                                         const u64 (&tb)[R + 1], int tid, int nthreads) {
+  const int dp_ehs_dbg = map_stride / ews;   // rows of a plane (bounds checks only)
+  (void)dp_ehs_dbg;
   constexpr int NV4 = (4 + 2 * R + 3) / 4;
   const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
   const int nx4 = (tw + 3) >> 2;
@@ -353,6 +355,7 @@ __device__ __forceinline__ void hpass_x(float* maps, int map_stride, int ews, in
           float v[NV4 * 4];
 #pragma unroll
           for (int i = 0; i < NV4; ++i) {
+            GBK_CHECK(row < dp_ehs_dbg && x0 + 4 * i + 3 < ews);
             const float4 f = *reinterpret_cast<const float4*>(rowp + q * map_stride + 4 * i);
             v[4 * i] = f.x, v[4 * i + 1] = f.y, v[4 * i + 2] = f.z, v[4 * i + 3] = f.w;
           }
@@ -378,9 +381,9 @@ __device__ __forceinline__ void hpass_x(float* maps, int map_stride, int ews, in
 
 // Vertical pass fused with moments and chi^2 (u == 1): a thread owns BY consecutive rows of a
 // column PAIR; lanes run along x, so the 8-byte shared-memory reads are conflict-free and the
-// global accesses coalesced.  Rows past the tile are read from the (allocated, possibly
-// uninitialised) padding of the plane and only feed outputs that are discarded; likewise the
-// second column of the last pair when the tile width is odd.
+// global accesses coalesced.  Rows past the tile are read from the (allocated, never written)
+// padding of the plane and only feed outputs that are discarded; likewise the second column of the
+// last pair when the tile width is odd.
 template <int R, int BY, bool OUT>
 __device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const EvalArgs& a,
                                                  const RowConst& rc, long long k, const float* maps,
@@ -400,6 +403,7 @@ __device__ __forceinline__ float vpass_x_moments(const DevProblem& dp, const Eva
       for (int m = 0; m < BY; ++m) res[q][m] = pk(0.f, 0.f);
 #pragma unroll
       for (int i = 0; i < BY + 2 * R; ++i) {
+        GBK_CHECK(col + 1 < maps + (q + 1) * map_stride && col >= maps + q * map_stride);
         const u64 v = *reinterpret_cast<const u64*>(col);
         col += ews;
 #pragma unroll
@@ -748,6 +752,8 @@ __device__ __forceinline__ bool poly_block(const RowConst& rc, const Smem& sm, i
   for (int j = 1; j < kPairs; ++j) any_g |= g[j];
   if (!__any_sync(0xffffffffu, any_g != 0ull)) return false;
   // scalar coefficients: FFMA2 takes a broadcast FP32 operand, so no (C, C) pairs are needed
+  GBK_CHECK(b >= 0 && (const float*)((FWD ? sm.coef : sm.coefb) + (b + 1) * (3 * kChanBlock)) <=
+                          (FWD ? (const float*)sm.coefb : (const float*)sm.rcd));
   const float4* C = reinterpret_cast<const float4*>((FWD ? sm.coef : sm.coefb) + b * (3 * kChanBlock));
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
@@ -900,7 +906,10 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       for (int b = b_lo; b <= b_b; ++b) n_poly += poly_block<PRECISE, false>(rc, sm, b, v) ? 1 : 0;
       for (int b = b_b + 1; b < b_f; ++b) {      // lines of this item on both sides of the block
 #pragma unroll
-        for (int cc = 0; cc < kChanBlock; ++cc) direct_channel<PRECISE>(rc, sm.chan[b * kChanBlock + cc], v);
+        for (int cc = 0; cc < kChanBlock; ++cc) {
+          GBK_CHECK(b >= 0 && b * kChanBlock + cc < dp.nvx_pad);
+          direct_channel<PRECISE>(rc, sm.chan[b * kChanBlock + cc], v);
+        }
         n_direct += kChanBlock;
       }
       for (int b = b_f; b <= b_hi; ++b) n_poly += poly_block<PRECISE, true>(rc, sm, b, v) ? 1 : 0;
@@ -909,7 +918,10 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       const int c_lo = min(max(__float2int_rd((-D - dmax) * inv_step), 0), dp.nvx);
       const int c_hi = max(min(__float2int_ru((D - dmin) * inv_step), dp.nvx) - 1, -1);
 #pragma unroll 4
-      for (int c = c_lo; c <= c_hi; ++c) direct_channel<PRECISE>(rc, sm.chan[c], v);
+      for (int c = c_lo; c <= c_hi; ++c) {
+        GBK_CHECK(c >= 0 && c < dp.nvx);
+        direct_channel<PRECISE>(rc, sm.chan[c], v);
+      }
       n_direct += max(c_hi - c_lo + 1, 0);
     }
     ++n_items;
@@ -917,6 +929,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
     for (int j = 0; j < kPairs; ++j)
       if (sidx[j] >= 0) {
         float2 o;
+        GBK_CHECK(sidx[j] + 1 < map_stride && (sidx[j] & 1) == 0);
         upk(mul2(v.s0[j], In[j]), o.x, o.y);
         *reinterpret_cast<float2*>(sm.maps + sidx[j]) = o;
         upk(mul2(v.s1[j], In[j]), o.x, o.y);
@@ -1018,6 +1031,11 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   } else {
     const int R = rc.r_p;
     const int EW = tw + 2 * R, EH = th + 2 * R;
+    // The PSF passes read whole register blocks, i.e. up to 10 columns and 7 rows past the extended tile
+    // inside the plane's allocation (ews x ehs, sized for that in gbk_api.cu).  Nobody writes that padding:
+    // what is read there only feeds outputs that are discarded (columns >= tw, rows >= th), and zeroing it
+    // would cost 5 % on config 5 and 10 % on config 1 for no change in any result.  -DGBK_DEBUG_BOUNDS
+    // checks that every such access stays inside the allocation.
     if (rc.precise)
       voxel_phase_precise(dp, smem_raw, tx0, ty0, EW, EH, R, tid, nthreads, COUNT ? a.counters : nullptr);
     else
