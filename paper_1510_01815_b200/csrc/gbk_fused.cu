@@ -50,7 +50,8 @@ constexpr float kTruncD = GBK_TRUNC_D;        // lines centred in the band are s
 
 // floats of the PSF tap area: image taps of the register-tiled pass are stored as (w, w) pairs
 __host__ __device__ __forceinline__ int taps_floats(const DevProblem& dp) {
-  return round_up4(dp.psf_stride) * (dp.img_fast ? 2 : 1);
+  const int n = 2 * dp.r_p_max + 1;
+  return dp.img_fast ? round_up4(2 * n * (n + 1)) : round_up4(dp.psf_stride);
 }
 
 struct Smem {
@@ -498,7 +499,7 @@ __device__ __noinline__ float conv2d_moments(const DevProblem& dp, const EvalArg
 // 8-pixel chunk of two rows (y and y + th/2): per kernel row it holds the N taps as (w, w) pairs
 // (one 8-byte broadcast read each) and applies them to the two input rows (float4 reads; lanes run
 // along y and the row stride is 4 mod 8 floats, so they are conflict-free), i.e. 8 N FFMA2 for
-// N + 2 NV4 shared-memory reads.  `out` is a different plane than `in`.
+// N + 1 + 2 NV4 shared-memory reads.  `out` is a different plane than `in`.
 template <int N>
 __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ews, int tw, int th,
                                              const u64* w64, int tid, int nthreads) {
@@ -516,9 +517,11 @@ __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ew
       for (int p = 0; p < 4; ++p) acc[m][p] = pk(0.f, 0.f);
 #pragma unroll 1
     for (int ky = 0; ky < N; ++ky) {
-      u64 w[N];
+      // an output pair (x + 2p, x + 2p + 1) receives from input v[i] the tap pair (W[i - 2p], W[i - 2p - 1])
+      // times the broadcast input: N + 1 FFMA2 per pair and kernel row, and no register shuffling
+      u64 w[N + 1];
 #pragma unroll
-      for (int kx = 0; kx < N; ++kx) w[kx] = w64[ky * N + kx];
+      for (int j = 0; j <= N; ++j) w[j] = w64[ky * (N + 1) + j];
 #pragma unroll
       for (int m = 0; m < 2; ++m) {
         const float* rowp = in + (yy[m] + ky) * ews + (xc << 3);
@@ -529,10 +532,10 @@ __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ew
           v[4 * i] = f.x, v[4 * i + 1] = f.y, v[4 * i + 2] = f.z, v[4 * i + 3] = f.w;
         }
 #pragma unroll
-        for (int kx = 0; kx < N; ++kx)
+        for (int i = 0; i < 8 + N - 1; ++i)
 #pragma unroll
           for (int p = 0; p < 4; ++p)
-            acc[m][p] = fma2(w[kx], pk(v[kx + 2 * p], v[kx + 2 * p + 1]), acc[m][p]);
+            if (i - 2 * p >= 0 && i - 2 * p <= N) acc[m][p] = fma2(w[i - 2 * p], pk1(v[i]), acc[m][p]);
       }
     }
 #pragma unroll
@@ -1005,12 +1008,16 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   }
   __syncthreads();
   const RowConst rc = *sm.rc;   // by value: registers, no aliasing with the map stores
-  for (int j = tid; j < dp.psf_stride; j += nthreads) {
-    const float t = dp.psf_taps[(size_t)rc.psf_set * dp.psf_stride + j];
-    if (dp.img_fast)
-      reinterpret_cast<u64*>(sm.taps)[j] = pk1(t);
-    else
-      sm.taps[j] = t;
+  if (dp.img_fast) {   // rows of tap pairs (W[ky][i], W[ky][i-1]), i = 0..N, with W[ky][-1] = W[ky][N] = 0
+    const int n = 2 * rc.r_p + 1;
+    const float* W = dp.psf_taps + (size_t)rc.psf_set * dp.psf_stride;
+    for (int j = tid; j < n * (n + 1); j += nthreads) {
+      const int ky = j / (n + 1), i = j - ky * (n + 1);
+      reinterpret_cast<u64*>(sm.taps)[j] = pk(i < n ? W[ky * n + i] : 0.0f, i >= 1 ? W[ky * n + i - 1] : 0.0f);
+    }
+  } else {
+    for (int j = tid; j < dp.psf_stride; j += nthreads)
+      sm.taps[j] = dp.psf_taps[(size_t)rc.psf_set * dp.psf_stride + j];
   }
 
   float chi = 0.0f;
