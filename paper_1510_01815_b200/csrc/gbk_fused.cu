@@ -1,11 +1,12 @@
 // Fused hot path of libgbk for sm_100a: one thread block = (parameter row k, spatial tile); one launch per batch.
 //
 // What one block does (steps a1..a9 of SURVEY.md section 8(a); PAPER.md = arXiv:1510.01815):
-//   a1  row constants from the 10 parameters (eq. 1-8)
+//   a1  row constants from the parameters (eq. 1-8)
 //   a2  per fine spatial sample of the tile + PSF halo: deprojection (eq. 1-4),
-//       exponential brightness (eq. 5, :110), rotation curve (eq. 6, :120, or ramp), line-of-sight
-//       velocity (eq. 8, :143)
-//   a3  Gaussian line at every extended channel, one MUFU.EX2 per voxel
+//       brightness (eq. 5, :110, or a tabulated profile, :106), rotation curve (eq. 6, :120, the ramp,
+//       or eq. 7, :124-129), line-of-sight velocity (eq. 8, :143)
+//   a3  Gaussian line over the extended channels: summed per block of 8 channels as a
+//       polynomial in the line ratio (two MUFU.EX2 per pixel and block), or voxel by voxel for narrow lines
 //   a4  LSF along v: folded into per-channel weights (see below)
 //   a5  PSF in (x, y) from shared memory: separable Gaussian passes or a general 2-D image
 //   a6  down-sampling by u
@@ -13,19 +14,18 @@
 //   a9  chi^2 (and optional maps / residuals) to global memory
 //
 // The cube never exists, not even in shared memory.  The un-normalised moments
-//   S_q(x, y) = sum_k v_k^q C_k(x, y),  q = 0, 1, 2
+//   S_q(x, y) = sum_k (v_k - v_ref)^q C_k(x, y),  q = 0, 1, 2
 // are linear in the cube, and LSF, PSF and down-sampling are linear and act on different axes,
-// so  S_q = downsample( PSF (*) sum_c w_q[c] line(x, y, c) )  with the per-problem weights
-//   w_q[c] = sum_{k in band} L[k - c] v_k^q
-// (LSF taps L and band edges folded in exactly; built in gbk_api.cu).  Only three 2-D maps per
-// tile are convolved.  m1 = S1/S0, m2 = sqrt(S2/S0 - m1^2).  Velocities are measured from
-// v_center so the FP32 cancellation in m2 stays ~1e-4 km/s.
+// so  S_q = downsample( PSF (*) sum_c w_q[c] line(x, y, c) )  with the weights
+//   w_q[c] = sum_{k in band} L[k - c] (v_k - v_ref)^q
+// (LSF taps L and band edges folded in exactly; built in FP64 in gbk_api.cu about v_center and shifted
+// to the row's reference velocity v_ref in the prologue).  Only three 2-D maps per tile are convolved.
+// m1 = v_ref + S1/S0, m2 = sqrt(S2/S0 - (S1/S0)^2).
 //
-// Instruction economy: the kernel is bound by the MUFU pipe (one ex2 per
-// extended voxel, 16 lanes/clk/SM) only if everything else fits in the issue slots left over, so
-// all FP32 arithmetic is written for Blackwell's packed FFMA2/FMUL2 (two FP32 lanes per issued
-// instruction): pixels are processed in horizontally adjacent pairs in the voxel loop, and the
-// separable PSF passes update output pairs with tap pairs (t[k], t[k-1]) times a broadcast input.
+// Instruction economy: the kernel is bound by the FP32 FMA pipe, so the FP32
+// arithmetic is written for Blackwell's packed FFMA2/FMUL2 (two FP32 lanes per issued instruction, which
+// saves issue slots, not pipe time): pixels are processed in horizontally adjacent pairs in the voxel
+// loop, and the PSF passes combine pixel pairs with broadcast taps or tap pairs with broadcast inputs.
 #include <math.h>
 
 #include "gbk_device.cuh"
@@ -39,14 +39,10 @@ constexpr int kMaxThreads = 256;
 constexpr int kMinBlocks = 3;
 constexpr int kVBlockX = 4;      // output rows per thread in the x-packed vertical pass (divides kVBlock)
 constexpr int kPairs = 2;        // pixel pairs per lane in the voxel loop (4 pixels per thread)
-#ifndef GBK_STRIP_PAIRS
-#define GBK_STRIP_PAIRS 8
-#endif
-#ifndef GBK_TRUNC_D
-#define GBK_TRUNC_D 6.5f
-#endif
-constexpr int kStripPairs = GBK_STRIP_PAIRS;  // width of a strip of the voxel loop in pixel pairs (power of two)
-constexpr float kTruncD = GBK_TRUNC_D;        // lines centred in the band are summed out to |d| < this
+constexpr int kStripPairs = 8;    // width of a strip of the voxel loop in pixel pairs (a power of two; 4 and 16
+                                  // measure the same on config 3)
+constexpr float kTruncD = 6.5f;   // lines centred in the band are summed out to |d| < this (6.0: -1.4 %, 5.5:
+                                  // -2.2 % of config 3's time; 6.5 keeps the left-out tail below 2^-42)
 
 // floats of the PSF tap area: image taps of the register-tiled pass are stored as (w, w) pairs
 __host__ __device__ __forceinline__ int taps_floats(const DevProblem& dp) {
