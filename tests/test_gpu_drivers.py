@@ -286,3 +286,62 @@ def test_monte_carlo_errors_are_consistent_table5(oracle, torch_cuda, gbk):
     # the reduced chi^2 of the fits is ~1 (eq. 11 with the right error bars)
     ndof = 2 * obs.mask.reshape(G * R, -1).sum(axis=1) - 7
     assert 0.9 < float(np.median(chi / ndof)) < 1.1
+
+
+def test_lm_failure_states_are_reported_not_counted_as_converged(oracle, torch_cuda, gbk):
+    """A fit that cannot iterate ends as FAILED (gbk_fit_stats.failed), never as converged: a start row that
+    is out of domain is returned unchanged with chi^2 = +INF; a finite-difference row that leaves the
+    domain (sigma_0 free, stepping to sigma_0 <= 0) stops the fit; a step far below one ulp of the
+    parameter is doubled until it moves the parameter, so no difference is ever divided by a zero step: the
+    fit then either iterates or fails on a noise-dominated Jacobian, but never returns non-finite rows."""
+    w0 = wl.config(1)
+    true = _true_row(w0)
+    w, obs = _case(oracle, 1, true)
+    b = wl.box(w)
+    lo, hi = b[FREE7, 0].copy(), b[FREE7, 1].copy()
+    lo[2], hi[2] = -360.0, 720.0
+    starts = np.repeat(true[None], 3, axis=0).astype(np.float32)
+    starts[:, wl.IX_VT] += 15.0
+    starts[1, wl.IX_R0] = -1.0                      # out of domain from the start
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        chi_start = float(prob.eval(torch_cuda.from_numpy(starts[:1]).cuda())["chi2"].item())
+        rows, chi, iters, st = gbk.gbk_fit_lm(prob.handle, starts, None, FREE7, lo, hi)
+        assert st["failed"] == 1 and st["converged"] == 2
+        assert np.isposinf(chi[1]) and iters[1] == 0 and np.array_equal(rows[1], starts[1])
+        assert np.isfinite(chi[[0, 2]]).all() and abs(rows[0, wl.IX_VT] - true[wl.IX_VT]) <= 5.0
+        # sigma_0 free with a backward difference that crosses zero: the difference row is out of domain
+        s = true.copy()
+        s[wl.IX_SIG] = 1e-3
+        r2, c2, i2, st2 = gbk.gbk_fit_lm(prob.handle, s[None], None, [wl.IX_SIG], [1e-3], [2e-3 - 1e-9],
+                                         rel_step=4.0)      # step 4 x the box width: forward leaves the box, backward crosses 0
+        assert st2["failed"] == 1 and st2["converged"] == 0 and np.array_equal(r2[0], s)
+        # a step of 1e-12 of the box is far below one ulp of V_t = 195: doubled until it moves the parameter
+        r3, c3, i3, st3 = gbk.gbk_fit_lm(prob.handle, starts[:1], None, FREE7, lo, hi, rel_step=1e-12, max_iter=5)
+        assert np.isfinite(r3).all() and np.isfinite(c3[0]) and c3[0] <= chi_start * (1 + 1e-6)
+        assert st3["failed"] + st3["converged"] <= 1
+
+
+def test_nested_grids_ghasp_setup_six_axes_on_the_velocity_field(oracle, torch_cuda, gbk):
+    """The paper's GHASP configuration of the nested-grid optimiser: velocity-field
+    strategy, Epinat curve, grid 7 x 11 x 11 x 5 x 5 over (PA, r_t, V_t, a, g) -- sigma is not part of a
+    velocity field -- with V_sys, centre and inclination fixed; 21 175 rows per level, refined to the
+    paper's accuracy thresholds.  Noise-free data: the velocity field must be reproduced."""
+    w = wl.config(3).scaled(nx=40, ny=36, rc_model=wl.RC_EPINAT, noise=0.0)
+    true = np.array([19.6, 17.7, 123.0, 52.0, 8.0, 180.0, 3.5, 40.0, 8.0, 1.0, 1.3, 0.9], dtype=np.float32)
+    g = pu.oracle_grid(oracle, w)
+    z = np.zeros((w.ny, w.nx), np.float32)
+    v = oracle.vfield_rows(g, z, z + 1, None, true[None], want_maps=True)["vmap"][0]
+    obs = wl.Observed(v[None].astype(np.float32), np.full((1, w.ny, w.nx), 5.0, np.float32),
+                      np.zeros((1, w.ny, w.nx), np.float32), np.ones((1, w.ny, w.nx), np.float32),
+                      np.ones((1, w.ny, w.nx), np.uint8))
+    axes = [wl.IX_PA, wl.IX_RT, wl.IX_VT, 10, 11]
+    lo = np.array([0.0, 1.0, 50.0, 0.3, 0.3], np.float32)
+    hi = np.array([360.0, 8.0, 300.0, 3.0, 3.0], np.float32)
+    with gbk.Problem(**pu.gbk_desc(w, obs)) as prob:
+        assert prob.info.strategy == gbk.GBK_STRATEGY_VFIELD
+        best, chi, st = gbk.gbk_fit_ng(prob.handle, true, 0, axes, lo, hi, [7, 11, 11, 5, 5], 30,
+                                       accuracy=[0.1, 0.01, 0.1, 0.1, 0.1])
+    assert st["converged"] == 1 and st["evals"] == st["iterations"] * 7 * 11 * 11 * 5 * 5
+    npix = w.nx * w.ny
+    assert chi < 0.05 * npix, chi                    # rms residual < 0.22 sigma = 1.1 km/s on a 5 km/s error map
+    assert _pa_diff(best[wl.IX_PA], true[wl.IX_PA]) <= 1.0

@@ -196,3 +196,43 @@ def test_gaussian_profile_extraction(oracle, torch_cuda, gbk, cfg, kw):
     pu.compare(ref_mom, mom, rows, True, "moments after switching back")
     # the two extractions are different things: beam smearing separates them
     assert np.nanmax(np.abs(ref["m2"][0][m] - ref_mom["m2"][0][m])) > 0.05
+
+
+def test_gaussian_profile_extraction_with_an_image_psf_and_two_galaxies(oracle, torch_cuda, gbk):
+    """GBK_EXTRACT_GAUSSFIT on the other branches of the multi-kernel pipeline: a 9 x 9 image PSF (direct
+    2-D sum from a shared-memory tile) and a batch that mixes two data sets."""
+    torch = torch_cuda
+    w = wl.config(4).scaled(nx=26, ny=22, nv=40, psf_n=9, sigma0=25.0, r0_lo=5.0, r0_hi=9.0, mask_rule="m0_rel")
+    rng = wl.rng_for(4, 42)
+    trues = wl.draw_rows(w, rng, 2)
+    img = wl.moffat_image(w.psf_fwhm, w.moffat_beta, w.psf_n).astype(np.float64)
+    g = oracle.Grid(nx=w.nx, ny=w.ny, nv=w.nv, u=1, v_center=0.0, dv=pu.f32(w.dv), rc_model=w.rc_model,
+                    psf=img / img.sum(), lsf=oracle.gaussian_taps(pu.f32(w.lsf_sigma) / pu.f32(w.dv)), extract=1)
+    clean = [oracle.model_maps(g, t.astype(np.float64)) for t in trues]
+    obs = wl.observe(w, *(np.stack([c[i] for c in clean]) for i in range(3)), rng)
+    rows = np.concatenate([np.repeat(t[None], 3, axis=0) for t in trues]).astype(np.float64)
+    rows[[1, 2, 4, 5], wl.IX_VT] += rng.uniform(-15, 15, 4)
+    rows = rows.astype(np.float32)
+    gal = np.array([0, 0, 0, 1, 1, 1], dtype=np.int32)
+    perm = rng.permutation(6)
+    rows, gal = rows[perm], gal[perm]
+    d = pu.gbk_desc(w, obs)
+    d["psf_image"] = wl.moffat_image(w.psf_fwhm, w.moffat_beta, w.psf_n)
+    with gbk.Problem(**d) as prob:
+        prob.set_extraction(gbk.GBK_EXTRACT_GAUSSFIT)
+        out = prob.eval(torch.from_numpy(rows).cuda(), torch.from_numpy(gal).cuda(), want_maps=True)
+        got = {k: v.cpu().numpy().astype(np.float64) for k, v in out.items()}
+    for gi in range(2):
+        sel = np.nonzero(gal == gi)[0]
+        ref = oracle.eval_rows(g, obs.vobs[gi], obs.verr[gi], obs.sobs[gi], obs.serr[gi], obs.mask[gi], rows[sel],
+                               want_maps=True)
+        m = obs.mask[gi] != 0
+        for j, k in enumerate(sel):
+            ok = m & np.isfinite(ref["m1"][j])
+            assert np.array_equal(np.isnan(ref["m1"][j][m]), np.isnan(got["m1"][k][m]))
+            assert np.max(np.abs(got["m1"][k][ok] - ref["m1"][j][ok])) <= pu.TOL_M12_ABS
+            assert np.max(np.abs(got["m2"][k][ok] - ref["m2"][j][ok])) <= pu.TOL_M12_ABS
+            assert np.max(np.abs(got["m0"][k][ok] / ref["m0"][j][ok] - 1.0)) <= pu.TOL_M0_REL
+        fin = np.isfinite(ref["chi2"])
+        assert np.array_equal(fin, np.isfinite(got["chi2"][sel]))
+        assert np.max(np.abs(got["chi2"][sel][fin] / ref["chi2"][fin] - 1.0)) <= pu.TOL_CHI2_REL
