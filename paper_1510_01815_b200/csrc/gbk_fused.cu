@@ -973,7 +973,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   if (tid == 0) row_constants(dp, a, k, sm.rc, sm.rcd);
   {
     // Channel table, and the coefficients of the block polynomial of this row (voxel loop below):
-    // C_m[c] = w_m[c] q^(j(j-1)/2), j = c mod 8, q = 2^(-2 step^2), stored as (C, C) pairs.
+    // C_m[c] = w_m[c] q^(j(j-1)/2), j = c mod 8, q = 2^(-2 step^2), stored as scalars (and the mirrored table).
     const float sigma0 = a.params[k * dp.row_stride + 7];
     const float s_ = 1.0f / (sigma0 * 1.1774100225154747f);
     const float step = s_ * dp.dv;
