@@ -520,9 +520,12 @@ def run_ours(args, ranks) -> None:
     achieved = nominal["ops_per_eval"] * evals_per_s_rank / 1e9
     roofline = {"bound": "alu", "pipe": "FP32 FMA pipe, 128 lanes/clk/SM (FFMA2 = 2 lanes x 2 clk)",
                 "achieved": achieved, "peak": peak_fp32, "unit": "Gop/s", "frac": achieved / peak_fp32,
-                "traffic": None,
-                "traffic_source": "not measured live; dram__bytes of one launch are in profiles/ (ncu --set full): "
-                                  "~0.3 MB per launch of 4096 rows, irrelevant to an ALU-bound kernel",
+                # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, copied from the committed ncu --set full
+                # capture of this command (config 3 only) -- NOT measured in this run
+                "traffic": 423680 if (cfg == 3 and tuple(args.tile) == (0, 0)) else None,
+                "traffic_unit": "bytes per launch",
+                "traffic_source": "profiles/r02_fused_kernel_ncu.md (325.6 KB read + 98.0 KB written per launch of 4096 "
+                                  "rows); a constant from that capture, not measured live; irrelevant to an ALU-bound kernel",
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
                 "ops_per_eval": int(nominal["ops_per_eval"]),
                 "ops_how": "ALGORITHMIC FP32 lane-ops of SURVEY.md 8(d): 5/ext voxel + 45/ext sample + 3 maps x "

@@ -123,7 +123,8 @@ def test_cube_with_a_tabulated_intensity_profile(oracle, torch_cuda, gbk, cfg, t
         rows[:, wl.IX_R0] = true[wl.IX_R0] * rng.uniform(0.6, 1.6, rows.shape[0])     # the table's scale length
         rows[:, wl.IX_INC] = np.clip(rows[:, wl.IX_INC], 5.0, 85.0)
         rows[:, wl.IX_RT] = np.clip(rows[:, wl.IX_RT], 0.5, None)
-        rows = rows.astype(np.float32)
+        rows[-1, wl.IX_VSYS] = 0.5 * w.nv * w.dv + 7.0 * true[wl.IX_SIG]    # line centred 7 sigma_0 outside the band:
+        rows = rows.astype(np.float32)                                       # the FP64 geometry path with the table
         ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows,
                                want_maps=True)
         desc = pu.gbk_desc(w, obs, tile_w=tile[0], tile_h=tile[1], intensity_table=tab, intensity_dx=dx)
