@@ -617,6 +617,34 @@ def run_ours(args, ranks) -> None:
     prob.close()
 
 
+def run_probe_umma() -> None:
+    """--probe-umma: the tcgen05.mma sequence that one 64x64 tile of config 4's 15x15 PSF pass would need as a
+    banded BF16 contraction (gbk_probe_umma), timed with CUDA events: how long the tensor pipe would be busy per
+    tile, to set beside the FFMA2 pass (profiles/r02_tcgen05_probe.md)."""
+    import torch
+    from paper_1510_01815_b200 import gbk
+    gbk.lib()
+    torch.cuda.set_device(0)
+    chk = torch.full((1,), -1.0, dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    out = {"probe": "tcgen05 banded contraction of the 15x15 pass", "sm_count": sms, "runs": []}
+    for per_sm, iters in ((1, 400), (2, 400)):
+        gbk.gbk_probe_umma(iters, per_sm * sms, chk, st)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        flops = gbk.gbk_probe_umma(iters, per_sm * sms, chk, st)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        out["runs"].append({"ctas_per_sm": per_sm, "tile_sequences_per_cta": iters, "ms": ms,
+                            "tflops_bf16_issued": flops / ms / 1e9,
+                            "us_of_tensor_pipe_per_tile_per_sm": ms * 1e3 / (iters * per_sm)})
+    out["check_max_abs_error"] = float(chk[0].item())
+    print(json.dumps(out), flush=True)
+
+
 def time_fits(gbk, torch, prob3, w3, true3) -> dict:
     """Wall time to a converged fit through the host drivers (outside the timed region; rank 0):
     nested grids on the config-3 problem (4 levels x 8^4 rows) and LM on a config-2
@@ -824,10 +852,14 @@ def main() -> None:
     ap.add_argument("--no-fits", action="store_true", help="skip the wall-time-to-fit legs")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config table (configs 1-5)")
     ap.add_argument("--config-launches", type=int, default=25, help="timed launches per config of the table")
+    ap.add_argument("--probe-umma", action="store_true", help="run the tcgen05 probe of the 15x15 pass and exit")
     ap.add_argument("--tile", type=int, nargs=2, default=(0, 0), metavar=("W", "H"),
                     help="spatial tile in spaxels (default 0 0 = the library's automatic tiling)")
     args = ap.parse_args()
     from paper_1510_01815_b200 import dist
+    if args.probe_umma:
+        run_probe_umma()
+        return
     if args.impl == "reference":
         rank = int(os.environ.get("RANK", "0"))
         if rank == 0:

@@ -264,6 +264,18 @@ const char *gbk_last_error(void);
 int gbk_probe_pipe(int which, int64_t iters, int blocks, int threads, float *sink,
                    double *ops_per_launch, void *cuda_stream);
 
+/*
+ * A measured answer to "would tcgen05 help the 15 x 15 image-PSF pass of config 4?" (DESIGN.md
+ * section 5, profiles/): every CTA issues, `iters` times, the tcgen05.mma sequence that one 64 x 64 tile
+ * of that pass would need as a banded contraction -- 15 kernel rows x 3 BF16 split products x 5 K-steps
+ * x (one M = 128 and one M = 64 MMA, N = 64, K = 16), operands in shared memory, accumulators in
+ * TMEM -- after checking ONE MMA on known integers against the exact product.  `check` is a DEVICE
+ * float that receives the largest error of that check (0 = the descriptors mean what they should);
+ * *flops_per_launch receives 2 x multiply-adds issued.  One launch of `blocks` CTAs of 128 threads on
+ * `cuda_stream`; the caller times it.  A probe, not a product path.
+ */
+int gbk_probe_umma(int iters, int blocks, float *check, double *flops_per_launch, void *cuda_stream);
+
 /* ------------------------------------------------------------------------------------------
  * Host drivers: the paper's three optimisers re-stated as callers of the
  * batched hot path.  Each builds batches of rows, calls gbk_eval_batch on `cuda_stream`, reduces

@@ -638,3 +638,12 @@ extern "C" int gbk_probe_pipe(int which, int64_t iters, int blocks, int threads,
   GBK_CUDA(launch_probe(which, iters, blocks, threads, sink, (cudaStream_t)cuda_stream));
   return GBK_OK;
 }
+
+extern "C" int gbk_probe_umma(int iters, int blocks, float* check, double* flops_per_launch, void* cuda_stream) {
+  g_err[0] = 0;
+  if (iters < 1 || blocks < 1 || !check) return fail(GBK_ERR_ARG, "bad probe arguments");
+  if (flops_per_launch)
+    *flops_per_launch = (double)blocks * iters * (15.0 * 3.0 * 5.0) * ((128.0 + 64.0) * 64.0 * 16.0 * 2.0);
+  GBK_CUDA(launch_probe_umma(iters, blocks, check, (cudaStream_t)cuda_stream));
+  return GBK_OK;
+}

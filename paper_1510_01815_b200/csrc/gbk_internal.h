@@ -147,6 +147,7 @@ struct DeviceGuard {
 int fail(int code, const char* fmt, ...);
 void clear_error();
 
+cudaError_t launch_probe_umma(int iters, int blocks, float* out, cudaStream_t st);   // gbk_probe_umma.cu
 cudaError_t launch_probe(int which, long long iters, int blocks, int threads, float* sink,
                          cudaStream_t st);
 

@@ -28,7 +28,7 @@ EXPORTS = (   # every symbol include/gbk.h declares (tests/test_abi_and_dist.py 
     "gbk_create_problem", "gbk_get_info", "gbk_set_strategy", "gbk_set_extraction", "gbk_reserve", "gbk_eval_batch",
     "gbk_eval_batch_counted",
     "gbk_eval_batch_unfused", "gbk_eval_vfield_batch", "gbk_eval_batch_host", "gbk_destroy",
-    "gbk_last_error", "gbk_probe_pipe", "gbk_fit_ng", "gbk_fit_lm", "gbk_fit_ns",
+    "gbk_last_error", "gbk_probe_pipe", "gbk_probe_umma", "gbk_fit_ng", "gbk_fit_lm", "gbk_fit_ns",
 )
 
 
@@ -117,6 +117,8 @@ def lib():
         L.gbk_probe_pipe.argtypes = [C.c_int, C.c_int64, C.c_int, C.c_int, vp,
                                      C.POINTER(C.c_double), vp]
         L.gbk_probe_pipe.restype = C.c_int
+        L.gbk_probe_umma.argtypes = [C.c_int, C.c_int, vp, C.POINTER(C.c_double), vp]
+        L.gbk_probe_umma.restype = C.c_int
         sp = C.POINTER(gbk_fit_stats)
         L.gbk_fit_ng.argtypes = [vp, vp, C.c_int32, C.c_int32, vp, vp, vp, vp, vp, C.c_int32, vp,
                                  vp, sp, vp]
@@ -261,6 +263,13 @@ def gbk_probe_pipe(which: int, iters: int, blocks: int, threads: int, sink, stre
     _check(lib().gbk_probe_pipe(which, iters, blocks, threads, _ptr(sink), C.byref(ops),
                                 stream or None))
     return ops.value
+
+
+def gbk_probe_umma(iters: int, blocks: int, check, stream=0) -> float:
+    """The tcgen05.mma sequence of the 15 x 15 pass as a banded contraction; returns 2 x multiply-adds issued."""
+    fl = C.c_double()
+    _check(lib().gbk_probe_umma(int(iters), int(blocks), _ptr(check), C.byref(fl), stream or None))
+    return fl.value
 
 
 def _stats_dict(st: gbk_fit_stats) -> dict:

@@ -78,3 +78,15 @@ def test_unfused_chunks_rows(oracle, torch_cuda, gbk):
     b = np.concatenate([_gpu_eval(torch_cuda, gbk, pu.gbk_desc(w, obs), rows[i:i + 1], want_maps=False,
                                   unfused=True)["chi2"] for i in (0, 33, 69)])
     assert np.array_equal(a[[0, 33, 69]], b)
+
+
+def test_tcgen05_probe_computes_the_exact_product(torch_cuda, gbk):
+    """gbk_probe_umma checks one tcgen05.mma (M = 128, N = 64, K = 16, BF16 operands from shared memory in
+    the K-major no-swizzle canonical layout, FP32 accumulator in TMEM read back with tcgen05.ld) against the
+    exact integer product before it times the sequence of the 15 x 15 pass: the error must be exactly 0."""
+    torch = torch_cuda
+    chk = torch.full((1,), -1.0, dtype=torch.float32, device="cuda")
+    flops = gbk.gbk_probe_umma(2, 4, chk, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert chk[0].item() == 0.0
+    assert flops == 4 * 2 * 15 * 3 * 5 * (128 + 64) * 64 * 16 * 2
