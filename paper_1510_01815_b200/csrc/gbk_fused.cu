@@ -41,6 +41,7 @@ constexpr int kVBlockX = 4;      // output rows per thread in the x-packed verti
 constexpr int kPairs = 2;        // pixel pairs per lane in the voxel loop (4 pixels per thread)
 constexpr int kStripPairs = 8;    // width of a strip of the voxel loop in pixel pairs (a power of two; 4 and 16
                                   // measure the same on config 3)
+constexpr float kSqueezedMargin = 3.5f;   // like kPreciseMargin: rows that also keep per-pixel central moments
 constexpr float kTruncD = 6.5f;   // lines centred in the band are summed out to |d| < this (6.0: -1.4 %, 5.5:
                                   // -2.2 % of config 3's time; 6.5 keeps the left-out tail below 2^-42)
 
@@ -48,6 +49,11 @@ constexpr float kTruncD = 6.5f;   // lines centred in the band are summed out to
 __host__ __device__ __forceinline__ int taps_floats(const DevProblem& dp) {
   const int n = 2 * dp.r_p_max + 1;
   return dp.img_fast ? round_up4(2 * n * (n + 1)) : round_up4(dp.psf_stride);
+}
+
+// Velocity (from v_center) of the centre of channel block b of the extended band (precise rows).
+__device__ __forceinline__ float block_centre_velocity(const DevProblem& dp, int b) {
+  return dp.vrel_first + ((float)(b * kChanBlock) + 0.5f * (float)(kChanBlock - 1)) * dp.dv;
 }
 
 struct Smem {
@@ -134,18 +140,11 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   // further than kPreciseMargin outside the band shows only its far wing, where the voxel values need
   // d to ~1e-6: those rows take the FP64 geometry.  (A non-finite test value is a row that is out of
   // domain anyway.)
-  float fsup = dp.rc_model == GBK_RC_ARCTAN ? 1.5707963267948966f : 1.0f;
-  if (dp.rc_model == GBK_RC_EPINAT && v[11] > v[10]) {
-    // q^g / (1 + q^a) <= max(1, q^(g - a)): bounded by the largest deprojected radius of the extended field
-    const float R = (float)dp.r_p_max * dp.inv_u + 1.0f;
-    const float ax = fmaxf(fabsf(v[0] + R), fabsf((float)dp.nx + R - v[0]));
-    const float ay = fmaxf(fabsf(v[1] + R), fabsf((float)dp.ny + R - v[1]));
-    const float qmax = sqrtf(ax * ax + ay * ay) * fabsf(inv_ci) / rt;
-    fsup = fmaxf(1.0f, powf(qmax, v[11] - v[10]));
-  }
-  const float tmax = fabsf(rc->k1) * fsup * 1.0001f + 1e-3f;
-  const float band = (float)(dp.nvx - 1) * rc->step;
-  rc->precise = (rc->k0 + tmax > kPreciseMargin || rc->k0 - tmax < -(band + kPreciseMargin)) ? 1 : 0;
+  const float fsup = curve_sup(dp, v, inv_ci);
+  rc->precise = line_leaves_band(dp, rc->k0, rc->k1, fsup, rc->step, kPreciseMargin) ? 1 : 0;
+  // ... and further out than kSqueezedMargin a spaxel may see its line squeezed into the band's edge channel:
+  // those rows also keep per-pixel central moments (precise_finish)
+  rc->squeezed = (rc->precise && line_leaves_band(dp, rc->k0, rc->k1, fsup, rc->step, kSqueezedMargin)) ? 1 : 0;
   rc->step_lo = 0.0f;
   if (rc->precise && rc->valid) {
     double dsp, dcp, dsi, dci;
@@ -170,16 +169,12 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
 // One spaxel: moments from the block sums, residuals, chi^2 contribution, optional outputs.
 // The packed observation has 1/E = 0 where masked and {0, 0} for a missing dispersion map, so
 // neither needs a branch.  OUT = false is the chi^2-only instantiation (no output predicates).
+// The tail of one spaxel from its moments: m1r = velocity about the row's v_ref, var = central variance
+// (NaN m1r marks a model-dark spaxel).
 template <bool OUT>
-__device__ __forceinline__ float spaxel_finish(const DevProblem& dp, const EvalArgs& a,
-                                               const RowConst& rc, long long k, int pix,
-                                               const float4 ob, float S0, float S1, float S2) {
-  // A model-dark spaxel (S0 below the threshold, or not a number) poisons the moments with NaN,
-  // so the one test "contrib < inf" below catches dark, NaN and overflowing spaxels alike.
-  const bool dark = !(S0 >= rc.dark_s0);
-  const float inv = dark ? f_nan() : rcp_approx(S0);
-  float m1r = S1 * inv;
-  const float var = fmaf(-m1r, m1r, S2 * inv);
+__device__ __forceinline__ float spaxel_finish_moments(const DevProblem& dp, const EvalArgs& a,
+                                                       const RowConst& rc, long long k, int pix, const float4 ob,
+                                                       float S0, float m1r, float var, bool dark) {
   float m2 = sqrt_approx(fmaxf(var, 0.0f));                     // fmaxf drops a NaN var: m1r carries it
   const bool unmasked = ob.y > 0.0f;
   float t = (m1r + (rc.v_ref - ob.x)) * ob.y;
@@ -202,6 +197,18 @@ __device__ __forceinline__ float spaxel_finish(const DevProblem& dp, const EvalA
     }
   }
   return contrib;
+}
+
+template <bool OUT>
+__device__ __forceinline__ float spaxel_finish(const DevProblem& dp, const EvalArgs& a,
+                                               const RowConst& rc, long long k, int pix,
+                                               const float4 ob, float S0, float S1, float S2) {
+  // A model-dark spaxel (S0 below the threshold, or not a number) poisons the moments with NaN,
+  // so the one test "contrib < inf" in the tail catches dark, NaN and overflowing spaxels alike.
+  const bool dark = !(S0 >= rc.dark_s0);
+  const float inv = dark ? f_nan() : rcp_approx(S0);
+  const float m1r = S1 * inv;
+  return spaxel_finish_moments<OUT>(dp, a, rc, k, pix, ob, S0, m1r, fmaf(-m1r, m1r, S2 * inv), dark);
 }
 
 __device__ __forceinline__ float4 load_obs(const DevProblem& dp, const RowConst& rc, int pix) {
@@ -721,10 +728,23 @@ __device__ __noinline__ void sample_geometry_f64(const DevProblem& dp, const Row
 struct VoxelAcc {
   u64 d0[kPairs], d0lo[kPairs];              // line-centre offset at extended channel 0 (hi, lo)
   u64 s0[kPairs], s1[kPairs], s2[kPairs];    // the three weighted sums
+  u64 refp[kPairs];                          // precise rows: the pixel's own reference velocity of s1, s2
 };
 
+// Precise rows: a block's sums P0, P1, P2 are about the block's centre velocity vb (build_row_tables); the
+// pixel accumulates them about its own reference ref (its line centre clamped to the band), D = vb - ref:
+//   s0 += g P0,   s1 += g (P1 + D P0),   s2 += g (P2 + 2 D P1 + D^2 P0).
+// The blocks that matter for a pixel lie around ref, so D is small where g is not: no cancellation.
+__device__ __forceinline__ void accumulate_recentred(VoxelAcc& v, int j, u64 g, u64 P0, u64 P1, u64 P2, float vb) {
+  const u64 D = add2(pk1(vb), mul2(v.refp[j], pk1(-1.0f)));
+  v.s0[j] = fma2(g, P0, v.s0[j]);
+  v.s1[j] = fma2(g, fma2(D, P0, P1), v.s1[j]);
+  v.s2[j] = fma2(g, fma2(D, fma2(D, P0, add2(P1, P1)), P2), v.s2[j]);
+}
+
 template <bool PRECISE, bool FWD>
-__device__ __forceinline__ bool poly_block(const RowConst& rc, const Smem& sm, int b, VoxelAcc& v) {
+__device__ __forceinline__ bool poly_block(const DevProblem& dp, const RowConst& rc, const Smem& sm, int b,
+                                           VoxelAcc& v) {
   const float nchan = (float)(b * kChanBlock + (FWD ? 0 : kChanBlock - 1));   // the anchor channel
   const float anchor_hi = nchan * rc.step;
   const u64 slope = pk1(FWD ? rc.m2step : -rc.m2step), ms2 = pk1(rc.mstep2);
@@ -754,6 +774,7 @@ __device__ __forceinline__ bool poly_block(const RowConst& rc, const Smem& sm, i
   GBK_CHECK(b >= 0 && (const float*)((FWD ? sm.coef : sm.coefb) + (b + 1) * (3 * kChanBlock)) <=
                           (FWD ? (const float*)sm.coefb : (const float*)sm.rcd));
   const float4* C = reinterpret_cast<const float4*>((FWD ? sm.coef : sm.coefb) + b * (3 * kChanBlock));
+  u64 P[3][kPairs];
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
     float c[kChanBlock];
@@ -764,12 +785,29 @@ __device__ __forceinline__ bool poly_block(const RowConst& rc, const Smem& sm, i
     }
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) {
-      u64 P = pk1(c[kChanBlock - 1]);
+      u64 Q = pk1(c[kChanBlock - 1]);
 #pragma unroll
-      for (int i = kChanBlock - 2; i >= 0; --i) P = fma2(P, r[j], pk1(c[i]));
-      if (m == 0) v.s0[j] = fma2(g[j], P, v.s0[j]);
-      if (m == 1) v.s1[j] = fma2(g[j], P, v.s1[j]);
-      if (m == 2) v.s2[j] = fma2(g[j], P, v.s2[j]);
+      for (int i = kChanBlock - 2; i >= 0; --i) Q = fma2(Q, r[j], pk1(c[i]));
+      if (PRECISE) {
+        P[m][j] = Q;
+      } else {
+        if (m == 0) v.s0[j] = fma2(g[j], Q, v.s0[j]);
+        if (m == 1) v.s1[j] = fma2(g[j], Q, v.s1[j]);
+        if (m == 2) v.s2[j] = fma2(g[j], Q, v.s2[j]);
+      }
+    }
+  }
+  if (PRECISE) {
+    const float vb = block_centre_velocity(dp, b);
+#pragma unroll
+    for (int j = 0; j < kPairs; ++j) {
+      if (rc.squeezed) {
+        accumulate_recentred(v, j, g[j], P[0][j], P[1][j], P[2][j], vb);
+      } else {
+        v.s0[j] = fma2(g[j], P[0][j], v.s0[j]);
+        v.s1[j] = fma2(g[j], P[1][j], v.s1[j]);
+        v.s2[j] = fma2(g[j], P[2][j], v.s2[j]);
+      }
     }
   }
   return true;
@@ -777,7 +815,7 @@ __device__ __forceinline__ bool poly_block(const RowConst& rc, const Smem& sm, i
 
 // One channel summed directly: the Gaussian line of PAPER.md:199 by one ex2 per voxel.
 template <bool PRECISE>
-__device__ __forceinline__ void direct_channel(const RowConst& rc, const float4 w, VoxelAcc& v) {
+__device__ __forceinline__ void direct_channel(const DevProblem& dp, const RowConst& rc, const float4 w, VoxelAcc& v) {
 #pragma unroll
   for (int j = 0; j < kPairs; ++j) {
     u64 d = fma2(pk1(w.x), pk1(rc.step), v.d0[j]);
@@ -785,9 +823,13 @@ __device__ __forceinline__ void direct_channel(const RowConst& rc, const float4 
     float ea, eb;
     upk(mul2(d, d), ea, eb);
     const u64 g = pk(ex2_approx(-ea), ex2_approx(-eb));
-    v.s0[j] = fma2(pk1(w.y), g, v.s0[j]);
-    v.s1[j] = fma2(pk1(w.z), g, v.s1[j]);
-    v.s2[j] = fma2(pk1(w.w), g, v.s2[j]);
+    if (PRECISE && rc.squeezed) {   // the channel's weights are about the centre of its block
+      accumulate_recentred(v, j, g, pk1(w.y), pk1(w.z), pk1(w.w), block_centre_velocity(dp, (int)w.x >> 3));
+    } else {
+      v.s0[j] = fma2(pk1(w.y), g, v.s0[j]);
+      v.s1[j] = fma2(pk1(w.z), g, v.s1[j]);
+      v.s2[j] = fma2(pk1(w.w), g, v.s2[j]);
+    }
   }
 }
 
@@ -855,6 +897,11 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
         sample_geometry_f64(dp, sm.rcd, rc.nl2e_inv_r0, xa, y, &ha, &la, &ba);
         sample_geometry_f64(dp, sm.rcd, rc.nl2e_inv_r0, xa + inv_ud, y, &hb, &lb, &bb);
         v.d0[j] = pk(ha, hb), v.d0lo[j] = pk(la, lb), In[j] = pk(ba, bb);
+        // the pixel's reference velocity: its line centre (offset -d0 from extended channel 0, in units of
+        // dv / step), clamped to the in-band channels
+        const float to_v = dp.dv / rc.step;
+        v.refp[j] = pk(fminf(fmaxf(dp.vrel_first - ha * to_v, -dp.vhalf), dp.vhalf),
+                       fminf(fmaxf(dp.vrel_first - hb * to_v, -dp.vhalf), dp.vhalf));
       } else {
         const float gx = (float)(tx0 + ex - R), gy = (float)(ty0 + ey - R);
         const float xa = (gx + 0.5f) * inv_u - 0.5f, xb = (gx + 1.5f) * inv_u - 0.5f;
@@ -902,16 +949,16 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       // the mirrored anchor up to block b_b (every line centred at most A before its last channel)
       const int b_f = min(max(__float2int_ru((-A - dmin) * rc.inv_bstep), b_lo), b_hi + 1);
       const int b_b = max(min(__float2int_rd((A - span - dmax) * rc.inv_bstep), b_f - 1), b_lo - 1);
-      for (int b = b_lo; b <= b_b; ++b) n_poly += poly_block<PRECISE, false>(rc, sm, b, v) ? 1 : 0;
+      for (int b = b_lo; b <= b_b; ++b) n_poly += poly_block<PRECISE, false>(dp, rc, sm, b, v) ? 1 : 0;
       for (int b = b_b + 1; b < b_f; ++b) {      // lines of this item on both sides of the block
 #pragma unroll
         for (int cc = 0; cc < kChanBlock; ++cc) {
           GBK_CHECK(b >= 0 && b * kChanBlock + cc < dp.nvx_pad);
-          direct_channel<PRECISE>(rc, sm.chan[b * kChanBlock + cc], v);
+          direct_channel<PRECISE>(dp, rc, sm.chan[b * kChanBlock + cc], v);
         }
         n_direct += kChanBlock;
       }
-      for (int b = b_f; b <= b_hi; ++b) n_poly += poly_block<PRECISE, true>(rc, sm, b, v) ? 1 : 0;
+      for (int b = b_f; b <= b_hi; ++b) n_poly += poly_block<PRECISE, true>(dp, rc, sm, b, v) ? 1 : 0;
     } else {
       const float inv_step = rc.inv_bstep * (float)kChanBlock;
       const int c_lo = min(max(__float2int_rd((-D - dmax) * inv_step), 0), dp.nvx);
@@ -919,7 +966,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
 #pragma unroll 4
       for (int c = c_lo; c <= c_hi; ++c) {
         GBK_CHECK(c >= 0 && c < dp.nvx);
-        direct_channel<PRECISE>(rc, sm.chan[c], v);
+        direct_channel<PRECISE>(dp, rc, sm.chan[c], v);
       }
       n_direct += max(c_hi - c_lo + 1, 0);
     }
@@ -929,6 +976,26 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       if (sidx[j] >= 0) {
         float2 o;
         GBK_CHECK(sidx[j] + 1 < map_stride && (sidx[j] & 1) == 0);
+        if (PRECISE && rc.squeezed) {
+          // these rows keep, per fine pixel, the flux S0 I, the mean velocity M1 (about the row's v_ref) and the
+          // CENTRAL variance V of its line sums -- both formed about the pixel's own reference, where nothing
+          // cancels; precise_finish mixes them through the PSF by the parallel-axis rule
+          float s0a, s0b, s1a, s1b, s2a, s2b, ra, rb;
+          upk(v.s0[j], s0a, s0b), upk(v.s1[j], s1a, s1b), upk(v.s2[j], s2a, s2b), upk(v.refp[j], ra, rb);
+          // a line sum below 1e-36 (it would overflow the reciprocal) counts as no flux at all
+          const bool ha = s0a > 1e-36f, hb = s0b > 1e-36f;
+          const float ia = ha ? 1.0f / s0a : 0.0f, ib = hb ? 1.0f / s0b : 0.0f;
+          const float ma = s1a * ia, mb = s1b * ib;
+          upk(mul2(v.s0[j], In[j]), o.x, o.y);
+          if (!ha) o.x = 0.0f;
+          if (!hb) o.y = 0.0f;
+          *reinterpret_cast<float2*>(sm.maps + sidx[j]) = o;
+          o.x = ha ? (ra - rc.v_ref) + ma : 0.0f, o.y = hb ? (rb - rc.v_ref) + mb : 0.0f;
+          *reinterpret_cast<float2*>(sm.maps + map_stride + sidx[j]) = o;
+          o.x = fmaxf(fmaf(-ma, ma, s2a * ia), 0.0f), o.y = fmaxf(fmaf(-mb, mb, s2b * ib), 0.0f);
+          *reinterpret_cast<float2*>(sm.maps + 2 * map_stride + sidx[j]) = o;
+          continue;
+        }
         upk(mul2(v.s0[j], In[j]), o.x, o.y);
         *reinterpret_cast<float2*>(sm.maps + sidx[j]) = o;
         upk(mul2(v.s1[j], In[j]), o.x, o.y);
@@ -945,6 +1012,55 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
   }
 }
 
+// a5..a9 of a precise row.  The planes hold, per fine pixel i, the flux F_i = S0_i I_i, the mean velocity
+// M_i (about the row's v_ref) and the central variance V_i of its line sums.  A spaxel is the PSF-weighted
+// (and u x u block-summed) mixture of its pixels, so by the parallel-axis rule
+//   S0 = sum_i w_i F_i,   m1 = sum_i w_i F_i M_i / S0,   var = sum_i w_i F_i (V_i + (M_i - m1)^2) / S0
+// -- two passes over the footprint, the second about the spaxel's own mean: nothing cancels even when the
+// spectrum is squeezed into the band's edge channel a hundred km/s from v_ref (m2 ~ 0.1 km/s), where
+// S2/S0 - m1^2 in FP32 is off by more than the tolerance.  Direct 2-D sums, (2R+1)^2 taps per pass: about
+// ten times the work of the separable passes, on rows that are rare.
+template <bool OUT>
+__device__ __noinline__ float precise_finish(const DevProblem& dp, const EvalArgs& a, const RowConst* rcp, long long k,
+                                             const float* maps, int map_stride, int tw, int th, int tx0, int ty0,
+                                             const float* taps, int tid, int nthreads) {
+  const RowConst rc = *rcp;
+  const int u = dp.u, sw = tw / u, sh = th / u, n = 2 * rc.r_p + 1, ews = dp.ews;
+  const bool image = dp.psf_kind == GBK_PSF_IMAGE;
+  float chi = 0.0f;
+  for (int item = tid; item < sw * sh; item += nthreads) {
+    const int Y = item / sw, X = item - Y * sw;
+    const int pix = (ty0 / u + Y) * dp.nx + tx0 / u + X;
+    const float4 ob = load_obs(dp, rc, pix);
+    float A0 = 0.0f, A1 = 0.0f, A2 = 0.0f, m1 = 0.0f;
+    for (int pass = 0; pass < 2; ++pass) {
+      for (int dy = 0; dy < u; ++dy)
+        for (int dx = 0; dx < u; ++dx) {
+          const float* base = maps + (Y * u + dy) * ews + X * u + dx;
+          for (int ky = 0; ky < n; ++ky)
+            for (int kx = 0; kx < n; ++kx) {
+              // Gaussian: outer product of the 1-D taps; image: the flipped image (pairs layout on the fast path)
+              const float w = !image ? taps[ky] * taps[kx]
+                                     : (dp.img_fast ? taps[2 * (ky * (n + 1) + kx)] : taps[ky * n + kx]);
+              const float* q = base + ky * ews + kx;
+              const float wf = w * q[0];
+              if (pass == 0) {
+                A0 += wf;
+                A1 = fmaf(wf, q[map_stride], A1);
+              } else {
+                const float dm = q[map_stride] - m1;
+                A2 = fmaf(wf, fmaf(dm, dm, q[2 * map_stride]), A2);
+              }
+            }
+        }
+      if (pass == 0) m1 = A1 / A0;
+    }
+    const bool dark = !(A0 >= rc.dark_s0);
+    chi += spaxel_finish_moments<OUT>(dp, a, rc, k, pix, ob, A0, dark ? f_nan() : m1, A2 / A0, dark);
+  }
+  return chi;
+}
+
 // Out of line: precise rows are rare, and the FP64 path must not weigh on the register allocation of
 // the common one.
 __device__ __noinline__ void voxel_phase_precise(const DevProblem& dp, unsigned char* smem_raw, int tx0,
@@ -953,6 +1069,43 @@ __device__ __noinline__ void voxel_phase_precise(const DevProblem& dp, unsigned 
   const Smem sm = carve(dp, smem_raw);
   const RowConst rc = *sm.rc;
   voxel_phase<true>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, counters);
+}
+
+// Channel table, and the coefficients of the block polynomial of this row (voxel loop):
+// C_m[c] = w_m[c] q^(j(j-1)/2), j = c mod 8, q = 2^(-2 step^2), stored as scalars (and the mirrored table).
+// The row's moment weights are the problem's w_q about v_center shifted in FP64 to a reference velocity vr,
+//   w1' = w1 - vr w0,   w2' = w2 - 2 vr w1 + vr^2 w0:
+// the row's v_ref (RowConst::v_ref) for ordinary rows; for precise rows (per_block) the velocity of the
+// centre of the channel's own block, so that the block sums of the voxel loop involve small velocities only
+// and each pixel can re-reference them to a velocity of its own without cancellation (precise_finish).
+__device__ __forceinline__ void build_row_tables(const DevProblem& dp, const EvalArgs& a, long long k, const Smem& sm,
+                                                 bool per_block, int tid, int nthreads) {
+  const float sigma0 = a.params[k * dp.row_stride + 7];
+  const float s_ = 1.0f / (sigma0 * 1.1774100225154747f);
+  const float step = s_ * dp.dv;
+  const bool poly = step <= kPolyMaxStep;        // false for NaN: the row is out of domain anyway
+  const double vrow = (double)fminf(fmaxf(a.params[k * dp.row_stride + 4] - dp.v_center, -dp.vhalf), dp.vhalf);
+  for (int c = tid; c < dp.nvx_pad; c += nthreads) {
+    const double vr = per_block ? (double)block_centre_velocity(dp, c >> 3) : vrow;
+    const double w0 = dp.chan_w[3 * c], w1 = dp.chan_w[3 * c + 1], w2 = dp.chan_w[3 * c + 2];
+    const float4 w = make_float4((float)c, (float)w0, (float)(w1 - vr * w0),
+                                 (float)(w2 - vr * (2.0 * w1 - vr * w0)));
+    sm.chan[c] = w;
+    if (poly) {
+      const int j = c & (kChanBlock - 1);
+      const float f = exp2f(-step * step * (float)(j * (j - 1)));
+      float* dst = sm.coef + (c >> 3) * (3 * kChanBlock) + j;
+      dst[0] = w.y * f;
+      dst[kChanBlock] = w.z * f;
+      dst[2 * kChanBlock] = w.w * f;
+      const int i = kChanBlock - 1 - j;            // the same channel counted from the block's end
+      const float fb = exp2f(-step * step * (float)(i * (i - 1)));
+      dst = sm.coefb + (c >> 3) * (3 * kChanBlock) + i;
+      dst[0] = w.y * fb;
+      dst[kChanBlock] = w.z * fb;
+      dst[2 * kChanBlock] = w.w * fb;
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------ the kernel ---
@@ -971,39 +1124,13 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   const int map_stride = dp.ehs * dp.ews;
 
   if (tid == 0) row_constants(dp, a, k, sm.rc, sm.rcd);
-  {
-    // Channel table, and the coefficients of the block polynomial of this row (voxel loop below):
-    // C_m[c] = w_m[c] q^(j(j-1)/2), j = c mod 8, q = 2^(-2 step^2), stored as scalars (and the mirrored table).
-    const float sigma0 = a.params[k * dp.row_stride + 7];
-    const float s_ = 1.0f / (sigma0 * 1.1774100225154747f);
-    const float step = s_ * dp.dv;
-    const bool poly = step <= kPolyMaxStep;        // false for NaN: the row is out of domain anyway
-    // the row's moment weights: the problem's w_q about v_center shifted to v_ref (RowConst::v_ref) in FP64,
-    //   w1' = w1 - v_ref w0,   w2' = w2 - 2 v_ref w1 + v_ref^2 w0
-    const double vr = (double)fminf(fmaxf(a.params[k * dp.row_stride + 4] - dp.v_center, -dp.vhalf), dp.vhalf);
-    for (int c = tid; c < dp.nvx_pad; c += nthreads) {
-      const double w0 = dp.chan_w[3 * c], w1 = dp.chan_w[3 * c + 1], w2 = dp.chan_w[3 * c + 2];
-      const float4 w = make_float4((float)c, (float)w0, (float)(w1 - vr * w0),
-                                   (float)(w2 - vr * (2.0 * w1 - vr * w0)));
-      sm.chan[c] = w;
-      if (poly) {
-        const int j = c & (kChanBlock - 1);
-        const float f = exp2f(-step * step * (float)(j * (j - 1)));
-        float* dst = sm.coef + (c >> 3) * (3 * kChanBlock) + j;
-        dst[0] = w.y * f;
-        dst[kChanBlock] = w.z * f;
-        dst[2 * kChanBlock] = w.w * f;
-        const int i = kChanBlock - 1 - j;            // the same channel counted from the block's end
-        const float fb = exp2f(-step * step * (float)(i * (i - 1)));
-        dst = sm.coefb + (c >> 3) * (3 * kChanBlock) + i;
-        dst[0] = w.y * fb;
-        dst[kChanBlock] = w.z * fb;
-        dst[2 * kChanBlock] = w.w * fb;
-      }
-    }
-  }
+  build_row_tables(dp, a, k, sm, false, tid, nthreads);
   __syncthreads();
   const RowConst rc = *sm.rc;   // by value: registers, no aliasing with the map stores
+  if (rc.squeezed && rc.valid) {  // moment weights about the centre of every channel block (build_row_tables)
+    build_row_tables(dp, a, k, sm, true, tid, nthreads);
+    __syncthreads();
+  }
   if (dp.img_fast) {   // rows of tap pairs (W[ky][i], W[ky][i-1]), i = 0..N, with W[ky][-1] = W[ky][N] = 0
     const int n = 2 * rc.r_p + 1;
     const float* W = dp.psf_taps + (size_t)rc.psf_set * dp.psf_stride;
@@ -1045,7 +1172,9 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
       voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, COUNT ? a.counters : nullptr);
     __syncthreads();
     // ------------------------------------------------------------------ a5 .. a9 ---------
-    if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {
+    if (rc.squeezed) {
+      chi = precise_finish<OUT>(dp, a, sm.rc, k, sm.maps, map_stride, tw, th, tx0, ty0, sm.taps, tid, nthreads);
+    } else if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {
 #define GBK_IMG_CASE(NN)                                                                          \
   case NN:                                                                                        \
     chi = image_phase<NN, OUT>(dp, a, rc, k, sm.maps, sm.spare, map_stride, tw, th, tx0, ty0,     \

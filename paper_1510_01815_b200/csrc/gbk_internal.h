@@ -88,6 +88,9 @@ struct RowConst {
   int psf_set, gal;
   int precise;        // some line of this row may be centred outside the extended band by more than
                       // kPreciseMargin: the voxel loop takes the FP64-geometry path
+  int squeezed;       // precise, and a line may be centred more than kSqueezedMargin outside the band: a spaxel
+                      // can then see its line squeezed into the edge channel (m2 << dv), where S2/S0 - m1^2
+                      // cancels in FP32 -- such rows keep per-pixel central moments (gbk_fused.cu, precise_finish)
   float step_lo;      // step = step + step_lo to FP64 accuracy (precise rows only)
 };
 
@@ -106,6 +109,31 @@ struct RowConstD {
 };
 
 constexpr float kPreciseMargin = 2.5f;   // in units of the line offset d (1.18 sigma_0 each)
+
+#ifdef __CUDACC__
+// sup over the extended field of |f(r / r_t)|, the shape of the rotation curve (v_rot = V_t f, with the 2/pi
+// of eq. 6 left out): bounds how far from V_sys a line of the row can be centred.  v = the parameter row.
+__device__ inline float curve_sup(const DevProblem& dp, const float* v, float inv_ci) {
+  float fsup = dp.rc_model == GBK_RC_ARCTAN ? 1.5707963267948966f : 1.0f;
+  if (dp.rc_model == GBK_RC_EPINAT && v[11] > v[10]) {
+    // q^g / (1 + q^a) <= max(1, q^(g - a)): bounded by the largest deprojected radius of the extended field
+    const float R = (float)dp.r_p_max * dp.inv_u + 1.0f;
+    const float ax = fmaxf(fabsf(v[0] + R), fabsf((float)dp.nx + R - v[0]));
+    const float ay = fmaxf(fabsf(v[1] + R), fabsf((float)dp.ny + R - v[1]));
+    const float qmax = sqrtf(ax * ax + ay * ay) * fabsf(inv_ci) / v[6];
+    fsup = fmaxf(1.0f, powf(qmax, v[11] - v[10]));
+  }
+  return fsup;
+}
+// With d0 = k1 f cos(theta) + k0 the offset of a line from extended channel 0 in units of `step` per channel:
+// can a line of the row be centred more than `margin` outside the extended band?
+__device__ inline bool line_leaves_band(const DevProblem& dp, float k0, float k1, float fsup, float step,
+                                        float margin) {
+  const float tmax = fabsf(k1) * fsup * 1.0001f + 1e-3f;
+  const float band = (float)(dp.nvx - 1) * step;
+  return k0 + tmax > margin || k0 - tmax < -(band + margin);
+}
+#endif
 
 struct FusedLaunch {
   int threads;

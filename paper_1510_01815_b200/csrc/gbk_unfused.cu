@@ -26,6 +26,8 @@ namespace {
 struct URow {          // constants of one parameter row (a1)
   float xo, yo, sp, cp, si, inv_ci, vsys, vt, inv_rt, inv_r0, i0, sigma0, ea, eg;
   int gal, psf_set, r_p, valid;
+  int precise;         // a line may be centred well outside the band: FP64 geometry (as in the fused kernel)
+  double dsp, dcp, dsi, dinv_ci, drt;
 };
 
 __device__ URow uf_row(const DevProblem& dp, const float* params, const int32_t* gal_index, long long k) {
@@ -48,6 +50,19 @@ __device__ URow uf_row(const DevProblem& dp, const float* params, const int32_t*
   r.r_p = dp.psf_r[r.psf_set];
   r.valid = finite && gal_ok && p[7] > 0.f && p[8] > 0.f && p[6] > 0.f && p[9] > 0.f && !(fabsf(ci) < 1e-6f) &&
             r.ea > 0.f && r.eg > 0.f;
+  // the fused kernel's criterion: only the far wing of such a line is in the band, where
+  // the voxel values need the line offset to ~1e-6 sigma_0
+  const float s = 1.0f / (p[7] * 1.1774100225154747f);
+  const float k1 = -s * (dp.rc_model == GBK_RC_ARCTAN ? 0.63661977236758134f : 1.0f) * p[5] * r.si;
+  const float k0 = s * dp.vrel_first - s * (p[4] - dp.v_center);
+  r.precise = r.valid && line_leaves_band(dp, k0, k1, curve_sup(dp, p, r.inv_ci), s * dp.dv, kPreciseMargin);
+  r.dsp = r.dcp = r.dsi = r.dinv_ci = 0.0, r.drt = (double)p[6];
+  if (r.precise) {
+    double dci;
+    sincospi((double)p[2] * (1.0 / 180.0), &r.dsp, &r.dcp);
+    sincospi((double)p[3] * (1.0 / 180.0), &r.dsi, &dci);
+    r.dinv_ci = 1.0 / dci;
+  }
   return r;
 }
 
@@ -110,6 +125,26 @@ __global__ void uf_cube_kernel(const __grid_constant__ DevProblem dp, const URow
     const float vlos = (r.vsys - dp.v_center) + vrot * r.si * cos_t;        // eq. 8, from v_center
     const float amp = bright * dp.dv / (r.sigma0 * 2.5066282746310002f) ; // A3
     const float inv_s = 1.0f / r.sigma0;
+    if (r.precise) {   // the same formulas with the line offset in FP64 (rare rows)
+      const double dx = ((double)(ex - g.R) + 0.5) / (double)dp.u - 0.5 - (double)r.xo;
+      const double dy = ((double)(ey - g.R) + 0.5) / (double)dp.u - 0.5 - (double)r.yo;
+      const double dxe = -dx * r.dsp + dy * r.dcp, dye = (-dx * r.dcp - dy * r.dsp) * r.dinv_ci;
+      const double drad = sqrt(dxe * dxe + dye * dye);
+      const double dcos = drad > 0.0 ? dxe / drad : 0.0;
+      const double dq = drad / r.drt;
+      double dvrot;
+      if (dp.rc_model == GBK_RC_ARCTAN) dvrot = 0.63661977236758134 * (double)r.vt * atan(dq);
+      else if (dp.rc_model == GBK_RC_RAMP) dvrot = (double)r.vt * fmin(dq, 1.0);
+      else dvrot = dq > 0.0 ? (double)r.vt * pow(dq, (double)r.eg) / (1.0 + pow(dq, (double)r.ea)) : 0.0;
+      const double dvlos = ((double)r.vsys - (double)dp.v_center) + dvrot * r.dsi * dcos;
+      const double first = (-(double)dp.r_v - 0.5 * (double)(dp.nv - 1)) * (double)dp.dv - dvlos;
+      const double dinv_s = 1.0 / (double)r.sigma0;
+      for (int c = 0; c < g.nvx; ++c) {
+        const float t = (float)(((double)c * (double)dp.dv + first) * dinv_s);
+        out[(size_t)c * g.plane] = amp * expf(-0.5f * t * t);
+      }
+      continue;
+    }
     for (int c = 0; c < g.nvx; ++c) {
       const float t = (dp.vrel_first + (float)c * dp.dv - vlos) * inv_s;
       out[(size_t)c * g.plane] = amp * expf(-0.5f * t * t);
@@ -311,8 +346,10 @@ __global__ void __launch_bounds__(256) uf_psf2d_kernel(const __grid_constant__ D
 
 // Steps 3-5: per spaxel, down-sample every channel (mean over the u x u block),
 // moments, residuals against the packed observation, and the spaxel's chi^2 contribution.  One pass
-// over the spectrum: S0, S1, S2 about a reference velocity close to the line (V_sys clamped to the
-// band, as in the fused kernel), then m1 = S1/S0, m2^2 = S2/S0 - m1^2.
+// over the spectrum with the weighted running-mean update (W' = W + w; mean += (w / W')(v - mean);
+// M2 += (v - mean_old)^2 W w / W'), velocities from a reference close to the line (V_sys clamped
+// to the band, as in the fused kernel): m1 = mean, m2^2 = M2 / W.  Unlike S2/S0 - m1^2 this does not
+// cancel where a line centred far outside the band leaves m2 << dv.
 __global__ void uf_moments_kernel(const __grid_constant__ DevProblem dp, const URow* __restrict__ rows,
                                   long long k0, int nrows, const float* __restrict__ cube,
                                   float* __restrict__ contrib, const EvalArgs a) {
@@ -336,15 +373,17 @@ __global__ void uf_moments_kernel(const __grid_constant__ DevProblem dp, const U
       const float* src = cube + (size_t)row * g.cube + (size_t)(Y * dp.u) * dp.fw + X * dp.u;
       const float v_ref = fminf(fmaxf(r.vsys - dp.v_center, -dp.vhalf), dp.vhalf);
       const float v_first = -dp.vhalf - v_ref;                               // channel 0 from the reference
-      float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f;
+      float s0 = 0.0f, mean = 0.0f, s2 = 0.0f;
       if (dp.u == 1) {
 #pragma unroll 8
         for (int c = 0; c < dp.nv; ++c) {
           const float blk = src[(size_t)c * cplane];
           const float v = fmaf((float)c, dp.dv, v_first);
+          const float w_old = s0;
           s0 += blk;
-          s1 = fmaf(blk, v, s1);
-          s2 = fmaf(blk * v, v, s2);
+          const float dl = v - mean, rw = s0 > 0.0f ? __fdividef(blk, s0) : 0.0f;
+          mean = fmaf(rw, dl, mean);
+          s2 = fmaf(dl * dl, w_old * rw, s2);
         }
       } else {
         for (int c = 0; c < dp.nv; ++c) {
@@ -353,14 +392,16 @@ __global__ void uf_moments_kernel(const __grid_constant__ DevProblem dp, const U
             for (int dx = 0; dx < dp.u; ++dx) blk += src[(size_t)c * cplane + (size_t)dy * dp.fw + dx];
           blk *= dp.inv_u2;
           const float v = fmaf((float)c, dp.dv, v_first);
+          const float w_old = s0;
           s0 += blk;
-          s1 = fmaf(blk, v, s1);
-          s2 = fmaf(blk * v, v, s2);
+          const float dl = v - mean, rw = s0 > 0.0f ? __fdividef(blk, s0) : 0.0f;
+          mean = fmaf(rw, dl, mean);
+          s2 = fmaf(dl * dl, w_old * rw, s2);
         }
       }
       m0 = s0;
-      m1 = s1 / s0;
-      const float var = s2 / s0 - m1 * m1;
+      m1 = s0 > 0.0f ? mean : nan;
+      const float var = s2 / s0;
       m2 = var > 0.0f ? sqrtf(var) : (var == var ? 0.0f : var);            // A5
       const bool dark = !(m0 >= 1e-30f * r.i0);                             // A15
       t = (m1 + (v_ref - ob.x)) * ob.y;
@@ -537,7 +578,7 @@ inline unsigned grid_for(long long n, int threads, int sm_count) {
 
 size_t unfused_bytes_per_row(const DevProblem& dp) {
   const UGeom g = uf_geom(dp);
-  return sizeof(float) * (2 * g.cube + (size_t)dp.nx * dp.ny) + sizeof(URow);
+  return sizeof(float) * (2 * g.cube + (size_t)dp.nx * dp.ny) + sizeof(URow) + 16;   // + 16: URow alignment
 }
 
 // Algorithmic HBM bytes of the unfused pipeline per row: every array written once and read once by
@@ -567,7 +608,8 @@ cudaError_t launch_unfused(const DevProblem& dp, const EvalArgs& a, const float*
   float* A = scratch;
   float* B = A + (size_t)chunk_rows * g.cube;
   float* contrib = B + (size_t)chunk_rows * g.cube;
-  URow* rows = reinterpret_cast<URow*>(contrib + (size_t)chunk_rows * npix);
+  const uintptr_t rows_at = reinterpret_cast<uintptr_t>(contrib + (size_t)chunk_rows * npix);
+  URow* rows = reinterpret_cast<URow*>((rows_at + 15) & ~(uintptr_t)15);   // URow holds doubles
   const unsigned wide = (unsigned)sm_count * 16;      // block-per-job kernels: grid-stride over the jobs
   for (long long k0 = 0; k0 < a.K; k0 += chunk_rows) {
     const int n = (int)std::min(chunk_rows, a.K - k0);

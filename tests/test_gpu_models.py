@@ -237,3 +237,67 @@ def test_gaussian_profile_extraction_with_an_image_psf_and_two_galaxies(oracle, 
         fin = np.isfinite(ref["chi2"])
         assert np.array_equal(fin, np.isfinite(got["chi2"][sel]))
         assert np.max(np.abs(got["chi2"][sel][fin] / ref["chi2"][fin] - 1.0)) <= pu.TOL_CHI2_REL
+
+
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("GBK_MODEL_FUZZ_CASES", "60"))))
+def test_random_shapes_with_the_epinat_curve_and_tabulated_profiles(oracle, torch_cuda, gbk, seed):
+    """Seeded random problems for the section-8(f) models: odd grid sizes, up-sampling, Gaussian or image PSFs,
+    delta or wide LSFs, explicit or automatic tiles -- with the Epinat curve (random slopes), a random tabulated
+    profile, or both; chi^2 and maps against the oracle, fused path (and the unfused one on every fourth case)."""
+    rng = np.random.default_rng(7_1510_01815 + seed)
+    nx, ny = int(rng.integers(4, 30)), int(rng.integers(4, 26))
+    u = int(rng.choice([1, 1, 2, 3]))
+    nv = int(rng.integers(14, 60))
+    dv = float(rng.choice([10.0, 20.0, 30.0]))
+    epinat = bool(rng.random() < 0.7)
+    table = bool(rng.random() < 0.6) or not epinat
+    image = bool(rng.random() < 0.35)
+    kw = dict(nx=nx, ny=ny, nv=nv, u=u, dv=dv, rc_model=wl.RC_EPINAT if epinat else int(rng.integers(0, 2)),
+              lsf_sigma=float(rng.choice([0.0, 0.7, 1.5])) * dv)
+    if image:
+        n = int(rng.choice([3, 5, 9, 13]))
+        img = rng.random((n, n)).astype(np.float32) + 0.05
+        w = wl.config(4).scaled(psf_n=n, sigma0=float(rng.uniform(0.6, 2.5)) * dv, r0_lo=4.0, r0_hi=9.0,
+                                mask_rule="m0_rel", **kw)
+        psf = img.astype(np.float64) / img.astype(np.float64).sum()
+    else:
+        fw = float(rng.choice([0.0, 0.9, 1.8, 2.7]))
+        w = wl.config(1).scaled(psf_fwhm=fw, sigma0=float(rng.uniform(0.6, 2.5)) * dv, **kw)
+        psf = oracle.psf_gaussian_image(pu.f32(fw), u)
+    tab, tab_dx = None, 0.0
+    if table:
+        ntab = int(rng.integers(2, 40))
+        tab_dx = float(rng.uniform(0.05, 0.8))
+        tab = (rng.uniform(0.1, 1.0, ntab) * np.exp(-0.3 * tab_dx * np.arange(ntab))).astype(np.float32)
+    lsf = oracle.gaussian_taps(pu.f32(w.lsf_sigma) / pu.f32(w.dv) if w.lsf_sigma > 0 else 0.0)
+    g = oracle.Grid(nx=nx, ny=ny, nv=nv, u=u, v_center=0.0, dv=pu.f32(dv), rc_model=w.rc_model, psf=psf, lsf=lsf,
+                    tab=None if tab is None else tab.astype(np.float64), tab_dx=pu.f32(tab_dx))
+    true = [0.5 * nx + rng.uniform(-1, 1), 0.5 * ny + rng.uniform(-1, 1), rng.uniform(0, 360), rng.uniform(20, 75),
+            rng.uniform(-40, 40), rng.uniform(60, 280), rng.uniform(1, 6), w.sigma0, rng.uniform(3, 8),
+            rng.uniform(0.5, 3)]
+    if epinat:
+        true += [rng.uniform(0.5, 2.5), rng.uniform(0.5, 2.5)]
+    true = np.asarray(true, dtype=np.float32)
+    m0, m1, m2 = oracle.model_maps(g, true.astype(np.float64))
+    obs = wl.observe(w, m0[None], m1[None], m2[None], rng)
+    K = int(rng.choice([1, 4, 9]))
+    rows = np.repeat(true[None].astype(np.float64), K, axis=0)
+    width = np.array([0.2 * nx, 0.2 * ny, 360.0, 60.0, 100.0, 250.0, 7.0, 0.0, 0.0, 0.0] + ([2.0, 2.0] if epinat else []))
+    rows[1:] += 0.1 * width * rng.uniform(-1, 1, (K - 1, rows.shape[1]))
+    rows[:, wl.IX_INC] = np.clip(rows[:, wl.IX_INC], 5.0, 85.0)
+    rows[:, wl.IX_RT] = np.clip(rows[:, wl.IX_RT], 0.5, None)
+    if epinat:
+        rows[:, 10:] = np.clip(rows[:, 10:], 0.3, 3.0)
+    rows = rows.astype(np.float32)
+    ref = oracle.eval_rows(g, obs.vobs[0], obs.verr[0], obs.sobs[0], obs.serr[0], obs.mask[0], rows, want_maps=True)
+    d = pu.gbk_desc(w, obs)
+    if image:
+        d["psf_image"] = img
+    if table:
+        d["intensity_table"], d["intensity_dx"] = tab, tab_dx
+    if rng.random() < 0.5:
+        d["tile_w"], d["tile_h"] = int(rng.integers(1, nx + 1)), int(rng.integers(1, ny + 1))
+    label = f"model fuzz {seed}: {kw} epinat={epinat} table={table} image={image}"
+    pu.compare(ref, _eval(torch_cuda, gbk, d, rows), rows, True, label)
+    if seed % 4 == 0:
+        pu.compare(ref, _eval(torch_cuda, gbk, d, rows, unfused=True), rows, True, label + " unfused")
