@@ -41,6 +41,7 @@ constexpr int kVBlockX = 4;      // output rows per thread in the x-packed verti
 constexpr int kPairs = 2;        // pixel pairs per lane in the voxel loop (4 pixels per thread)
 constexpr int kStripPairs = 8;    // width of a strip of the voxel loop in pixel pairs (a power of two; 4 and 16
                                   // measure the same on config 3)
+constexpr int kSqueezed = 2;               // RowConst::precise of such rows
 constexpr float kSqueezedMargin = 3.5f;   // like kPreciseMargin: rows that also keep per-pixel central moments
 constexpr float kTruncD = 6.5f;   // lines centred in the band are summed out to |d| < this (6.0: -1.4 %, 5.5:
                                   // -2.2 % of config 3's time; 6.5 keeps the left-out tail below 2^-42)
@@ -144,7 +145,7 @@ __device__ void row_constants(const DevProblem& dp, const EvalArgs& a, long long
   rc->precise = line_leaves_band(dp, rc->k0, rc->k1, fsup, rc->step, kPreciseMargin) ? 1 : 0;
   // ... and further out than kSqueezedMargin a spaxel may see its line squeezed into the band's edge channel:
   // those rows also keep per-pixel central moments (precise_finish)
-  rc->squeezed = (rc->precise && line_leaves_band(dp, rc->k0, rc->k1, fsup, rc->step, kSqueezedMargin)) ? 1 : 0;
+  if (rc->precise && line_leaves_band(dp, rc->k0, rc->k1, fsup, rc->step, kSqueezedMargin)) rc->precise = kSqueezed;
   rc->step_lo = 0.0f;
   if (rc->precise && rc->valid) {
     double dsp, dcp, dsi, dci;
@@ -801,7 +802,7 @@ __device__ __forceinline__ bool poly_block(const DevProblem& dp, const RowConst&
     const float vb = block_centre_velocity(dp, b);
 #pragma unroll
     for (int j = 0; j < kPairs; ++j) {
-      if (rc.squeezed) {
+      if ((rc.precise == kSqueezed)) {
         accumulate_recentred(v, j, g[j], P[0][j], P[1][j], P[2][j], vb);
       } else {
         v.s0[j] = fma2(g[j], P[0][j], v.s0[j]);
@@ -823,7 +824,7 @@ __device__ __forceinline__ void direct_channel(const DevProblem& dp, const RowCo
     float ea, eb;
     upk(mul2(d, d), ea, eb);
     const u64 g = pk(ex2_approx(-ea), ex2_approx(-eb));
-    if (PRECISE && rc.squeezed) {   // the channel's weights are about the centre of its block
+    if (PRECISE && (rc.precise == kSqueezed)) {   // the channel's weights are about the centre of its block
       accumulate_recentred(v, j, g, pk1(w.y), pk1(w.z), pk1(w.w), block_centre_velocity(dp, (int)w.x >> 3));
     } else {
       v.s0[j] = fma2(pk1(w.y), g, v.s0[j]);
@@ -976,7 +977,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       if (sidx[j] >= 0) {
         float2 o;
         GBK_CHECK(sidx[j] + 1 < map_stride && (sidx[j] & 1) == 0);
-        if (PRECISE && rc.squeezed) {
+        if (PRECISE && (rc.precise == kSqueezed)) {
           // these rows keep, per fine pixel, the flux S0 I, the mean velocity M1 (about the row's v_ref) and the
           // CENTRAL variance V of its line sums -- both formed about the pixel's own reference, where nothing
           // cancels; precise_finish mixes them through the PSF by the parallel-axis rule
@@ -1108,6 +1109,11 @@ __device__ __forceinline__ void build_row_tables(const DevProblem& dp, const Eva
   }
 }
 
+__device__ __noinline__ void build_block_tables(const DevProblem& dp, const EvalArgs& a, long long k,
+                                                unsigned char* smem_raw, int tid, int nthreads) {
+  build_row_tables(dp, a, k, carve(dp, smem_raw), true, tid, nthreads);
+}
+
 // ------------------------------------------------------------------------------ the kernel ---
 template <bool OUT, bool COUNT>
 __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
@@ -1127,8 +1133,8 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   build_row_tables(dp, a, k, sm, false, tid, nthreads);
   __syncthreads();
   const RowConst rc = *sm.rc;   // by value: registers, no aliasing with the map stores
-  if (rc.squeezed && rc.valid) {  // moment weights about the centre of every channel block (build_row_tables)
-    build_row_tables(dp, a, k, sm, true, tid, nthreads);
+  if ((rc.precise == kSqueezed) && rc.valid) {  // moment weights about the centre of every channel block (build_row_tables)
+    build_block_tables(dp, a, k, smem_raw, tid, nthreads);
     __syncthreads();
   }
   if (dp.img_fast) {   // rows of tap pairs (W[ky][i], W[ky][i-1]), i = 0..N, with W[ky][-1] = W[ky][N] = 0
@@ -1172,7 +1178,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
       voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, COUNT ? a.counters : nullptr);
     __syncthreads();
     // ------------------------------------------------------------------ a5 .. a9 ---------
-    if (rc.squeezed) {
+    if ((rc.precise == kSqueezed)) {
       chi = precise_finish<OUT>(dp, a, sm.rc, k, sm.maps, map_stride, tw, th, tx0, ty0, sm.taps, tid, nthreads);
     } else if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {
 #define GBK_IMG_CASE(NN)                                                                          \

@@ -88,7 +88,7 @@ struct RowConst {
   int psf_set, gal;
   int precise;        // some line of this row may be centred outside the extended band by more than
                       // kPreciseMargin: the voxel loop takes the FP64-geometry path
-  int squeezed;       // precise, and a line may be centred more than kSqueezedMargin outside the band: a spaxel
+                      // = 2 (kSqueezed) when a line may be centred more than kSqueezedMargin outside: a spaxel
                       // can then see its line squeezed into the edge channel (m2 << dv), where S2/S0 - m1^2
                       // cancels in FP32 -- such rows keep per-pixel central moments (gbk_fused.cu, precise_finish)
   float step_lo;      // step = step + step_lo to FP64 accuracy (precise rows only)
