@@ -212,6 +212,31 @@ int gbk_eval_batch_counted(gbk_problem *p, const float *params, const int32_t *g
 int gbk_reserve(gbk_problem *p, int64_t K_max, void *cuda_stream);
 
 /*
+ * gbk_eval_batch for callers that cannot allocate at all (a stream capture without a gbk_reserve
+ * beforehand, a serving loop or a harness that forbids cudaMalloc): same arguments, same kernel,
+ * same results, but the cross-tile scratch of a tiled launch (one chi^2 partial per row and tile,
+ * one tile counter per row) lives in a fixed array in the library's device image instead of the
+ * per-stream scratch that gbk_eval_batch grows with cudaMalloc.  The call never calls cudaMalloc,
+ * cudaFree or any allocating routine, and never synchronises: it clears the K tile counters with a
+ * cudaMemsetAsync on `cuda_stream` and launches the kernel there.
+ * Limits (the size of the array, 4.25 MiB, which every GPU that loads the library holds until the
+ * process exits):  K <= GBK_STATIC_MAX_ROWS  and  K x tiles <= GBK_STATIC_MAX_PARTIALS, tiles being
+ * the tiles per row of the tiling the library picks for K rows (tiles_x x tiles_y of gbk_get_info
+ * for large K or an explicit tile; never more for small K than ceil(nx / 4) ceil(ny / 4)).  Larger
+ * batches are rejected with GBK_ERR_ARG (split them, or use gbk_eval_batch); so is
+ * GBK_EXTRACT_GAUSSFIT (GBK_ERR_UNSUPPORTED: that pipeline needs a model cube of scratch).
+ * ONE array per device serves every problem and every stream: two gbk_eval_batch_static calls that
+ * may overlap on the GPU (different streams, or a replayed graph beside a live call) RACE on it --
+ * order them on one stream or with events.  It keeps the last call's contents between calls;
+ * nothing in it needs to survive from one call to the next.
+ */
+#define GBK_STATIC_MAX_ROWS (1 << 16)
+#define GBK_STATIC_MAX_PARTIALS (1 << 20)
+int gbk_eval_batch_static(gbk_problem *p, const float *params, const int32_t *gal_index, int64_t K,
+                          float *chi2, float *m0, float *m1, float *m2, float *resid,
+                          void *cuda_stream);
+
+/*
  * Comparison path, same contract: one kernel per step of the paper's pipeline
  * (PAPER.md:197-251), with the FP32 model cube written to device memory
  * between steps (the paper's own structure minus the FFT).  Processes the rows

@@ -99,6 +99,36 @@ struct gbk_problem {
   float* lsf_taps = nullptr;    // [2 r_v + 1], unfused path only
 };
 
+// ---- gbk_eval_batch_static: cross-tile scratch that nobody allocates ---------------------------
+// [GBK_STATIC_MAX_PARTIALS] chi^2 partials (float) followed by [GBK_STATIC_MAX_ROWS] tile counters (unsigned,
+// same size), in the device image of this translation unit: every device that loads the library holds it.
+// The NAME below is a host-side stand-in in host code, not a device address: kernels get the address that
+// cudaGetSymbolAddress returns for the current device (static_scratch_address).
+static __device__ __align__(256) float g_static_scratch[GBK_STATIC_MAX_PARTIALS + GBK_STATIC_MAX_ROWS];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+float* g_static_addr[kMaxDevices] = {};        // device address of g_static_scratch on device i
+cudaError_t g_static_err[kMaxDevices] = {};    // why it is missing
+
+// Looks the address up once per device.  `device` must be current (cudaGetSymbolAddress answers for the
+// current device; the first call also loads this unit's device image, which is why gbk_create_problem
+// makes it at set-up and gbk_eval_batch_static only reads the table).
+float* static_scratch_address(int device, bool lookup) {
+  if (device < 0 || device >= kMaxDevices) return nullptr;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_addr[device] && lookup) {
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+    g_static_err[device] = e;
+    if (e == cudaSuccess) g_static_addr[device] = static_cast<float*>(ptr);
+    else (void)cudaGetLastError();             // not sticky for the caller's next CUDA call
+  }
+  return g_static_addr[device];
+}
+}  // namespace
+
 extern "C" const char* gbk_last_error(void) { return g_err; }
 
 extern "C" int gbk_destroy(gbk_problem* p) {
@@ -381,6 +411,8 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     dp = dp0;
   }
 #undef GBK_CUDA_P
+  // set-up of gbk_eval_batch_static on this device (a failure is reported by that call, not here)
+  (void)static_scratch_address(dev, true);
   // host pointers of the descriptor are not kept
   p->d.vobs = p->d.verr = p->d.sobs = p->d.serr = nullptr;
   p->d.mask = nullptr;
@@ -557,6 +589,45 @@ static int eval_batch_impl(gbk_problem* p, const float* params, const int32_t* g
   }
   EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, partial, tile_count, counters};
   GBK_CUDA(launch_fused(dp, a, p->levels[lv].fl, st));
+  return GBK_OK;
+}
+
+// gbk_eval_batch with the cross-tile scratch in g_static_scratch: no allocation of any kind (no scratch table,
+// no cudaMalloc), one cudaMemsetAsync and one launch on the caller's stream.
+extern "C" int gbk_eval_batch_static(gbk_problem* p, const float* params, const int32_t* gal_index, int64_t K,
+                                     float* chi2, float* m0, float* m1, float* m2, float* resid,
+                                     void* cuda_stream) {
+  g_err[0] = 0;
+  if (int rc = check_eval_args(p, params, K, chi2)) return rc;
+  if (K == 0) return GBK_OK;
+  if (p->extraction == GBK_EXTRACT_GAUSSFIT)
+    return fail(GBK_ERR_UNSUPPORTED, "gbk_eval_batch_static: GBK_EXTRACT_GAUSSFIT runs the multi-kernel pipeline, "
+                                     "which needs a model cube of scratch; use gbk_eval_batch");
+  const DevProblem& dp = p->levels[pick_level(p, K)].dp;
+  const FusedLaunch& fl = p->levels[pick_level(p, K)].fl;
+  if (K > (int64_t)GBK_STATIC_MAX_ROWS)
+    return fail(GBK_ERR_ARG, "gbk_eval_batch_static: K = %lld rows exceeds GBK_STATIC_MAX_ROWS = %d; split the batch "
+                             "or use gbk_eval_batch", (long long)K, (int)GBK_STATIC_MAX_ROWS);
+  if (K * (int64_t)dp.ntiles > (int64_t)GBK_STATIC_MAX_PARTIALS)
+    return fail(GBK_ERR_ARG, "gbk_eval_batch_static: K x tiles = %lld x %d exceeds GBK_STATIC_MAX_PARTIALS = %d; "
+                             "split the batch or use gbk_eval_batch", (long long)K, dp.ntiles,
+                (int)GBK_STATIC_MAX_PARTIALS);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DeviceGuard guard(p->device);
+  GBK_CUDA(guard.status);
+  float* scratch = static_scratch_address(p->device, false);
+  if (!scratch)
+    return fail(GBK_ERR_CUDA, "gbk_eval_batch_static: no device address of the static scratch on device %d "
+                              "(cudaGetSymbolAddress at gbk_create_problem: %s)", p->device,
+                p->device >= 0 && p->device < kMaxDevices ? cudaGetErrorString(g_static_err[p->device])
+                                                          : "device ordinal beyond the table");
+  float* partial = scratch;
+  unsigned* tile_count = reinterpret_cast<unsigned*>(scratch + GBK_STATIC_MAX_PARTIALS);
+  // the array keeps whatever the last call (of any problem) left: the counters must start at zero; the
+  // partials are all written before they are read
+  if (dp.ntiles > 1) GBK_CUDA(cudaMemsetAsync(tile_count, 0, sizeof(unsigned) * (size_t)K, st));
+  EvalArgs a{params, gal_index, (long long)K, chi2, m0, m1, m2, resid, partial, tile_count, nullptr};
+  GBK_CUDA(launch_fused(dp, a, fl, st));
   return GBK_OK;
 }
 

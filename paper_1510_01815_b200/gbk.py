@@ -26,7 +26,7 @@ GBK_EXTRACT_MOMENTS, GBK_EXTRACT_GAUSSFIT = 0, 1
 
 EXPORTS = (   # every symbol include/gbk.h declares (tests/test_abi_and_dist.py checks them all)
     "gbk_create_problem", "gbk_get_info", "gbk_set_strategy", "gbk_set_extraction", "gbk_reserve", "gbk_eval_batch",
-    "gbk_eval_batch_counted",
+    "gbk_eval_batch_counted", "gbk_eval_batch_static",
     "gbk_eval_batch_unfused", "gbk_eval_vfield_batch", "gbk_eval_batch_host", "gbk_destroy",
     "gbk_last_error", "gbk_probe_pipe", "gbk_probe_umma", "gbk_fit_ng", "gbk_fit_lm", "gbk_fit_ns",
 )
@@ -94,7 +94,7 @@ def lib():
         L.gbk_create_problem.restype = C.c_int
         L.gbk_get_info.argtypes = [vp, C.POINTER(gbk_problem_info)]
         L.gbk_get_info.restype = C.c_int
-        for name in ("gbk_eval_batch", "gbk_eval_batch_unfused"):
+        for name in ("gbk_eval_batch", "gbk_eval_batch_unfused", "gbk_eval_batch_static"):
             f = getattr(L, name)
             f.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp]
             f.restype = C.c_int
@@ -224,6 +224,16 @@ def gbk_eval_batch_counted(handle, params, gal_index, K, chi2, counters, stream=
     """gbk_eval_batch (chi^2 only) adding the voxel loop's work counts to `counters` (device int64 [4])."""
     _check(lib().gbk_eval_batch_counted(handle, _ptr(params), _ptr(gal_index), int(K), _ptr(chi2),
                                         _ptr(counters), stream or None))
+
+
+GBK_STATIC_MAX_ROWS, GBK_STATIC_MAX_PARTIALS = 1 << 16, 1 << 20
+
+
+def gbk_eval_batch_static(handle, params, gal_index, K, chi2, m0=None, m1=None, m2=None, resid=None, stream=0):
+    """gbk_eval_batch that allocates nothing: cross-tile scratch in the library's static device array
+    (K <= GBK_STATIC_MAX_ROWS, K x tiles <= GBK_STATIC_MAX_PARTIALS; overlapping calls race on it)."""
+    _check(lib().gbk_eval_batch_static(handle, _ptr(params), _ptr(gal_index), int(K), _ptr(chi2), _ptr(m0),
+                                       _ptr(m1), _ptr(m2), _ptr(resid), stream or None))
 
 
 def gbk_reserve(handle, K_max: int, stream=0):
