@@ -279,7 +279,8 @@ def psf_radius(w: wl.Workload, fwhm: float) -> int:
 
 
 def ext_samples_per_eval(info, w: wl.Workload, R: int) -> int:
-    """Extended fine samples a row of PSF radius R evaluates: sum over its tiles of (tw+2R)(th+2R)."""
+    """Extended fine samples a row of PSF radius R EVALUATES in the kernel's tiling: sum over its tiles of
+    (tw+2R)(th+2R) -- every tile carries its own PSF halo."""
     tw, th, fw, fh = info.tile_w * w.u, info.tile_h * w.u, w.nx * w.u, w.ny * w.u
     tot = 0
     for ty in range(info.tiles_y):
@@ -291,19 +292,27 @@ def ext_samples_per_eval(info, w: wl.Workload, R: int) -> int:
 def op_counts(info, w: wl.Workload, radii: np.ndarray) -> dict:
     """Algorithmic FP32 lane-ops per evaluation: 5 per extended voxel, 45 per
     extended sample, 3 maps x (2 x taps separable | taps^2 image) per fine pixel, 12 per spaxel --
-    averaged over the PSF radii of the batch's rows."""
+    averaged over the PSF radii of the batch's rows.  "Extended" is the WHOLE FIELD plus one PSF halo
+    (SURVEY's table: 270 x 270 x 56 for config 4), whatever tiling the kernel uses: the halos that tiles
+    re-evaluate are the kernel's overhead, not the method's work.  `*_tiled` are the figures of the tiling
+    (equal for one tile per row: configs 3 and 5)."""
     nvx = info.nv + 2 * info.r_v
-    fine = (w.u * w.nx) * (w.u * w.ny)
-    tot = 0.0
-    samples = 0.0
+    fw, fh = w.u * w.nx, w.u * w.ny
+    tot = tot_tiled = samples = samples_tiled = 0.0
     for R in np.unique(radii):
         share = float(np.mean(radii == R))
-        ns = ext_samples_per_eval(info, w, int(R))
+        ns = (fw + 2 * int(R)) * (fh + 2 * int(R))
+        ns_tiled = ext_samples_per_eval(info, w, int(R))
         taps = 2 * int(R) + 1
         psf = taps * taps if w.psf_kind == wl.PSF_IMAGE else 2 * taps
-        tot += share * (5.0 * ns * nvx + 45.0 * ns + 3.0 * psf * fine + 12.0 * w.nx * w.ny)
+        rest = 3.0 * psf * fw * fh + 12.0 * w.nx * w.ny
+        tot += share * (5.0 * ns * nvx + 45.0 * ns + rest)
+        tot_tiled += share * (5.0 * ns_tiled * nvx + 45.0 * ns_tiled + rest)
         samples += share * ns
-    return {"ops_per_eval": tot, "ext_samples_per_eval": samples, "ext_voxels_per_eval": samples * nvx}
+        samples_tiled += share * ns_tiled
+    return {"ops_per_eval": tot, "ext_samples_per_eval": samples, "ext_voxels_per_eval": samples * nvx,
+            "ops_per_eval_tiled": tot_tiled, "ext_samples_per_eval_tiled": samples_tiled,
+            "ext_voxels_per_eval_tiled": samples_tiled * nvx}
 
 
 def executed_ops(counters: np.ndarray, K: int, nominal: dict, info, w: wl.Workload) -> float:
@@ -414,6 +423,8 @@ def time_case(gbk, torch, case: dict, launches: int, flush, sm_max_mhz: float, t
            "tile_of_large_batches": [info.tile_w, info.tile_h], "block_threads": info.block_threads,
            "ops_per_eval": int(nominal["ops_per_eval"]),
            "frac": nominal["ops_per_eval"] * K / (med * 1e-3) / 1e9 / peak,
+           "ops_per_eval_tiled": int(nominal["ops_per_eval_tiled"]),
+           "frac_tiled": nominal["ops_per_eval_tiled"] * K / (med * 1e-3) / 1e9 / peak,
            "ops_executed_per_eval": int(ex), "frac_executed": ex * K / (med * 1e-3) / 1e9 / peak,
            "voxel_loop": {"warp_items": int(cnt[0]), "poly_blocks": int(cnt[1]), "direct_channels": int(cnt[2]),
                           "precise_items": int(cnt[3])},
@@ -529,7 +540,9 @@ def run_ours(args, ranks) -> None:
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
                 "ops_per_eval": int(nominal["ops_per_eval"]),
                 "ops_how": "ALGORITHMIC FP32 lane-ops of SURVEY.md 8(d): 5/ext voxel + 45/ext sample + 3 maps x "
-                           "(2 x taps separable | taps^2 image)/fine pixel + 12/spaxel",
+                           "(2 x taps separable | taps^2 image)/fine pixel + 12/spaxel; ext = the whole field plus ONE "
+                           "PSF halo, whatever the tiling (halos re-evaluated per tile are overhead, not work)",
+                "ops_per_eval_tiled": int(nominal["ops_per_eval_tiled"]),
                 "ops_executed_per_eval": int(executed),
                 "achieved_executed": executed * evals_per_s_rank / 1e9,
                 "frac_executed": executed * evals_per_s_rank / 1e9 / peak_fp32,

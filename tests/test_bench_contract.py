@@ -28,7 +28,7 @@ def test_reference_arm_prints_the_contract_line():
 
 def test_algorithmic_op_count_is_the_survey_figure():
     """Config 3: 5 x 415 872 + 45 x 5 776 + 3 x 26 x 4 096 + 12 x 4 096 = 2 707 920 lane-ops per evaluation
-    (SURVEY.md section 8(d)); config 4 with its 225-tap image: 5 x 4 082 400 x ... per tile layout."""
+    (SURVEY.md section 8(d)); config 4 with its 225-tap image: 68 715 732."""
     sys.path.insert(0, ROOT)
     import bench
     from paper_1510_01815_b200 import workloads as wl
@@ -41,5 +41,9 @@ def test_algorithmic_op_count_is_the_survey_figure():
     w4 = wl.config(4)
     info4 = types.SimpleNamespace(nv=48, r_v=4, tile_w=64, tile_h=64, tiles_x=4, tiles_y=4)
     n4 = bench.op_counts(info4, w4, np.full(256, 7))
-    assert n4["ext_samples_per_eval"] == 16 * 78 * 78
-    assert n4["ops_per_eval"] == 5 * 16 * 78 * 78 * 56 + 45 * 16 * 78 * 78 + 3 * 225 * 65536 + 12 * 65536
+    # the algorithmic count extends the WHOLE FIELD by one PSF halo (SURVEY's 6.87e7 for config 4), whatever the
+    # tiling; the halos the 16 tiles re-evaluate are reported apart
+    assert n4["ext_samples_per_eval"] == 270 * 270 and n4["ext_samples_per_eval_tiled"] == 16 * 78 * 78
+    assert n4["ops_per_eval"] == 5 * 270 * 270 * 56 + 45 * 270 * 270 + 3 * 225 * 65536 + 12 * 65536 == 68715732
+    assert n4["ops_per_eval_tiled"] == 5 * 16 * 78 * 78 * 56 + 45 * 16 * 78 * 78 + 3 * 225 * 65536 + 12 * 65536
+    assert n["ops_per_eval_tiled"] == n["ops_per_eval"]
