@@ -503,7 +503,8 @@ __device__ __noinline__ float conv2d_moments(const DevProblem& dp, const EvalArg
 // 8-pixel chunk of two rows (y and y + th/2): per kernel row it holds the N taps as (w, w) pairs
 // (one 8-byte broadcast read each) and applies them to the two input rows (float4 reads; lanes run
 // along y and the row stride is 4 mod 8 floats, so they are conflict-free), i.e. 8 N FFMA2 for
-// N + 1 + 2 NV4 shared-memory reads.  `out` is a different plane than `in`.
+// N + 1 + 2 NV4 shared-memory reads.  `out` is a different plane than `in`.  (The two end terms of an
+// output pair's N + 1 tap pairs carry half a pair each and share one FFMA2: 8 N - 8 + 8 per kernel row.)
 template <int N>
 __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ews, int tw, int th,
                                              const u64* w64, int tid, int nthreads) {
@@ -526,6 +527,12 @@ __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ew
       u64 w[N + 1];
 #pragma unroll
       for (int j = 0; j <= N; ++j) w[j] = w64[ky * (N + 1) + j];
+      u64 wend;
+      {
+        float w0, wz, wl;
+        upk(w[0], w0, wz), upk(w[N], wz, wl);
+        wend = pk(w0, wl);
+      }
 #pragma unroll
       for (int m = 0; m < 2; ++m) {
         const float* rowp = in + (yy[m] + ky) * ews + (xc << 3);
@@ -539,7 +546,10 @@ __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ew
         for (int i = 0; i < 8 + N - 1; ++i)
 #pragma unroll
           for (int p = 0; p < 4; ++p)
-            if (i - 2 * p >= 0 && i - 2 * p <= N) acc[m][p] = fma2(w[i - 2 * p], pk1(v[i]), acc[m][p]);
+            if (i - 2 * p >= 1 && i - 2 * p <= N - 1) acc[m][p] = fma2(w[i - 2 * p], pk1(v[i]), acc[m][p]);
+        // the two end terms have half a tap pair each, (W[0], 0) v[2p] and (0, W[N-1]) v[2p+N]: one FFMA2
+#pragma unroll
+        for (int p = 0; p < 4; ++p) acc[m][p] = fma2(wend, pk(v[2 * p], v[2 * p + N]), acc[m][p]);
       }
     }
 #pragma unroll
