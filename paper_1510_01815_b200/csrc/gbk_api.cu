@@ -390,7 +390,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
     cap.smem_bytes = (int)smem_cap;
     GBK_CUDA_P(fused_prepare(cap));
   }
-  GBK_CUDA_P(fused_occupancy(p->fl, &p->blocks_per_sm));
+  GBK_CUDA_P(fused_occupancy(dp, p->fl, &p->blocks_per_sm));
   auto rounds_for = [&](const DevProblem& q, const FusedLaunch& f) {
     const int ne = (q.tile_w + 2 * r_p_max) * (q.tile_h + 2 * r_p_max);
     return (ne + 4 * f.threads - 1) / (4 * f.threads);
@@ -405,7 +405,7 @@ extern "C" int gbk_create_problem(const gbk_problem_desc* d, gbk_problem** out) 
       lf.smem_bytes = (int)set_tile(lw, lh);
       lf.threads = threads_for(dp);
       int bps = 1;
-      GBK_CUDA_P(fused_occupancy(lf, &bps));
+      GBK_CUDA_P(fused_occupancy(dp, lf, &bps));
       p->levels.push_back({dp, lf, std::max(1, bps), rounds_for(dp, lf)});
     }
     dp = dp0;

@@ -585,12 +585,12 @@ __device__ __forceinline__ float image_phase(const DevProblem& dp, const EvalArg
                              nthreads);
 }
 
-template <int R, bool OUT>
+template <int R, bool OUT, bool U1>
 __device__ __forceinline__ float separable_phase(const DevProblem& dp, const EvalArgs& a,
                                               const RowConst& rc, long long k, float* maps,
                                               int map_stride, int EH, int tw, int th, int tx0,
                                               int ty0, const float* taps, int tid, int nthreads) {
-  if (dp.u == 1) {
+  if (U1 || dp.u == 1) {   // U1: the instantiation for u == 1 holds nothing else
     u64 tb[R + 1];
     load_tap_bcast<R>(taps, tb);
     hpass_x<R>(maps, map_stride, dp.ews, EH, tw, tb, tid, nthreads);
@@ -598,6 +598,7 @@ __device__ __forceinline__ float separable_phase(const DevProblem& dp, const Eva
     return vpass_x_moments<R, kVBlockX, OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0,
                                              tb, tid, nthreads);
   }
+  if (U1) return 0.0f;
   u64 tp[2 * R + 2];
   load_tap_pairs<R>(taps, tp);
   hpass<R>(maps, map_stride, dp.ews, EH, tw, tp, tid, nthreads);
@@ -1125,7 +1126,11 @@ __device__ __noinline__ void build_block_tables(const DevProblem& dp, const Eval
 }
 
 // ------------------------------------------------------------------------------ the kernel ---
-template <bool OUT, bool COUNT>
+// PATH: which PSF passes the instantiation holds -- kPathAny everything (chosen at run time), kPathSepU1 the
+// separable Gaussian passes without down-sampling only (configs 1, 3, 5), kPathImage the register-tiled image
+// pass only (config 4).  The specialised ones exist for the register allocation of their hot loops.
+constexpr int kPathAny = 0, kPathSepU1 = 1, kPathImage = 2;
+template <bool OUT, bool COUNT, int PATH>
 __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     fused_kernel(const __grid_constant__ DevProblem dp, const __grid_constant__ EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1147,7 +1152,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     build_block_tables(dp, a, k, smem_raw, tid, nthreads);
     __syncthreads();
   }
-  if (dp.img_fast) {   // rows of tap pairs (W[ky][i], W[ky][i-1]), i = 0..N, with W[ky][-1] = W[ky][N] = 0
+  if (PATH == kPathImage || (PATH == kPathAny && dp.img_fast)) {   // rows of tap pairs (W[ky][i], W[ky][i-1]), i = 0..N, with W[ky][-1] = W[ky][N] = 0
     const int n = 2 * rc.r_p + 1;
     const float* W = dp.psf_taps + (size_t)rc.psf_set * dp.psf_stride;
     for (int j = tid; j < n * (n + 1); j += nthreads) {
@@ -1190,7 +1195,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     // ------------------------------------------------------------------ a5 .. a9 ---------
     if ((rc.precise == kSqueezed)) {
       chi = precise_finish<OUT>(dp, a, sm.rc, k, sm.maps, map_stride, tw, th, tx0, ty0, sm.taps, tid, nthreads);
-    } else if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) {
+    } else if (PATH == kPathImage || (PATH == kPathAny && dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast)) {
 #define GBK_IMG_CASE(NN)                                                                          \
   case NN:                                                                                        \
     chi = image_phase<NN, OUT>(dp, a, rc, k, sm.maps, sm.spare, map_stride, tw, th, tx0, ty0,     \
@@ -1202,13 +1207,13 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
         default: break;
       }
 #undef GBK_IMG_CASE
-    } else if (dp.psf_kind == GBK_PSF_IMAGE) {
+    } else if (PATH == kPathAny && dp.psf_kind == GBK_PSF_IMAGE) {
       chi = conv2d_moments<OUT>(dp, a, rc, k, sm.maps, map_stride, dp.ews, tw, th, tx0, ty0, sm.taps,
                                 tid, nthreads);
     } else {
 #define GBK_SEP_CASE(RR)                                                                          \
   case RR:                                                                                        \
-    chi = separable_phase<RR, OUT>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0,       \
+    chi = separable_phase<RR, OUT, PATH == kPathSepU1>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0, \
                                    sm.taps, tid, nthreads);                                       \
     break;
       switch (R) {
@@ -1259,30 +1264,47 @@ size_t fused_smem_bytes(const DevProblem& dp) {
          sizeof(float) * 32;
 }
 
+namespace {
+// the instantiation a problem runs (see kPath* above)
+int path_of(const DevProblem& dp) {
+  if (dp.psf_kind == GBK_PSF_GAUSSIAN && dp.u == 1) return kPathSepU1;
+  if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) return kPathImage;
+  return kPathAny;
+}
+typedef void (*FusedFn)(const DevProblem, const EvalArgs);
+FusedFn fused_fn(int path, bool out, bool count) {
+#define GBK_PATH_FN(PP)                                                  \
+  case PP:                                                               \
+    return out ? fused_kernel<true, false, PP> : (count ? fused_kernel<false, true, PP> : fused_kernel<false, false, PP>);
+  switch (path) {
+    GBK_PATH_FN(kPathSepU1) GBK_PATH_FN(kPathImage)
+    default: break;
+  }
+  return out ? fused_kernel<true, false, kPathAny> : (count ? fused_kernel<false, true, kPathAny> : fused_kernel<false, false, kPathAny>);
+#undef GBK_PATH_FN
+}
+}  // namespace
+
 cudaError_t fused_prepare(const FusedLaunch& fl) {
-  cudaError_t e = cudaFuncSetAttribute(fused_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       fl.smem_bytes);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(fused_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fl.smem_bytes);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(fused_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              fl.smem_bytes);
+  for (int path = 0; path < 3; ++path)
+    for (int v = 0; v < 3; ++v) {
+      const cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(fused_fn(path, v == 1, v == 2)),
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, fl.smem_bytes);
+      if (e != cudaSuccess) return e;
+    }
+  return cudaSuccess;
 }
 
-cudaError_t fused_occupancy(const FusedLaunch& fl, int* n) {
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(n, fused_kernel<false, false>, fl.threads,
-                                                       fl.smem_bytes);
+cudaError_t fused_occupancy(const DevProblem& dp, const FusedLaunch& fl, int* n) {
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(n, reinterpret_cast<const void*>(fused_fn(path_of(dp), false, false)),
+                                                       fl.threads, fl.smem_bytes);
 }
 
 cudaError_t launch_fused(const DevProblem& dp, const EvalArgs& a, const FusedLaunch& fl,
                          cudaStream_t st) {
   const long long nblocks = a.K * dp.ntiles;
-  if (a.m0 || a.m1 || a.m2 || a.resid)
-    fused_kernel<true, false><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
-  else if (a.counters)
-    fused_kernel<false, true><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
-  else
-    fused_kernel<false, false><<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
+  const bool out = a.m0 || a.m1 || a.m2 || a.resid;
+  fused_fn(path_of(dp), out, !out && a.counters)<<<(unsigned)nblocks, fl.threads, fl.smem_bytes, st>>>(dp, a);
   return cudaGetLastError();
 }
 

@@ -142,7 +142,7 @@ struct FusedLaunch {
 
 cudaError_t launch_fused(const DevProblem& dp, const EvalArgs& a, const FusedLaunch& fl,
                          cudaStream_t st);
-cudaError_t fused_occupancy(const FusedLaunch& fl, int* blocks_per_sm);
+cudaError_t fused_occupancy(const DevProblem& dp, const FusedLaunch& fl, int* blocks_per_sm);
 cudaError_t fused_prepare(const FusedLaunch& fl);  // opt in to large dynamic shared memory
 size_t fused_smem_bytes(const DevProblem& dp);
 
