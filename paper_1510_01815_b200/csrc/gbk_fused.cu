@@ -49,7 +49,7 @@ constexpr float kTruncD = 6.5f;   // lines centred in the band are summed out to
 // floats of the PSF tap area: image taps of the register-tiled pass are stored as (w, w) pairs
 __host__ __device__ __forceinline__ int taps_floats(const DevProblem& dp) {
   const int n = 2 * dp.r_p_max + 1;
-  return dp.img_fast ? round_up4(2 * n * (n + 1)) : round_up4(dp.psf_stride);
+  return dp.img_fast ? round_up4(2 * n * (n + 1)) : round_up4(dp.psf_stride) + 2 * (n + 1);   // + (w[i], w[i-1]) pairs
 }
 
 // Velocity (from v_center) of the centre of channel block b of the extended band (precise rows).
@@ -384,6 +384,60 @@ __device__ __forceinline__ void hpass_x(float* maps, int map_stride, int ews, in
   }
 }
 
+// The same pass with BROADCAST inputs: an output pair (x, x + 1) receives from input v[i] the tap pair
+// (w[i], w[i - 1]) (w[-1] = w[2R + 1] = 0) -- 2R + 2 FFMA2 per pair instead of 2R + 1, but FFMA2 takes the
+// scalar v[i] as it is, where the pass above has to build every odd-offset input pair with two MOVs.  The tap
+// pairs are read from shared memory (`tp`, one 8-byte broadcast read each).
+template <int R>
+__device__ __forceinline__ void hpass_b(float* maps, int map_stride, int ews, int EH, int tw, const u64* tp,
+                                        int tid, int nthreads) {
+  constexpr int NV4 = (4 + 2 * R + 3) / 4;
+  const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
+  const int nx4 = (tw + 3) >> 2;
+  int lpr_log = 0;
+  while ((1 << lpr_log) < nx4 && lpr_log < 5) ++lpr_log;
+  const int lpr = 1 << lpr_log;                 // lanes per row
+  const int rpp = 32 >> lpr_log;                // rows per pass
+  const int l = lane & (lpr - 1), rsub = lane >> lpr_log;
+  const int nchunks = (nx4 + lpr - 1) >> lpr_log;
+  const int npass = (EH + rpp - 1) / rpp;
+  for (int job = warp; job < npass; job += nwarps) {
+    const int row = job * rpp + rsub;
+    for (int chunk = 0; chunk < nchunks; ++chunk) {
+      const int x0 = ((chunk << lpr_log) + l) << 2;
+      const bool active = row < EH && x0 < tw;
+      float* rowp = maps + row * ews + x0;
+      float4 res[3];
+      if (active) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+          float v[NV4 * 4];
+#pragma unroll
+          for (int i = 0; i < NV4; ++i) {
+            const float4 f = *reinterpret_cast<const float4*>(rowp + q * map_stride + 4 * i);
+            v[4 * i] = f.x, v[4 * i + 1] = f.y, v[4 * i + 2] = f.z, v[4 * i + 3] = f.w;
+          }
+          u64 o0 = pk(0.f, 0.f), o1 = o0;
+#pragma unroll
+          for (int i = 0; i < 2 * R + 2; ++i) {
+            const u64 t = tp[i];
+            o0 = fma2(t, pk1(v[i]), o0);
+            if (i + 2 < NV4 * 4) o1 = fma2(t, pk1(v[i + 2]), o1);
+          }
+          upk(o0, res[q].x, res[q].y);
+          upk(o1, res[q].z, res[q].w);
+        }
+      }
+      __syncwarp();
+      if (active) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) *reinterpret_cast<float4*>(rowp + q * map_stride) = res[q];
+      }
+      __syncwarp();
+    }
+  }
+}
+
 // Vertical pass fused with moments and chi^2 (u == 1): a thread owns BY consecutive rows of a
 // column PAIR; lanes run along x, so the 8-byte shared-memory reads are conflict-free and the
 // global accesses coalesced.  Rows past the tile are read from the (allocated, never written)
@@ -593,7 +647,9 @@ __device__ __forceinline__ float separable_phase(const DevProblem& dp, const Eva
   if (U1 || dp.u == 1) {   // U1: the instantiation for u == 1 holds nothing else
     u64 tb[R + 1];
     load_tap_bcast<R>(taps, tb);
-    hpass_x<R>(maps, map_stride, dp.ews, EH, tw, tb, tid, nthreads);
+    if (U1) hpass_b<R>(maps, map_stride, dp.ews, EH, tw, reinterpret_cast<const u64*>(taps + round_up4(dp.psf_stride)),
+                       tid, nthreads);
+    else hpass_x<R>(maps, map_stride, dp.ews, EH, tw, tb, tid, nthreads);
     __syncthreads();
     return vpass_x_moments<R, kVBlockX, OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0,
                                              tb, tid, nthreads);
@@ -1162,6 +1218,12 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
   } else {
     for (int j = tid; j < dp.psf_stride; j += nthreads)
       sm.taps[j] = dp.psf_taps[(size_t)rc.psf_set * dp.psf_stride + j];
+    if (PATH == kPathSepU1) {   // tap pairs (w[i], w[i - 1]) of the horizontal pass (hpass_b)
+      const float* W = dp.psf_taps + (size_t)rc.psf_set * dp.psf_stride;
+      const int n = 2 * rc.r_p + 1;
+      u64* tp = reinterpret_cast<u64*>(sm.taps + round_up4(dp.psf_stride));
+      for (int i = tid; i <= n; i += nthreads) tp[i] = pk(i < n ? W[i] : 0.0f, i >= 1 ? W[i - 1] : 0.0f);
+    }
   }
 
   float chi = 0.0f;
