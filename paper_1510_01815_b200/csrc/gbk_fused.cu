@@ -182,7 +182,8 @@ __device__ __forceinline__ float spaxel_finish_moments(const DevProblem& dp, con
   float s = (m2 - ob.z) * ob.w;
   float contrib = fmaf(t, t, s * s);
   const bool bad = !(contrib < f_inf());                        // NaN or Inf moments
-  contrib = unmasked ? (bad ? f_inf() : contrib) : 0.0f;
+  contrib = fminf(contrib, f_inf());                            // ... count +INF (fminf drops the NaN): no branch
+  contrib = unmasked ? contrib : 0.0f;
   if (OUT) {
     if (dark) m1r = m2 = f_nan();
     if (!unmasked) t = s = 0.0f;
