@@ -760,7 +760,9 @@ def time_survey(gbk, torch) -> dict:
     starts[:, wl.IX_RT] = np.clip(starts[:, wl.IX_RT], 1.0, 8.0)
     gal = np.repeat(np.arange(n, dtype=np.int32), 2)
     with gbk.Problem(**d) as prob:
-        gbk.gbk_fit_lm(prob.handle, starts[:64], gal[:64], free7, lo, hi, max_iter=2)     # warm-up
+        # warm-up at the full size, so that the library's cached workspace is sized before the timed call (on a
+        # fresh box the first large cudaMalloc alone can take tens of ms of the wall-clock fit time)
+        gbk.gbk_fit_lm(prob.handle, starts, gal, free7, lo, hi, max_iter=2)
         rows, chi2, iters, st = gbk.gbk_fit_lm(prob.handle, starts, gal, free7, lo, hi,
                                                rel_step=1e-3, max_iter=50, ftol=1e-6)
     best = np.where(chi2[0::2] <= chi2[1::2], 0, 1) + 2 * np.arange(n)
