@@ -533,9 +533,9 @@ def run_ours(args, ranks) -> None:
                 "achieved": achieved, "peak": peak_fp32, "unit": "Gop/s", "frac": achieved / peak_fp32,
                 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, copied from the committed ncu --set full
                 # capture of this command (config 3 only) -- NOT measured in this run
-                "traffic": 423680 if (cfg == 3 and tuple(args.tile) == (0, 0)) else None,
+                "traffic": 319744 if (cfg == 3 and tuple(args.tile) == (0, 0)) else None,
                 "traffic_unit": "bytes per launch",
-                "traffic_source": "profiles/r02_fused_kernel_ncu.md (325.6 KB read + 98.0 KB written per launch of 4096 "
+                "traffic_source": "profiles/r02_fused_kernel_ncu.md (319.7 KB read + 0 B written -- the 16 KB of chi^2 stay in L2 -- per launch of 4096 "
                                   "rows); a constant from that capture, not measured live; irrelevant to an ALU-bound kernel",
                 "peak_how": f"derived: {info.sm_count} SMs x 128 FP32 lanes x {sm_max:.0f} MHz (max SM clock)",
                 "ops_per_eval": int(nominal["ops_per_eval"]),
