@@ -640,12 +640,13 @@ __device__ __forceinline__ float image_phase(const DevProblem& dp, const EvalArg
                              nthreads);
 }
 
-template <int R, bool OUT, bool U1>
+template <int R, bool OUT, int UMODE>   // UMODE 0: u read at run time, 1: u == 1 only, 2: u > 1 only
 __device__ __forceinline__ float separable_phase(const DevProblem& dp, const EvalArgs& a,
                                               const RowConst& rc, long long k, float* maps,
                                               int map_stride, int EH, int tw, int th, int tx0,
                                               int ty0, const float* taps, int tid, int nthreads) {
-  if (U1 || dp.u == 1) {   // U1: the instantiation for u == 1 holds nothing else
+  constexpr bool U1 = UMODE == 1;
+  if (U1 || (UMODE == 0 && dp.u == 1)) {   // the instantiations for u == 1 / u > 1 hold nothing else
     u64 tb[R + 1];
     load_tap_bcast<R>(taps, tb);
     if (U1) hpass_b<R>(maps, map_stride, dp.ews, EH, tw, reinterpret_cast<const u64*>(taps + round_up4(dp.psf_stride)),
@@ -1186,7 +1187,7 @@ __device__ __noinline__ void build_block_tables(const DevProblem& dp, const Eval
 // PATH: which PSF passes the instantiation holds -- kPathAny everything (chosen at run time), kPathSepU1 the
 // separable Gaussian passes without down-sampling only (configs 1, 3, 5), kPathImage the register-tiled image
 // pass only (config 4).  The specialised ones exist for the register allocation of their hot loops.
-constexpr int kPathAny = 0, kPathSepU1 = 1, kPathImage = 2;
+constexpr int kPathAny = 0, kPathSepU1 = 1, kPathImage = 2, kPathSepUN = 3;   // kPathSepUN: separable, u > 1 (config 2)
 template <bool OUT, bool COUNT, int PATH>
 __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     fused_kernel(const __grid_constant__ DevProblem dp, const __grid_constant__ EvalArgs a) {
@@ -1276,7 +1277,7 @@ __global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
     } else {
 #define GBK_SEP_CASE(RR)                                                                          \
   case RR:                                                                                        \
-    chi = separable_phase<RR, OUT, PATH == kPathSepU1>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0, \
+    chi = separable_phase<RR, OUT, PATH == kPathSepU1 ? 1 : (PATH == kPathSepUN ? 2 : 0)>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0, \
                                    sm.taps, tid, nthreads);                                       \
     break;
       switch (R) {
@@ -1330,7 +1331,7 @@ size_t fused_smem_bytes(const DevProblem& dp) {
 namespace {
 // the instantiation a problem runs (see kPath* above)
 int path_of(const DevProblem& dp) {
-  if (dp.psf_kind == GBK_PSF_GAUSSIAN && dp.u == 1) return kPathSepU1;
+  if (dp.psf_kind == GBK_PSF_GAUSSIAN) return dp.u == 1 ? kPathSepU1 : kPathSepUN;
   if (dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast) return kPathImage;
   return kPathAny;
 }
@@ -1340,7 +1341,7 @@ FusedFn fused_fn(int path, bool out, bool count) {
   case PP:                                                               \
     return out ? fused_kernel<true, false, PP> : (count ? fused_kernel<false, true, PP> : fused_kernel<false, false, PP>);
   switch (path) {
-    GBK_PATH_FN(kPathSepU1) GBK_PATH_FN(kPathImage)
+    GBK_PATH_FN(kPathSepU1) GBK_PATH_FN(kPathImage) GBK_PATH_FN(kPathSepUN)
     default: break;
   }
   return out ? fused_kernel<true, false, kPathAny> : (count ? fused_kernel<false, true, kPathAny> : fused_kernel<false, false, kPathAny>);
@@ -1349,7 +1350,7 @@ FusedFn fused_fn(int path, bool out, bool count) {
 }  // namespace
 
 cudaError_t fused_prepare(const FusedLaunch& fl) {
-  for (int path = 0; path < 3; ++path)
+  for (int path = 0; path < 4; ++path)
     for (int v = 0; v < 3; ++v) {
       const cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(fused_fn(path, v == 1, v == 2)),
                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, fl.smem_bytes);
