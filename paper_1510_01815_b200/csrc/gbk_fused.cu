@@ -560,9 +560,19 @@ __device__ __noinline__ float conv2d_moments(const DevProblem& dp, const EvalArg
 // along y and the row stride is 4 mod 8 floats, so they are conflict-free), i.e. 8 N FFMA2 for
 // N + 1 + 2 NV4 shared-memory reads.  `out` is a different plane than `in`.  (The two end terms of an
 // output pair's N + 1 tap pairs carry half a pair each and share one FFMA2: 8 N - 8 + 8 per kernel row.)
-template <int N>
-__device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ews, int tw, int th,
-                                             const u64* w64, int tid, int nthreads) {
+// FIN (u == 1 only): the plane convolved is S2, the last of the three; its outputs stay in registers and each
+// pixel is finished on the spot with its S0 and S1 read from `fin.s0`, `fin.s1` (the planes the first two
+// passes wrote) -- no store of S2, no barrier and no separate pass over the spaxels.  Returns the thread's chi^2.
+struct ConvFinish {
+  const float *s0, *s1;     // convolved planes (same row stride)
+  long long k;
+  int tx0, ty0;
+};
+template <int N, bool FIN, bool OUT>
+__device__ __forceinline__ float conv2d_plane(const DevProblem& dp, const EvalArgs& a, const RowConst& rc,
+                                              const ConvFinish& fin, const float* in, float* out, int ews, int tw,
+                                              int th, const u64* w64, int tid, int nthreads) {
+  float chi = 0.0f;
   constexpr int NV4 = (8 + N - 1 + 3) / 4;
   const int nxc = (tw + 7) >> 3, half = (th + 1) >> 1;
   const unsigned magic = div_magic(half);
@@ -615,11 +625,27 @@ __device__ __forceinline__ void conv2d_plane(const float* in, float* out, int ew
         upk(acc[m][1], f0.z, f0.w);
         upk(acc[m][2], f1.x, f1.y);
         upk(acc[m][3], f1.z, f1.w);
-        float* o = out + yy[m] * ews + (xc << 3);
-        *reinterpret_cast<float4*>(o) = f0;
-        *reinterpret_cast<float4*>(o + 4) = f1;
+        const int o = yy[m] * ews + (xc << 3);
+        if (FIN) {
+          const float s2[8] = {f0.x, f0.y, f0.z, f0.w, f1.x, f1.y, f1.z, f1.w};
+          const float4 a0 = *reinterpret_cast<const float4*>(fin.s0 + o), a1 = *reinterpret_cast<const float4*>(fin.s0 + o + 4);
+          const float4 b0 = *reinterpret_cast<const float4*>(fin.s1 + o), b1 = *reinterpret_cast<const float4*>(fin.s1 + o + 4);
+          const float s0[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+          const float s1[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+          const int pix0 = (fin.ty0 + yy[m]) * dp.nx + fin.tx0 + (xc << 3);
+          float part = 0.0f;
+#pragma unroll
+          for (int e = 0; e < 8; ++e)
+            if ((xc << 3) + e < tw)
+              part += spaxel_finish<OUT>(dp, a, rc, fin.k, pix0 + e, load_obs(dp, rc, pix0 + e), s0[e], s1[e], s2[e]);
+          chi += part;
+        } else {
+          *reinterpret_cast<float4*>(out + o) = f0;
+          *reinterpret_cast<float4*>(out + o + 4) = f1;
+        }
       }
   }
+  return chi;
 }
 
 // a5..a9 for an image PSF on the fast path: the three maps are convolved plane by plane, each into
@@ -630,11 +656,16 @@ __device__ __forceinline__ float image_phase(const DevProblem& dp, const EvalArg
                                           int th, int tx0, int ty0, const float* taps, int tid,
                                           int nthreads) {
   const u64* w64 = reinterpret_cast<const u64*>(taps);
-  conv2d_plane<N>(maps, spare, dp.ews, tw, th, w64, tid, nthreads);
+  const ConvFinish fin{spare, maps, k, tx0, ty0};
+  conv2d_plane<N, false, OUT>(dp, a, rc, fin, maps, spare, dp.ews, tw, th, w64, tid, nthreads);
   __syncthreads();
-  conv2d_plane<N>(maps + map_stride, maps, dp.ews, tw, th, w64, tid, nthreads);
+  conv2d_plane<N, false, OUT>(dp, a, rc, fin, maps + map_stride, maps, dp.ews, tw, th, w64, tid, nthreads);
   __syncthreads();
-  conv2d_plane<N>(maps + 2 * map_stride, maps + map_stride, dp.ews, tw, th, w64, tid, nthreads);
+  if (dp.u == 1)   // no down-sampling: finish every pixel from the registers of the third pass
+    return conv2d_plane<N, true, OUT>(dp, a, rc, fin, maps + 2 * map_stride, nullptr, dp.ews, tw, th, w64, tid,
+                                      nthreads);
+  conv2d_plane<N, false, OUT>(dp, a, rc, fin, maps + 2 * map_stride, maps + map_stride, dp.ews, tw, th, w64, tid,
+                              nthreads);
   __syncthreads();
   return moments_blocks<OUT>(dp, a, rc, k, spare, maps, maps + map_stride, dp.ews, tw, th, tx0, ty0, tid,
                              nthreads);
@@ -1189,7 +1220,7 @@ __device__ __noinline__ void build_block_tables(const DevProblem& dp, const Eval
 // pass only (config 4).  The specialised ones exist for the register allocation of their hot loops.
 constexpr int kPathAny = 0, kPathSepU1 = 1, kPathImage = 2, kPathSepUN = 3;   // kPathSepUN: separable, u > 1 (config 2)
 template <bool OUT, bool COUNT, int PATH>
-__global__ void __launch_bounds__(kMaxThreads, kMinBlocks)
+__global__ void __launch_bounds__(kMaxThreads, PATH == kPathImage ? 2 : kMinBlocks)
     fused_kernel(const __grid_constant__ DevProblem dp, const __grid_constant__ EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Smem sm = carve(dp, smem_raw);
