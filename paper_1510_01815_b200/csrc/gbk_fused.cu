@@ -1220,7 +1220,7 @@ __device__ __noinline__ void build_block_tables(const DevProblem& dp, const Eval
 // pass only (config 4).  The specialised ones exist for the register allocation of their hot loops.
 constexpr int kPathAny = 0, kPathSepU1 = 1, kPathImage = 2, kPathSepUN = 3;   // kPathSepUN: separable, u > 1 (config 2)
 template <bool OUT, bool COUNT, int PATH>
-__global__ void __launch_bounds__(kMaxThreads, PATH == kPathImage ? 2 : kMinBlocks)
+__global__ void __launch_bounds__(kMaxThreads, (PATH == kPathImage || PATH == kPathSepUN) ? 2 : kMinBlocks)
     fused_kernel(const __grid_constant__ DevProblem dp, const __grid_constant__ EvalArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Smem sm = carve(dp, smem_raw);
