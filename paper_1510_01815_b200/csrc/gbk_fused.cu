@@ -826,32 +826,34 @@ __device__ __noinline__ void sample_geometry_f64(const DevProblem& dp, const Row
 // channel (FWD, ratio r_0 <= 2^14.6), blocks they are approaching at their last one with the mirrored
 // table (g_{7-i} = g_7 rho^i q^(i(i-1)/2), rho = 2^(2 d_7 step - step^2)), and the rare block where the
 // item's lines do both is summed voxel by voxel.
+template <int NP>
 struct VoxelAcc {
-  u64 d0[kPairs], d0lo[kPairs];              // line-centre offset at extended channel 0 (hi, lo)
-  u64 s0[kPairs], s1[kPairs], s2[kPairs];    // the three weighted sums
-  u64 refp[kPairs];                          // precise rows: the pixel's own reference velocity of s1, s2
+  u64 d0[NP], d0lo[NP];              // line-centre offset at extended channel 0 (hi, lo)
+  u64 s0[NP], s1[NP], s2[NP];    // the three weighted sums
+  u64 refp[NP];                          // precise rows: the pixel's own reference velocity of s1, s2
 };
 
 // Precise rows: a block's sums P0, P1, P2 are about the block's centre velocity vb (build_row_tables); the
 // pixel accumulates them about its own reference ref (its line centre clamped to the band), D = vb - ref:
 //   s0 += g P0,   s1 += g (P1 + D P0),   s2 += g (P2 + 2 D P1 + D^2 P0).
 // The blocks that matter for a pixel lie around ref, so D is small where g is not: no cancellation.
-__device__ __forceinline__ void accumulate_recentred(VoxelAcc& v, int j, u64 g, u64 P0, u64 P1, u64 P2, float vb) {
+template <int NP>
+__device__ __forceinline__ void accumulate_recentred(VoxelAcc<NP>& v, int j, u64 g, u64 P0, u64 P1, u64 P2, float vb) {
   const u64 D = add2(pk1(vb), mul2(v.refp[j], pk1(-1.0f)));
   v.s0[j] = fma2(g, P0, v.s0[j]);
   v.s1[j] = fma2(g, fma2(D, P0, P1), v.s1[j]);
   v.s2[j] = fma2(g, fma2(D, fma2(D, P0, add2(P1, P1)), P2), v.s2[j]);
 }
 
-template <bool PRECISE, bool FWD>
+template <bool PRECISE, bool FWD, int NP>
 __device__ __forceinline__ bool poly_block(const DevProblem& dp, const RowConst& rc, const Smem& sm, int b,
-                                           VoxelAcc& v) {
+                                           VoxelAcc<NP>& v) {
   const float nchan = (float)(b * kChanBlock + (FWD ? 0 : kChanBlock - 1));   // the anchor channel
   const float anchor_hi = nchan * rc.step;
   const u64 slope = pk1(FWD ? rc.m2step : -rc.m2step), ms2 = pk1(rc.mstep2);
-  u64 g[kPairs], r[kPairs];
+  u64 g[NP], r[NP];
 #pragma unroll
-  for (int j = 0; j < kPairs; ++j) {
+  for (int j = 0; j < NP; ++j) {
     u64 d;
     if (PRECISE) {   // n * step as a float pair (n * step_hi is not exact in FP32)
       const float anchor_lo = fmaf(nchan, rc.step, -anchor_hi) + nchan * rc.step_lo;
@@ -869,13 +871,13 @@ __device__ __forceinline__ bool poly_block(const DevProblem& dp, const RowConst&
   // whose anchors have all flushed to zero contributes exactly 0: skipping is bit-identical.
   u64 any_g = g[0];
 #pragma unroll
-  for (int j = 1; j < kPairs; ++j) any_g |= g[j];
+  for (int j = 1; j < NP; ++j) any_g |= g[j];
   if (!__any_sync(0xffffffffu, any_g != 0ull)) return false;
   // scalar coefficients: FFMA2 takes a broadcast FP32 operand, so no (C, C) pairs are needed
   GBK_CHECK(b >= 0 && (const float*)((FWD ? sm.coef : sm.coefb) + (b + 1) * (3 * kChanBlock)) <=
                           (FWD ? (const float*)sm.coefb : (const float*)sm.rcd));
   const float4* C = reinterpret_cast<const float4*>((FWD ? sm.coef : sm.coefb) + b * (3 * kChanBlock));
-  u64 P[3][kPairs];
+  u64 P[3][NP];
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
     float c[kChanBlock];
@@ -885,7 +887,7 @@ __device__ __forceinline__ bool poly_block(const DevProblem& dp, const RowConst&
       c[4 * i] = t.x, c[4 * i + 1] = t.y, c[4 * i + 2] = t.z, c[4 * i + 3] = t.w;
     }
 #pragma unroll
-    for (int j = 0; j < kPairs; ++j) {
+    for (int j = 0; j < NP; ++j) {
       u64 Q = pk1(c[kChanBlock - 1]);
 #pragma unroll
       for (int i = kChanBlock - 2; i >= 0; --i) Q = fma2(Q, r[j], pk1(c[i]));
@@ -901,7 +903,7 @@ __device__ __forceinline__ bool poly_block(const DevProblem& dp, const RowConst&
   if (PRECISE) {
     const float vb = block_centre_velocity(dp, b);
 #pragma unroll
-    for (int j = 0; j < kPairs; ++j) {
+    for (int j = 0; j < NP; ++j) {
       if ((rc.precise == kSqueezed)) {
         accumulate_recentred(v, j, g[j], P[0][j], P[1][j], P[2][j], vb);
       } else {
@@ -915,10 +917,10 @@ __device__ __forceinline__ bool poly_block(const DevProblem& dp, const RowConst&
 }
 
 // One channel summed directly: the Gaussian line of PAPER.md:199 by one ex2 per voxel.
-template <bool PRECISE>
-__device__ __forceinline__ void direct_channel(const DevProblem& dp, const RowConst& rc, const float4 w, VoxelAcc& v) {
+template <bool PRECISE, int NP>
+__device__ __forceinline__ void direct_channel(const DevProblem& dp, const RowConst& rc, const float4 w, VoxelAcc<NP>& v) {
 #pragma unroll
-  for (int j = 0; j < kPairs; ++j) {
+  for (int j = 0; j < NP; ++j) {
     u64 d = fma2(pk1(w.x), pk1(rc.step), v.d0[j]);
     if (PRECISE) d = add2(d, fma2(pk1(w.x), pk1(rc.step_lo), v.d0lo[j]));
     float ea, eb;
@@ -967,7 +969,7 @@ __device__ __forceinline__ void strip_pixel(const StripMap& m, int pi, int& ey, 
 // PRECISE (rows whose lines may be centred outside the band, RowConst::precise): the geometry is
 // evaluated in FP64 and the line offset is carried as hi + lo, with the channel offsets c * step
 // compensated likewise, so that d at the voxels that matter (|d| < 12) is good to ~5e-7.
-template <bool PRECISE>
+template <bool PRECISE, int NP>
 __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst& rc, const Smem& sm,
                                             int tx0, int ty0, int EW, int EH, int R, int tid,
                                             int nthreads, unsigned long long* counters) {
@@ -976,16 +978,16 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
   int n_poly = 0, n_direct = 0, n_items = 0;     // work counters of this warp (gbk_eval_batch_counted)
   const int npairs = smap.ppr * EH;
   const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
-  constexpr int kPerItem = 32 * kPairs;
+  constexpr int kPerItem = 32 * NP;
   const int nitems = (npairs + kPerItem - 1) / kPerItem;
   const int map_stride = dp.ehs * dp.ews;
   const float inv_u = dp.inv_u;
   for (int item = warp; item < nitems; item += nwarps) {
-    VoxelAcc v;
-    u64 In[kPairs];
-    int sidx[kPairs];
+    VoxelAcc<NP> v;
+    u64 In[NP];
+    int sidx[NP];
 #pragma unroll
-    for (int j = 0; j < kPairs; ++j) {
+    for (int j = 0; j < NP; ++j) {
       const int pi = item * kPerItem + j * 32 + lane;
       int ey, ex;
       strip_pixel(smap, min(pi, npairs - 1), ey, ex);
@@ -1020,7 +1022,7 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
     // range of the line-centre offsets of the item's 128 pixels (at extended channel 0)
     float dmin = 3.0e38f, dmax = -3.0e38f;
 #pragma unroll
-    for (int j = 0; j < kPairs; ++j) {
+    for (int j = 0; j < NP; ++j) {
       float da, db;
       upk(v.d0[j], da, db);
       dmin = fminf(dmin, fminf(da, db));
@@ -1050,16 +1052,16 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
       // the mirrored anchor up to block b_b (every line centred at most A before its last channel)
       const int b_f = min(max(__float2int_ru((-A - dmin) * rc.inv_bstep), b_lo), b_hi + 1);
       const int b_b = max(min(__float2int_rd((A - span - dmax) * rc.inv_bstep), b_f - 1), b_lo - 1);
-      for (int b = b_lo; b <= b_b; ++b) n_poly += poly_block<PRECISE, false>(dp, rc, sm, b, v) ? 1 : 0;
+      for (int b = b_lo; b <= b_b; ++b) n_poly += poly_block<PRECISE, false, NP>(dp, rc, sm, b, v) ? NP / 2 : 0;
       for (int b = b_b + 1; b < b_f; ++b) {      // lines of this item on both sides of the block
 #pragma unroll
         for (int cc = 0; cc < kChanBlock; ++cc) {
           GBK_CHECK(b >= 0 && b * kChanBlock + cc < dp.nvx_pad);
-          direct_channel<PRECISE>(dp, rc, sm.chan[b * kChanBlock + cc], v);
+          direct_channel<PRECISE, NP>(dp, rc, sm.chan[b * kChanBlock + cc], v);
         }
-        n_direct += kChanBlock;
+        n_direct += kChanBlock * (NP / 2);
       }
-      for (int b = b_f; b <= b_hi; ++b) n_poly += poly_block<PRECISE, true>(dp, rc, sm, b, v) ? 1 : 0;
+      for (int b = b_f; b <= b_hi; ++b) n_poly += poly_block<PRECISE, true, NP>(dp, rc, sm, b, v) ? NP / 2 : 0;
     } else {
       const float inv_step = rc.inv_bstep * (float)kChanBlock;
       const int c_lo = min(max(__float2int_rd((-D - dmax) * inv_step), 0), dp.nvx);
@@ -1067,13 +1069,13 @@ __device__ __forceinline__ void voxel_phase(const DevProblem& dp, const RowConst
 #pragma unroll 4
       for (int c = c_lo; c <= c_hi; ++c) {
         GBK_CHECK(c >= 0 && c < dp.nvx);
-        direct_channel<PRECISE>(dp, rc, sm.chan[c], v);
+        direct_channel<PRECISE, NP>(dp, rc, sm.chan[c], v);
       }
-      n_direct += max(c_hi - c_lo + 1, 0);
+      n_direct += max(c_hi - c_lo + 1, 0) * (NP / 2);
     }
-    ++n_items;
+    n_items += NP / 2;     // the counters' unit is 128 samples (gbk.h)
 #pragma unroll
-    for (int j = 0; j < kPairs; ++j)
+    for (int j = 0; j < NP; ++j)
       if (sidx[j] >= 0) {
         float2 o;
         GBK_CHECK(sidx[j] + 1 < map_stride && (sidx[j] & 1) == 0);
@@ -1169,7 +1171,7 @@ __device__ __noinline__ void voxel_phase_precise(const DevProblem& dp, unsigned 
                                                  unsigned long long* counters) {
   const Smem sm = carve(dp, smem_raw);
   const RowConst rc = *sm.rc;
-  voxel_phase<true>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, counters);
+  voxel_phase<true, kPairs>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, counters);
 }
 
 // Channel table, and the coefficients of the block polynomial of this row (voxel loop):
@@ -1285,7 +1287,8 @@ __global__ void __launch_bounds__(kMaxThreads, (PATH == kPathImage || PATH == kP
     if (rc.precise)
       voxel_phase_precise(dp, smem_raw, tx0, ty0, EW, EH, R, tid, nthreads, COUNT ? a.counters : nullptr);
     else
-      voxel_phase<false>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads, COUNT ? a.counters : nullptr);
+      voxel_phase<false, PATH == kPathImage ? 2 * kPairs : kPairs>(dp, rc, sm, tx0, ty0, EW, EH, R, tid, nthreads,
+                                                                    COUNT ? a.counters : nullptr);
     __syncthreads();
     // ------------------------------------------------------------------ a5 .. a9 ---------
     if ((rc.precise == kSqueezed)) {
