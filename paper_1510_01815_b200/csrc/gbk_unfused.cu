@@ -198,6 +198,55 @@ __global__ void __launch_bounds__(256) uf_lsf_kernel(const __grid_constant__ Dev
   }
 }
 
+// Step 2a for the usual small LSF radii (RV <= kLsfRegMaxR): no shared memory at all.  A thread owns one pixel and
+// walks its channels with the last 2 RV + 1 inputs in a register ring (static indices: the loop is unrolled by
+// the ring length), so every input is loaded from device memory exactly once, 128-byte coalesced across the
+// warp, with a whole group of 2 RV + 1 loads in flight per thread; 2 RV + 1 FMAs per output and nothing else.
+constexpr int kLsfRegMaxR = 6;
+template <int RV>
+__global__ void __launch_bounds__(256, 4) uf_lsf_reg_kernel(const __grid_constant__ DevProblem dp,
+                                                         const float* __restrict__ lsf, int nrows,
+                                                         const float* __restrict__ in, float* __restrict__ out) {
+  constexpr int NT = 2 * RV + 1;
+  float L[NT];
+#pragma unroll
+  for (int j = 0; j < NT; ++j) L[j] = lsf[j];
+  const UGeom g = uf_geom(dp);
+  const long long n = (long long)nrows * (long long)g.plane;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const int row = (int)(idx / (long long)g.plane);
+    const size_t pix = (size_t)(idx - (long long)row * (long long)g.plane);
+    const float* src = in + (size_t)row * g.cube + pix;
+    float* dst = out + (size_t)row * g.cube + pix;
+    // a group of NT outputs c .. c + NT - 1 needs the inputs c .. c + 2 NT - 2: NT - 1 carried over from the
+    // group before, NT new ones, which are requested one group ahead (`nxt`) so that their latency hides
+    // behind the arithmetic of the current group
+    float v[2 * NT - 1], nxt[NT];
+#pragma unroll
+    for (int e = 0; e < NT - 1; ++e) v[e] = src[(size_t)e * g.plane];
+#pragma unroll
+    for (int e = 0; e < NT; ++e) nxt[e] = e < dp.nv ? src[(size_t)(NT - 1 + e) * g.plane] : 0.0f;
+    for (int c = 0; c < dp.nv; c += NT) {
+#pragma unroll
+      for (int e = 0; e < NT; ++e) v[NT - 1 + e] = nxt[e];
+#pragma unroll
+      for (int e = 0; e < NT; ++e)                 // inputs of the next group (output c + NT + e exists)
+        nxt[e] = c + NT + e < dp.nv ? src[(size_t)(c + 2 * NT - 1 + e) * g.plane] : 0.0f;
+#pragma unroll
+      for (int k = 0; k < NT; ++k)
+        if (c + k < dp.nv) {
+          float sum = 0.0f;
+#pragma unroll
+          for (int j = 0; j < NT; ++j) sum = fmaf(L[j], v[k + NT - 1 - j], sum);   // out[c] = sum_j L[j] in[c - j]
+          dst[(size_t)(c + k) * g.plane] = sum;
+        }
+#pragma unroll
+      for (int e = 0; e < NT - 1; ++e) v[e] = v[NT + e];
+    }
+  }
+}
+
 // Step 2b, separable Gaussian PSF: both 1-D passes in one kernel.  A block takes one tile of one
 // channel of one row: the extended tile (tile + 2R each way) is read once into shared memory, the x
 // pass writes an intermediate (tile width x extended height) there, the y pass writes the fine-grid
@@ -618,7 +667,15 @@ cudaError_t launch_unfused(const DevProblem& dp, const EvalArgs& a, const float*
     {
       const long long jobs = (long long)n * (((long long)g.plane + kLsfPix - 1) / kLsfPix);
       const size_t smem = sizeof(float) * kLsfPix * (kLsfPiece + 2 * dp.r_v);
-      uf_lsf_kernel<<<(unsigned)std::min<long long>(jobs, wide), 256, smem, st>>>(dp, lsf_taps, n, A, B);
+      const unsigned rgrid = grid_for((long long)n * g.plane, 256, sm_count);
+#define GBK_LSF_CASE(RR) case RR: uf_lsf_reg_kernel<RR><<<rgrid, 256, 0, st>>>(dp, lsf_taps, n, A, B); break;
+      switch (dp.r_v) {
+        GBK_LSF_CASE(0) GBK_LSF_CASE(1) GBK_LSF_CASE(2) GBK_LSF_CASE(3) GBK_LSF_CASE(4) GBK_LSF_CASE(5) GBK_LSF_CASE(6)
+        default:
+          uf_lsf_kernel<<<(unsigned)std::min<long long>(jobs, wide), 256, smem, st>>>(dp, lsf_taps, n, A, B);
+      }
+#undef GBK_LSF_CASE
+      static_assert(kLsfRegMaxR == 6, "the switch above lists the register-ring instantiations");
     }
     // PSF: B (extended layout) -> A (compact fine-grid layout)
     if (dp.psf_kind == GBK_PSF_GAUSSIAN) {
