@@ -247,6 +247,69 @@ __global__ void __launch_bounds__(256, 4) uf_lsf_reg_kernel(const __grid_constan
   }
 }
 
+constexpr int kPsfTileW = 64;
+// The two passes of one tile from shared memory (shared by the two kernels below): x pass tin -> tmid, y pass
+// tmid -> device memory.
+template <int R, int IW, int IH>
+__device__ __forceinline__ void psf_tile_passes(const float (*tin)[IW], float (*tmid)[kPsfTileW + 1], const float* taps,
+                                                int tw, int th, float* dst, int fw) {
+  // Tap pairs for packed FP32 (FFMA2): an output pair (o[x], o[x+1]) receives from input v[i],
+  // i = 0..2R+1, the pair (f[i], f[i-1]) of flipped taps f[j] = taps[2R - j] (f[-1] = f[2R+1] = 0)
+  // times the broadcast input, i.e. 2R + 2 instructions per two outputs instead of 2 (2R + 1).
+  u64 tp[2 * R + 2];
+#pragma unroll
+  for (int i = 0; i < 2 * R + 2; ++i)
+    tp[i] = pk(i <= 2 * R ? taps[2 * R - i] : 0.0f, i >= 1 ? taps[2 * R - (i - 1)] : 0.0f);
+  constexpr int NX4 = kPsfTileW / 4;
+  for (int i = threadIdx.x; i < (th + 2 * R) * NX4; i += blockDim.x) {      // x pass
+    const int yy = i / NX4, xx = (i - yy * NX4) * 4;
+    float v[4 + 2 * R + 3];
+#pragma unroll
+    for (int q = 0; q < (4 + 2 * R + 3) / 4; ++q) {
+      const float4 f = *reinterpret_cast<const float4*>(&tin[yy][xx + 4 * q]);
+      v[4 * q] = f.x, v[4 * q + 1] = f.y, v[4 * q + 2] = f.z, v[4 * q + 3] = f.w;
+    }
+    u64 o01 = pk(0.f, 0.f), o23 = o01;
+#pragma unroll
+    for (int j = 0; j < 2 * R + 2; ++j) {
+      o01 = fma2(tp[j], pk1(v[j]), o01);
+      o23 = fma2(tp[j], pk1(v[j + 2]), o23);
+    }
+    float o0, o1, o2, o3;
+    upk(o01, o0, o1);
+    upk(o23, o2, o3);
+    tmid[yy][xx] = o0, tmid[yy][xx + 1] = o1, tmid[yy][xx + 2] = o2, tmid[yy][xx + 3] = o3;
+  }
+  __syncthreads();
+  const int ny4 = (th + 3) / 4;
+  for (int i = threadIdx.x; i < ny4 * tw; i += blockDim.x) {                // y pass
+    const int yb = i / tw, xx = i - yb * tw, yy = yb * 4;
+    u64 o01 = pk(0.f, 0.f), o23 = o01;
+    if (yy + 4 + 2 * R <= IH) {          // all 4 + 2R rows lie inside tmid (always, for a full tile): no checks;
+      const float* col = &tmid[yy][xx];  // rows past th + 2R hold older values and only feed outputs not stored
+#pragma unroll
+      for (int j = 0; j < 4 + 2 * R; ++j) {
+        const float vv = col[j * (kPsfTileW + 1)];
+        if (j < 2 * R + 2) o01 = fma2(tp[j], pk1(vv), o01);
+        if (j >= 2) o23 = fma2(tp[j - 2], pk1(vv), o23);
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < 4 + 2 * R; ++j) {
+        const float vv = yy + j < th + 2 * R ? tmid[yy + j][xx] : 0.0f;
+        if (j < 2 * R + 2) o01 = fma2(tp[j], pk1(vv), o01);
+        if (j >= 2) o23 = fma2(tp[j - 2], pk1(vv), o23);
+      }
+    }
+    float o[4];
+    upk(o01, o[0], o[1]);
+    upk(o23, o[2], o[3]);
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+      if (yy + m < th) dst[(size_t)(yy + m) * fw + xx] = o[m];
+  }
+}
+
 // Step 2b, separable Gaussian PSF: both 1-D passes in one kernel.  A block takes one tile of one
 // channel of one row: the extended tile (tile + 2R each way) is read once into shared memory, the x
 // pass writes an intermediate (tile width x extended height) there, the y pass writes the fine-grid
@@ -254,7 +317,6 @@ __global__ void __launch_bounds__(256, 4) uf_lsf_reg_kernel(const __grid_constan
 // in registers.  R is the problem's largest tap radius; a data set with a narrower PSF has its taps
 // centred and zero-padded to that radius (the same sums).
 // in: extended layout [row][c][EH][EW]; out: compact [row][c][fh][fw].
-constexpr int kPsfTileW = 64;
 template <int R>
 __global__ void __launch_bounds__(256) uf_psf_sep_kernel(const __grid_constant__ DevProblem dp,
                                                          const URow* __restrict__ rows, int nrows,
@@ -302,52 +364,75 @@ __global__ void __launch_bounds__(256) uf_psf_sep_kernel(const __grid_constant__
       }
     }
     __syncthreads();
-    // Tap pairs for packed FP32 (FFMA2): an output pair (o[x], o[x+1]) receives from input v[i],
-    // i = 0..2R+1, the pair (f[i], f[i-1]) of flipped taps f[j] = taps[2R - j] (f[-1] = f[2R+1] = 0)
-    // times the broadcast input, i.e. 2R + 2 instructions per two outputs instead of 2 (2R + 1).
-    u64 tp[2 * R + 2];
-#pragma unroll
-    for (int i = 0; i < 2 * R + 2; ++i)
-      tp[i] = pk(i <= 2 * R ? taps[2 * R - i] : 0.0f, i >= 1 ? taps[2 * R - (i - 1)] : 0.0f);
-    constexpr int NX4 = kPsfTileW / 4;
-    for (int i = threadIdx.x; i < (th + 2 * R) * NX4; i += blockDim.x) {      // x pass
-      const int yy = i / NX4, xx = (i - yy * NX4) * 4;
-      float v[4 + 2 * R + 3];
-#pragma unroll
-      for (int q = 0; q < (4 + 2 * R + 3) / 4; ++q) {
-        const float4 f = *reinterpret_cast<const float4*>(&tin[yy][xx + 4 * q]);
-        v[4 * q] = f.x, v[4 * q + 1] = f.y, v[4 * q + 2] = f.z, v[4 * q + 3] = f.w;
-      }
-      u64 o01 = pk(0.f, 0.f), o23 = o01;
-#pragma unroll
-      for (int j = 0; j < 2 * R + 2; ++j) {
-        o01 = fma2(tp[j], pk1(v[j]), o01);
-        o23 = fma2(tp[j], pk1(v[j + 2]), o23);
-      }
-      float o0, o1, o2, o3;
-      upk(o01, o0, o1);
-      upk(o23, o2, o3);
-      tmid[yy][xx] = o0, tmid[yy][xx + 1] = o1, tmid[yy][xx + 2] = o2, tmid[yy][xx + 3] = o3;
-    }
-    __syncthreads();
     float* dst = out + (size_t)row * g.cube + (size_t)c * dp.fw * dp.fh + (size_t)y0 * dp.fw + x0;
-    const int ny4 = (th + 3) / 4;
-    for (int i = threadIdx.x; i < ny4 * tw; i += blockDim.x) {                // y pass
-      const int yb = i / tw, xx = i - yb * tw, yy = yb * 4;
-      u64 o01 = pk(0.f, 0.f), o23 = o01;
-#pragma unroll
-      for (int j = 0; j < 4 + 2 * R; ++j) {
-        const float vv = yy + j < th + 2 * R ? tmid[yy + j][xx] : 0.0f;
-        if (j < 2 * R + 2) o01 = fma2(tp[j], pk1(vv), o01);
-        if (j >= 2) o23 = fma2(tp[j - 2], pk1(vv), o23);
-      }
-      float o[4];
-      upk(o01, o[0], o[1]);
-      upk(o23, o[2], o[3]);
-#pragma unroll
-      for (int m = 0; m < 4; ++m)
-        if (yy + m < th) dst[(size_t)(yy + m) * dp.fw + xx] = o[m];
+    psf_tile_passes<R, IW, IH>(tin, tmid, taps, tw, th, dst, dp.fw);
+  }
+}
+
+// The same step with the tile loads taken off the critical path: the block walks its jobs with TWO input
+// buffers and requests the tile of its next job with cp.async (16-byte copies straight into shared memory)
+// before it computes the current one, so a block always has a tile in flight.  For the aligned case only
+// (extended rows a multiple of 16 bytes, full-width tiles): the launcher falls back to the kernel above otherwise.
+template <int R>
+__global__ void __launch_bounds__(256) uf_psf_sep_pipe_kernel(const __grid_constant__ DevProblem dp,
+                                                              const URow* __restrict__ rows, int nrows,
+                                                              const float* __restrict__ in, float* __restrict__ out) {
+  constexpr int kPsfTileH = R <= 8 ? 64 : 32;
+  constexpr int IW = (kPsfTileW + 2 * R + 3) & ~3, IH = kPsfTileH + 2 * R;
+  extern __shared__ __align__(16) unsigned char psf_smem[];
+  float (*tin0)[IW] = reinterpret_cast<float (*)[IW]>(psf_smem);
+  float (*tin1)[IW] = reinterpret_cast<float (*)[IW]>(psf_smem + sizeof(float) * IH * IW);
+  float (*tmid)[kPsfTileW + 1] = reinterpret_cast<float (*)[kPsfTileW + 1]>(psf_smem + 2 * sizeof(float) * IH * IW);
+  __shared__ float taps[2 * R + 1];
+  const UGeom g = uf_geom(dp);
+  const int ntx = dp.fw / kPsfTileW, nty = (dp.fh + kPsfTileH - 1) / kPsfTileH;
+  const long long per_row = (long long)dp.nv * ntx * nty, njobs = (long long)nrows * per_row;
+  struct Job {
+    int row, c, x0, y0, th;
+  };
+  auto decode = [&](long long job) {
+    Job j;
+    j.row = (int)(job / per_row);
+    long long rem = job - (long long)j.row * per_row;
+    j.c = (int)(rem / (ntx * nty));
+    rem -= (long long)j.c * ntx * nty;
+    const int ty = (int)(rem / ntx), tx = (int)(rem - (long long)ty * ntx);
+    j.x0 = tx * kPsfTileW, j.y0 = ty * kPsfTileH;
+    j.th = min(kPsfTileH, dp.fh - j.y0);
+    return j;
+  };
+  auto request = [&](const Job& j, float (*buf)[IW]) {      // all IW columns lie inside the extended row
+    const float* src = in + (size_t)j.row * g.cube + (size_t)j.c * g.plane + (size_t)j.y0 * g.EW + j.x0;
+    for (int i = threadIdx.x; i < (j.th + 2 * R) * (IW / 4); i += blockDim.x) {
+      const int yy = i / (IW / 4), xx = (i - yy * (IW / 4)) * 4;
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(&buf[yy][xx]);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src + (size_t)yy * g.EW + xx) : "memory");
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  long long job = blockIdx.x;
+  if (job < njobs) request(decode(job), tin0);
+  int cur = 0;
+  for (; job < njobs; job += gridDim.x, cur ^= 1) {
+    const Job j = decode(job);
+    const long long next = job + gridDim.x;
+    // the other buffer was last read by the x pass of the job before this one, which every thread has left
+    // (barrier after that pass), so it is free
+    if (next < njobs) {
+      request(decode(next), cur ? tin0 : tin1);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    const URow r = rows[j.row];
+    if (threadIdx.x < 2 * R + 1) {     // nobody reads `taps` or `tmid` of the previous job any more: see the last barrier
+      const int idx = (int)threadIdx.x - (R - r.r_p);
+      taps[threadIdx.x] = idx >= 0 && idx <= 2 * r.r_p ? dp.psf_taps[(size_t)r.psf_set * dp.psf_stride + idx] : 0.0f;
+    }
+    __syncthreads();                   // this job's tile (everybody's copies) and taps are visible
+    float* dst = out + (size_t)j.row * g.cube + (size_t)j.c * dp.fw * dp.fh + (size_t)j.y0 * dp.fw + j.x0;
+    psf_tile_passes<R, IW, IH>(cur ? tin1 : tin0, tmid, taps, kPsfTileW, j.th, dst, dp.fw);
+    __syncthreads();                   // the y pass is done with tmid and taps before the next job rewrites them
   }
 }
 
@@ -644,8 +729,21 @@ namespace {
 template <int R>
 void launch_psf_sep(const DevProblem& dp, const URow* rows, int n, unsigned cap, const float* in, float* out,
                     cudaStream_t st) {
-  const int th = R <= 8 ? 64 : 32;
+  constexpr int th = R <= 8 ? 64 : 32;
   const long long jobs = (long long)n * dp.nv * ((dp.fw + kPsfTileW - 1) / kPsfTileW) * ((dp.fh + th - 1) / th);
+  const UGeom g = uf_geom(dp);
+  constexpr int IW = (kPsfTileW + 2 * R + 3) & ~3, IH = th + 2 * R;
+  // cp.async pipeline: every 16-byte copy must be aligned and inside the extended row (IW <= EW)
+  const bool aligned = (g.EW & 3) == 0 && dp.fw % kPsfTileW == 0 && IW <= g.EW && (reinterpret_cast<uintptr_t>(in) & 15) == 0 &&
+                       (g.plane & 3) == 0 && (g.cube & 3) == 0;
+  if (aligned) {
+    const size_t smem = sizeof(float) * (2 * (size_t)IH * IW + (size_t)IH * (kPsfTileW + 1));
+    // per device and cheap: set on every launch rather than remembered (the library serves several devices)
+    cudaFuncSetAttribute(uf_psf_sep_pipe_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const unsigned blocks = (unsigned)std::min<long long>(jobs, cap);
+    uf_psf_sep_pipe_kernel<R><<<blocks, 256, smem, st>>>(dp, rows, n, in, out);
+    return;
+  }
   uf_psf_sep_kernel<R><<<(unsigned)std::min<long long>(jobs, cap), 256, 0, st>>>(dp, rows, n, in, out);
 }
 }  // namespace
