@@ -317,10 +317,10 @@ __device__ __forceinline__ void vpass_inplace(float* maps, int map_stride, int e
   }
 }
 
-// ---- x-packed passes (the fast path) -----------------------------------------------------
-// Both passes keep two horizontally adjacent pixels in one 64-bit register pair and multiply by a
-// broadcast tap pair (t, t), so every FFMA2 does two useful FMAs and no instruction is spent on
-// building broadcast inputs.  Symmetric taps: only R + 1 tap pairs live in registers.
+// ---- the passes of the fast path (u == 1) ------------------------------------------------
+// The vertical pass keeps two horizontally adjacent pixels in one 64-bit register pair and multiplies by a
+// broadcast tap pair (t, t), so every FFMA2 does two useful FMAs on aligned pairs; symmetric taps: only
+// R + 1 tap pairs live in registers.  The horizontal pass broadcasts the INPUT instead (hpass_b).
 template <int R>
 __device__ __forceinline__ void load_tap_bcast(const float* taps, u64 (&tb)[R + 1]) {
 #pragma unroll
@@ -331,64 +331,12 @@ __device__ __forceinline__ u64 tap_sym(const u64 (&tb)[R + 1], int j) {   // j i
   return tb[j <= R ? j : 2 * R - j];
 }
 
-// Horizontal pass, in place.  A row of one map is owned by a group of lanes of one warp (each lane
-// 4 consecutive outputs), which loads everything it needs before it stores.
-template <int R>
-__device__ __forceinline__ void hpass_x(float* maps, int map_stride, int ews, int EH, int tw,
-                                        const u64 (&tb)[R + 1], int tid, int nthreads) {
-  const int dp_ehs_dbg = map_stride / ews;   // rows of a plane (bounds checks only)
-  (void)dp_ehs_dbg;
-  constexpr int NV4 = (4 + 2 * R + 3) / 4;
-  const int lane = tid & 31, warp = tid >> 5, nwarps = nthreads >> 5;
-  const int nx4 = (tw + 3) >> 2;
-  int lpr_log = 0;
-  while ((1 << lpr_log) < nx4 && lpr_log < 5) ++lpr_log;
-  const int lpr = 1 << lpr_log;                 // lanes per row
-  const int rpp = 32 >> lpr_log;                // rows per pass
-  const int l = lane & (lpr - 1), rsub = lane >> lpr_log;
-  const int nchunks = (nx4 + lpr - 1) >> lpr_log;
-  const int npass = (EH + rpp - 1) / rpp;
-  for (int job = warp; job < npass; job += nwarps) {
-    const int row = job * rpp + rsub;
-    for (int chunk = 0; chunk < nchunks; ++chunk) {
-      const int x0 = ((chunk << lpr_log) + l) << 2;
-      const bool active = row < EH && x0 < tw;
-      float* rowp = maps + row * ews + x0;
-      float4 res[3];
-      if (active) {
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-          float v[NV4 * 4];
-#pragma unroll
-          for (int i = 0; i < NV4; ++i) {
-            GBK_CHECK(row < dp_ehs_dbg && x0 + 4 * i + 3 < ews);
-            const float4 f = *reinterpret_cast<const float4*>(rowp + q * map_stride + 4 * i);
-            v[4 * i] = f.x, v[4 * i + 1] = f.y, v[4 * i + 2] = f.z, v[4 * i + 3] = f.w;
-          }
-          u64 o0 = pk(0.f, 0.f), o1 = o0;
-#pragma unroll
-          for (int j = 0; j <= 2 * R; ++j) {
-            o0 = fma2(tap_sym<R>(tb, j), pk(v[j], v[j + 1]), o0);
-            o1 = fma2(tap_sym<R>(tb, j), pk(v[j + 2], v[j + 3]), o1);
-          }
-          upk(o0, res[q].x, res[q].y);
-          upk(o1, res[q].z, res[q].w);
-        }
-      }
-      __syncwarp();
-      if (active) {
-#pragma unroll
-        for (int q = 0; q < 3; ++q) *reinterpret_cast<float4*>(rowp + q * map_stride) = res[q];
-      }
-      __syncwarp();
-    }
-  }
-}
-
-// The same pass with BROADCAST inputs: an output pair (x, x + 1) receives from input v[i] the tap pair
-// (w[i], w[i - 1]) (w[-1] = w[2R + 1] = 0) -- 2R + 2 FFMA2 per pair instead of 2R + 1, but FFMA2 takes the
-// scalar v[i] as it is, where the pass above has to build every odd-offset input pair with two MOVs.  The tap
-// pairs are read from shared memory (`tp`, one 8-byte broadcast read each).
+// Horizontal pass, in place, with BROADCAST inputs.  A row of one map is owned by a group of lanes of one warp
+// (each lane 4 consecutive outputs), which loads everything it needs before it stores.  An output pair
+// (x, x + 1) receives from input v[i] the tap pair (w[i], w[i - 1]) (w[-1] = w[2R + 1] = 0) -- 2R + 2 FFMA2 per
+// pair instead of 2R + 1, but FFMA2 takes the scalar v[i] as it is, where multiplying aligned pixel pairs by a
+// broadcast tap has to build every odd-offset input pair with two MOVs (the earlier form of this pass: 78 FFMA2
+// + 56 MOV per 12 outputs).  The tap pairs are read from shared memory (`tp`, one 8-byte broadcast read each).
 template <int R>
 __device__ __forceinline__ void hpass_b(float* maps, int map_stride, int ews, int EH, int tw, const u64* tp,
                                         int tid, int nthreads) {
@@ -671,23 +619,20 @@ __device__ __forceinline__ float image_phase(const DevProblem& dp, const EvalArg
                              nthreads);
 }
 
-template <int R, bool OUT, int UMODE>   // UMODE 0: u read at run time, 1: u == 1 only, 2: u > 1 only
+template <int R, bool OUT, bool U1>   // U1: no down-sampling (u == 1); otherwise u > 1
 __device__ __forceinline__ float separable_phase(const DevProblem& dp, const EvalArgs& a,
                                               const RowConst& rc, long long k, float* maps,
                                               int map_stride, int EH, int tw, int th, int tx0,
                                               int ty0, const float* taps, int tid, int nthreads) {
-  constexpr bool U1 = UMODE == 1;
-  if (U1 || (UMODE == 0 && dp.u == 1)) {   // the instantiations for u == 1 / u > 1 hold nothing else
+  if (U1) {
     u64 tb[R + 1];
     load_tap_bcast<R>(taps, tb);
-    if (U1) hpass_b<R>(maps, map_stride, dp.ews, EH, tw, reinterpret_cast<const u64*>(taps + round_up4(dp.psf_stride)),
-                       tid, nthreads);
-    else hpass_x<R>(maps, map_stride, dp.ews, EH, tw, tb, tid, nthreads);
+    hpass_b<R>(maps, map_stride, dp.ews, EH, tw, reinterpret_cast<const u64*>(taps + round_up4(dp.psf_stride)), tid,
+               nthreads);
     __syncthreads();
     return vpass_x_moments<R, kVBlockX, OUT>(dp, a, rc, k, maps, map_stride, dp.ews, tw, th, tx0, ty0,
                                              tb, tid, nthreads);
   }
-  if (U1) return 0.0f;
   u64 tp[2 * R + 2];
   load_tap_pairs<R>(taps, tp);
   hpass<R>(maps, map_stride, dp.ews, EH, tw, tp, tid, nthreads);
@@ -1217,10 +1162,12 @@ __device__ __noinline__ void build_block_tables(const DevProblem& dp, const Eval
 }
 
 // ------------------------------------------------------------------------------ the kernel ---
-// PATH: which PSF passes the instantiation holds -- kPathAny everything (chosen at run time), kPathSepU1 the
-// separable Gaussian passes without down-sampling only (configs 1, 3, 5), kPathImage the register-tiled image
-// pass only (config 4).  The specialised ones exist for the register allocation of their hot loops.
-constexpr int kPathAny = 0, kPathSepU1 = 1, kPathImage = 2, kPathSepUN = 3;   // kPathSepUN: separable, u > 1 (config 2)
+// PATH: which PSF passes the instantiation holds (path_of picks by problem) -- kPathSepU1 the separable Gaussian
+// passes without down-sampling (configs 1, 3, 5), kPathSepUN the separable passes with down-sampling (config 2),
+// kPathImage the register-tiled image pass (config 4; images up to kMaxFastPsfN a side, any u), kPathAny the
+// general 2-D sum for larger images.  One function with every path inlined spilt ~1750 B inside 80 registers;
+// separate instantiations also let each path have the launch bounds that fit it (fused_kernel below).
+constexpr int kPathAny = 0, kPathSepU1 = 1, kPathImage = 2, kPathSepUN = 3;
 template <bool OUT, bool COUNT, int PATH>
 __global__ void __launch_bounds__(kMaxThreads, (PATH == kPathImage || PATH == kPathSepUN) ? 2 : kMinBlocks)
     fused_kernel(const __grid_constant__ DevProblem dp, const __grid_constant__ EvalArgs a) {
@@ -1243,7 +1190,7 @@ __global__ void __launch_bounds__(kMaxThreads, (PATH == kPathImage || PATH == kP
     build_block_tables(dp, a, k, smem_raw, tid, nthreads);
     __syncthreads();
   }
-  if (PATH == kPathImage || (PATH == kPathAny && dp.img_fast)) {   // rows of tap pairs (W[ky][i], W[ky][i-1]), i = 0..N, with W[ky][-1] = W[ky][N] = 0
+  if (PATH == kPathImage) {   // rows of tap pairs (W[ky][i], W[ky][i-1]), i = 0..N, with W[ky][-1] = W[ky][N] = 0
     const int n = 2 * rc.r_p + 1;
     const float* W = dp.psf_taps + (size_t)rc.psf_set * dp.psf_stride;
     for (int j = tid; j < n * (n + 1); j += nthreads) {
@@ -1293,7 +1240,7 @@ __global__ void __launch_bounds__(kMaxThreads, (PATH == kPathImage || PATH == kP
     // ------------------------------------------------------------------ a5 .. a9 ---------
     if ((rc.precise == kSqueezed)) {
       chi = precise_finish<OUT>(dp, a, sm.rc, k, sm.maps, map_stride, tw, th, tx0, ty0, sm.taps, tid, nthreads);
-    } else if (PATH == kPathImage || (PATH == kPathAny && dp.psf_kind == GBK_PSF_IMAGE && dp.img_fast)) {
+    } else if (PATH == kPathImage) {
 #define GBK_IMG_CASE(NN)                                                                          \
   case NN:                                                                                        \
     chi = image_phase<NN, OUT>(dp, a, rc, k, sm.maps, sm.spare, map_stride, tw, th, tx0, ty0,     \
@@ -1305,13 +1252,13 @@ __global__ void __launch_bounds__(kMaxThreads, (PATH == kPathImage || PATH == kP
         default: break;
       }
 #undef GBK_IMG_CASE
-    } else if (PATH == kPathAny && dp.psf_kind == GBK_PSF_IMAGE) {
+    } else if (PATH == kPathAny) {
       chi = conv2d_moments<OUT>(dp, a, rc, k, sm.maps, map_stride, dp.ews, tw, th, tx0, ty0, sm.taps,
                                 tid, nthreads);
-    } else {
+    } else if (PATH == kPathSepU1 || PATH == kPathSepUN) {
 #define GBK_SEP_CASE(RR)                                                                          \
   case RR:                                                                                        \
-    chi = separable_phase<RR, OUT, PATH == kPathSepU1 ? 1 : (PATH == kPathSepUN ? 2 : 0)>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0, \
+    chi = separable_phase<RR, OUT, PATH == kPathSepU1>(dp, a, rc, k, sm.maps, map_stride, EH, tw, th, tx0, ty0, \
                                    sm.taps, tid, nthreads);                                       \
     break;
       switch (R) {
