@@ -67,8 +67,8 @@ __device__ __forceinline__ u64 vf_velocity2(const DevProblem& dp, const VRow& r,
   const u64 r2 = fma2(xe, xe, mul2(yd, yd));                    // eq. 3
   float r2a, r2b;
   upk(r2, r2a, r2b);
-  // r = 0: cos(theta) := 0 (A8)
-  const u64 rs = pk(r2a > 1e-30f ? rsqrt_approx(r2a) : 0.0f, r2b > 1e-30f ? rsqrt_approx(r2b) : 0.0f);
+  // r = 0: cos(theta) := 0 (A8) -- xe = 0 there, so a finite 1/r gives exactly that without a select
+  const u64 rs = pk(rsqrt_approx(fmaxf(r2a, 1e-30f)), rsqrt_approx(fmaxf(r2b, 1e-30f)));
   const u64 rad = mul2(r2, rs), cos_t = mul2(xe, rs);           // eq. 4
   const u64 q = mul2(rad, r.inv_rt);
   float qa, qb;
@@ -77,10 +77,10 @@ __device__ __forceinline__ u64 vf_velocity2(const DevProblem& dp, const VRow& r,
   if (dp.rc_model == GBK_RC_ARCTAN) {                           // eq. 6 without (2/pi) V_t
     float ia, ib;
     upk(mul2(rs, r.rt), ia, ib);                                // 1/q = r_t / r
-    const bool biga = qa > 1.0f, bigb = qb > 1.0f;
-    const u64 at = atan01_2(pk(biga ? ia : qa, bigb ? ib : qb));
-    f = fma2(at, pk(biga ? -1.0f : 1.0f, bigb ? -1.0f : 1.0f),
-             pk(biga ? 1.5707963267948966f : 0.0f, bigb ? 1.5707963267948966f : 0.0f));
+    // atan q = pi/2 - atan(1/q) for q > 1: the polynomial argument is the smaller of q and 1/q (one min)
+    float ata, atb;
+    upk(atan01_2(pk(fminf(qa, ia), fminf(qb, ib))), ata, atb);
+    f = pk(qa > 1.0f ? 1.5707963267948966f - ata : ata, qb > 1.0f ? 1.5707963267948966f - atb : atb);
   } else if (dp.rc_model == GBK_RC_RAMP) {
     f = pk(fminf(qa, 1.0f), fminf(qb, 1.0f));                   // ramp (A7)
   } else {                                                      // eq. 7: q^g / (1 + q^a)
@@ -132,11 +132,12 @@ __global__ void __launch_bounds__(kThreads) vfield_kernel(const __grid_constant_
       }
       float va, vb;
       upk(vf_velocity2(dp, r, pk(x - r.xo, x + 1.0f - r.xo), y - r.yo), va, vb);
-      if (!r.valid) va = vb = nan;
+      if (OUT && !r.valid) va = vb = nan;     // chi^2 of an out-of-domain row is set to +INF at the end whatever its sum
       const float ta = (va - oa.x) * oa.y, tb = (vb - ob.x) * ob.y;
       float ca = ta * ta, cb = tb * tb;
-      ca = oa.y > 0.0f ? (ca < inf ? ca : inf) : 0.0f;
-      cb = ob.y > 0.0f ? (cb < inf ? cb : inf) : 0.0f;     // ob.y = 0 for the missing second spaxel
+      // NaN or Inf -> +INF (fminf drops the NaN), masked -> 0: one min and one select each, no nested branch
+      ca = oa.y > 0.0f ? fminf(ca, inf) : 0.0f;
+      cb = ob.y > 0.0f ? fminf(cb, inf) : 0.0f;           // ob.y = 0 for the missing second spaxel
       chi[j] += ca + cb;
       if (OUT) {
         const size_t o = (size_t)(k0 + j) * npix + pix;
