@@ -679,8 +679,9 @@ __device__ __forceinline__ u64 pair_geometry(const DevProblem& dp, const RowCons
   const u64 r2 = fma2(xe, xe, mul2(yd, yd));                         // eq. 3
   float r2a, r2b;
   upk(r2, r2a, r2b);
-  // r < 1e-15 px is r = 0: cos(theta) := 0 and V_rot(0) = 0 (A8)
-  const u64 rs = pk(r2a > 1e-30f ? rsqrt_approx(r2a) : 0.0f, r2b > 1e-30f ? rsqrt_approx(r2b) : 0.0f);
+  // r = 0: cos(theta) := 0 and V_rot(0) = 0 (A8) -- x_e = r^2 = 0 there, so a finite 1/r gives exactly that
+  // without a select
+  const u64 rs = pk(rsqrt_approx(fmaxf(r2a, 1e-30f)), rsqrt_approx(fmaxf(r2b, 1e-30f)));
   const u64 r = mul2(r2, rs);
   const u64 cos_t = mul2(xe, rs);                                    // eq. 4
   if (GENERAL && dp.tab_n > 0) {                                     // tabulated T(r / r0)
@@ -698,11 +699,10 @@ __device__ __forceinline__ u64 pair_geometry(const DevProblem& dp, const RowCons
     float qa, qb, ia, ib;
     upk(q, qa, qb);
     upk(mul2(rs, pk1(rc.rt)), ia, ib);                               // 1/q = r_t / r
-    const bool biga = qa > 1.0f, bigb = qb > 1.0f;
-    const u64 at = atan01_2(pk(biga ? ia : qa, bigb ? ib : qb));
-    // atan(q) = pi/2 - atan(1/q) for q > 1
-    f = fma2(at, pk(biga ? -1.0f : 1.0f, bigb ? -1.0f : 1.0f),
-             pk(biga ? 1.5707963267948966f : 0.0f, bigb ? 1.5707963267948966f : 0.0f));
+    // atan(q) = pi/2 - atan(1/q) for q > 1: the polynomial argument is the smaller of q and 1/q (one min)
+    float ata, atb;
+    upk(atan01_2(pk(fminf(qa, ia), fminf(qb, ib))), ata, atb);
+    f = pk(qa > 1.0f ? 1.5707963267948966f - ata : ata, qb > 1.0f ? 1.5707963267948966f - atb : atb);
   } else {                                                           // ramp: min(r/r_t, 1)
     float qa, qb;
     upk(q, qa, qb);
