@@ -248,10 +248,11 @@ __global__ void __launch_bounds__(256, 4) uf_lsf_reg_kernel(const __grid_constan
 }
 
 constexpr int kPsfTileW = 64;
+constexpr int kPsfMidW = kPsfTileW + 4;   // row stride of the intermediate: 16-byte rows
 // The two passes of one tile from shared memory (shared by the two kernels below): x pass tin -> tmid, y pass
 // tmid -> device memory.
 template <int R, int IW, int IH>
-__device__ __forceinline__ void psf_tile_passes(const float (*tin)[IW], float (*tmid)[kPsfTileW + 1], const float* taps,
+__device__ __forceinline__ void psf_tile_passes(const float (*tin)[IW], float (*tmid)[kPsfMidW], const float* taps,
                                                 int tw, int th, float* dst, int fw) {
   // Tap pairs for packed FP32 (FFMA2): an output pair (o[x], o[x+1]) receives from input v[i],
   // i = 0..2R+1, the pair (f[i], f[i-1]) of flipped taps f[j] = taps[2R - j] (f[-1] = f[2R+1] = 0)
@@ -275,38 +276,47 @@ __device__ __forceinline__ void psf_tile_passes(const float (*tin)[IW], float (*
       o01 = fma2(tp[j], pk1(v[j]), o01);
       o23 = fma2(tp[j], pk1(v[j + 2]), o23);
     }
-    float o0, o1, o2, o3;
-    upk(o01, o0, o1);
-    upk(o23, o2, o3);
-    tmid[yy][xx] = o0, tmid[yy][xx + 1] = o1, tmid[yy][xx + 2] = o2, tmid[yy][xx + 3] = o3;
+    float4 o;
+    upk(o01, o.x, o.y);
+    upk(o23, o.z, o.w);
+    *reinterpret_cast<float4*>(&tmid[yy][xx]) = o;
   }
   __syncthreads();
-  const int ny4 = (th + 3) / 4;
-  for (int i = threadIdx.x; i < ny4 * tw; i += blockDim.x) {                // y pass
-    const int yb = i / tw, xx = i - yb * tw, yy = yb * 4;
-    u64 o01 = pk(0.f, 0.f), o23 = o01;
-    if (yy + 4 + 2 * R <= IH) {          // all 4 + 2R rows lie inside tmid (always, for a full tile): no checks;
-      const float* col = &tmid[yy][xx];  // rows past th + 2R hold older values and only feed outputs not stored
+  // y pass: a thread owns a column PAIR (one 8-byte read per row, both columns in one FFMA2 with the tap as the
+  // broadcast scalar operand) and 4 output rows: 4 (2R + 1) FFMA2 and 4 + 2R reads for 8 outputs
+  float f[2 * R + 1];                    // out[y] = sum_t f[t] in[y + t], f[t] = taps[2R - t] as in the x pass
 #pragma unroll
-      for (int j = 0; j < 4 + 2 * R; ++j) {
-        const float vv = col[j * (kPsfTileW + 1)];
-        if (j < 2 * R + 2) o01 = fma2(tp[j], pk1(vv), o01);
-        if (j >= 2) o23 = fma2(tp[j - 2], pk1(vv), o23);
-      }
-    } else {
+  for (int t = 0; t < 2 * R + 1; ++t) f[t] = taps[2 * R - t];
+  const int ny4 = (th + 3) / 4, nxp = (tw + 1) >> 1;
+  const bool pair_store = (fw & 1) == 0 && (reinterpret_cast<size_t>(dst) & 7) == 0;
+  for (int i = threadIdx.x; i < ny4 * nxp; i += blockDim.x) {
+    const int yb = i / nxp, xx = (i - yb * nxp) << 1, yy = yb * 4;
+    u64 acc[4];
 #pragma unroll
-      for (int j = 0; j < 4 + 2 * R; ++j) {
-        const float vv = yy + j < th + 2 * R ? tmid[yy + j][xx] : 0.0f;
-        if (j < 2 * R + 2) o01 = fma2(tp[j], pk1(vv), o01);
-        if (j >= 2) o23 = fma2(tp[j - 2], pk1(vv), o23);
-      }
+    for (int m = 0; m < 4; ++m) acc[m] = pk(0.f, 0.f);
+    const bool inside = yy + 4 + 2 * R <= IH;   // all 4 + 2R rows lie inside tmid (always, for a full tile): no checks;
+                                                // rows past th + 2R hold older values and only feed outputs not stored
+#pragma unroll
+    for (int j = 0; j < 4 + 2 * R; ++j) {
+      u64 v = pk(0.f, 0.f);
+      if (inside || yy + j < th + 2 * R) v = *reinterpret_cast<const u64*>(&tmid[yy + j][xx]);
+#pragma unroll
+      for (int m = 0; m < 4; ++m)
+        if (j - m >= 0 && j - m <= 2 * R) acc[m] = fma2(pk1(f[j - m]), v, acc[m]);
     }
-    float o[4];
-    upk(o01, o[0], o[1]);
-    upk(o23, o[2], o[3]);
 #pragma unroll
     for (int m = 0; m < 4; ++m)
-      if (yy + m < th) dst[(size_t)(yy + m) * fw + xx] = o[m];
+      if (yy + m < th) {
+        float* q = dst + (size_t)(yy + m) * fw + xx;
+        float oa, ob;
+        upk(acc[m], oa, ob);
+        if (pair_store && xx + 1 < tw) {
+          *reinterpret_cast<float2*>(q) = make_float2(oa, ob);
+        } else {
+          q[0] = oa;
+          if (xx + 1 < tw) q[1] = ob;
+        }
+      }
   }
 }
 
@@ -324,7 +334,7 @@ __global__ void __launch_bounds__(256) uf_psf_sep_kernel(const __grid_constant__
   constexpr int kPsfTileH = R <= 8 ? 64 : 32;     // the taller tile has less halo; R > 8 would not fit 48 KB
   constexpr int IW = (kPsfTileW + 2 * R + 3) & ~3, IH = kPsfTileH + 2 * R;
   __shared__ __align__(16) float tin[IH][IW];
-  __shared__ float tmid[IH][kPsfTileW + 1];
+  __shared__ __align__(16) float tmid[IH][kPsfMidW];
   __shared__ float taps[2 * R + 1];
   const UGeom g = uf_geom(dp);
   const int ntx = (dp.fw + kPsfTileW - 1) / kPsfTileW, nty = (dp.fh + kPsfTileH - 1) / kPsfTileH;
@@ -382,7 +392,7 @@ __global__ void __launch_bounds__(256) uf_psf_sep_pipe_kernel(const __grid_const
   extern __shared__ __align__(16) unsigned char psf_smem[];
   float (*tin0)[IW] = reinterpret_cast<float (*)[IW]>(psf_smem);
   float (*tin1)[IW] = reinterpret_cast<float (*)[IW]>(psf_smem + sizeof(float) * IH * IW);
-  float (*tmid)[kPsfTileW + 1] = reinterpret_cast<float (*)[kPsfTileW + 1]>(psf_smem + 2 * sizeof(float) * IH * IW);
+  float (*tmid)[kPsfMidW] = reinterpret_cast<float (*)[kPsfMidW]>(psf_smem + 2 * sizeof(float) * IH * IW);
   __shared__ float taps[2 * R + 1];
   const UGeom g = uf_geom(dp);
   const int ntx = dp.fw / kPsfTileW, nty = (dp.fh + kPsfTileH - 1) / kPsfTileH;
@@ -737,7 +747,7 @@ void launch_psf_sep(const DevProblem& dp, const URow* rows, int n, unsigned cap,
   const bool aligned = (g.EW & 3) == 0 && dp.fw % kPsfTileW == 0 && IW <= g.EW && (reinterpret_cast<uintptr_t>(in) & 15) == 0 &&
                        (g.plane & 3) == 0 && (g.cube & 3) == 0;
   if (aligned) {
-    const size_t smem = sizeof(float) * (2 * (size_t)IH * IW + (size_t)IH * (kPsfTileW + 1));
+    const size_t smem = sizeof(float) * (2 * (size_t)IH * IW + (size_t)IH * kPsfMidW);
     // per device and cheap: set on every launch rather than remembered (the library serves several devices)
     cudaFuncSetAttribute(uf_psf_sep_pipe_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const unsigned blocks = (unsigned)std::min<long long>(jobs, cap);
